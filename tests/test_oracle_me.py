@@ -1,0 +1,459 @@
+"""Pins for the oracle's matrix elements (SURVEY §8(c) 'Pins').  None of these re-types the oracle's
+formulas: they use closed forms, symmetries, defining eigenvalue equations solved by numpy.linalg,
+and a brute-force explicit-colour tensor recursion written with explicit 4x4 gamma matrices."""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+PRM = dict(mz=91.188, wz=2.441404, aewm1=132.507, sw2=0.2222, mt=173.0, alpha_s=0.118)
+GS = math.sqrt(4 * math.pi * PRM["alpha_s"])
+
+# ---------------------------------------------------------------- explicit Dirac algebra (chiral basis)
+S0 = np.eye(2, dtype=complex)
+SIG = [np.array([[0, 1], [1, 0]], complex), np.array([[0, -1j], [1j, 0]], complex), np.array([[1, 0], [0, -1]], complex)]
+Z2 = np.zeros((2, 2), complex)
+GAM = np.array([np.block([[Z2, S0], [S0, Z2]])] + [np.block([[Z2, s], [-s, Z2]]) for s in SIG])   # gamma^mu
+METRIC = np.diag([1.0, -1.0, -1.0, -1.0])
+SIGMA3 = [np.block([[s, Z2], [Z2, s]]) for s in SIG]                                               # spin operator
+I4 = np.eye(4, dtype=complex)
+
+
+def slash(v):
+    return sum(METRIC[m, m] * v[m] * GAM[m] for m in range(4))
+
+
+def null_vector(M):
+    _, s, vh = np.linalg.svd(M)
+    assert s[-1] < 1e-9 * s[0]
+    return vh[-1].conj()
+
+
+def def_u(p, m, lam):
+    """u(p,lam) from its defining equations: (pslash - m)u = 0, (Sigma.phat)u = lam u, u^dag u = 2E."""
+    ph = p[1:] / np.linalg.norm(p[1:])
+    hel = sum(ph[i] * SIGMA3[i] for i in range(3))
+    u = null_vector(np.vstack([slash(p) - m * I4, (hel - lam * I4) * p[0]]))
+    return u * math.sqrt(2 * p[0]) / np.linalg.norm(u)
+
+
+def def_v(p, m, lam):
+    """v(p,lam): (pslash + m)v = 0, (Sigma.phat)v = -lam v (lam = physical antiparticle helicity), v^dag v = 2E."""
+    ph = p[1:] / np.linalg.norm(p[1:])
+    hel = sum(ph[i] * SIGMA3[i] for i in range(3))
+    v = null_vector(np.vstack([slash(p) + m * I4, (hel + lam * I4) * p[0]]))
+    return v * math.sqrt(2 * p[0]) / np.linalg.norm(v)
+
+
+def def_eps(p, lam):
+    """eps(p,lam): eps^0 = 0, eps.p = 0, i phat x eps = lam eps, |eps| = 1."""
+    ph = p[1:] / np.linalg.norm(p[1:])
+    cross = np.array([[0, -ph[2], ph[1]], [ph[2], 0, -ph[0]], [-ph[1], ph[0], 0]], complex)
+    e = null_vector(np.vstack([1j * cross - lam * np.eye(3), ph[None, :]]))
+    return np.concatenate([[0], e / np.linalg.norm(e)])
+
+
+def rand_p(rng, m):
+    k = rng.normal(size=3) * 300
+    return np.array([math.sqrt(m * m + k @ k), *k])
+
+
+# ---------------------------------------------------------------- external states (SURVEY C2 invariants)
+@pytest.mark.parametrize("m", [0.0, 173.0])
+def test_external_spinor_invariants(orc, m):
+    rng = np.random.default_rng(1)
+    pts = [rand_p(rng, m) for _ in range(20)]
+    pts += [np.array([750.0 if m == 0 else math.hypot(750, m), 0, 0, 750.0]),
+            np.array([750.0 if m == 0 else math.hypot(750, m), 0, 0, -750.0])]          # beam-axis branches (Q8)
+    for p in pts:
+        E = p[0]
+        ph = p[1:] / np.linalg.norm(p[1:])
+        hel = sum(ph[i] * SIGMA3[i] for i in range(3))
+        us, vs = {}, {}
+        for lam in (+1, -1):
+            u, v = orc.external("u", p, m, lam), orc.external("v", p, m, lam)
+            us[lam], vs[lam] = u, v
+            assert np.abs((slash(p) - m * I4) @ u).max() < 1e-12 * E ** 1.5            # Dirac equation
+            assert np.abs((slash(p) + m * I4) @ v).max() < 1e-12 * E ** 1.5
+            assert np.abs(hel @ u - lam * u).max() < 1e-12 * E ** 0.5                  # helicity labels
+            assert np.abs(hel @ v + lam * v).max() < 1e-12 * E ** 0.5
+            ub, vb = u.conj() @ GAM[0], v.conj() @ GAM[0]
+            assert abs(ub @ u - 2 * m) < 1e-10 * E and abs(vb @ v + 2 * m) < 1e-10 * E
+            if m == 0.0:   # explicit m=0 branch: the wrong-chirality block is an exact zero
+                assert np.count_nonzero(u) <= 2 and np.count_nonzero(v) <= 2
+            # same ray as the eigenvector definition
+            for w, d in ((u, def_u(p, m, lam)), (v, def_v(p, m, lam))):
+                assert abs(abs(np.vdot(d, w)) - 2 * E) < 1e-9 * E
+        su = sum(np.outer(us[l], us[l].conj() @ GAM[0]) for l in (1, -1))
+        sv = sum(np.outer(vs[l], vs[l].conj() @ GAM[0]) for l in (1, -1))
+        assert np.abs(su - (slash(p) + m * I4)).max() < 1e-11 * E                      # completeness
+        assert np.abs(sv - (slash(p) - m * I4)).max() < 1e-11 * E
+
+
+def test_external_polarisation_invariants(orc):
+    rng = np.random.default_rng(2)
+    pts = [rand_p(rng, 0.0) for _ in range(20)] + [np.array([750.0, 0, 0, 750.0]), np.array([750.0, 0, 0, -750.0])]
+    for p in pts:
+        ph = p[1:] / p[0]
+        e = {lam: orc.external("eps", p, 0.0, lam) for lam in (1, -1)}
+        for lam in (1, -1):
+            assert e[lam][0] == 0
+            assert abs(e[lam] @ METRIC @ p) < 1e-13 * p[0]                              # transverse
+            assert np.abs(1j * np.cross(ph, e[lam][1:]) - lam * e[lam][1:]).max() < 1e-13
+            for lp in (1, -1):                                                         # eps(l).eps(l')* = -delta
+                assert abs(e[lam] @ METRIC @ e[lp].conj() + (1.0 if lam == lp else 0.0)) < 1e-13
+            assert abs(abs(np.vdot(def_eps(p, lam), e[lam])) - 1) < 1e-12
+    # beam-axis special values: e1=(0,1,0,0), e2=(0,0,sgn pz,0); eps = (-lam e1 - i e2)/sqrt2
+    r = 1 / math.sqrt(2)
+    assert np.allclose(orc.external("eps", [750.0, 0, 0, 750.0], 0, +1), [0, -r, -1j * r, 0], atol=0, rtol=1e-16)
+    assert np.allclose(orc.external("eps", [750.0, 0, 0, -750.0], 0, +1), [0, -r, +1j * r, 0], atol=0, rtol=1e-16)
+
+
+# ---------------------------------------------------------------- cfg 1: closed form and cross-section
+def epem_closed_form(p):
+    e2 = 4 * math.pi / PRM["aewm1"]
+    sw2 = PRM["sw2"]
+    sw, cw = math.sqrt(sw2), math.sqrt(1 - sw2)
+    g = {"L": (-0.5 + sw2) / (sw * cw), "R": sw2 / (sw * cw)}
+    s = 1500.0 ** 2
+    A = {a + b: 1 + g[a] * g[b] * s / (s - PRM["mz"] ** 2 + 1j * PRM["mz"] * PRM["wz"]) for a in "LR" for b in "LR"}
+    # c = cos angle(e-, mu-); 1 +- c = |n1 +- n3|^2 / 2 avoids the cancellation near the beam axis
+    n1 = p[:, 1, 1:] / np.linalg.norm(p[:, 1, 1:], axis=1, keepdims=True)
+    n3 = p[:, 3, 1:] / np.linalg.norm(p[:, 3, 1:], axis=1, keepdims=True)
+    opc, omc = ((n1 + n3) ** 2).sum(-1) / 2, ((n1 - n3) ** 2).sum(-1) / 2
+    me = e2 ** 2 / 4 * ((abs(A["LL"]) ** 2 + abs(A["RR"]) ** 2) * opc ** 2 + (abs(A["LR"]) ** 2 + abs(A["RL"]) ** 2) * omc ** 2)
+    sigma = math.pi * (e2 / (4 * math.pi)) ** 2 / (3 * s) * sum(abs(x) ** 2 for x in A.values())
+    return me, sigma
+
+
+def test_cfg1_epem_closed_form_mask_and_cross_section(orc):
+    p, w = orc.events(0, 16384, seed=20230331)
+    me, mh = orc.me(0, p, per_helicity=True)
+    ref, sigma = epem_closed_form(p)
+    rel = np.abs(me / ref - 1)
+    # the few worst events are RAMBO points whose momenta are off shell at 1e-12 (|p| == E is taken for m = 0)
+    assert np.median(rel) < 2e-15 and np.quantile(rel, 0.999) < 1e-12 and rel.max() < 1e-10
+    assert abs(sigma - 1.21298820395e-10) < 1e-20                                       # SURVEY pin value, GeV^-2
+    est = w * me / (2 * 1500.0 ** 2)
+    assert abs(est.mean() - sigma) < 3 * est.std() / math.sqrt(len(est))
+    assert orc.helicity_mask(mh[:32]) == 0x0660                                         # helicities {5,6,9,10}
+    assert (mh[:, [h for h in range(16) if not (0x0660 >> h) & 1]] == 0).all()          # structural zeros are exact
+
+
+# ---------------------------------------------------------------- cfg 2: closed form and cross-section
+def ggtt_closed_form(p):
+    shat = 1500.0 ** 2
+    mt = PRM["mt"]
+    dot = lambda a, b: a[:, 0] * b[:, 0] - (a[:, 1:] * b[:, 1:]).sum(-1)
+    t1, t2 = 2 * dot(p[:, 0], p[:, 2]) / shat, 2 * dot(p[:, 1], p[:, 2]) / shat
+    rho = 4 * mt ** 2 / shat
+    me = GS ** 4 * (1 / (6 * t1 * t2) - 3 / 8) * (t1 ** 2 + t2 ** 2 + rho - rho ** 2 / (4 * t1 * t2))
+    beta = math.sqrt(1 - rho)
+    sigma = math.pi * PRM["alpha_s"] ** 2 / (3 * shat) * ((1 + rho + rho ** 2 / 16) * math.log((1 + beta) / (1 - beta))
+                                                         - beta * (7 / 4 + 31 * rho / 16))
+    return me, sigma
+
+
+def test_cfg2_ggtt_closed_form_mask_and_cross_section(orc):
+    p, w = orc.events(1, 100000, seed=1)
+    me, mh = orc.me(1, p, per_helicity=True)
+    ref, sigma = ggtt_closed_form(p)
+    rel = np.abs(me / ref - 1)
+    # worst events: RAMBO points with |sum p| ~ 1e-7 GeV (boost from a nearly collinear q-pair), for which
+    # the closed form (uses p1.pt, p2.pt only) and the full amplitude see inconsistent inputs; the oracle's
+    # own double-vs-long-double difference on those same events is ~1e-16
+    assert np.median(rel) < 1e-14 and np.quantile(rel, 0.999) < 1e-12 and rel.max() < 1e-9
+    assert abs(sigma - 1.76189425098e-8) < 1e-18                                        # SURVEY pin value, GeV^-2
+    est = w * me / (2 * 1500.0 ** 2)
+    assert abs(est.mean() - sigma) < 3 * est.std() / math.sqrt(len(est))
+    assert orc.helicity_mask(mh[:32]) == 0x9FF9
+    frac = mh / mh.sum(1, keepdims=True)
+    bad = [h for h in range(16) if not (0x9FF9 >> h) & 1]
+    assert frac[:, bad].max() < 1e-18 and np.median(frac[:, bad]) < 1e-27           # Q7: far below the 1e-12 threshold
+
+
+# ---------------------------------------------------------------- diagram counts and colour matrices (C4, C5)
+def test_diagram_and_subtree_counts(orc):
+    assert [orc.info(k)["ndiagrams"] for k in range(5)] == [2, 3, 16, 123, 1240]
+    assert [orc.count_gluon_subtrees(n) for n in range(1, 6)] == [1, 1, 4, 25, 220]
+    assert [orc.info(k)["ncol"] for k in range(5)] == [1, 2, 6, 24, 120]
+    assert [orc.info(k)["avg_denom"] for k in range(5)] == [4, 256, 256, 512, 1536]
+
+
+def lex_perms(n):
+    return list(itertools.permutations(range(n)))
+
+
+@pytest.mark.parametrize("process,denom,diag", [(1, 3, 16), (2, 9, 64), (3, 54, 512), (4, 324, 4096)])
+def test_colour_matrix_values(orc, process, denom, diag):
+    C = orc.color_matrix(process)
+    n = process + 1
+    nc = math.factorial(n)
+    N = C * denom
+    assert np.abs(N - np.round(N)).max() < 1e-9                                         # integer numerators
+    N = np.round(N).astype(int)
+    assert (N == N.T).all() and (np.diag(N) == diag).all()
+    assert abs(C[0, 0] - 3 * (4 / 3) ** n) < 1e-11                                      # N_c C_F^n
+    ev = np.linalg.eigvalsh(C)
+    lo, hi = {1: (4.67, 6), 2: (5, 9), 3: (3.90, 14.85), 4: (1.90, 30.18)}[process]
+    assert abs(ev[0] - lo) < 0.01 and abs(ev[-1] - hi) < 0.01                           # SURVEY C5 eigenvalue ranges
+    perms = lex_perms(n)
+    row = {perms[t]: N[0, t] for t in range(nc)}
+    if process == 1:
+        assert row == {(0, 1): 16, (1, 0): -2}
+    if process == 2:
+        assert row == {(0, 1, 2): 64, (0, 2, 1): -8, (1, 0, 2): -8, (1, 2, 0): 1, (2, 0, 1): 1, (2, 1, 0): 10}
+    if process == 3:
+        vals, cnt = np.unique(N[0], return_counts=True)
+        assert dict(zip(vals.tolist(), cnt.tolist())) == {512: 1, 80: 2, 71: 1, 62: 3, 8: 5, -1: 4, -10: 4, -28: 1, -64: 3}
+    if process == 4:
+        assert sorted(set(N[0].tolist())) == [-512, -224, -134, -116, -80, -71, -62, -53, -44, -8, 1, 10, 19, 28, 64, 100,
+                                              136, 442, 496, 505, 514, 568, 640, 4096]
+    assert max(abs(v).bit_length() for v in N.ravel().tolist()) <= 13
+    # every numerator has <= 11 significant bits (exact in TF32/FP16), SURVEY C5
+    assert all((abs(v) >> ((abs(v) & -abs(v)).bit_length() - 1)).bit_length() <= 11 for v in N.ravel().tolist() if v)
+
+
+def gell_mann():
+    l = np.zeros((8, 3, 3), complex)
+    l[0][0, 1] = l[0][1, 0] = 1
+    l[1][0, 1], l[1][1, 0] = -1j, 1j
+    l[2][0, 0], l[2][1, 1] = 1, -1
+    l[3][0, 2] = l[3][2, 0] = 1
+    l[4][0, 2], l[4][2, 0] = -1j, 1j
+    l[5][1, 2] = l[5][2, 1] = 1
+    l[6][1, 2], l[6][2, 1] = -1j, 1j
+    l[7] = np.diag([1, 1, -2]) / math.sqrt(3)
+    return l / 2
+
+
+def test_colour_matrix_random_entries_direct_trace(orc):
+    # entries other than row 0, straight from sum_a Tr(T^sigma T^tau^dagger) with explicit matrices
+    T = gell_mann()
+    rng = np.random.default_rng(3)
+    for process in (2, 3):
+        n = process + 1
+        perms = lex_perms(n)
+        C = orc.color_matrix(process)
+        for _ in range(4):
+            s, t = rng.integers(len(perms)), rng.integers(len(perms))
+            tot = 0
+            for a in itertools.product(range(8), repeat=n):
+                Ms = np.linalg.multi_dot([T[a[k]] for k in perms[s]]) if n > 1 else T[a[0]]
+                Mt = np.linalg.multi_dot([T[a[k]] for k in perms[t]])
+                tot += np.trace(Ms @ Mt.conj().T)
+            assert abs(tot - C[s, t]) < 1e-10
+
+
+# ---------------------------------------------------------------- symmetries (diagram set, signs)
+def boost_rotate(p, rng):
+    """Random proper Lorentz transformation applied to every momentum of every event."""
+    A = rng.normal(size=(3, 3))
+    Q, _ = np.linalg.qr(A)
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] *= -1
+    b = rng.normal(size=3)
+    b *= 0.6 / np.linalg.norm(b)
+    g = 1 / math.sqrt(1 - b @ b)
+    L = np.eye(4)
+    L[0, 0] = g
+    L[0, 1:] = L[1:, 0] = g * b
+    L[1:, 1:] += (g - 1) * np.outer(b, b) / (b @ b)
+    R = np.eye(4)
+    R[1:, 1:] = Q
+    return p @ (L @ R).T
+
+
+@pytest.mark.parametrize("process,nev", [(1, 16), (2, 16), (3, 8), (4, 2)])
+def test_ward_identity(orc, process, nev):
+    """eps_k -> p_k for any one gluon gives zero: fails at O(1) if a diagram, a relative sign or a colour
+    coefficient is wrong (SURVEY §8(c) pins (ii))."""
+    p, _ = orc.events(process, nev, seed=100 + process)
+    me = orc.me(process, p)
+    for leg in range(process + 1):
+        mw = orc.me(process, p, ward_leg=leg)
+        assert (mw / (750.0 ** 2 * me)).max() < 1e-22
+
+
+@pytest.mark.parametrize("process,nev", [(2, 16), (3, 8), (4, 2)])
+def test_bose_symmetry(orc, process, nev):
+    p, _ = orc.events(process, nev, seed=200 + process)
+    me = orc.me(process, p)
+    q = p.copy()
+    q[:, [0, 1]] = q[:, [1, 0]]                                  # relabel the incoming gluons
+    assert np.abs(orc.me(process, q) / me - 1).max() < 1e-11
+    if process >= 3:
+        for i, j in itertools.combinations(range(4, 4 + process - 1), 2):
+            q = p.copy()
+            q[:, [i, j]] = q[:, [j, i]]                          # swap identical final-state gluons
+            assert np.abs(orc.me(process, q) / me - 1).max() < 1e-11
+
+
+@pytest.mark.parametrize("process,nev", [(0, 32), (1, 32), (2, 16), (3, 8), (4, 2)])
+def test_lorentz_invariance(orc, process, nev):
+    p, _ = orc.events(process, nev, seed=300 + process)
+    me = orc.me(process, p)
+    rng = np.random.default_rng(process)
+    q = boost_rotate(p, rng)                                      # beams leave the z axis: general branches
+    assert np.abs(orc.me(process, q) / me - 1).max() < 1e-10
+
+
+@pytest.mark.parametrize("process,nev", [(1, 32), (2, 16), (3, 8), (4, 2)])
+def test_parity_pairs_of_helicities(orc, process, nev):
+    p, _ = orc.events(process, nev, seed=400 + process)
+    _, mh = orc.me(process, p, per_helicity=True)
+    ncomb = mh.shape[1]
+    flipped = mh[:, [ncomb - 1 - h for h in range(ncomb)]]       # -h has the complemented bit pattern
+    tot = mh.sum(1, keepdims=True)
+    assert np.abs(mh - flipped).max() < 1e-12 * tot.max() and (np.abs(mh - flipped) / tot).max() < 1e-11
+
+
+@pytest.mark.parametrize("process,nev", [(0, 64), (1, 64), (2, 64), (3, 64), (4, 4)])
+def test_double_vs_long_double(orc, process, nev):
+    p, _ = orc.events(process, nev, seed=500 + process)
+    d, l = orc.me(process, p), orc.me(process, p, long_double=True)
+    assert np.abs(d / l - 1).max() < 1e-11
+    assert np.median(np.abs(d / l - 1)) < 1e-13
+
+
+@pytest.mark.parametrize("process,mask", [(2, 0xFFFFFFFF), (3, 2 ** 64 - 1)])
+def test_all_helicities_contribute_cfg3_cfg4(orc, process, mask):
+    p, _ = orc.events(process, 32, seed=[0, 1, 2, 3, 4][process])
+    _, mh = orc.me(process, p, per_helicity=True)
+    assert orc.helicity_mask(mh) == mask
+    assert (mh / mh.sum(1, keepdims=True)).max(0).min() > 1e-7   # smallest genuine contribution, Q7
+
+
+def test_all_helicities_contribute_cfg5(orc):
+    p, _ = orc.events(4, 4, seed=4)
+    _, mh = orc.me(4, p, per_helicity=True)
+    assert orc.helicity_mask(mh) == 2 ** 128 - 1
+
+
+# ---------------------------------------------------------------- SURVEY worked examples (golden fixture)
+def load_worked_examples():
+    out = []
+    with open(os.path.join(GOLD, "worked_examples.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if not line:
+                continue
+            tok = line.split()
+            process, value = int(tok[0]), float(tok[1])
+            mom = np.array([float(x) for x in tok[2:]]).reshape(-1, 4)
+            out.append((process, value, mom))
+    return out
+
+
+def test_worked_examples_third_opinion(orc):
+    for process, value, fin in load_worked_examples():
+        p = np.concatenate([[[750.0, 0, 0, 750.0], [750.0, 0, 0, -750.0]], fin])[None]
+        me = orc.me(process, p)[0]
+        assert abs(me / value - 1) < 1e-10, (process, me, value)
+
+
+# ---------------------------------------------------------------- brute force: explicit colour, no diagram list
+def explicit_colour_me_hel(n, p, hel):
+    """sum over all external colours of |M|^2 for one helicity configuration, by a colour-dressed off-shell
+    recursion with explicit f^{abc}, T^a_{ij} and 4x4 gamma matrices; external states from their defining
+    eigenvalue equations (def_u, def_v, def_eps).  No diagram enumeration, no colour-flow basis."""
+    T = gell_mann()
+    f = np.zeros((8, 8, 8), complex)
+    for a in range(8):
+        for b in range(8):
+            comm = T[a] @ T[b] - T[b] @ T[a]
+            for c in range(8):
+                f[a, b, c] = -2j * np.trace(comm @ T[c])
+    mt = PRM["mt"]
+    part = lambda g: g if g < 2 else g + 2
+    full = (1 << n) - 1
+    K = {m: sum((1 if g < 2 else -1) * p[part(g)] for g in range(n) if m >> g & 1) for m in range(1, full + 1)}
+    K[0] = np.zeros(4)
+    L = "ABCDEFGH"                                                # einsum letter of each gluon's external colour
+    letters = lambda m: "".join(L[g] for g in range(n) if m >> g & 1)
+    low = lambda V: np.tensordot(METRIC, V, axes=(1, 0))
+    G = {}
+    masks = sorted(range(1, full + 1), key=lambda m: (bin(m).count("1"), m))
+    for m in masks:
+        bits = [g for g in range(n) if m >> g & 1]
+        if len(bits) == 1:
+            g = bits[0]
+            e = def_eps(p[part(g)], hel[part(g)])
+            e = e if g < 2 else e.conj()
+            G[m] = np.einsum("m,ca->mca", e, np.eye(8))          # [mu, open colour, external colour]
+            continue
+        acc = 0
+        lowbit = m & -m
+        subs = [A for A in range(1, m) if (A & m) == A]
+        for A in subs:                                           # three-gluon vertex
+            B = m ^ A
+            if not A & lowbit:
+                continue
+            k1, k2 = K[A], K[B]
+            k3 = -(k1 + k2)
+            V1, V2 = G[A], G[B]
+            la, lb, ls = letters(A), letters(B), letters(m)
+            t1 = np.einsum(f"ma{la},mb{lb},r->rab{la}{lb}", low(V1), V2, k1 - k2)
+            t2 = np.einsum(f"m,ma{la},rb{lb}->rab{la}{lb}", METRIC @ (k2 - k3), V1, V2)
+            t3 = np.einsum(f"m,mb{lb},ra{la}->rab{la}{lb}", METRIC @ (k3 - k1), V2, V1)
+            acc = acc + GS * np.einsum(f"abc,rab{la}{lb}->rc{ls}", f, t1 + t2 + t3)
+        for A in subs:                                           # four-gluon vertex
+            if not A & lowbit:
+                continue
+            rest = m ^ A
+            lowr = rest & -rest
+            for B in [x for x in range(1, rest) if (x & rest) == x and x & lowr]:
+                Cc = rest ^ B
+                V1, V2, V3 = G[A], G[B], G[Cc]
+                la, lb, lc, ls = letters(A), letters(B), letters(Cc), letters(m)
+                tot = 0
+                for fa, fb, kin in (("abe", "cde", (("13", 2, +1), ("23", 1, -1))),
+                                    ("ace", "bde", (("12", 3, +1), ("23", 1, -1))),
+                                    ("ade", "bce", (("12", 3, +1), ("13", 2, -1)))):
+                    for pair, free, sign in kin:
+                        idx = {1: f"a{la}", 2: f"b{lb}", 3: f"c{lc}"}
+                        Vs = {1: V1, 2: V2, 3: V3}
+                        i, j = int(pair[0]), int(pair[1])
+                        tot = tot + sign * np.einsum(f"{fa},{fb},m{idx[i]},m{idx[j]},s{idx[free]}->sd{ls}",
+                                                     f, f, low(Vs[i]), Vs[j], Vs[free], optimize=True)
+                acc = acc + (-1j * GS ** 2) * tot
+        k2 = K[m] @ METRIC @ K[m]
+        G[m] = (-1j / k2) * acc
+    # quark line from the outgoing t: Psi[S][spinor, i, j, colours]
+    pt, ptb = p[2], p[3]
+    ub = def_u(pt, mt, hel[2]).conj() @ GAM[0]
+    v = def_v(ptb, mt, hel[3])
+    Psi = {0: np.einsum("b,ij->bij", ub, np.eye(3))}
+    for m in masks:
+        if m == full:
+            continue
+        q = pt - K[m]
+        prop = 1j * (slash(q) + mt * I4) / (q @ METRIC @ q - mt ** 2)
+        acc = 0
+        for A in [x for x in range(1, m + 1) if (x & m) == x]:
+            S = m ^ A
+            ls, la, lm = letters(S), letters(A), letters(m)
+            acc = acc + np.einsum(f"bij{ls},mbe,mc{la},cjk,ea->aik{lm}", Psi[S], GAM, low(G[A]), T, prop, optimize=True) * (1j * GS)
+        Psi[m] = acc
+    M = 0
+    for A in [x for x in range(1, full + 1)]:
+        S = full ^ A
+        ls, la, lm = letters(S), letters(A), letters(full)
+        M = M + np.einsum(f"bij{ls},mbe,mc{la},cjk,e->ik{lm}", Psi[S], GAM, low(G[A]), T, v, optimize=True) * (1j * GS)
+    return float((abs(M) ** 2).sum())
+
+
+@pytest.mark.parametrize("process,hels", [(1, range(16)), (2, range(32)), (3, (0, 5, 27, 38, 63)), (4, (77,))])
+def test_brute_force_explicit_colour(orc, process, hels):
+    n = process + 1
+    p, _ = orc.events(process, 1, seed=600 + process)
+    _, mh = orc.me(process, p, per_helicity=True)
+    npar = n + 2
+    scale = mh[0].max()
+    for ih in hels:
+        hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
+        ref = explicit_colour_me_hel(n, p[0], hel)
+        assert abs(mh[0, ih] - ref) < 1e-10 * max(ref, 1e-6 * scale), (process, ih, mh[0, ih], ref)
