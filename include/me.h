@@ -1,0 +1,156 @@
+/* =====================================================================================
+ * me.h — C-ABI boundary of the B200-native tree-level matrix-element engine.
+ *
+ * What it computes.  For each phase-space point of one of five fixed processes the
+ * library evaluates the tree-level matrix element "based on Feynman diagrams and
+ * helicity amplitudes" (section 2), one event per GPU thread in
+ * lockstep, in double, float or mixed precision, where mixed
+ * means Feynman diagrams in double and "color algebra" in single precision (PAPER.md
+ * line 81, section 3):
+ *
+ *     ME(p) = (1/D) * sum_{h good} sum_{sigma,tau} conj(J_sigma(p,h)) C_{sigma tau} J_tau(p,h)
+ *
+ * J = colour-flow amplitudes ("jamp"), C = colour matrix, D = averaging denominator
+ * (the paper itself prints no formula — every reading is listed in
+ * DESIGN.md).  The paper's interface is "batch of momenta in, batch of MEs out"
+ * (PAPER.md line 41); the entry-point names are those of BASELINE.json `north_star`.
+ *
+ * Conventions: metric (+,-,-,-), GeV, p = (E,px,py,pz); the two
+ * initial-state particles come first with their physical incoming momenta, final-state
+ * particles are outgoing.  Particle order: e+ e- mu+ mu- / g g t t~ [g [g [g]]].
+ * Helicity index ihel in [0, 2^npar): bit (npar-1-k) set <=> particle k has helicity +1.
+ *
+ * Pointers named d_* are DEVICE pointers, everything else is HOST memory.  The caller
+ * owns every buffer it passes; the library owns me_ctx and its internal scratch.
+ * No function throws or aborts; every function returns an me_status.
+ * Every entry point runs on the CUDA device that was current at me_create time.
+ * ===================================================================================== */
+#ifndef PAPER_2303_18244_B200_ME_H
+#define PAPER_2303_18244_B200_ME_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct me_ctx me_ctx; /* opaque; one per (process, parameters, device) */
+
+typedef enum {
+  ME_OK = 0,
+  ME_EINVAL = 1,       /* null pointer, negative n, unknown enum value */
+  ME_EPROCESS = 2,     /* unknown process id */
+  ME_ENOTFILTERED = 3, /* me_compute before me_filter_helicities / me_set_helicities */
+  ME_EALIGN = 4,       /* d_momenta / d_me not 16-byte aligned */
+  ME_ENOMEM = 5,       /* host or device allocation failed */
+  ME_ECUDA = 6         /* a CUDA call failed; me_strerror(ME_ECUDA) names the last one */
+} me_status;
+
+typedef enum {
+  ME_EPEM_MUPMUM = 0, /* e+ e- -> mu+ mu-   (2 diagrams, 16 helicities, 1 colour)        */
+  ME_GG_TTX = 1,      /* g g -> t t~        (3 diagrams, 16 helicities, 2 colour flows)  */
+  ME_GG_TTXG = 2,     /* g g -> t t~ g      (16 diagrams, 32 helicities, 6 flows)        */
+  ME_GG_TTXGG = 3,    /* g g -> t t~ g g    (123 diagrams, 64 helicities, 24 flows)      */
+  ME_GG_TTXGGG = 4    /* g g -> t t~ g g g  (1240 diagrams, 128 helicities, 120 flows)   */
+} me_process;
+
+/* "double", "float" and "mixed" (diagrams FP64, colour algebra FP32). */
+typedef enum { ME_FP64 = 0, ME_MIXED = 1, ME_FP32 = 2 } me_precision;
+
+/* Standard-Model inputs (BASELINE.json configs): cfg 1 uses mz, wz, aewm1 (=1/alpha_EM),
+ * sw2 (=sin^2 theta_W); the QCD processes use mt, alpha_s.  wt must be 0 (reading Q4). */
+typedef struct {
+  double mz, wz, aewm1, sw2;
+  double mt, wt, alpha_s;
+} me_sm_params;
+
+typedef struct {
+  int npar, ninitial, ndiagrams, ncomb, ncolor, color_denom, avg_denom;
+  int page;                   /* P of the AoSoA momentum layout (events per page), 32       */
+  int nkernels;               /* diagram kernels one me_compute pass launches per helicity chunk */
+  int namplitudes;            /* amplitudes per helicity (a 4-gluon vertex yields three)    */
+  double mass[8];             /* external masses in particle order, GeV                      */
+  double flops_per_helicity[3]; /* counted algorithmic real flops per (event, helicity), by me_precision */
+  double flops_per_event_fixed[3]; /* helicity-independent flops per event (invariants, bases)   */
+} me_info;
+
+/* Create a context for `process` on the current CUDA device.  Builds the colour matrix and
+ * helicity tables on the device.  *out is untouched on failure.
+ * Errors: ME_EINVAL (null), ME_EPROCESS, ME_EINVAL (wt != 0 or mt <= 0 for a QCD process), ME_ECUDA. */
+me_status me_create(me_process process, const me_sm_params* params, me_ctx** out);
+
+/* Frees the context and its device scratch.  Synchronises the device.  Null is ME_EINVAL. */
+me_status me_destroy(me_ctx* ctx);
+
+me_status me_get_info(const me_ctx* ctx, me_info* out);
+
+/* Helicity filtering (reading Q7; BASELINE.json north_star
+ * "me_filter_helicities(momenta, n)").  Evaluates, ALWAYS in FP64, every helicity combination
+ * on the first n events of d_momenta; helicity h is "good" iff
+ *     max_events  ME_h(evt) / sum_h' ME_h'(evt)  >  1e-12.
+ * mask_out[w] bit b <=> helicity index 64*w+b is good.  The mask is stored in the context and
+ * returned.  Synchronises `stream`.  n must be >= 1; the buffer must hold ceil(n/P) pages.
+ * d_momenta layout: see me_compute. */
+me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
+                               uint64_t mask_out[2], int* ngood_out, void* stream);
+
+/* Install a helicity mask without filtering (e.g. one returned by an earlier context). */
+me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
+
+/* The hot path.  Asynchronous on `stream`
+ * (a cudaStream_t passed as void*; null = default stream).  No host<->device copy, no
+ * synchronisation (except a one-off scratch allocation for ME_GG_TTXGGG the first time a
+ * larger n is seen).
+ *   d_momenta : DEVICE, FP64 in every precision mode, AoSoA [ceil(n/P)][npar][4][P] with
+ *               P = me_info.page and component order (E,px,py,pz); event e lives at page e/P,
+ *               lane e%P.  The last page must be allocated in full; lanes >= n are read
+ *               but their results discarded (they must hold finite numbers, e.g. a repeated event).
+ *   d_me      : DEVICE, FP64 [n]; ME averaged over initial helicities/colours and divided by
+ *               the identical-particle factor (avg_denom).  Non-finite values are not an error.
+ * n = 0 is a no-op returning ME_OK.
+ * Errors: ME_EINVAL, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA (launch failure). */
+me_status me_compute(me_ctx* ctx, const double* d_momenta, int64_t n, me_precision precision,
+                     double* d_me, void* stream);
+
+/* Same pass, but also returns the per-helicity colour-summed |M_h|^2 (not averaged) for ALL
+ * ncomb helicities (masked ones evaluate too): d_me_hel is DEVICE FP64 [ncomb][n].
+ * Used by the filter and by the parity tests.  d_me may be null. */
+me_status me_compute_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
+                                me_precision precision, double* d_me, double* d_me_hel, void* stream);
+
+/* Colour-flow amplitudes of one helicity (test hook for step a6): d_jamp is DEVICE FP64
+ * [ncolor][2][n] (re, im), in units where the overall factor g_s^(npar-2) and a global
+ * phase are stripped; QCD processes only. */
+me_status me_compute_jamps(me_ctx* ctx, const double* d_momenta, int64_t n, int ihel,
+                           double* d_jamp, void* stream);
+
+/* Host copy of the colour matrix numerators (row-major [ncolor][ncolor], exact integers);
+ * C = numerators / color_denom. */
+me_status me_color_matrix(const me_ctx* ctx, double* numerators_out);
+
+/* Counter-based RNG (reading Q14): Philox4x32-10 with
+ * key = (seed lo32, seed hi32), counter = (event lo32, event hi32, k, j), k in [0,per_event),
+ * j in {0,1}; the 8 output words of (k; j=0,1) give 4 uniforms
+ *     u_i = ((w_2i >> 5) * 2^26 + (w_2i+1 >> 6) + 0.5) * 2^-53   in (0,1).
+ * d_rnd: DEVICE FP64 [n][per_event][4]; event index = first_event + row.  Asynchronous. */
+me_status me_philox_uniform(uint64_t seed, uint64_t first_event, int64_t n, int per_event,
+                            double* d_rnd, void* stream);
+
+/* RAMBO flat phase space (step a1, reading Q12) for the context's process at sqrt_s:
+ * d_rnd [n][nfinal][4] -> d_momenta AoSoA (layout of me_compute, last page padded with copies
+ * of event n-1), d_weight [n] (nullable) = phase-space weight in GeV^(2 nfinal - 4).
+ * Massive final particles by xi rescaling (Newton).  Asynchronous. */
+me_status me_rambo(const me_ctx* ctx, double sqrt_s, const double* d_rnd, int64_t n,
+                   double* d_momenta, double* d_weight, void* stream);
+
+/* Measured-peak microbenchmarks used by bench.py for the roofline denominator: run a
+ * register-resident FMA-chain kernel (FP64 if fp64 != 0 else FP32) on the whole GPU and
+ * return the achieved TFLOP/s in *tflops_out (2 flops per FMA).  Synchronises. */
+me_status me_fma_peak(int fp64, double* tflops_out);
+
+const char* me_strerror(me_status status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,286 @@
+// =====================================================================================
+// hel_amp.cuh — device wavefunction / vertex routines.
+//
+// External states, off-shell currents and amplitudes of the tree-level Feynman rules
+// restated in DESIGN.md ("Readings" C1-C3): metric (+,-,-,-), chiral Dirac basis
+//   gamma^0 = [[0,1],[1,0]],  gamma^i = [[0,s^i],[-s^i,0]],
+// all gluon momenta counted INTO the vertex.  PAPER.md gives no formulas ("Feynman
+// diagrams and helicity amplitudes"); these are the textbook rules.
+//
+// "Stripped" convention: every factor of i and of g_s is removed from the routines here.
+// The generator (codegen/topology.py) folds the phases i^k into the Gaussian-integer colour
+// coefficients c_{d,sigma} and the overall g_s^(2n) into the final normalisation, so all
+// arithmetic below has real scalar coefficients only.
+//
+// Everything is a template on the real type R (double or float) and is force-inlined into
+// the generated per-process kernels: one event per thread, no memory traffic in here.
+// =====================================================================================
+#pragma once
+#include <cuda_runtime.h>
+
+namespace me {
+
+#define ME_DEV __device__ __forceinline__
+
+template <typename R> struct P4 { R e, x, y, z; };            // real four-vector (E,px,py,pz)
+template <typename R> struct Cx { R re, im; };
+// four complex numbers: a Lorentz vector (contravariant 0..3) or a chiral-basis spinor
+template <typename R> struct W4 { R r0, i0, r1, i1, r2, i2, r3, i3; };
+
+template <typename R> ME_DEV R rsqrt_(R x);
+template <> ME_DEV double rsqrt_<double>(double x) { return 1.0 / sqrt(x); }
+template <> ME_DEV float rsqrt_<float>(float x) { return 1.0f / sqrtf(x); }
+template <typename R> ME_DEV R sqrt_(R x);
+template <> ME_DEV double sqrt_<double>(double x) { return sqrt(x); }
+template <> ME_DEV float sqrt_<float>(float x) { return sqrtf(x); }
+
+template <typename R> ME_DEV P4<R> padd(const P4<R>& a, const P4<R>& b) { return {a.e + b.e, a.x + b.x, a.y + b.y, a.z + b.z}; }
+template <typename R> ME_DEV P4<R> psub(const P4<R>& a, const P4<R>& b) { return {a.e - b.e, a.x - b.x, a.y - b.y, a.z - b.z}; }
+template <typename R> ME_DEV P4<R> pneg(const P4<R>& a) { return {-a.e, -a.x, -a.y, -a.z}; }
+ME_DEV double pdot(const P4<double>& a, const P4<double>& b) { return a.e * b.e - a.x * b.x - a.y * b.y - a.z * b.z; }
+template <typename R> ME_DEV P4<R> pcast(const P4<double>& a) { return {(R)a.e, (R)a.x, (R)a.y, (R)a.z}; }
+
+// ------------------------------------------------------------------------------------
+// External gluons (step a3).  eps(p,lam) = (-lam e1 - i e2)/sqrt2 with real e1,e2 that do
+// not depend on the helicity, so the basis is built once per event and a helicity flip is
+// a sign.  pT = 0 branch: e1 = x^, e2 = sgn(pz) y^ (hit by both beams on every event).
+// ------------------------------------------------------------------------------------
+template <typename R> struct GluonBasis { R ax, ay, az, bx, by; };   // a = e1/sqrt2, b = e2/sqrt2
+
+template <typename R> ME_DEV GluonBasis<R> gluon_basis(const P4<R>& p) {
+  const R rs2 = (R)0.70710678118654752440;
+  const R pt2 = p.x * p.x + p.y * p.y;
+  GluonBasis<R> g;
+  if (pt2 == (R)0) {
+    g.ax = rs2; g.ay = 0; g.az = 0; g.bx = 0; g.by = p.z >= (R)0 ? rs2 : -rs2;
+  } else {
+    const R ipt = rsqrt_<R>(pt2), ipabs = rsqrt_<R>(pt2 + p.z * p.z);
+    const R c = p.z * ipabs * ipt * rs2;
+    g.ax = p.x * c; g.ay = p.y * c; g.az = -pt2 * ipt * ipabs * rs2;
+    g.bx = -p.y * ipt * rs2; g.by = p.x * ipt * rs2;
+  }
+  return g;
+}
+// lam = +-1; outgoing gluons carry eps*
+template <typename R> ME_DEV W4<R> gluon_pol(const GluonBasis<R>& g, R lam, bool outgoing) {
+  W4<R> w;
+  const R s = outgoing ? (R)1 : (R)-1;
+  w.r0 = 0; w.i0 = 0;
+  w.r1 = -lam * g.ax; w.i1 = s * g.bx;
+  w.r2 = -lam * g.ay; w.i2 = s * g.by;
+  w.r3 = -lam * g.az; w.i3 = 0;
+  return w;
+}
+
+// ------------------------------------------------------------------------------------
+// External fermions (step a3).  Two-spinors chi+ = (a, b+ic), chi- = (-b+ic, a) with
+// a = N(|p|+pz), b = N px, c = N py, N = 1/sqrt(2|p|(|p|+pz)); |p|+pz = 0: chi+ = (0,1),
+// chi- = (-1,0).  wp = sqrt(E+|p|), wm = sqrt(E-|p|) = m/wp (exactly 0 for m = 0).
+// ------------------------------------------------------------------------------------
+template <typename R> struct SpinorBasis { R a, b, c, wp, wm; };
+
+template <typename R> ME_DEV SpinorBasis<R> spinor_basis(const P4<R>& p, R m) {
+  SpinorBasis<R> s;
+  const R pt2 = p.x * p.x + p.y * p.y;
+  R pabs;
+  if (m == (R)0) { pabs = p.e; s.wp = sqrt_<R>((R)2 * p.e); s.wm = 0; }
+  else { pabs = sqrt_<R>(pt2 + p.z * p.z); s.wp = sqrt_<R>(p.e + pabs); s.wm = m / s.wp; }
+  const R ppz = p.z >= (R)0 ? pabs + p.z : pt2 / (pabs - p.z);
+  if (ppz == (R)0) { s.a = 0; s.b = 1; s.c = 0; }
+  else { const R N = rsqrt_<R>((R)2 * pabs * ppz); s.a = N * ppz; s.b = N * p.x; s.c = N * p.y; }
+  return s;
+}
+// ubar(p,lam) = u^dagger gamma^0 (row spinor) — outgoing fermion
+template <typename R> ME_DEV W4<R> spinor_ubar(const SpinorBasis<R>& s, R lam) {
+  W4<R> w;
+  if (lam > (R)0) {   // chi+^* = (a, b - ic)
+    w.r0 = s.wp * s.a; w.i0 = 0; w.r1 = s.wp * s.b; w.i1 = -s.wp * s.c;
+    w.r2 = s.wm * s.a; w.i2 = 0; w.r3 = s.wm * s.b; w.i3 = -s.wm * s.c;
+  } else {            // chi-^* = (-b - ic, a)
+    w.r0 = -s.wm * s.b; w.i0 = -s.wm * s.c; w.r1 = s.wm * s.a; w.i1 = 0;
+    w.r2 = -s.wp * s.b; w.i2 = -s.wp * s.c; w.r3 = s.wp * s.a; w.i3 = 0;
+  }
+  return w;
+}
+// v(p,lam) (column spinor) — outgoing antifermion of physical helicity lam
+template <typename R> ME_DEV W4<R> spinor_v(const SpinorBasis<R>& s, R lam) {
+  W4<R> w;
+  if (lam > (R)0) {   // (-wp chi-, wm chi-)
+    w.r0 = s.wp * s.b; w.i0 = -s.wp * s.c; w.r1 = -s.wp * s.a; w.i1 = 0;
+    w.r2 = -s.wm * s.b; w.i2 = s.wm * s.c; w.r3 = s.wm * s.a; w.i3 = 0;
+  } else {            // (wm chi+, -wp chi+)
+    w.r0 = s.wm * s.a; w.i0 = 0; w.r1 = s.wm * s.b; w.i1 = s.wm * s.c;
+    w.r2 = -s.wp * s.a; w.i2 = 0; w.r3 = -s.wp * s.b; w.i3 = -s.wp * s.c;
+  }
+  return w;
+}
+// u(p,lam) (column spinor) — incoming fermion
+template <typename R> ME_DEV W4<R> spinor_u(const SpinorBasis<R>& s, R lam) {
+  W4<R> w;
+  if (lam > (R)0) {   // (wm chi+, wp chi+)
+    w.r0 = s.wm * s.a; w.i0 = 0; w.r1 = s.wm * s.b; w.i1 = s.wm * s.c;
+    w.r2 = s.wp * s.a; w.i2 = 0; w.r3 = s.wp * s.b; w.i3 = s.wp * s.c;
+  } else {            // (wp chi-, wm chi-)
+    w.r0 = -s.wp * s.b; w.i0 = s.wp * s.c; w.r1 = s.wp * s.a; w.i1 = 0;
+    w.r2 = -s.wm * s.b; w.i2 = s.wm * s.c; w.r3 = s.wm * s.a; w.i3 = 0;
+  }
+  return w;
+}
+// psibar = psi^dagger gamma^0: swap the chirality blocks and conjugate
+template <typename R> ME_DEV W4<R> dirac_bar(const W4<R>& s) {
+  return {s.r2, -s.i2, s.r3, -s.i3, s.r0, -s.i0, s.r1, -s.i1};
+}
+
+// ------------------------------------------------------------------------------------
+// Dirac algebra.  V-slash = [[0, S],[Sb, 0]],  S = [[A,-C],[-D,B]],  Sb = [[B,C],[D,A]],
+// A = V0-V3, B = V0+V3, C = V1-iV2, D = V1+iV2.
+// ------------------------------------------------------------------------------------
+#define ME_CMUL_RE(ar, ai, br, bi) ((ar) * (br) - (ai) * (bi))
+#define ME_CMUL_IM(ar, ai, br, bi) ((ar) * (bi) + (ai) * (br))
+
+// row spinor times V-slash (complex V)
+template <typename R> ME_DEV W4<R> row_slash(const W4<R>& r, const W4<R>& V) {
+  const R Ar = V.r0 - V.r3, Ai = V.i0 - V.i3, Br = V.r0 + V.r3, Bi = V.i0 + V.i3;
+  const R Cr = V.r1 + V.i2, Ci = V.i1 - V.r2, Dr = V.r1 - V.i2, Di = V.i1 + V.r2;
+  W4<R> o;
+  o.r2 = ME_CMUL_RE(r.r0, r.i0, Ar, Ai) - ME_CMUL_RE(r.r1, r.i1, Dr, Di);
+  o.i2 = ME_CMUL_IM(r.r0, r.i0, Ar, Ai) - ME_CMUL_IM(r.r1, r.i1, Dr, Di);
+  o.r3 = ME_CMUL_RE(r.r1, r.i1, Br, Bi) - ME_CMUL_RE(r.r0, r.i0, Cr, Ci);
+  o.i3 = ME_CMUL_IM(r.r1, r.i1, Br, Bi) - ME_CMUL_IM(r.r0, r.i0, Cr, Ci);
+  o.r0 = ME_CMUL_RE(r.r2, r.i2, Br, Bi) + ME_CMUL_RE(r.r3, r.i3, Dr, Di);
+  o.i0 = ME_CMUL_IM(r.r2, r.i2, Br, Bi) + ME_CMUL_IM(r.r3, r.i3, Dr, Di);
+  o.r1 = ME_CMUL_RE(r.r2, r.i2, Cr, Ci) + ME_CMUL_RE(r.r3, r.i3, Ar, Ai);
+  o.i1 = ME_CMUL_IM(r.r2, r.i2, Cr, Ci) + ME_CMUL_IM(r.r3, r.i3, Ar, Ai);
+  return o;
+}
+// V-slash (complex V) times column spinor
+template <typename R> ME_DEV W4<R> slash_col(const W4<R>& V, const W4<R>& c) {
+  const R Ar = V.r0 - V.r3, Ai = V.i0 - V.i3, Br = V.r0 + V.r3, Bi = V.i0 + V.i3;
+  const R Cr = V.r1 + V.i2, Ci = V.i1 - V.r2, Dr = V.r1 - V.i2, Di = V.i1 + V.r2;
+  W4<R> o;
+  o.r0 = ME_CMUL_RE(Ar, Ai, c.r2, c.i2) - ME_CMUL_RE(Cr, Ci, c.r3, c.i3);
+  o.i0 = ME_CMUL_IM(Ar, Ai, c.r2, c.i2) - ME_CMUL_IM(Cr, Ci, c.r3, c.i3);
+  o.r1 = ME_CMUL_RE(Br, Bi, c.r3, c.i3) - ME_CMUL_RE(Dr, Di, c.r2, c.i2);
+  o.i1 = ME_CMUL_IM(Br, Bi, c.r3, c.i3) - ME_CMUL_IM(Dr, Di, c.r2, c.i2);
+  o.r2 = ME_CMUL_RE(Br, Bi, c.r0, c.i0) + ME_CMUL_RE(Cr, Ci, c.r1, c.i1);
+  o.i2 = ME_CMUL_IM(Br, Bi, c.r0, c.i0) + ME_CMUL_IM(Cr, Ci, c.r1, c.i1);
+  o.r3 = ME_CMUL_RE(Dr, Di, c.r0, c.i0) + ME_CMUL_RE(Ar, Ai, c.r1, c.i1);
+  o.i3 = ME_CMUL_IM(Dr, Di, c.r0, c.i0) + ME_CMUL_IM(Ar, Ai, c.r1, c.i1);
+  return o;
+}
+// row . column
+template <typename R> ME_DEV Cx<R> row_col(const W4<R>& r, const W4<R>& c) {
+  Cx<R> o;
+  o.re = ME_CMUL_RE(r.r0, r.i0, c.r0, c.i0) + ME_CMUL_RE(r.r1, r.i1, c.r1, c.i1) +
+         ME_CMUL_RE(r.r2, r.i2, c.r2, c.i2) + ME_CMUL_RE(r.r3, r.i3, c.r3, c.i3);
+  o.im = ME_CMUL_IM(r.r0, r.i0, c.r0, c.i0) + ME_CMUL_IM(r.r1, r.i1, c.r1, c.i1) +
+         ME_CMUL_IM(r.r2, r.i2, c.r2, c.i2) + ME_CMUL_IM(r.r3, r.i3, c.r3, c.i3);
+  return o;
+}
+// Minkowski products
+template <typename R> ME_DEV Cx<R> wdot(const W4<R>& a, const W4<R>& b) {
+  Cx<R> o;
+  o.re = ME_CMUL_RE(a.r0, a.i0, b.r0, b.i0) - ME_CMUL_RE(a.r1, a.i1, b.r1, b.i1) -
+         ME_CMUL_RE(a.r2, a.i2, b.r2, b.i2) - ME_CMUL_RE(a.r3, a.i3, b.r3, b.i3);
+  o.im = ME_CMUL_IM(a.r0, a.i0, b.r0, b.i0) - ME_CMUL_IM(a.r1, a.i1, b.r1, b.i1) -
+         ME_CMUL_IM(a.r2, a.i2, b.r2, b.i2) - ME_CMUL_IM(a.r3, a.i3, b.r3, b.i3);
+  return o;
+}
+template <typename R> ME_DEV Cx<R> kdot(const P4<R>& k, const W4<R>& w) {
+  return {k.e * w.r0 - k.x * w.r1 - k.y * w.r2 - k.z * w.r3, k.e * w.i0 - k.x * w.i1 - k.y * w.i2 - k.z * w.i3};
+}
+
+// ------------------------------------------------------------------------------------
+// Off-shell currents (step a4), stripped of i and g_s.
+// ------------------------------------------------------------------------------------
+// Quark line grown from the outgoing t (row spinor): psibar' = psibar V-slash (q-slash + m) * iden,
+// q = fermion-flow momentum of the new propagator, iden = 1/(q^2 - m^2).
+template <typename R> ME_DEV W4<R> quark_step(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden) {
+  const W4<R> r = row_slash(psibar, V);
+  const R A = q.e - q.z, B = q.e + q.z;   // real; C = qx - i qy, D = qx + i qy
+  const R ms = m * iden;
+  W4<R> o;
+  // (r qslash)_2 = r0 A - r1 D ; _3 = -r0 C + r1 B ; _0 = r2 B + r3 D ; _1 = r2 C + r3 A
+  o.r2 = (r.r0 * A - (r.r1 * q.x - r.i1 * q.y)) * iden + ms * r.r2;
+  o.i2 = (r.i0 * A - (r.r1 * q.y + r.i1 * q.x)) * iden + ms * r.i2;
+  o.r3 = (r.r1 * B - (r.r0 * q.x + r.i0 * q.y)) * iden + ms * r.r3;
+  o.i3 = (r.i1 * B - (r.i0 * q.x - r.r0 * q.y)) * iden + ms * r.i3;
+  o.r0 = (r.r2 * B + (r.r3 * q.x - r.i3 * q.y)) * iden + ms * r.r0;
+  o.i0 = (r.i2 * B + (r.r3 * q.y + r.i3 * q.x)) * iden + ms * r.i0;
+  o.r1 = (r.r3 * A + (r.r2 * q.x + r.i2 * q.y)) * iden + ms * r.r1;
+  o.i1 = (r.i3 * A + (r.i2 * q.x - r.r2 * q.y)) * iden + ms * r.i1;
+  return o;
+}
+// Three-gluon vertex current, legs 1,2 with incoming momenta k1,k2, open leg momentum -(k1+k2):
+//   W = [ (W1.W2)(k1-k2) + ((k1+2k2).W1) W2 - ((2k1+k2).W2) W1 ] * ik2 ,  ik2 = 1/(k1+k2)^2
+template <typename R> ME_DEV W4<R> v3_current(const W4<R>& W1, const W4<R>& W2, const P4<R>& k1, const P4<R>& k2, R ik2) {
+  Cx<R> w12 = wdot(W1, W2);
+  const P4<R> ka = {k1.e + (R)2 * k2.e, k1.x + (R)2 * k2.x, k1.y + (R)2 * k2.y, k1.z + (R)2 * k2.z};
+  const P4<R> kb = {(R)2 * k1.e + k2.e, (R)2 * k1.x + k2.x, (R)2 * k1.y + k2.y, (R)2 * k1.z + k2.z};
+  Cx<R> a = kdot(ka, W1), b = kdot(kb, W2);
+  w12.re *= ik2; w12.im *= ik2; a.re *= ik2; a.im *= ik2; b.re *= ik2; b.im *= ik2;
+  const P4<R> d = psub(k1, k2);
+  W4<R> o;
+  o.r0 = w12.re * d.e + ME_CMUL_RE(a.re, a.im, W2.r0, W2.i0) - ME_CMUL_RE(b.re, b.im, W1.r0, W1.i0);
+  o.i0 = w12.im * d.e + ME_CMUL_IM(a.re, a.im, W2.r0, W2.i0) - ME_CMUL_IM(b.re, b.im, W1.r0, W1.i0);
+  o.r1 = w12.re * d.x + ME_CMUL_RE(a.re, a.im, W2.r1, W2.i1) - ME_CMUL_RE(b.re, b.im, W1.r1, W1.i1);
+  o.i1 = w12.im * d.x + ME_CMUL_IM(a.re, a.im, W2.r1, W2.i1) - ME_CMUL_IM(b.re, b.im, W1.r1, W1.i1);
+  o.r2 = w12.re * d.y + ME_CMUL_RE(a.re, a.im, W2.r2, W2.i2) - ME_CMUL_RE(b.re, b.im, W1.r2, W1.i2);
+  o.i2 = w12.im * d.y + ME_CMUL_IM(a.re, a.im, W2.r2, W2.i2) - ME_CMUL_IM(b.re, b.im, W1.r2, W1.i2);
+  o.r3 = w12.re * d.z + ME_CMUL_RE(a.re, a.im, W2.r3, W2.i3) - ME_CMUL_RE(b.re, b.im, W1.r3, W1.i3);
+  o.i3 = w12.im * d.z + ME_CMUL_IM(a.re, a.im, W2.r3, W2.i3) - ME_CMUL_IM(b.re, b.im, W1.r3, W1.i3);
+  return o;
+}
+// Four-gluon vertex: the three kinematic structures share the products W1.W2, W1.W3, W2.W3
+//   s0 = (W1.W3) W2 - (W2.W3) W1     [f^{abe}f^{cde}]
+//   s1 = (W1.W2) W3 - (W2.W3) W1     [f^{ace}f^{bde}]
+//   s2 = (W1.W2) W3 - (W1.W3) W2     [f^{ade}f^{bce}]      each times ik2
+template <typename R> struct V4Dots { Cx<R> w12, w13, w23; };
+template <typename R> ME_DEV V4Dots<R> v4_dots(const W4<R>& W1, const W4<R>& W2, const W4<R>& W3, R ik2) {
+  V4Dots<R> d; d.w12 = wdot(W1, W2); d.w13 = wdot(W1, W3); d.w23 = wdot(W2, W3);
+  d.w12.re *= ik2; d.w12.im *= ik2; d.w13.re *= ik2; d.w13.im *= ik2; d.w23.re *= ik2; d.w23.im *= ik2;
+  return d;
+}
+template <typename R> ME_DEV W4<R> cx_comb(const Cx<R>& a, const W4<R>& X, const Cx<R>& b, const W4<R>& Y) {   // a X - b Y
+  W4<R> o;
+  o.r0 = ME_CMUL_RE(a.re, a.im, X.r0, X.i0) - ME_CMUL_RE(b.re, b.im, Y.r0, Y.i0);
+  o.i0 = ME_CMUL_IM(a.re, a.im, X.r0, X.i0) - ME_CMUL_IM(b.re, b.im, Y.r0, Y.i0);
+  o.r1 = ME_CMUL_RE(a.re, a.im, X.r1, X.i1) - ME_CMUL_RE(b.re, b.im, Y.r1, Y.i1);
+  o.i1 = ME_CMUL_IM(a.re, a.im, X.r1, X.i1) - ME_CMUL_IM(b.re, b.im, Y.r1, Y.i1);
+  o.r2 = ME_CMUL_RE(a.re, a.im, X.r2, X.i2) - ME_CMUL_RE(b.re, b.im, Y.r2, Y.i2);
+  o.i2 = ME_CMUL_IM(a.re, a.im, X.r2, X.i2) - ME_CMUL_IM(b.re, b.im, Y.r2, Y.i2);
+  o.r3 = ME_CMUL_RE(a.re, a.im, X.r3, X.i3) - ME_CMUL_RE(b.re, b.im, Y.r3, Y.i3);
+  o.i3 = ME_CMUL_IM(a.re, a.im, X.r3, X.i3) - ME_CMUL_IM(b.re, b.im, Y.r3, Y.i3);
+  return o;
+}
+template <typename R> ME_DEV W4<R> v4_current(int k, const V4Dots<R>& d, const W4<R>& W1, const W4<R>& W2, const W4<R>& W3) {
+  if (k == 0) return cx_comb(d.w13, W2, d.w23, W1);
+  if (k == 1) return cx_comb(d.w12, W3, d.w23, W1);
+  return cx_comb(d.w12, W3, d.w13, W2);
+}
+// fermion bilinear  J^mu = row gamma^mu col  (contravariant), used to close a gluon tree on the bare line:
+//   row Vslash col = V . J
+template <typename R> ME_DEV W4<R> bilinear(const W4<R>& r, const W4<R>& c) {
+  // gamma^0: blocks [[0,1],[1,0]]; gamma^i: [[0,s^i],[-s^i,0]]
+  // upper-right block couples (r0,r1) with (c2,c3); lower-left couples (r2,r3) with (c0,c1)
+  const R u00r = ME_CMUL_RE(r.r0, r.i0, c.r2, c.i2), u00i = ME_CMUL_IM(r.r0, r.i0, c.r2, c.i2);
+  const R u01r = ME_CMUL_RE(r.r0, r.i0, c.r3, c.i3), u01i = ME_CMUL_IM(r.r0, r.i0, c.r3, c.i3);
+  const R u10r = ME_CMUL_RE(r.r1, r.i1, c.r2, c.i2), u10i = ME_CMUL_IM(r.r1, r.i1, c.r2, c.i2);
+  const R u11r = ME_CMUL_RE(r.r1, r.i1, c.r3, c.i3), u11i = ME_CMUL_IM(r.r1, r.i1, c.r3, c.i3);
+  const R l00r = ME_CMUL_RE(r.r2, r.i2, c.r0, c.i0), l00i = ME_CMUL_IM(r.r2, r.i2, c.r0, c.i0);
+  const R l01r = ME_CMUL_RE(r.r2, r.i2, c.r1, c.i1), l01i = ME_CMUL_IM(r.r2, r.i2, c.r1, c.i1);
+  const R l10r = ME_CMUL_RE(r.r3, r.i3, c.r0, c.i0), l10i = ME_CMUL_IM(r.r3, r.i3, c.r0, c.i0);
+  const R l11r = ME_CMUL_RE(r.r3, r.i3, c.r1, c.i1), l11i = ME_CMUL_IM(r.r3, r.i3, c.r1, c.i1);
+  W4<R> J;
+  // J^0 = u00+u11 + l00+l11
+  J.r0 = u00r + u11r + l00r + l11r; J.i0 = u00i + u11i + l00i + l11i;
+  // J^1: sigma^1 = [[0,1],[1,0]] : (u01+u10) - (l01+l10)
+  J.r1 = u01r + u10r - l01r - l10r; J.i1 = u01i + u10i - l01i - l10i;
+  // J^2: sigma^2 = [[0,-i],[i,0]] : -i u01 + i u10 - (-i l01 + i l10)
+  J.r2 = u01i - u10i - l01i + l10i; J.i2 = -u01r + u10r + l01r - l10r;
+  // J^3: sigma^3 = diag(1,-1): (u00-u11) - (l00-l11)
+  J.r3 = u00r - u11r - l00r + l11r; J.i3 = u00i - u11i - l00i + l11i;
+  return J;
+}
+
+}  // namespace me

@@ -1,0 +1,51 @@
+// kernels.h — internal launch interface between the C-ABI layer (me_api.cu) and the per-process
+// kernels (hand-written epem.cu, generated gen_*.cu).  Not part of the public boundary.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define ME_BLOCK 128   // threads per CTA of the diagram kernels (one event per thread)
+#define ME_PAGE 32     // events per AoSoA page
+
+namespace me {
+
+// arguments common to every per-process launcher
+struct LaunchArgs {
+  const double* mom;          // device AoSoA momenta
+  long n, npad;               // events, events rounded up to a whole page
+  const unsigned char* hels;  // device list of helicity indices to evaluate
+  int nhel;
+  double mt;                  // quark mass (QCD) — unused for e+e-
+  double norm_hel;            // per-helicity normalisation (couplings, colour denominator)
+  double inv_avg;             // 1 / averaging denominator
+  double* me_out;             // [n] or null
+  double* me_hel;             // [ncomb][n] or null
+  double* jamp_out;           // [ncol][2][n] or null (single helicity expected)
+  void* scratch;              // process-specific device scratch (gg->tt~ggg jamp staging)
+  size_t scratch_bytes;
+  cudaStream_t stream;
+};
+
+// static description of a generated process
+struct ProcTable {
+  int nglu, ndiagrams, namplitudes, ncol, color_denom, nkernels;
+  double flops_per_helicity[3];   // by me_precision
+  double fixed_flops;
+  const double* color_num;        // [ncol*ncol] host
+  cudaError_t (*launch)(int precision, const LaunchArgs&);
+  size_t (*scratch_bytes)(int precision, long npad);   // may be null
+};
+
+extern const ProcTable tab_gg_ttx, tab_gg_ttxg, tab_gg_ttxgg, tab_gg_ttxggg;
+
+// e+ e- -> mu+ mu-: couplings passed explicitly
+struct EpemCouplings { double gL, gR, mz, wz; };
+cudaError_t launch_epem(int precision, const LaunchArgs&, const EpemCouplings&);
+extern const double epem_flops_per_helicity;
+
+cudaError_t launch_philox(uint64_t seed, uint64_t first_event, long n, int per_event, double* d_rnd, cudaStream_t s);
+cudaError_t launch_rambo(int nfinal, const double* masses /*host, nfinal*/, double sqrt_s, const double* d_rnd, long n,
+                         double* d_mom, double* d_wt, cudaStream_t s);
+cudaError_t run_fma_peak(int fp64, double* tflops);
+
+}  // namespace me

@@ -1,0 +1,237 @@
+// me_api.cu — the C-ABI boundary declared in include/me.h: context, helicity filtering, dispatch.
+// Host logic only; every arithmetic step of the path runs in the kernels (hel_amp.cuh, epem.cu,
+// gen_*.cu, rng_rambo.cu).  No CPU fallback: without a CUDA device every entry point returns ME_ECUDA.
+#include "../../include/me.h"
+#include "kernels.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+struct me_ctx {
+  me_process process;
+  me_sm_params prm;
+  me_info info;
+  int device;
+  const me::ProcTable* tab;      // null for e+e-
+  me::EpemCouplings epem;
+  double norm_hel, inv_avg;
+  unsigned char* d_hels_all;     // [ncomb] 0..ncomb-1
+  unsigned char* d_hels_good;    // [ngood]
+  int ngood;
+  uint64_t mask[2];
+  bool filtered;
+  void* scratch; size_t scratch_bytes;
+};
+
+static thread_local char g_errbuf[256] = "CUDA error (none recorded)";
+static me_status cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+  return ME_ECUDA;
+}
+#define ME_CUDA(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+extern "C" const char* me_strerror(me_status s) {
+  switch (s) {
+    case ME_OK: return "ok";
+    case ME_EINVAL: return "invalid argument";
+    case ME_EPROCESS: return "unknown process";
+    case ME_ENOTFILTERED: return "helicities not filtered: call me_filter_helicities or me_set_helicities first";
+    case ME_EALIGN: return "device buffer not 16-byte aligned";
+    case ME_ENOMEM: return "out of memory";
+    case ME_ECUDA: return g_errbuf;
+  }
+  return "unknown status";
+}
+
+static const me::ProcTable* table_of(me_process p) {
+  switch (p) {
+    case ME_GG_TTX: return &me::tab_gg_ttx;
+    case ME_GG_TTXG: return &me::tab_gg_ttxg;
+    case ME_GG_TTXGG: return &me::tab_gg_ttxgg;
+    case ME_GG_TTXGGG: return &me::tab_gg_ttxggg;
+    default: return nullptr;
+  }
+}
+
+extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_ctx** out) {
+  if (prm == nullptr || out == nullptr) return ME_EINVAL;
+  if ((int)process < 0 || (int)process > (int)ME_GG_TTXGGG) return ME_EPROCESS;
+  me_ctx* c = new (std::nothrow) me_ctx();
+  if (c == nullptr) return ME_ENOMEM;
+  c->process = process; c->prm = *prm; c->filtered = false; c->ngood = 0; c->mask[0] = c->mask[1] = 0;
+  c->scratch = nullptr; c->scratch_bytes = 0; c->d_hels_all = c->d_hels_good = nullptr;
+  me_info& I = c->info; memset(&I, 0, sizeof(I));
+  I.page = ME_PAGE; I.ninitial = 2;
+  const double PI = 3.14159265358979323846;
+  if (process == ME_EPEM_MUPMUM) {
+    if (!(prm->aewm1 > 0) || !(prm->sw2 > 0 && prm->sw2 < 1) || !(prm->mz > 0)) { delete c; return ME_EINVAL; }
+    c->tab = nullptr;
+    I.npar = 4; I.ndiagrams = 2; I.ncomb = 16; I.ncolor = 1; I.color_denom = 1; I.avg_denom = 4; I.nkernels = 1; I.namplitudes = 2;
+    const double sw = std::sqrt(prm->sw2), cw = std::sqrt(1.0 - prm->sw2);
+    c->epem.gL = (-0.5 + prm->sw2) / (sw * cw); c->epem.gR = prm->sw2 / (sw * cw); c->epem.mz = prm->mz; c->epem.wz = prm->wz;
+    const double e2 = 4.0 * PI / prm->aewm1;
+    c->norm_hel = e2 * e2;
+    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = me::epem_flops_per_helicity; I.flops_per_event_fixed[k] = 60; }
+  } else {
+    if (!(prm->mt > 0) || prm->wt != 0.0 || !(prm->alpha_s > 0)) { delete c; return ME_EINVAL; }
+    const me::ProcTable* t = table_of(process);
+    c->tab = t;
+    const int n = t->nglu;
+    I.npar = n + 2; I.ndiagrams = t->ndiagrams; I.ncomb = 1 << (n + 2); I.ncolor = t->ncol; I.color_denom = t->color_denom;
+    int fact = 1; for (int i = 2; i <= n - 2; ++i) fact *= i;
+    I.avg_denom = 4 * 64 * fact; I.nkernels = t->nkernels; I.namplitudes = t->namplitudes;
+    I.mass[2] = I.mass[3] = prm->mt;
+    const double gs2 = 4.0 * PI * prm->alpha_s;
+    // |M|^2 carries g_s^(2n); the generated colour sum returns half the numerator of J^dagger C J
+    c->norm_hel = std::pow(gs2, n) * 2.0 / t->color_denom;
+    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = t->flops_per_helicity[k]; I.flops_per_event_fixed[k] = t->fixed_flops; }
+  }
+  c->inv_avg = 1.0 / I.avg_denom;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_hels_all, 128);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_hels_good, 128);
+  if (e == cudaSuccess) {
+    unsigned char all[128]; for (int i = 0; i < 128; ++i) all[i] = (unsigned char)i;
+    e = cudaMemcpy(c->d_hels_all, all, 128, cudaMemcpyHostToDevice);
+  }
+  if (e != cudaSuccess) { cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); delete c; return cuda_fail(e, "me_create"); }
+  *out = c;
+  return ME_OK;
+}
+
+extern "C" me_status me_destroy(me_ctx* c) {
+  if (c == nullptr) return ME_EINVAL;
+  cudaDeviceSynchronize();
+  cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); cudaFree(c->scratch);
+  delete c;
+  return ME_OK;
+}
+
+extern "C" me_status me_get_info(const me_ctx* c, me_info* out) {
+  if (c == nullptr || out == nullptr) return ME_EINVAL;
+  *out = c->info;
+  return ME_OK;
+}
+
+extern "C" me_status me_color_matrix(const me_ctx* c, double* out) {
+  if (c == nullptr || out == nullptr) return ME_EINVAL;
+  if (c->tab == nullptr) { out[0] = 1.0; return ME_OK; }
+  memcpy(out, c->tab->color_num, sizeof(double) * c->tab->ncol * c->tab->ncol);
+  return ME_OK;
+}
+
+static me_status run(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, const unsigned char* hels, int nhel,
+                     double* d_me, double* d_me_hel, double* d_jamp, void* stream) {
+  if ((int)prec < 0 || (int)prec > 2) return ME_EINVAL;
+  if (((uintptr_t)d_mom & 15) || ((uintptr_t)d_me & 7) || ((uintptr_t)d_me_hel & 7)) return ME_EALIGN;
+  me::LaunchArgs a;
+  a.mom = d_mom; a.n = n; a.npad = (n + ME_PAGE - 1) / ME_PAGE * ME_PAGE; a.hels = hels; a.nhel = nhel;
+  a.mt = c->prm.mt; a.norm_hel = c->norm_hel; a.inv_avg = c->inv_avg;
+  a.me_out = d_me; a.me_hel = d_me_hel; a.jamp_out = d_jamp; a.stream = (cudaStream_t)stream;
+  a.scratch = nullptr; a.scratch_bytes = 0;
+  if (c->tab != nullptr && c->tab->scratch_bytes != nullptr) {
+    const size_t need = c->tab->scratch_bytes((int)prec, a.npad);
+    if (need > c->scratch_bytes) {
+      ME_CUDA(cudaStreamSynchronize(a.stream), "scratch sync");
+      cudaFree(c->scratch); c->scratch = nullptr; c->scratch_bytes = 0;
+      cudaError_t e = cudaMalloc(&c->scratch, need);
+      if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return ME_ENOMEM; }
+      ME_CUDA(e, "scratch alloc");
+      c->scratch_bytes = need;
+    }
+    a.scratch = c->scratch; a.scratch_bytes = c->scratch_bytes;
+  }
+  cudaError_t e = c->tab != nullptr ? c->tab->launch((int)prec, a) : me::launch_epem((int)prec, a, c->epem);
+  if (e != cudaSuccess) return cuda_fail(e, "kernel launch");
+  return ME_OK;
+}
+
+extern "C" me_status me_set_helicities(me_ctx* c, const uint64_t mask[2]) {
+  if (c == nullptr || mask == nullptr) return ME_EINVAL;
+  unsigned char good[128]; int ng = 0;
+  for (int h = 0; h < c->info.ncomb; ++h) if (mask[h >> 6] >> (h & 63) & 1) good[ng++] = (unsigned char)h;
+  if (ng == 0) return ME_EINVAL;
+  ME_CUDA(cudaMemcpy(c->d_hels_good, good, ng, cudaMemcpyHostToDevice), "me_set_helicities");
+  c->ngood = ng; c->mask[0] = mask[0]; c->mask[1] = c->info.ncomb > 64 ? mask[1] : 0; c->filtered = true;
+  return ME_OK;
+}
+
+extern "C" me_status me_filter_helicities(me_ctx* c, const double* d_mom, int64_t n, uint64_t mask_out[2], int* ngood_out, void* stream) {
+  if (c == nullptr || d_mom == nullptr || mask_out == nullptr || n < 1) return ME_EINVAL;
+  const int nc = c->info.ncomb;
+  double* d_mh = nullptr;
+  cudaError_t e = cudaMalloc(&d_mh, sizeof(double) * (size_t)nc * n);
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return ME_ENOMEM; }
+  ME_CUDA(e, "filter alloc");
+  me_status st = run(c, d_mom, n, ME_FP64, c->d_hels_all, nc, nullptr, d_mh, nullptr, stream);
+  if (st != ME_OK) { cudaFree(d_mh); return st; }
+  std::vector<double> mh((size_t)nc * n);
+  e = cudaMemcpyAsync(mh.data(), d_mh, sizeof(double) * mh.size(), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+  cudaFree(d_mh);
+  if (e != cudaSuccess) return cuda_fail(e, "me_filter_helicities");
+  // reading Q7: good <=> max_evt ME_h / sum_h' ME_h' > 1e-12
+  uint64_t mask[2] = {0, 0};
+  std::vector<double> tot(n, 0.0);
+  for (int h = 0; h < nc; ++h) for (int64_t i = 0; i < n; ++i) tot[i] += mh[(size_t)h * n + i];
+  for (int h = 0; h < nc; ++h) {
+    double mx = 0;
+    for (int64_t i = 0; i < n; ++i) { const double f = mh[(size_t)h * n + i] / tot[i]; if (f > mx) mx = f; }
+    if (mx > 1e-12) mask[h >> 6] |= (uint64_t)1 << (h & 63);
+  }
+  st = me_set_helicities(c, mask);
+  if (st != ME_OK) return st;
+  mask_out[0] = mask[0]; mask_out[1] = mask[1];
+  if (ngood_out != nullptr) *ngood_out = c->ngood;
+  return ME_OK;
+}
+
+extern "C" me_status me_compute(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, double* d_me, void* stream) {
+  if (c == nullptr || n < 0) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  if (d_mom == nullptr || d_me == nullptr) return ME_EINVAL;
+  if (!c->filtered) return ME_ENOTFILTERED;
+  return run(c, d_mom, n, prec, c->d_hels_good, c->ngood, d_me, nullptr, nullptr, stream);
+}
+
+extern "C" me_status me_compute_helicities(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, double* d_me, double* d_me_hel, void* stream) {
+  if (c == nullptr || n < 0) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  if (d_mom == nullptr || d_me_hel == nullptr) return ME_EINVAL;
+  return run(c, d_mom, n, prec, c->d_hels_all, c->info.ncomb, d_me, d_me_hel, nullptr, stream);
+}
+
+extern "C" me_status me_compute_jamps(me_ctx* c, const double* d_mom, int64_t n, int ihel, double* d_jamp, void* stream) {
+  if (c == nullptr || n < 0 || d_mom == nullptr || d_jamp == nullptr) return ME_EINVAL;
+  if (c->tab == nullptr || ihel < 0 || ihel >= c->info.ncomb) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  return run(c, d_mom, n, ME_FP64, c->d_hels_all + ihel, 1, nullptr, nullptr, d_jamp, stream);
+}
+
+extern "C" me_status me_philox_uniform(uint64_t seed, uint64_t first_event, int64_t n, int per_event, double* d_rnd, void* stream) {
+  if (n < 0 || per_event < 1 || (n > 0 && d_rnd == nullptr)) return ME_EINVAL;
+  if ((uintptr_t)d_rnd & 15) return ME_EALIGN;
+  ME_CUDA(me::launch_philox(seed, first_event, n, per_event, d_rnd, (cudaStream_t)stream), "philox");
+  return ME_OK;
+}
+
+extern "C" me_status me_rambo(const me_ctx* c, double sqrt_s, const double* d_rnd, int64_t n, double* d_mom, double* d_wt, void* stream) {
+  if (c == nullptr || n < 0 || !(sqrt_s > 0)) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  if (d_rnd == nullptr || d_mom == nullptr) return ME_EINVAL;
+  if (((uintptr_t)d_rnd & 15) || ((uintptr_t)d_mom & 15)) return ME_EALIGN;
+  const int nf = c->info.npar - 2;
+  double msum = 0; for (int k = 0; k < nf; ++k) msum += c->info.mass[2 + k];
+  if (!(msum < sqrt_s)) return ME_EINVAL;
+  ME_CUDA(me::launch_rambo(nf, c->info.mass + 2, sqrt_s, d_rnd, n, d_mom, d_wt, (cudaStream_t)stream), "rambo");
+  return ME_OK;
+}
+
+extern "C" me_status me_fma_peak(int fp64, double* out) {
+  if (out == nullptr) return ME_EINVAL;
+  ME_CUDA(me::run_fma_peak(fp64, out), "fma peak");
+  return ME_OK;
+}
