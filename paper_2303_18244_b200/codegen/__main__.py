@@ -3,14 +3,17 @@ import json
 import os
 import sys
 
-from . import emit
+from . import emit, emit_blocked
 
 
 def main(outdir):
     os.makedirs(outdir, exist_ok=True)
     summary = {}
     for n, name in ((2, "gg_ttx"), (3, "gg_ttxg"), (4, "gg_ttxgg")):
-        src, info = emit.emit_single_kernel_process(n, name)
+        if n >= 4:
+            src, info = emit_blocked.emit_blocked_process(n, name)
+        else:
+            src, info = emit.emit_single_kernel_process(n, name)
         _write(os.path.join(outdir, "gen_%s.cu" % name), src)
         info.pop("color_num")
         summary[name] = info

@@ -1,0 +1,121 @@
+// color_sum.cu — batched colour sum for the multi-kernel process:
+//     ME_h(evt) = sum_ij conj(J_i) C_ij J_j = Jr^T C Jr + Ji^T C Ji          (C real symmetric)
+// evaluated as a dense contraction over a tile of events: Y = C X with X = [ncol x (2*events)],
+// then the column-wise dot X.Y.  This file holds the plain-FMA version (FP64 or FP32):
+// a CTA owns 32 events (one per lane); each of its 8 warps owns ncol/8 rows of C and keeps their
+// 2*ncol/8 accumulators in registers, so every shared-memory load of X feeds ncol/8 FMAs whose
+// C operand is a warp-uniform (broadcast) load.
+#include "multi.h"
+
+namespace me {
+
+#define CS_NCOL 120
+#define CS_WARPS 8
+#define CS_ROWS (CS_NCOL / CS_WARPS)   // 15
+
+// colour-matrix numerators (exact small integers); 115 KB in FP64, too large for the constant bank
+__device__ double c_color_d[CS_NCOL * CS_NCOL];
+__device__ float c_color_f[CS_NCOL * CS_NCOL];
+
+template <typename RC> __device__ __forceinline__ RC cmat(int i);
+template <> __device__ __forceinline__ double cmat<double>(int i) { return __ldg(&c_color_d[i]); }
+template <> __device__ __forceinline__ float cmat<float>(int i) { return __ldg(&c_color_f[i]); }
+
+// RJ: staging type, RC: arithmetic type of the contraction
+template <typename RJ, typename RC>
+__global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restrict__ gj, long npad, long n, int nh,
+                                                             const unsigned char* __restrict__ hels, int first,
+                                                             double norm_hel, double inv_avg,
+                                                             double* __restrict__ me_out, double* __restrict__ me_hel) {
+  extern __shared__ __align__(16) unsigned char cs_smem[];
+  RC (*sx)[32] = reinterpret_cast<RC (*)[32]>(cs_smem);                 // [2*CS_NCOL][32]
+  RC (*red)[32] = sx + 2 * CS_NCOL;                                     // [CS_WARPS][32]
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const long e = (long)blockIdx.x * 32 + lane;
+  double acc = 0;
+  for (int hc = 0; hc < nh; ++hc) {
+    const RJ* g = gj + (long)hc * (2 * CS_NCOL) * npad + e;
+    __syncthreads();
+    for (int r = w; r < 2 * CS_NCOL; r += CS_WARPS) sx[r][lane] = (RC)g[(long)r * npad];
+    __syncthreads();
+    RC yr[CS_ROWS], yi[CS_ROWS];
+#pragma unroll
+    for (int r = 0; r < CS_ROWS; ++r) { yr[r] = 0; yi[r] = 0; }
+    const int row0 = w * CS_ROWS;
+#pragma unroll 4
+    for (int j = 0; j < CS_NCOL; ++j) {
+      const RC xr = sx[2 * j][lane], xi = sx[2 * j + 1][lane];
+#pragma unroll
+      for (int r = 0; r < CS_ROWS; ++r) {
+        const RC c = cmat<RC>((row0 + r) * CS_NCOL + j);
+        yr[r] += c * xr; yi[r] += c * xi;
+      }
+    }
+    RC part = 0;
+#pragma unroll
+    for (int r = 0; r < CS_ROWS; ++r) part += yr[r] * sx[2 * (row0 + r)][lane] + yi[r] * sx[2 * (row0 + r) + 1][lane];
+    red[w][lane] = part;
+    __syncthreads();
+    if (w == 0) {
+      RC s = 0;
+#pragma unroll
+      for (int k = 0; k < CS_WARPS; ++k) s += red[k][lane];
+      const double meh = (double)s;
+      if (me_hel != nullptr && e < n) me_hel[(long)hels[hc] * n + e] = meh * norm_hel * 0.5;
+      acc += meh;
+    }
+  }
+  if (w == 0 && me_out != nullptr && e < n) {
+    const double v = acc * norm_hel * 0.5 * inv_avg;
+    me_out[e] = first ? v : me_out[e] + v;
+  }
+}
+
+size_t multi_scratch_bytes(int precision, long npad, int ncol) {
+  return (size_t)ME_HEL_CHUNK * ncol * 2 * npad * (precision == 2 ? sizeof(float) : sizeof(double));
+}
+
+static bool g_color_loaded = false;
+
+cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
+                         const double* color_num_host) {
+  if (ncol != CS_NCOL) return cudaErrorInvalidValue;
+  if (!g_color_loaded) {
+    static float cf[CS_NCOL * CS_NCOL];
+    for (int i = 0; i < CS_NCOL * CS_NCOL; ++i) cf[i] = (float)color_num_host[i];
+    cudaError_t e = cudaMemcpyToSymbol(c_color_d, color_num_host, sizeof(double) * CS_NCOL * CS_NCOL);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_color_f, cf, sizeof(float) * CS_NCOL * CS_NCOL);
+    if (e != cudaSuccess) return e;
+    g_color_loaded = true;
+  }
+  const unsigned cgrid = (unsigned)(a.npad / 32);
+  for (int base = 0; base < a.nhel; base += ME_HEL_CHUNK) {
+    const int nh = a.nhel - base < ME_HEL_CHUNK ? a.nhel - base : ME_HEL_CHUNK;
+    MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream};
+    for (int k = 0; k < nparts; ++k) {
+      cudaError_t e = parts[k]->launch(precision, m);
+      if (e != cudaSuccess) return e;
+    }
+    if (a.jamp_out != nullptr && base == 0) {
+      const size_t esz = precision == 2 ? sizeof(float) : sizeof(double);
+      if (esz != sizeof(double)) return cudaErrorInvalidValue;   // jamp hook is FP64 only
+      cudaError_t e = cudaMemcpy2DAsync(a.jamp_out, a.n * sizeof(double), a.scratch, a.npad * sizeof(double), a.n * sizeof(double),
+                                        2 * ncol, cudaMemcpyDeviceToDevice, a.stream);
+      if (e != cudaSuccess) return e;
+    }
+    const int first = base == 0;
+    const size_t smd = sizeof(double) * (2 * CS_NCOL + CS_WARPS) * 32, smf = sizeof(float) * (2 * CS_NCOL + CS_WARPS) * 32;
+    cudaFuncSetAttribute(k_color_sum<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);
+    if (precision == 0)
+      k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+    else if (precision == 1)
+      k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+    else
+      k_color_sum<float, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const float*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+}  // namespace me

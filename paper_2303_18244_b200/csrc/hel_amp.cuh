@@ -284,3 +284,39 @@ template <typename R> ME_DEV W4<R> bilinear(const W4<R>& r, const W4<R>& c) {
 }
 
 }  // namespace me
+
+// ------------------------------------------------------------------------------------
+// Per-thread shared-memory slots (blocked kernels): slot i of this thread lives at
+// sm[i * ME_SM_STRIDE] with sm already offset by threadIdx.x -> conflict-free, static offsets.
+// ------------------------------------------------------------------------------------
+#ifndef ME_SM_STRIDE
+#define ME_SM_STRIDE 128
+#endif
+namespace me {
+template <typename R> ME_DEV W4<R> ldw(const R* sm, int s) {
+  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE],
+          sm[(s + 4) * ME_SM_STRIDE], sm[(s + 5) * ME_SM_STRIDE], sm[(s + 6) * ME_SM_STRIDE], sm[(s + 7) * ME_SM_STRIDE]};
+}
+template <typename R> ME_DEV void stw(R* sm, int s, const W4<R>& w) {
+  sm[(s + 0) * ME_SM_STRIDE] = w.r0; sm[(s + 1) * ME_SM_STRIDE] = w.i0; sm[(s + 2) * ME_SM_STRIDE] = w.r1; sm[(s + 3) * ME_SM_STRIDE] = w.i1;
+  sm[(s + 4) * ME_SM_STRIDE] = w.r2; sm[(s + 5) * ME_SM_STRIDE] = w.i2; sm[(s + 6) * ME_SM_STRIDE] = w.r3; sm[(s + 7) * ME_SM_STRIDE] = w.i3;
+}
+template <typename R> ME_DEV P4<R> ldp(const R* sm, int s) {
+  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE]};
+}
+template <typename R> ME_DEV void stp(R* sm, int s, const P4<R>& p) {
+  sm[(s + 0) * ME_SM_STRIDE] = p.e; sm[(s + 1) * ME_SM_STRIDE] = p.x; sm[(s + 2) * ME_SM_STRIDE] = p.y; sm[(s + 3) * ME_SM_STRIDE] = p.z;
+}
+template <typename R> ME_DEV GluonBasis<R> ldgb(const R* sm, int s) {
+  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE], sm[(s + 4) * ME_SM_STRIDE]};
+}
+template <typename R> ME_DEV void stgb(R* sm, int s, const GluonBasis<R>& g) {
+  sm[(s + 0) * ME_SM_STRIDE] = g.ax; sm[(s + 1) * ME_SM_STRIDE] = g.ay; sm[(s + 2) * ME_SM_STRIDE] = g.az; sm[(s + 3) * ME_SM_STRIDE] = g.bx; sm[(s + 4) * ME_SM_STRIDE] = g.by;
+}
+template <typename R> ME_DEV SpinorBasis<R> ldsb(const R* sm, int s) {
+  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE], sm[(s + 4) * ME_SM_STRIDE]};
+}
+template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) {
+  sm[(s + 0) * ME_SM_STRIDE] = g.a; sm[(s + 1) * ME_SM_STRIDE] = g.b; sm[(s + 2) * ME_SM_STRIDE] = g.c; sm[(s + 3) * ME_SM_STRIDE] = g.wp; sm[(s + 4) * ME_SM_STRIDE] = g.wm;
+}
+}  // namespace me

@@ -1,0 +1,21 @@
+// multi.h — pipeline of the multi-kernel process (g g -> t t~ g g g): diagram kernels write the
+// colour-flow amplitudes of a chunk of helicities into a global staging buffer
+//     gj[hc][ncol][2 (re,im)][npad]      (FP64 in double and mixed mode, FP32 in float mode)
+// and the batched colour-sum kernel (color_sum.cu) contracts them with the colour matrix.
+#pragma once
+#include "kernels.h"
+
+#define ME_HEL_CHUNK 8   // helicities staged per pass
+
+namespace me {
+
+struct MultiArgs {
+  const double* mom; long npad; const unsigned char* hels; int nh; double mt; void* gj; cudaStream_t stream;
+};
+struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); };
+
+cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
+                         const double* color_num_host);
+size_t multi_scratch_bytes(int precision, long npad, int ncol);
+
+}  // namespace me
