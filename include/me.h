@@ -70,8 +70,10 @@ typedef struct {
   int nkernels;               /* diagram kernels one me_compute pass launches per helicity chunk */
   int namplitudes;            /* amplitudes per helicity (a 4-gluon vertex yields three)    */
   double mass[8];             /* external masses in particle order, GeV                      */
-  double flops_per_helicity[3]; /* counted algorithmic real flops per (event, helicity), by me_precision */
+  double flops_per_helicity[3]; /* ALGORITHMIC real flops per (event, helicity), by me_precision: every current,
+                                   amplitude and colour-sum term evaluated exactly once */
   double flops_per_event_fixed[3]; /* helicity-independent flops per event (invariants, bases)   */
+  double flops_executed_per_helicity[3]; /* flops the kernels actually issue (>= algorithmic: recomputation) */
 } me_info;
 
 /* Create a context for `process` on the current CUDA device.  Builds the colour matrix and

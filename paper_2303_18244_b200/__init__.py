@@ -29,7 +29,7 @@ class me_info(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int) for k in ("npar", "ninitial", "ndiagrams", "ncomb", "ncolor", "color_denom", "avg_denom",
                                             "page", "nkernels", "namplitudes")] + \
                [("mass", ctypes.c_double * 8), ("flops_per_helicity", ctypes.c_double * 3),
-                ("flops_per_event_fixed", ctypes.c_double * 3)]
+                ("flops_per_event_fixed", ctypes.c_double * 3), ("flops_executed_per_helicity", ctypes.c_double * 3)]
 
 
 class MEError(RuntimeError):

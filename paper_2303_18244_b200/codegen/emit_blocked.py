@@ -13,7 +13,7 @@ The straight-line emitter of emit.py leaves every current to ptxas, which for g 
 
 Flop counting as in emit.py (routines of hel_amp.cuh as written).
 """
-from .emit import FLOPS, bits, particle_of, colour_sum_lines
+from .emit import FLOPS, bits, particle_of, colour_sum_lines, algorithmic_flops
 from .topology import Topology
 
 
@@ -440,10 +440,13 @@ def emit_blocked_process(n, name, block=128):
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in T.color_num for x in row)))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr};"
-      % (name, n, T.ndiagrams, B.namp, ncol, T.color_denom, float(per_hel), float(per_hel), float(per_hel), float(B.fixed_flops), name, name))
+    algo = algorithmic_flops(T)
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr};"
+      % (name, n, T.ndiagrams, B.namp, ncol, T.color_denom, float(algo), float(algo), float(algo),
+         float(per_hel), float(per_hel), float(per_hel), float(B.fixed_flops), name, name))
     S("}  // namespace me")
-    info = dict(n=n, ndiagrams=T.ndiagrams, namp=B.namp, ncol=ncol, color_denom=T.color_denom, flops_per_helicity=per_hel,
+    info = dict(n=n, ndiagrams=T.ndiagrams, namp=B.namp, ncol=ncol, color_denom=T.color_denom, flops_per_helicity=algo,
+                flops_executed_per_helicity=per_hel,
                 fixed_flops=B.fixed_flops, colour_flops=cs_flops, smem_slots=B.nslots, block=block,
                 persistent_g=len(B.persist_g), persistent_q=len(B.persist_q), color_num=T.color_num)
     return "\n".join(src) + "\n", info

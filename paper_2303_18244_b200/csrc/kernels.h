@@ -29,7 +29,8 @@ struct LaunchArgs {
 // static description of a generated process
 struct ProcTable {
   int nglu, ndiagrams, namplitudes, ncol, color_denom, nkernels;
-  double flops_per_helicity[3];   // by me_precision
+  double flops_per_helicity[3];   // algorithmic (single pass), by me_precision
+  double flops_executed[3];       // as emitted (with recomputation)
   double fixed_flops;
   const double* color_num;        // [ncol*ncol] host
   cudaError_t (*launch)(int precision, const LaunchArgs&);

@@ -74,7 +74,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
     c->epem.gL = (-0.5 + prm->sw2) / (sw * cw); c->epem.gR = prm->sw2 / (sw * cw); c->epem.mz = prm->mz; c->epem.wz = prm->wz;
     const double e2 = 4.0 * PI / prm->aewm1;
     c->norm_hel = e2 * e2;
-    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = me::epem_flops_per_helicity; I.flops_per_event_fixed[k] = 60; }
+    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = I.flops_executed_per_helicity[k] = me::epem_flops_per_helicity; I.flops_per_event_fixed[k] = 60; }
   } else {
     if (!(prm->mt > 0) || prm->wt != 0.0 || !(prm->alpha_s > 0)) { delete c; return ME_EINVAL; }
     const me::ProcTable* t = table_of(process);
@@ -87,7 +87,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
     const double gs2 = 4.0 * PI * prm->alpha_s;
     // |M|^2 carries g_s^(2n); the generated colour sum returns half the numerator of J^dagger C J
     c->norm_hel = std::pow(gs2, n) * 2.0 / t->color_denom;
-    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = t->flops_per_helicity[k]; I.flops_per_event_fixed[k] = t->fixed_flops; }
+    for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = t->flops_per_helicity[k]; I.flops_executed_per_helicity[k] = t->flops_executed[k]; I.flops_per_event_fixed[k] = t->fixed_flops; }
   }
   c->inv_avg = 1.0 / I.avg_denom;
   cudaError_t e = cudaGetDevice(&c->device);

@@ -1,0 +1,182 @@
+"""CPU-side checks (-m "not gpu"): the C-ABI library builds, loads and exports every symbol that
+include/me.h declares; the header is plain C; the generator's exact colour algebra and diagram counts
+agree with the oracle's independent numeric ones; host logic (layout transforms, sharding) incl. a
+world_size-2 gloo run.  No compute call is made here (no GPU)."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="session")
+def melib():
+    import __graft_entry__
+    __graft_entry__.build()
+    import paper_2303_18244_b200 as me
+    return me
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "me.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(me_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = declared_functions()
+    for required in ("me_create", "me_filter_helicities", "me_compute", "me_rambo", "me_philox_uniform", "me_destroy"):
+        assert required in names
+
+
+def test_library_exports_every_declared_symbol(melib):
+    lib = ctypes.CDLL(melib.LIB_PATH)
+    for name in declared_functions():
+        assert hasattr(lib, name), "libme_b200.so does not export %s" % name
+    assert set(melib.EXPORTS) == set(declared_functions())
+
+
+def test_header_is_plain_c_and_struct_layout_matches_binding(melib, tmp_path):
+    src = tmp_path / "t.c"
+    src.write_text('#include "me.h"\n#include <stdio.h>\n#include <stddef.h>\n'
+                   'int main(void){printf("%zu %zu %zu %zu\\n", sizeof(me_info), sizeof(me_sm_params), offsetof(me_info, mass), offsetof(me_info, flops_per_helicity));return 0;}\n')
+    exe = tmp_path / "t"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    assert int(out[0]) == ctypes.sizeof(melib.me_info)
+    assert int(out[1]) == ctypes.sizeof(melib.me_sm_params)
+    assert int(out[2]) == melib.me_info.mass.offset
+    assert int(out[3]) == melib.me_info.flops_per_helicity.offset
+
+
+def test_strerror_without_gpu(melib):
+    L = melib.lib()
+    assert L.me_strerror(0) == b"ok"
+    assert b"filter" in L.me_strerror(melib.ME_ENOTFILTERED)
+
+
+def test_null_arguments_are_rejected_without_touching_cuda(melib):
+    L = melib.lib()
+    assert L.me_create(1, None, None) == melib.ME_EINVAL
+    assert L.me_destroy(None) == melib.ME_EINVAL
+    assert L.me_get_info(None, None) == melib.ME_EINVAL
+    assert L.me_compute(None, None, 0, 0, None, None) == melib.ME_EINVAL
+    prm = melib.me_sm_params(**melib.DEFAULT_SM)
+    h = ctypes.c_void_p(0)
+    assert L.me_create(17, ctypes.byref(prm), ctypes.byref(h)) == melib.ME_EPROCESS
+
+
+def test_binding_fails_loudly_without_cuda(melib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    with pytest.raises(RuntimeError):
+        melib.MEContext(melib.ME_GG_TTX)
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2303_18244_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "liboracle" not in text, f
+
+
+# ------------------------------------------------------------------ generator vs oracle (independent colour algebra)
+@pytest.mark.parametrize("n,process,ndiag", [(2, 1, 3), (3, 2, 16), (4, 3, 123), (5, 4, 1240)])
+def test_generator_topology_against_oracle(orc, n, process, ndiag):
+    from paper_2303_18244_b200.codegen.topology import Topology
+    T = Topology(n)
+    assert T.ndiagrams == ndiag
+    info = orc.info(process)
+    assert T.ncol == info["ncol"] and len(T.Cl) == info["n_closures"]
+    # exact Fierz colour matrix (generator) == numeric Gell-Mann colour matrix (oracle)
+    C_gen = np.array(T.color_num, dtype=float) / T.color_denom
+    C_orc = orc.color_matrix(process)
+    assert np.abs(C_gen - C_orc).max() < 1e-10
+    assert T.color_denom == {2: 3, 3: 9, 4: 54, 5: 324}[n]
+    # every jamp coefficient is a unit Gaussian integer
+    for c in T.Cl:
+        for _, coef in c.jamp:
+            assert coef in (1, -1, 1j, -1j)
+
+
+def test_generated_flop_counts_are_recorded(melib):
+    import json
+    s = json.load(open(os.path.join(ROOT, "paper_2303_18244_b200", "csrc", "generated", "gen_summary.json")))
+    assert s["gg_ttxgg"]["ndiagrams"] == 123 and s["gg_ttxggg"]["ndiagrams"] == 1240
+    assert 2e4 < s["gg_ttxgg"]["flops_per_helicity"] < 6e4      # SURVEY §8(d) estimate 27-42 k + colour
+
+
+# ------------------------------------------------------------------ host logic
+def test_aosoa_roundtrip_and_padding():
+    import inputs
+    rng = np.random.default_rng(0)
+    for n in (1, 31, 32, 33, 100):
+        p = rng.normal(size=(n, 6, 4))
+        flat = inputs.aos_to_aosoa(p, 32)
+        assert flat.size == ((n + 31) // 32) * 6 * 4 * 32
+        assert np.array_equal(inputs.aosoa_to_aos(flat, n, 6, 32), p)
+        # element (event e, particle k, component c) sits at page e/32, lane e%32
+        e, k, c = n - 1, 3, 2
+        assert flat[(e // 32) * 6 * 4 * 32 + (k * 4 + c) * 32 + e % 32] == p[e, k, c]
+
+
+def test_shard_ranges_cover_exactly_once():
+    from paper_2303_18244_b200.shard import shard_range
+    for n in (0, 1, 31, 32, 33, 1000, 524288, 65536 + 5):
+        for world in (1, 2, 3, 8):
+            seen = np.zeros(n, dtype=int)
+            for r in range(world):
+                f, c = shard_range(n, r, world)
+                assert f % 32 == 0 or c == 0
+                seen[f:f + c] += 1
+            assert (seen == 1).all()
+
+
+def _gloo_worker(rank, world, port, n, q):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import oracle
+    from paper_2303_18244_b200.shard import shard_range
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    first, cnt = shard_range(n, rank, world)
+    # each rank generates ITS events from the global event index (counter-based Philox) — no exchange
+    p, w = oracle.events(oracle.GG_TTX, cnt, seed=1, first_event=first)
+    me = oracle.me(oracle.GG_TTX, p, nthreads=1)
+    # the only collective: one double per rank for the cross-section estimate
+    s = torch.tensor([float((w * me).sum()), float(cnt)], dtype=torch.float64)
+    dist.all_reduce(s)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, (first, me))
+    if rank == 0:
+        q.put((s.tolist(), gathered))
+    dist.destroy_process_group()
+
+
+def test_two_rank_gloo_sharding_reproduces_single_rank(orc):
+    import torch.multiprocessing as mp
+    n, world, port = 200, 2, 29511 + os.getpid() % 500
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, world, port, n, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    (tot, cnt), gathered = q.get(timeout=120)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    p_all, w_all = orc.events(orc.GG_TTX, n, seed=1)
+    me_all = orc.me(orc.GG_TTX, p_all, nthreads=1)
+    me_sharded = np.concatenate([m for _, m in sorted(gathered, key=lambda t: t[0])])
+    assert cnt == n
+    assert np.array_equal(me_sharded, me_all)            # bit-identical: same events, same arithmetic
+    assert abs(tot / float((w_all * me_all).sum()) - 1) < 1e-13
