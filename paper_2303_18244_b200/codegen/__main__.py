@@ -3,15 +3,15 @@ import json
 import os
 import sys
 
-from . import emit, emit_blocked
+from . import emit, emit_orbit
 
 
 def main(outdir):
     os.makedirs(outdir, exist_ok=True)
     summary = {}
     for n, name in ((2, "gg_ttx"), (3, "gg_ttxg"), (4, "gg_ttxgg")):
-        if n >= 4:
-            src, info = emit_blocked.emit_blocked_process(n, name)
+        if n == 4:
+            src, info = emit_orbit.emit_orbit_process(name)
         else:
             src, info = emit.emit_single_kernel_process(n, name)
         _write(os.path.join(outdir, "gen_%s.cu" % name), src)

@@ -1,0 +1,426 @@
+"""Orbit-looped emitter for g g -> t t~ g g (BASELINE.json config 4, the headline workload).
+
+Why (profiles/r1_ttxgg_fp64_blocked_v2.md): fully unrolled per-helicity code is ~40 k SASS instructions
+(~640 KB); on B200 the kernel then stalls on instruction fetch for half of its cycles.  The 123 diagrams
+fall into a handful of SHAPES that differ only by a relabelling of the four gluons, so each shape is
+emitted ONCE as a loop over its instances; everything that depends on the labels (shared-memory offsets
+of operands, helicity bits, colour-flow indices) comes from a small __constant__ table.  The loop body is
+straight-line register code; the whole helicity body is a few thousand instructions and stays in the
+instruction cache.
+
+Evaluation scheme (same Feynman diagrams, same amplitudes — one complex number per diagram term, 159 in
+total — as emit.py), organised to cut work:
+  * two-sided quark line: row currents grown from the t end (0..2 gluons attached) meet column currents
+    grown from the t~ end (0..1 gluons), so no current with three attached gluons is ever formed;
+  * amplitudes that share their two fermion ends use the bilinear J = row gamma col once and a 4-vector
+    dot per diagram; three-gluon vertices closing on the bare line use the dual current (hel_amp.cuh v3_dual).
+Storage: per-event constants, persistent currents (6 gluon pairs, 4+4 one-gluon quark currents) and the 24
+jamps in per-thread shared-memory slots [slot][thread] (north_star "jamp staging in shared memory").
+"""
+from itertools import permutations
+
+from .emit import FLOPS, colour_sum_lines
+from .topology import _pmul, _pcomm, _pscale, color_matrix
+
+N = 4
+NPAR = 6
+FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
+
+
+def lam_bit(label):
+    p = label if label < 2 else label + 2
+    return NPAR - 1 - p
+
+
+class Layout:
+    def __init__(self):
+        s = 0
+        self.MOM = s; s += 4 * N            # signed gluon momenta (+p incoming, -p outgoing)
+        self.PT = s; s += 4                 # p_t
+        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
+        self.IK2 = {m: s + i for i, m in enumerate(masks2)}; s += len(masks2)
+        masksq = [m for m in range(1, (1 << N) - 1)]
+        self.IQ = {m: s + i for i, m in enumerate(masksq)}; s += len(masksq)
+        self.GB = s; s += 5 * N
+        pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+        self.PAIR = {p: s + 8 * i for i, p in enumerate(pairs)}; s += 8 * len(pairs)
+        self.Q1 = s; s += 8 * N
+        self.CHI = s; s += 8 * N
+        self.J = s; s += 2 * 24
+        self.nslots = s
+
+
+def mask_of(*labels):
+    m = 0
+    for l in labels:
+        m |= 1 << l
+    return m
+
+
+class Inst:
+    """One instance of a block: records parameters; emits lines only when it is the template."""
+
+    def __init__(self, lay, stride):
+        self.lay, self.stride = lay, stride
+        self.params, self.lines, self.flops, self.namp = [], [], 0, 0
+        self.jamp_codes = []
+
+    def P(self, v):
+        self.params.append(int(v))
+        return "tb[%d]" % (len(self.params) - 1)
+
+    def off(self, slot):                       # shared-memory element offset of a slot
+        return self.P(slot * self.stride)
+
+    def L(self, s):
+        self.lines.append(s)
+
+    # ---- operand helpers
+    def leaf(self, name, l):
+        self.L("const W4<R> %s = gluon_pol_s<R>(sm + %s, lam_of<R>(h, %s));" % (name, self.off(self.lay.GB + 5 * l), self.P(lam_bit(l))))
+        self.flops += FL["gluon_pol"]
+
+    def kvec(self, name, labels):
+        terms = ["ldp<R>(sm + %s)" % self.off(self.lay.MOM + 4 * l) for l in labels]
+        expr = terms[0]
+        for t in terms[1:]:
+            expr = "padd(%s, %s)" % (expr, t)
+            self.flops += 4
+        self.L("const P4<R> %s = %s;" % (name, expr))
+
+    def qvec(self, name, labels):
+        expr = "ldp<R>(sm + %d)" % (self.lay.PT * self.stride)
+        for l in labels:
+            expr = "psub(%s, ldp<R>(sm + %s))" % (expr, self.off(self.lay.MOM + 4 * l))
+            self.flops += 4
+        self.L("const P4<R> %s = %s;" % (name, expr))
+
+    def ldw(self, name, slot):
+        self.L("const W4<R> %s = ldw<R>(sm + %s);" % (name, self.off(slot)))
+
+    def stw(self, slot, name):
+        self.L("stw<R>(sm + %s, %s);" % (self.off(slot), name))
+
+    def ik2(self, *labels):
+        return "sm[%s]" % self.off(self.lay.IK2[mask_of(*labels)])
+
+    def iq(self, *labels):
+        return "sm[%s]" % self.off(self.lay.IQ[mask_of(*labels)])
+
+    def jamp(self, amp, col, perm_index):
+        """J_sigma += c * amp for every string of the colour polynomial `col` (insertion order)"""
+        self.namp += 1
+        for st, c in col.items():
+            if c == 0:
+                continue
+            code = {1: 0, -1: 1, 1j: 2, -1j: 3}[complex(c) if not isinstance(c, int) else c]
+            self.jamp_codes.append(code)
+            j = "sm + %s" % self.off(self.lay.J + 2 * perm_index[st])
+            if code == 0:
+                self.L("{ R* j = %s; j[0] += %s.re; j[ME_SM_STRIDE] += %s.im; }" % (j, amp, amp))
+            elif code == 1:
+                self.L("{ R* j = %s; j[0] -= %s.re; j[ME_SM_STRIDE] -= %s.im; }" % (j, amp, amp))
+            elif code == 2:
+                self.L("{ R* j = %s; j[0] -= %s.im; j[ME_SM_STRIDE] += %s.re; }" % (j, amp, amp))
+            else:
+                self.L("{ R* j = %s; j[0] += %s.im; j[ME_SM_STRIDE] -= %s.re; }" % (j, amp, amp))
+            self.flops += FL["jamp_entry"]
+
+
+# colour polynomials (phases folded in, see topology.py): strings are tuples of gluon labels
+def c_leaf(l):
+    return {(l,): 1}
+
+
+def c_v3(x1, x2):
+    return _pscale(_pcomm(x1, x2), -1)
+
+
+def c_v4(k, x1, x2, x3):
+    if k == 0:
+        return _pcomm(_pcomm(x1, x2), x3)
+    if k == 1:
+        return _pcomm(_pcomm(x1, x3), x2)
+    return _pscale(_pcomm(x1, _pcomm(x2, x3)), -1)
+
+
+def c_step(prev, g):          # quark step (either end): phase i*i = -1
+    return _pscale(_pmul(prev, g), -1)
+
+
+def c_close(left, mid, right):  # closing vertex: phase i
+    return _pscale(_pmul(_pmul(left, mid), right), 1j)
+
+
+ONE = {(): 1}
+
+
+def build_groups(stride):
+    lay = Layout()
+    perms = list(permutations(range(N)))
+    pidx = {p: i for i, p in enumerate(perms)}
+    groups = []      # (name, template Inst, [param rows])
+
+    def add_group(name, instances):
+        tmpl = instances[0]
+        for it in instances[1:]:
+            assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
+            assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
+        groups.append((name, tmpl, [it.params for it in instances]))
+
+    labels = list(range(N))
+    cpair = lambda a, b: c_v3(c_leaf(a), c_leaf(b))       # colour of the stored pair(a,b), a<b
+    cq1 = lambda l: c_step(ONE, c_leaf(l))
+    cchi = lambda l: c_step(c_leaf(l), ONE)
+
+    # ---- A1: gluon pairs  V3(eps_a, eps_b)
+    insts = []
+    for (a, b) in lay.PAIR:
+        I = Inst(lay, stride)
+        I.leaf("ea", a); I.leaf("eb", b)
+        I.kvec("ka", [a]); I.kvec("kb", [b])
+        I.L("const W4<R> t = v3_current(ea, eb, ka, kb, %s);" % I.ik2(a, b)); I.flops += FL["v3_current"]
+        I.stw(lay.PAIR[(a, b)], "t")
+        insts.append(I)
+    add_group("pairs", insts)
+    # ---- A2: one-gluon row currents from the t end
+    insts = []
+    for l in labels:
+        I = Inst(lay, stride)
+        I.leaf("el", l); I.qvec("q", [l])
+        I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL["quark_step2"]
+        I.stw(lay.Q1 + 8 * l, "t")
+        insts.append(I)
+    add_group("q1", insts)
+    # ---- A3: one-gluon column currents from the t~ end: chi_w = (qslash+m)/(q^2-m^2) eps_w-slash v, q = p_t - K_{all but w}
+    insts = []
+    for w in labels:
+        rest = [l for l in labels if l != w]
+        I = Inst(lay, stride)
+        I.leaf("ew", w); I.qvec("q", rest)
+        I.L("const W4<R> t = col_step(slash_col(ew, vv), q, mt, %s);" % I.iq(*rest)); I.flops += FL["slash_col"] + FL["col_step"]
+        I.stw(lay.CHI + 8 * w, "t")
+        insts.append(I)
+    add_group("chi1", insts)
+    # ---- B1: three-gluon sub-trees on {a,b,c} (6 terms) closing three ways with the remaining gluon w
+    insts = []
+    for w in labels:
+        a, b, c = [l for l in labels if l != w]
+        I = Inst(lay, stride)
+        I.leaf("ea", a); I.leaf("eb", b); I.leaf("ec", c); I.leaf("ew", w)
+        I.kvec("ka", [a]); I.kvec("kb", [b]); I.kvec("kc", [c]); I.kvec("kw", [w])
+        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc), kabc = padd(kab, kc);"); I.flops += 16
+        I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pac", lay.PAIR[(a, c)]); I.ldw("pbc", lay.PAIR[(b, c)])
+        I.ldw("chiw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
+        I.L("const W4<R> j1 = bilinear(ub, chiw);"); I.L("const W4<R> j2 = bilinear(q1w, vv);"); I.flops += 2 * FL["bilinear"]
+        I.L("const W4<R> dd = v3_dual(ew, jtt, kabc, kw, %s);" % I.ik2(a, b, c, w)); I.flops += FL["v3_dual"]
+        ik3 = I.ik2(a, b, c)
+        I.L("const R ik3 = %s;" % ik3)
+        terms = [("t0", "v3_current(pab, ec, kab, kc, ik3)", c_v3(cpair(a, b), c_leaf(c))),
+                 ("t1", "v3_current(pac, eb, kac, kb, ik3)", c_v3(cpair(a, c), c_leaf(b))),
+                 ("t2", "v3_current(pbc, ea, kbc, ka, ik3)", c_v3(cpair(b, c), c_leaf(a)))]
+        I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL["v4_dots"]
+        for k in range(3):
+            terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
+        for i, (nm, expr, col) in enumerate(terms):
+            I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["v3_current"] if i < 3 else FL["v4_current"]
+            I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2), a3 = wdot(%s, dd);" % (nm, nm, nm)); I.flops += 3 * FL["wdot"]
+            I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)                    # ubar . t-slash . chi_w
+            I.jamp("a2", c_close(cq1(w), col, ONE), pidx)                     # q1(w) . t-slash . v
+            I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)       # V3(t, eps_w) on the bare line
+            I.L("}")
+        insts.append(I)
+    add_group("triples", insts)
+    # ---- B2: the three row currents with gluons {a,b} attached, each closing three ways on {c,d}
+    insts = []
+    for (a, b) in lay.PAIR:
+        c, d = [l for l in labels if l not in (a, b)]
+        I = Inst(lay, stride)
+        I.leaf("ea", a); I.leaf("eb", b); I.leaf("ec", c); I.leaf("ed", d)
+        I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pcd", lay.PAIR[(c, d)])
+        I.ldw("q1a", lay.Q1 + 8 * a); I.ldw("q1b", lay.Q1 + 8 * b)
+        I.ldw("chic", lay.CHI + 8 * c); I.ldw("chid", lay.CHI + 8 * d)
+        I.qvec("q", [a, b])
+        I.L("const R iq2 = %s;" % I.iq(a, b))
+        I.L("const W4<R> xp = slash_col(pcd, vv), xcd = slash_col(ec, chid), xdc = slash_col(ed, chic);"); I.flops += 3 * FL["slash_col"]
+        rows = [("ra", "quark_step2(ub, pab, q, mt, iq2)", c_step(ONE, cpair(a, b))),
+                ("rb", "quark_step2(q1a, eb, q, mt, iq2)", c_step(cq1(a), c_leaf(b))),
+                ("rc", "quark_step2(q1b, ea, q, mt, iq2)", c_step(cq1(b), c_leaf(a)))]
+        for nm, expr, col in rows:
+            I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["quark_step2"]
+            I.L("  const Cx<R> a1 = row_col(%s, xp), a2 = row_col(%s, xcd), a3 = row_col(%s, xdc);" % (nm, nm, nm)); I.flops += 3 * FL["row_col"]
+            I.jamp("a1", c_close(col, cpair(c, d), ONE), pidx)
+            I.jamp("a2", c_close(col, c_leaf(c), cchi(d)), pidx)
+            I.jamp("a3", c_close(col, c_leaf(d), cchi(c)), pidx)
+            I.L("}")
+        insts.append(I)
+    add_group("rows2", insts)
+    # ---- B3: q1(x) . pair(y,z)-slash . chi_w
+    insts = []
+    for x in labels:
+        for w in labels:
+            if w == x:
+                continue
+            y, z = [l for l in labels if l not in (x, w)]
+            I = Inst(lay, stride)
+            I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("pyz", lay.PAIR[(y, z)]); I.ldw("chiw", lay.CHI + 8 * w)
+            I.L("const Cx<R> a1 = row_col(row_slash(q1x, pyz), chiw);"); I.flops += FL["row_slash"] + FL["row_col"]
+            I.jamp("a1", c_close(cq1(x), cpair(y, z), cchi(w)), pidx)
+            insts.append(I)
+    add_group("q1_pair_chi", insts)
+    # ---- B4: V3(pair, pair') on the bare line
+    insts = []
+    for (a, b), (c, d) in (((0, 1), (2, 3)), ((0, 2), (1, 3)), ((0, 3), (1, 2))):
+        I = Inst(lay, stride)
+        I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pcd", lay.PAIR[(c, d)])
+        I.kvec("kab", [a, b]); I.kvec("kcd", [c, d])
+        I.L("const Cx<R> a1 = wdot(v3_current(pab, pcd, kab, kcd, %s), jtt);" % I.ik2(a, b, c, d)); I.flops += FL["v3_current"] + FL["wdot"]
+        I.jamp("a1", c_close(ONE, c_v3(cpair(a, b), cpair(c, d)), ONE), pidx)
+        insts.append(I)
+    add_group("pair_pair", insts)
+    # ---- B5: four-gluon vertex (pair, eps_c, eps_d) on the bare line, three colour structures
+    insts = []
+    for (a, b) in lay.PAIR:
+        c, d = [l for l in labels if l not in (a, b)]
+        I = Inst(lay, stride)
+        I.ldw("pab", lay.PAIR[(a, b)]); I.leaf("ec", c); I.leaf("ed", d)
+        I.L("const V4Dots<R> dots = v4_dots(pab, ec, ed, %s);" % I.ik2(a, b, c, d)); I.flops += FL["v4_dots"]
+        for k in range(3):
+            I.L("{ const Cx<R> a1 = wdot(v4_current(%d, dots, pab, ec, ed), jtt);" % k); I.flops += FL["v4_current"] + FL["wdot"]
+            I.jamp("a1", c_close(ONE, c_v4(k, cpair(a, b), c_leaf(c), c_leaf(d)), ONE), pidx)
+            I.L("}")
+        insts.append(I)
+    add_group("pair_v4", insts)
+    return lay, perms, groups
+
+
+def emit_orbit_process(name="gg_ttxgg", block=128):
+    stride = block
+    lay, perms, groups = build_groups(stride)
+    color_num, color_denom = color_matrix(perms)
+    ncol = len(perms)
+    cs_lines, cs_flops = colour_sum_lines(color_num, ncol, color_denom)
+    namp = sum(t.namp * len(rows) for _, t, rows in groups)
+    flops = sum(t.flops * len(rows) for _, t, rows in groups)
+    per_hel = flops + cs_flops + 2 * FL["spinor"] + FL["bilinear"]
+    sgn = lambda l: 1 if l < 2 else -1
+    part = lambda l: l if l < 2 else l + 2
+    src = []
+    S = src.append
+    S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter) — do not edit.")
+    S("// g g -> t t~ g g: 123 diagrams, %d amplitudes in %d looped shapes, 24 colour flows; %d shared-memory slots per thread." % (namp, len(groups), lay.nslots))
+    S("#define ME_SM_STRIDE %d" % block)
+    S("#include \"hel_amp.cuh\"")
+    S("#include \"kernels.h\"")
+    S("namespace me {")
+    for gname, tmpl, rows in groups:
+        nf = len(tmpl.params)
+        S("__constant__ int tab_%s_%s[%d][%d] = {" % (name, gname, len(rows), nf))
+        for r in rows:
+            S("  {%s}," % ", ".join(str(v) for v in r))
+        S("};")
+    S("template <typename R, typename RC>")
+    S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
+      " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out) {" % (block, name))
+    S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
+    S("  R* sm = reinterpret_cast<R*>(smem_raw) + threadIdx.x;")
+    S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
+    S("  if (e >= npad) return;")
+    S("  const R mt = (R)mt_d;")
+    S("  SpinorBasis<R> sbt, sbtb;")
+    S("  {")
+    S("    const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % NPAR)
+    for k in range(NPAR):
+        S("    const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
+    fixed = 0
+    for i in range(N):
+        for j in range(i + 1, N):
+            S("    const double d%d_%d = pdot(pd%d, pd%d);" % (i, j, part(i), part(j))); fixed += 7
+    for l in range(N):
+        S("    const double dt%d = pdot(pd2, pd%d);" % (l, part(l))); fixed += 7
+
+    def k2expr(m):
+        b = [i for i in range(N) if m >> i & 1]
+        terms = []
+        for i in range(len(b)):
+            for j in range(i + 1, len(b)):
+                terms.append(("+" if sgn(b[i]) * sgn(b[j]) > 0 else "-") + "d%d_%d" % (b[i], b[j]))
+        return "2.0*(" + "".join(terms).lstrip("+") + ")"
+
+    for l in range(N):
+        S("    stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
+    S("    stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
+    for m, slot in lay.IK2.items():
+        S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+    for m, slot in lay.IQ.items():
+        b = [i for i in range(N) if m >> i & 1]
+        lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
+        if len(b) == 1:
+            S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
+        else:
+            S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
+        fixed += 8
+    for l in range(N):
+        S("    { GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GB + 5 * l))
+        fixed += 22
+    S("    sbt = spinor_basis(pcast<R>(pd2), mt);")
+    S("    sbtb = spinor_basis(pcast<R>(pd3), mt);")
+    fixed += 40
+    S("  }")
+    S("  double acc = 0;")
+    S("  for (int ih = 0; ih < nhel; ++ih) {")
+    S("    const int h = hels[ih];")
+    S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
+    S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
+    S("    const W4<R> jtt = bilinear(ub, vv);")
+    S("#pragma unroll")
+    S("    for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * ncol, lay.J))
+    for gname, tmpl, rows in groups:
+        S("    // ---- %s: %d instances" % (gname, len(rows)))
+        S("#pragma unroll 1")
+        S("    for (int it = 0; it < %d; ++it) {" % len(rows))
+        S("      const int* tb = tab_%s_%s[it];" % (name, gname))
+        for l in tmpl.lines:
+            S("      " + l)
+        S("    }")
+    S("    if (jamp_out != nullptr && e < n) {")
+    S("#pragma unroll")
+    S("      for (int s = 0; s < %d; ++s) jamp_out[(long)s * n + e] = (double)sm[(%d + s) * ME_SM_STRIDE];" % (2 * ncol, lay.J))
+    S("    }")
+    S("    RC cr[%d], ci[%d];" % (ncol, ncol))
+    S("#pragma unroll")
+    S("    for (int s = 0; s < %d; ++s) { cr[s] = (RC)sm[(%d + 2 * s) * ME_SM_STRIDE]; ci[s] = (RC)sm[(%d + 2 * s + 1) * ME_SM_STRIDE]; }" % (ncol, lay.J, lay.J))
+    for l in cs_lines:
+        S("    " + l)
+    S("    const double meh = (double)cs;")
+    S("    if (me_hel != nullptr && e < n) me_hel[(long)h * n + e] = meh * norm_hel;")
+    S("    acc += meh;")
+    S("  }")
+    S("  if (me_out != nullptr && e < n) me_out[e] = acc * norm_hel * inv_avg;")
+    S("}")
+    S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
+    S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
+    S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d;" % (lay.nslots, block, lay.nslots, block))
+    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out")
+    S("  if (precision == 0) {")
+    S("    cudaFuncSetAttribute(k_%s<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);" % name)
+    S("    k_%s<double, double><<<grid, %d, smd, a.stream>>>(ME_ARGS);" % (name, block))
+    S("  } else if (precision == 1) {")
+    S("    cudaFuncSetAttribute(k_%s<double, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);" % name)
+    S("    k_%s<double, float><<<grid, %d, smd, a.stream>>>(ME_ARGS);" % (name, block))
+    S("  } else {")
+    S("    cudaFuncSetAttribute(k_%s<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smf);" % name)
+    S("    k_%s<float, float><<<grid, %d, smf, a.stream>>>(ME_ARGS);" % (name, block))
+    S("  }")
+    S("#undef ME_ARGS")
+    S("  return cudaGetLastError();")
+    S("}")
+    S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr};"
+      % (name, N, 123, namp, ncol, color_denom, float(per_hel), float(per_hel), float(per_hel),
+         float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name))
+    S("}  // namespace me")
+    info = dict(n=N, ndiagrams=123, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=per_hel,
+                flops_executed_per_helicity=per_hel, fixed_flops=fixed, colour_flops=cs_flops, smem_slots=lay.nslots, block=block,
+                shapes={g: len(r) for g, _, r in groups}, color_num=color_num)
+    return "\n".join(src) + "\n", info

@@ -320,3 +320,69 @@ template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) {
   sm[(s + 0) * ME_SM_STRIDE] = g.a; sm[(s + 1) * ME_SM_STRIDE] = g.b; sm[(s + 2) * ME_SM_STRIDE] = g.c; sm[(s + 3) * ME_SM_STRIDE] = g.wp; sm[(s + 4) * ME_SM_STRIDE] = g.wm;
 }
 }  // namespace me
+
+// ------------------------------------------------------------------------------------
+// Helpers of the orbit-looped kernels (codegen/emit_orbit.py): operands addressed through a
+// per-instance table of shared-memory offsets, two-sided quark line, dual currents.
+// ------------------------------------------------------------------------------------
+namespace me {
+template <typename R> ME_DEV W4<R> ldw(const R* p) { return ldw<R>(p, 0); }
+template <typename R> ME_DEV void stw(R* p, const W4<R>& w) { stw<R>(p, 0, w); }
+template <typename R> ME_DEV P4<R> ldp(const R* p) { return ldp<R>(p, 0); }
+template <typename R> ME_DEV R lam_of(int h, int bit) { return ((h >> bit) & 1) ? (R)1 : (R)-1; }
+// polarisation from a basis whose b part is pre-signed (+ for outgoing eps*, - for incoming eps)
+template <typename R> ME_DEV W4<R> gluon_pol_s(const R* p, R lam) {
+  const GluonBasis<R> g = ldgb<R>(p, 0);
+  return {(R)0, (R)0, -lam * g.ax, g.bx, -lam * g.ay, g.by, -lam * g.az, (R)0};
+}
+// column current grown from the t~ end: chi' = (q-slash + m) X * iden  (X = V-slash chi already formed)
+template <typename R> ME_DEV W4<R> col_step(const W4<R>& X, const P4<R>& q, R m, R iden) {
+  const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;
+  W4<R> o;
+  // (qslash X)_0 = A X2 - C X3 ; _1 = -D X2 + B X3 ; _2 = B X0 + C X1 ; _3 = D X0 + A X1 ; C = qx - i qy, D = qx + i qy
+  o.r0 = A * X.r2 - (qx * X.r3 + qy * X.i3) + ms * X.r0;
+  o.i0 = A * X.i2 - (qx * X.i3 - qy * X.r3) + ms * X.i0;
+  o.r1 = B * X.r3 - (qx * X.r2 - qy * X.i2) + ms * X.r1;
+  o.i1 = B * X.i3 - (qx * X.i2 + qy * X.r2) + ms * X.i1;
+  o.r2 = B * X.r0 + (qx * X.r1 + qy * X.i1) + ms * X.r2;
+  o.i2 = B * X.i0 + (qx * X.i1 - qy * X.r1) + ms * X.i2;
+  o.r3 = A * X.r1 + (qx * X.r0 - qy * X.i0) + ms * X.r3;
+  o.i3 = A * X.i1 + (qx * X.i0 + qy * X.r0) + ms * X.i3;
+  return o;
+}
+// same arithmetic order for the row current (scale q once, then 4 products per component)
+template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden) {
+  const W4<R> r = row_slash(psibar, V);
+  const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;
+  W4<R> o;
+  o.r2 = r.r0 * A - (r.r1 * qx - r.i1 * qy) + ms * r.r2;
+  o.i2 = r.i0 * A - (r.r1 * qy + r.i1 * qx) + ms * r.i2;
+  o.r3 = r.r1 * B - (r.r0 * qx + r.i0 * qy) + ms * r.r3;
+  o.i3 = r.i1 * B - (r.i0 * qx - r.r0 * qy) + ms * r.i3;
+  o.r0 = r.r2 * B + (r.r3 * qx - r.i3 * qy) + ms * r.r0;
+  o.i0 = r.i2 * B + (r.r3 * qy + r.i3 * qx) + ms * r.i0;
+  o.r1 = r.r3 * A + (r.r2 * qx + r.i2 * qy) + ms * r.r1;
+  o.i1 = r.i3 * A + (r.i2 * qx - r.r2 * qy) + ms * r.i1;
+  return o;
+}
+// dual of the three-gluon vertex:  v3_current(W1, W2, k1, k2, ik2) . J  ==  W1 . v3_dual(W2, J, k1, k2, ik2)
+//   D = [ W2 ((k1-k2).J) + (k1+2k2) (W2.J) - J ((2k1+k2).W2) ] * ik2
+template <typename R> ME_DEV W4<R> v3_dual(const W4<R>& W2, const W4<R>& J, const P4<R>& k1, const P4<R>& k2, R ik2) {
+  const P4<R> d = psub(k1, k2);
+  const P4<R> ka = {(k1.e + (R)2 * k2.e) * ik2, (k1.x + (R)2 * k2.x) * ik2, (k1.y + (R)2 * k2.y) * ik2, (k1.z + (R)2 * k2.z) * ik2};
+  const P4<R> kb = {(R)2 * k1.e + k2.e, (R)2 * k1.x + k2.x, (R)2 * k1.y + k2.y, (R)2 * k1.z + k2.z};
+  Cx<R> c1 = kdot(d, J), c3 = kdot(kb, W2);
+  const Cx<R> c2 = wdot(W2, J);
+  c1.re *= ik2; c1.im *= ik2; c3.re *= ik2; c3.im *= ik2;
+  W4<R> o;
+  o.r0 = ME_CMUL_RE(c1.re, c1.im, W2.r0, W2.i0) + c2.re * ka.e - ME_CMUL_RE(c3.re, c3.im, J.r0, J.i0);
+  o.i0 = ME_CMUL_IM(c1.re, c1.im, W2.r0, W2.i0) + c2.im * ka.e - ME_CMUL_IM(c3.re, c3.im, J.r0, J.i0);
+  o.r1 = ME_CMUL_RE(c1.re, c1.im, W2.r1, W2.i1) + c2.re * ka.x - ME_CMUL_RE(c3.re, c3.im, J.r1, J.i1);
+  o.i1 = ME_CMUL_IM(c1.re, c1.im, W2.r1, W2.i1) + c2.im * ka.x - ME_CMUL_IM(c3.re, c3.im, J.r1, J.i1);
+  o.r2 = ME_CMUL_RE(c1.re, c1.im, W2.r2, W2.i2) + c2.re * ka.y - ME_CMUL_RE(c3.re, c3.im, J.r2, J.i2);
+  o.i2 = ME_CMUL_IM(c1.re, c1.im, W2.r2, W2.i2) + c2.im * ka.y - ME_CMUL_IM(c3.re, c3.im, J.r2, J.i2);
+  o.r3 = ME_CMUL_RE(c1.re, c1.im, W2.r3, W2.i3) + c2.re * ka.z - ME_CMUL_RE(c3.re, c3.im, J.r3, J.i3);
+  o.i3 = ME_CMUL_IM(c1.re, c1.im, W2.r3, W2.i3) + c2.im * ka.z - ME_CMUL_IM(c3.re, c3.im, J.r3, J.i3);
+  return o;
+}
+}  // namespace me
