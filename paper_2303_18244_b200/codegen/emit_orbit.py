@@ -64,6 +64,7 @@ class Inst:
         self.lay, self.stride = lay, stride
         self.params, self.lines, self.flops, self.namp = [], [], 0, 0
         self.jamp_codes = []
+        self.pending = []          # (sigma, code, amp) waiting for flush_jamps()
 
     def P(self, v):
         self.params.append(int(v))
@@ -108,23 +109,29 @@ class Inst:
         return "sm[%s]" % self.off(self.lay.IQ[mask_of(*labels)])
 
     def jamp(self, amp, col, perm_index):
-        """J_sigma += c * amp for every string of the colour polynomial `col` (insertion order)"""
+        """queue J_sigma += c * amp for every string of the colour polynomial `col`"""
         self.namp += 1
         for st, c in col.items():
             if c == 0:
                 continue
             code = {1: 0, -1: 1, 1j: 2, -1j: 3}[complex(c) if not isinstance(c, int) else c]
             self.jamp_codes.append(code)
-            j = "sm + %s" % self.off(self.lay.J + 2 * perm_index[st])
-            if code == 0:
-                self.L("{ R* j = %s; j[0] += %s.re; j[ME_SM_STRIDE] += %s.im; }" % (j, amp, amp))
-            elif code == 1:
-                self.L("{ R* j = %s; j[0] -= %s.re; j[ME_SM_STRIDE] -= %s.im; }" % (j, amp, amp))
-            elif code == 2:
-                self.L("{ R* j = %s; j[0] -= %s.im; j[ME_SM_STRIDE] += %s.re; }" % (j, amp, amp))
-            else:
-                self.L("{ R* j = %s; j[0] += %s.im; j[ME_SM_STRIDE] -= %s.re; }" % (j, amp, amp))
-            self.flops += FL["jamp_entry"]
+            self.pending.append((perm_index[st], code, amp))
+
+    def flush_jamps(self):
+        """one shared-memory read-modify-write per colour flow touched since the last flush: amplitudes that
+        feed the same flow are combined in registers first"""
+        order, by = [], {}
+        for sigma, code, amp in self.pending:
+            if sigma not in by:
+                by[sigma] = []; order.append(sigma)
+            by[sigma].append((code, amp))
+        for sigma in order:
+            re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
+            im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
+            self.L("{ R* j = sm + %s; j[0] = j[0]%s; j[ME_SM_STRIDE] = j[ME_SM_STRIDE]%s; }" % (self.off(self.lay.J + 2 * sigma), re, im))
+            self.flops += 2 * len(by[sigma])
+        self.pending = []
 
 
 # colour polynomials (phases folded in, see topology.py): strings are tuples of gluon labels
@@ -228,6 +235,7 @@ def build_groups(stride):
             I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)                    # ubar . t-slash . chi_w
             I.jamp("a2", c_close(cq1(w), col, ONE), pidx)                     # q1(w) . t-slash . v
             I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)       # V3(t, eps_w) on the bare line
+            I.flush_jamps()
             I.L("}")
         insts.append(I)
     add_group("triples", insts)
@@ -252,6 +260,7 @@ def build_groups(stride):
             I.jamp("a1", c_close(col, cpair(c, d), ONE), pidx)
             I.jamp("a2", c_close(col, c_leaf(c), cchi(d)), pidx)
             I.jamp("a3", c_close(col, c_leaf(d), cchi(c)), pidx)
+            I.flush_jamps()
             I.L("}")
         insts.append(I)
     add_group("rows2", insts)
@@ -266,6 +275,7 @@ def build_groups(stride):
             I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("pyz", lay.PAIR[(y, z)]); I.ldw("chiw", lay.CHI + 8 * w)
             I.L("const Cx<R> a1 = row_col(row_slash(q1x, pyz), chiw);"); I.flops += FL["row_slash"] + FL["row_col"]
             I.jamp("a1", c_close(cq1(x), cpair(y, z), cchi(w)), pidx)
+            I.flush_jamps()
             insts.append(I)
     add_group("q1_pair_chi", insts)
     # ---- B4: V3(pair, pair') on the bare line
@@ -276,6 +286,7 @@ def build_groups(stride):
         I.kvec("kab", [a, b]); I.kvec("kcd", [c, d])
         I.L("const Cx<R> a1 = wdot(v3_current(pab, pcd, kab, kcd, %s), jtt);" % I.ik2(a, b, c, d)); I.flops += FL["v3_current"] + FL["wdot"]
         I.jamp("a1", c_close(ONE, c_v3(cpair(a, b), cpair(c, d)), ONE), pidx)
+        I.flush_jamps()
         insts.append(I)
     add_group("pair_pair", insts)
     # ---- B5: four-gluon vertex (pair, eps_c, eps_d) on the bare line, three colour structures
@@ -286,9 +297,9 @@ def build_groups(stride):
         I.ldw("pab", lay.PAIR[(a, b)]); I.leaf("ec", c); I.leaf("ed", d)
         I.L("const V4Dots<R> dots = v4_dots(pab, ec, ed, %s);" % I.ik2(a, b, c, d)); I.flops += FL["v4_dots"]
         for k in range(3):
-            I.L("{ const Cx<R> a1 = wdot(v4_current(%d, dots, pab, ec, ed), jtt);" % k); I.flops += FL["v4_current"] + FL["wdot"]
-            I.jamp("a1", c_close(ONE, c_v4(k, cpair(a, b), c_leaf(c), c_leaf(d)), ONE), pidx)
-            I.L("}")
+            I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, pab, ec, ed), jtt);" % (k, k)); I.flops += FL["v4_current"] + FL["wdot"]
+            I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(a, b), c_leaf(c), c_leaf(d)), ONE), pidx)
+        I.flush_jamps()
         insts.append(I)
     add_group("pair_v4", insts)
     return lay, perms, groups

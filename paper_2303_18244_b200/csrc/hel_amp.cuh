@@ -138,19 +138,22 @@ template <typename R> ME_DEV W4<R> dirac_bar(const W4<R>& s) {
 #define ME_CMUL_RE(ar, ai, br, bi) ((ar) * (br) - (ai) * (bi))
 #define ME_CMUL_IM(ar, ai, br, bi) ((ar) * (bi) + (ai) * (br))
 
+// All sums of products below are written as FLAT left-to-right chains (no parenthesised partial sums) so
+// that nvcc contracts them into one multiply followed by fused multiply-adds: the FP64 pipe issues one
+// instruction per term instead of a mul + an add (profiles/r1_*: only 38 % of FP64 instructions were DFMA).
 // row spinor times V-slash (complex V)
 template <typename R> ME_DEV W4<R> row_slash(const W4<R>& r, const W4<R>& V) {
   const R Ar = V.r0 - V.r3, Ai = V.i0 - V.i3, Br = V.r0 + V.r3, Bi = V.i0 + V.i3;
   const R Cr = V.r1 + V.i2, Ci = V.i1 - V.r2, Dr = V.r1 - V.i2, Di = V.i1 + V.r2;
   W4<R> o;
-  o.r2 = ME_CMUL_RE(r.r0, r.i0, Ar, Ai) - ME_CMUL_RE(r.r1, r.i1, Dr, Di);
-  o.i2 = ME_CMUL_IM(r.r0, r.i0, Ar, Ai) - ME_CMUL_IM(r.r1, r.i1, Dr, Di);
-  o.r3 = ME_CMUL_RE(r.r1, r.i1, Br, Bi) - ME_CMUL_RE(r.r0, r.i0, Cr, Ci);
-  o.i3 = ME_CMUL_IM(r.r1, r.i1, Br, Bi) - ME_CMUL_IM(r.r0, r.i0, Cr, Ci);
-  o.r0 = ME_CMUL_RE(r.r2, r.i2, Br, Bi) + ME_CMUL_RE(r.r3, r.i3, Dr, Di);
-  o.i0 = ME_CMUL_IM(r.r2, r.i2, Br, Bi) + ME_CMUL_IM(r.r3, r.i3, Dr, Di);
-  o.r1 = ME_CMUL_RE(r.r2, r.i2, Cr, Ci) + ME_CMUL_RE(r.r3, r.i3, Ar, Ai);
-  o.i1 = ME_CMUL_IM(r.r2, r.i2, Cr, Ci) + ME_CMUL_IM(r.r3, r.i3, Ar, Ai);
+  o.r2 = r.r0 * Ar - r.i0 * Ai - r.r1 * Dr + r.i1 * Di;
+  o.i2 = r.r0 * Ai + r.i0 * Ar - r.r1 * Di - r.i1 * Dr;
+  o.r3 = r.r1 * Br - r.i1 * Bi - r.r0 * Cr + r.i0 * Ci;
+  o.i3 = r.r1 * Bi + r.i1 * Br - r.r0 * Ci - r.i0 * Cr;
+  o.r0 = r.r2 * Br - r.i2 * Bi + r.r3 * Dr - r.i3 * Di;
+  o.i0 = r.r2 * Bi + r.i2 * Br + r.r3 * Di + r.i3 * Dr;
+  o.r1 = r.r2 * Cr - r.i2 * Ci + r.r3 * Ar - r.i3 * Ai;
+  o.i1 = r.r2 * Ci + r.i2 * Cr + r.r3 * Ai + r.i3 * Ar;
   return o;
 }
 // V-slash (complex V) times column spinor
@@ -158,32 +161,28 @@ template <typename R> ME_DEV W4<R> slash_col(const W4<R>& V, const W4<R>& c) {
   const R Ar = V.r0 - V.r3, Ai = V.i0 - V.i3, Br = V.r0 + V.r3, Bi = V.i0 + V.i3;
   const R Cr = V.r1 + V.i2, Ci = V.i1 - V.r2, Dr = V.r1 - V.i2, Di = V.i1 + V.r2;
   W4<R> o;
-  o.r0 = ME_CMUL_RE(Ar, Ai, c.r2, c.i2) - ME_CMUL_RE(Cr, Ci, c.r3, c.i3);
-  o.i0 = ME_CMUL_IM(Ar, Ai, c.r2, c.i2) - ME_CMUL_IM(Cr, Ci, c.r3, c.i3);
-  o.r1 = ME_CMUL_RE(Br, Bi, c.r3, c.i3) - ME_CMUL_RE(Dr, Di, c.r2, c.i2);
-  o.i1 = ME_CMUL_IM(Br, Bi, c.r3, c.i3) - ME_CMUL_IM(Dr, Di, c.r2, c.i2);
-  o.r2 = ME_CMUL_RE(Br, Bi, c.r0, c.i0) + ME_CMUL_RE(Cr, Ci, c.r1, c.i1);
-  o.i2 = ME_CMUL_IM(Br, Bi, c.r0, c.i0) + ME_CMUL_IM(Cr, Ci, c.r1, c.i1);
-  o.r3 = ME_CMUL_RE(Dr, Di, c.r0, c.i0) + ME_CMUL_RE(Ar, Ai, c.r1, c.i1);
-  o.i3 = ME_CMUL_IM(Dr, Di, c.r0, c.i0) + ME_CMUL_IM(Ar, Ai, c.r1, c.i1);
+  o.r0 = Ar * c.r2 - Ai * c.i2 - Cr * c.r3 + Ci * c.i3;
+  o.i0 = Ar * c.i2 + Ai * c.r2 - Cr * c.i3 - Ci * c.r3;
+  o.r1 = Br * c.r3 - Bi * c.i3 - Dr * c.r2 + Di * c.i2;
+  o.i1 = Br * c.i3 + Bi * c.r3 - Dr * c.i2 - Di * c.r2;
+  o.r2 = Br * c.r0 - Bi * c.i0 + Cr * c.r1 - Ci * c.i1;
+  o.i2 = Br * c.i0 + Bi * c.r0 + Cr * c.i1 + Ci * c.r1;
+  o.r3 = Dr * c.r0 - Di * c.i0 + Ar * c.r1 - Ai * c.i1;
+  o.i3 = Dr * c.i0 + Di * c.r0 + Ar * c.i1 + Ai * c.r1;
   return o;
 }
 // row . column
 template <typename R> ME_DEV Cx<R> row_col(const W4<R>& r, const W4<R>& c) {
   Cx<R> o;
-  o.re = ME_CMUL_RE(r.r0, r.i0, c.r0, c.i0) + ME_CMUL_RE(r.r1, r.i1, c.r1, c.i1) +
-         ME_CMUL_RE(r.r2, r.i2, c.r2, c.i2) + ME_CMUL_RE(r.r3, r.i3, c.r3, c.i3);
-  o.im = ME_CMUL_IM(r.r0, r.i0, c.r0, c.i0) + ME_CMUL_IM(r.r1, r.i1, c.r1, c.i1) +
-         ME_CMUL_IM(r.r2, r.i2, c.r2, c.i2) + ME_CMUL_IM(r.r3, r.i3, c.r3, c.i3);
+  o.re = r.r0 * c.r0 - r.i0 * c.i0 + r.r1 * c.r1 - r.i1 * c.i1 + r.r2 * c.r2 - r.i2 * c.i2 + r.r3 * c.r3 - r.i3 * c.i3;
+  o.im = r.r0 * c.i0 + r.i0 * c.r0 + r.r1 * c.i1 + r.i1 * c.r1 + r.r2 * c.i2 + r.i2 * c.r2 + r.r3 * c.i3 + r.i3 * c.r3;
   return o;
 }
 // Minkowski products
 template <typename R> ME_DEV Cx<R> wdot(const W4<R>& a, const W4<R>& b) {
   Cx<R> o;
-  o.re = ME_CMUL_RE(a.r0, a.i0, b.r0, b.i0) - ME_CMUL_RE(a.r1, a.i1, b.r1, b.i1) -
-         ME_CMUL_RE(a.r2, a.i2, b.r2, b.i2) - ME_CMUL_RE(a.r3, a.i3, b.r3, b.i3);
-  o.im = ME_CMUL_IM(a.r0, a.i0, b.r0, b.i0) - ME_CMUL_IM(a.r1, a.i1, b.r1, b.i1) -
-         ME_CMUL_IM(a.r2, a.i2, b.r2, b.i2) - ME_CMUL_IM(a.r3, a.i3, b.r3, b.i3);
+  o.re = a.r0 * b.r0 - a.i0 * b.i0 - a.r1 * b.r1 + a.i1 * b.i1 - a.r2 * b.r2 + a.i2 * b.i2 - a.r3 * b.r3 + a.i3 * b.i3;
+  o.im = a.r0 * b.i0 + a.i0 * b.r0 - a.r1 * b.i1 - a.i1 * b.r1 - a.r2 * b.i2 - a.i2 * b.r2 - a.r3 * b.i3 - a.i3 * b.r3;
   return o;
 }
 template <typename R> ME_DEV Cx<R> kdot(const P4<R>& k, const W4<R>& w) {
@@ -195,21 +194,9 @@ template <typename R> ME_DEV Cx<R> kdot(const P4<R>& k, const W4<R>& w) {
 // ------------------------------------------------------------------------------------
 // Quark line grown from the outgoing t (row spinor): psibar' = psibar V-slash (q-slash + m) * iden,
 // q = fermion-flow momentum of the new propagator, iden = 1/(q^2 - m^2).
+template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden);
 template <typename R> ME_DEV W4<R> quark_step(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden) {
-  const W4<R> r = row_slash(psibar, V);
-  const R A = q.e - q.z, B = q.e + q.z;   // real; C = qx - i qy, D = qx + i qy
-  const R ms = m * iden;
-  W4<R> o;
-  // (r qslash)_2 = r0 A - r1 D ; _3 = -r0 C + r1 B ; _0 = r2 B + r3 D ; _1 = r2 C + r3 A
-  o.r2 = (r.r0 * A - (r.r1 * q.x - r.i1 * q.y)) * iden + ms * r.r2;
-  o.i2 = (r.i0 * A - (r.r1 * q.y + r.i1 * q.x)) * iden + ms * r.i2;
-  o.r3 = (r.r1 * B - (r.r0 * q.x + r.i0 * q.y)) * iden + ms * r.r3;
-  o.i3 = (r.i1 * B - (r.i0 * q.x - r.r0 * q.y)) * iden + ms * r.i3;
-  o.r0 = (r.r2 * B + (r.r3 * q.x - r.i3 * q.y)) * iden + ms * r.r0;
-  o.i0 = (r.i2 * B + (r.r3 * q.y + r.i3 * q.x)) * iden + ms * r.i0;
-  o.r1 = (r.r3 * A + (r.r2 * q.x + r.i2 * q.y)) * iden + ms * r.r1;
-  o.i1 = (r.i3 * A + (r.i2 * q.x - r.r2 * q.y)) * iden + ms * r.i1;
-  return o;
+  return quark_step2(psibar, V, q, m, iden);
 }
 // Three-gluon vertex current, legs 1,2 with incoming momenta k1,k2, open leg momentum -(k1+k2):
 //   W = [ (W1.W2)(k1-k2) + ((k1+2k2).W1) W2 - ((2k1+k2).W2) W1 ] * ik2 ,  ik2 = 1/(k1+k2)^2
@@ -221,14 +208,14 @@ template <typename R> ME_DEV W4<R> v3_current(const W4<R>& W1, const W4<R>& W2, 
   w12.re *= ik2; w12.im *= ik2; a.re *= ik2; a.im *= ik2; b.re *= ik2; b.im *= ik2;
   const P4<R> d = psub(k1, k2);
   W4<R> o;
-  o.r0 = w12.re * d.e + ME_CMUL_RE(a.re, a.im, W2.r0, W2.i0) - ME_CMUL_RE(b.re, b.im, W1.r0, W1.i0);
-  o.i0 = w12.im * d.e + ME_CMUL_IM(a.re, a.im, W2.r0, W2.i0) - ME_CMUL_IM(b.re, b.im, W1.r0, W1.i0);
-  o.r1 = w12.re * d.x + ME_CMUL_RE(a.re, a.im, W2.r1, W2.i1) - ME_CMUL_RE(b.re, b.im, W1.r1, W1.i1);
-  o.i1 = w12.im * d.x + ME_CMUL_IM(a.re, a.im, W2.r1, W2.i1) - ME_CMUL_IM(b.re, b.im, W1.r1, W1.i1);
-  o.r2 = w12.re * d.y + ME_CMUL_RE(a.re, a.im, W2.r2, W2.i2) - ME_CMUL_RE(b.re, b.im, W1.r2, W1.i2);
-  o.i2 = w12.im * d.y + ME_CMUL_IM(a.re, a.im, W2.r2, W2.i2) - ME_CMUL_IM(b.re, b.im, W1.r2, W1.i2);
-  o.r3 = w12.re * d.z + ME_CMUL_RE(a.re, a.im, W2.r3, W2.i3) - ME_CMUL_RE(b.re, b.im, W1.r3, W1.i3);
-  o.i3 = w12.im * d.z + ME_CMUL_IM(a.re, a.im, W2.r3, W2.i3) - ME_CMUL_IM(b.re, b.im, W1.r3, W1.i3);
+  o.r0 = w12.re * d.e + a.re * W2.r0 - a.im * W2.i0 - b.re * W1.r0 + b.im * W1.i0;
+  o.i0 = w12.im * d.e + a.re * W2.i0 + a.im * W2.r0 - b.re * W1.i0 - b.im * W1.r0;
+  o.r1 = w12.re * d.x + a.re * W2.r1 - a.im * W2.i1 - b.re * W1.r1 + b.im * W1.i1;
+  o.i1 = w12.im * d.x + a.re * W2.i1 + a.im * W2.r1 - b.re * W1.i1 - b.im * W1.r1;
+  o.r2 = w12.re * d.y + a.re * W2.r2 - a.im * W2.i2 - b.re * W1.r2 + b.im * W1.i2;
+  o.i2 = w12.im * d.y + a.re * W2.i2 + a.im * W2.r2 - b.re * W1.i2 - b.im * W1.r2;
+  o.r3 = w12.re * d.z + a.re * W2.r3 - a.im * W2.i3 - b.re * W1.r3 + b.im * W1.i3;
+  o.i3 = w12.im * d.z + a.re * W2.i3 + a.im * W2.r3 - b.re * W1.i3 - b.im * W1.r3;
   return o;
 }
 // Four-gluon vertex: the three kinematic structures share the products W1.W2, W1.W3, W2.W3
@@ -243,14 +230,14 @@ template <typename R> ME_DEV V4Dots<R> v4_dots(const W4<R>& W1, const W4<R>& W2,
 }
 template <typename R> ME_DEV W4<R> cx_comb(const Cx<R>& a, const W4<R>& X, const Cx<R>& b, const W4<R>& Y) {   // a X - b Y
   W4<R> o;
-  o.r0 = ME_CMUL_RE(a.re, a.im, X.r0, X.i0) - ME_CMUL_RE(b.re, b.im, Y.r0, Y.i0);
-  o.i0 = ME_CMUL_IM(a.re, a.im, X.r0, X.i0) - ME_CMUL_IM(b.re, b.im, Y.r0, Y.i0);
-  o.r1 = ME_CMUL_RE(a.re, a.im, X.r1, X.i1) - ME_CMUL_RE(b.re, b.im, Y.r1, Y.i1);
-  o.i1 = ME_CMUL_IM(a.re, a.im, X.r1, X.i1) - ME_CMUL_IM(b.re, b.im, Y.r1, Y.i1);
-  o.r2 = ME_CMUL_RE(a.re, a.im, X.r2, X.i2) - ME_CMUL_RE(b.re, b.im, Y.r2, Y.i2);
-  o.i2 = ME_CMUL_IM(a.re, a.im, X.r2, X.i2) - ME_CMUL_IM(b.re, b.im, Y.r2, Y.i2);
-  o.r3 = ME_CMUL_RE(a.re, a.im, X.r3, X.i3) - ME_CMUL_RE(b.re, b.im, Y.r3, Y.i3);
-  o.i3 = ME_CMUL_IM(a.re, a.im, X.r3, X.i3) - ME_CMUL_IM(b.re, b.im, Y.r3, Y.i3);
+  o.r0 = a.re * X.r0 - a.im * X.i0 - b.re * Y.r0 + b.im * Y.i0;
+  o.i0 = a.re * X.i0 + a.im * X.r0 - b.re * Y.i0 - b.im * Y.r0;
+  o.r1 = a.re * X.r1 - a.im * X.i1 - b.re * Y.r1 + b.im * Y.i1;
+  o.i1 = a.re * X.i1 + a.im * X.r1 - b.re * Y.i1 - b.im * Y.r1;
+  o.r2 = a.re * X.r2 - a.im * X.i2 - b.re * Y.r2 + b.im * Y.i2;
+  o.i2 = a.re * X.i2 + a.im * X.r2 - b.re * Y.i2 - b.im * Y.r2;
+  o.r3 = a.re * X.r3 - a.im * X.i3 - b.re * Y.r3 + b.im * Y.i3;
+  o.i3 = a.re * X.i3 + a.im * X.r3 - b.re * Y.i3 - b.im * Y.r3;
   return o;
 }
 template <typename R> ME_DEV W4<R> v4_current(int k, const V4Dots<R>& d, const W4<R>& W1, const W4<R>& W2, const W4<R>& W3) {
@@ -340,14 +327,14 @@ template <typename R> ME_DEV W4<R> col_step(const W4<R>& X, const P4<R>& q, R m,
   const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;
   W4<R> o;
   // (qslash X)_0 = A X2 - C X3 ; _1 = -D X2 + B X3 ; _2 = B X0 + C X1 ; _3 = D X0 + A X1 ; C = qx - i qy, D = qx + i qy
-  o.r0 = A * X.r2 - (qx * X.r3 + qy * X.i3) + ms * X.r0;
-  o.i0 = A * X.i2 - (qx * X.i3 - qy * X.r3) + ms * X.i0;
-  o.r1 = B * X.r3 - (qx * X.r2 - qy * X.i2) + ms * X.r1;
-  o.i1 = B * X.i3 - (qx * X.i2 + qy * X.r2) + ms * X.i1;
-  o.r2 = B * X.r0 + (qx * X.r1 + qy * X.i1) + ms * X.r2;
-  o.i2 = B * X.i0 + (qx * X.i1 - qy * X.r1) + ms * X.i2;
-  o.r3 = A * X.r1 + (qx * X.r0 - qy * X.i0) + ms * X.r3;
-  o.i3 = A * X.i1 + (qx * X.i0 + qy * X.r0) + ms * X.i3;
+  o.r0 = A * X.r2 - qx * X.r3 - qy * X.i3 + ms * X.r0;
+  o.i0 = A * X.i2 - qx * X.i3 + qy * X.r3 + ms * X.i0;
+  o.r1 = B * X.r3 - qx * X.r2 + qy * X.i2 + ms * X.r1;
+  o.i1 = B * X.i3 - qx * X.i2 - qy * X.r2 + ms * X.i1;
+  o.r2 = B * X.r0 + qx * X.r1 + qy * X.i1 + ms * X.r2;
+  o.i2 = B * X.i0 + qx * X.i1 - qy * X.r1 + ms * X.i2;
+  o.r3 = A * X.r1 + qx * X.r0 - qy * X.i0 + ms * X.r3;
+  o.i3 = A * X.i1 + qx * X.i0 + qy * X.r0 + ms * X.i3;
   return o;
 }
 // same arithmetic order for the row current (scale q once, then 4 products per component)
@@ -355,14 +342,14 @@ template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>&
   const W4<R> r = row_slash(psibar, V);
   const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;
   W4<R> o;
-  o.r2 = r.r0 * A - (r.r1 * qx - r.i1 * qy) + ms * r.r2;
-  o.i2 = r.i0 * A - (r.r1 * qy + r.i1 * qx) + ms * r.i2;
-  o.r3 = r.r1 * B - (r.r0 * qx + r.i0 * qy) + ms * r.r3;
-  o.i3 = r.i1 * B - (r.i0 * qx - r.r0 * qy) + ms * r.i3;
-  o.r0 = r.r2 * B + (r.r3 * qx - r.i3 * qy) + ms * r.r0;
-  o.i0 = r.i2 * B + (r.r3 * qy + r.i3 * qx) + ms * r.i0;
-  o.r1 = r.r3 * A + (r.r2 * qx + r.i2 * qy) + ms * r.r1;
-  o.i1 = r.i3 * A + (r.i2 * qx - r.r2 * qy) + ms * r.i1;
+  o.r2 = r.r0 * A - r.r1 * qx + r.i1 * qy + ms * r.r2;
+  o.i2 = r.i0 * A - r.r1 * qy - r.i1 * qx + ms * r.i2;
+  o.r3 = r.r1 * B - r.r0 * qx - r.i0 * qy + ms * r.r3;
+  o.i3 = r.i1 * B - r.i0 * qx + r.r0 * qy + ms * r.i3;
+  o.r0 = r.r2 * B + r.r3 * qx - r.i3 * qy + ms * r.r0;
+  o.i0 = r.i2 * B + r.r3 * qy + r.i3 * qx + ms * r.i0;
+  o.r1 = r.r3 * A + r.r2 * qx + r.i2 * qy + ms * r.r1;
+  o.i1 = r.i3 * A + r.i2 * qx - r.r2 * qy + ms * r.i1;
   return o;
 }
 // dual of the three-gluon vertex:  v3_current(W1, W2, k1, k2, ik2) . J  ==  W1 . v3_dual(W2, J, k1, k2, ik2)
@@ -375,14 +362,14 @@ template <typename R> ME_DEV W4<R> v3_dual(const W4<R>& W2, const W4<R>& J, cons
   const Cx<R> c2 = wdot(W2, J);
   c1.re *= ik2; c1.im *= ik2; c3.re *= ik2; c3.im *= ik2;
   W4<R> o;
-  o.r0 = ME_CMUL_RE(c1.re, c1.im, W2.r0, W2.i0) + c2.re * ka.e - ME_CMUL_RE(c3.re, c3.im, J.r0, J.i0);
-  o.i0 = ME_CMUL_IM(c1.re, c1.im, W2.r0, W2.i0) + c2.im * ka.e - ME_CMUL_IM(c3.re, c3.im, J.r0, J.i0);
-  o.r1 = ME_CMUL_RE(c1.re, c1.im, W2.r1, W2.i1) + c2.re * ka.x - ME_CMUL_RE(c3.re, c3.im, J.r1, J.i1);
-  o.i1 = ME_CMUL_IM(c1.re, c1.im, W2.r1, W2.i1) + c2.im * ka.x - ME_CMUL_IM(c3.re, c3.im, J.r1, J.i1);
-  o.r2 = ME_CMUL_RE(c1.re, c1.im, W2.r2, W2.i2) + c2.re * ka.y - ME_CMUL_RE(c3.re, c3.im, J.r2, J.i2);
-  o.i2 = ME_CMUL_IM(c1.re, c1.im, W2.r2, W2.i2) + c2.im * ka.y - ME_CMUL_IM(c3.re, c3.im, J.r2, J.i2);
-  o.r3 = ME_CMUL_RE(c1.re, c1.im, W2.r3, W2.i3) + c2.re * ka.z - ME_CMUL_RE(c3.re, c3.im, J.r3, J.i3);
-  o.i3 = ME_CMUL_IM(c1.re, c1.im, W2.r3, W2.i3) + c2.im * ka.z - ME_CMUL_IM(c3.re, c3.im, J.r3, J.i3);
+  o.r0 = c1.re * W2.r0 - c1.im * W2.i0 + c2.re * ka.e - c3.re * J.r0 + c3.im * J.i0;
+  o.i0 = c1.re * W2.i0 + c1.im * W2.r0 + c2.im * ka.e - c3.re * J.i0 - c3.im * J.r0;
+  o.r1 = c1.re * W2.r1 - c1.im * W2.i1 + c2.re * ka.x - c3.re * J.r1 + c3.im * J.i1;
+  o.i1 = c1.re * W2.i1 + c1.im * W2.r1 + c2.im * ka.x - c3.re * J.i1 - c3.im * J.r1;
+  o.r2 = c1.re * W2.r2 - c1.im * W2.i2 + c2.re * ka.y - c3.re * J.r2 + c3.im * J.i2;
+  o.i2 = c1.re * W2.i2 + c1.im * W2.r2 + c2.im * ka.y - c3.re * J.i2 - c3.im * J.r2;
+  o.r3 = c1.re * W2.r3 - c1.im * W2.i3 + c2.re * ka.z - c3.re * J.r3 + c3.im * J.i3;
+  o.i3 = c1.re * W2.i3 + c1.im * W2.r3 + c2.im * ka.z - c3.re * J.i3 - c3.im * J.r3;
   return o;
 }
 }  // namespace me
