@@ -25,6 +25,8 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 N = 4
 NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
+# partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
+UNROLL = dict(pairs=2, q1=2, chi1=2, triples=1, rows2=1, q1_pair_chi=4, pair_pair=3, pair_v4=2)
 
 
 def lam_bit(label):
@@ -388,7 +390,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * ncol, lay.J))
     for gname, tmpl, rows in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
-        S("#pragma unroll 1")
+        S("#pragma unroll %d" % UNROLL.get(gname, 1))
         S("    for (int it = 0; it < %d; ++it) {" % len(rows))
         S("      const int* tb = tab_%s_%s[it];" % (name, gname))
         for l in tmpl.lines:
