@@ -3,7 +3,7 @@ import json
 import os
 import sys
 
-from . import emit, emit_orbit
+from . import emit, emit_orbit, emit_orbit5
 
 
 def main(outdir):
@@ -17,8 +17,11 @@ def main(outdir):
         _write(os.path.join(outdir, "gen_%s.cu" % name), src)
         info.pop("color_num")
         summary[name] = info
-    if hasattr(emit, "emit_multi_kernel_process"):
-        files, info = emit.emit_multi_kernel_process(5, "gg_ttxggg")
+    if True:
+        files, info = emit_orbit5.emit_orbit5_process("gg_ttxggg")
+        for f in os.listdir(outdir):                      # drop files of an earlier generator version
+            if f.startswith("gen_gg_ttxggg_") and f not in files:
+                os.remove(os.path.join(outdir, f))
         for fn, src in files.items():
             _write(os.path.join(outdir, fn), src)
         info.pop("color_num", None)

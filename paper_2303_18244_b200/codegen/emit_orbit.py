@@ -29,12 +29,14 @@ FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 UNROLL = dict(pairs=2, q1=2, chi1=2, triples=1, rows2=1, q1_pair_chi=4, pair_pair=3, pair_v4=2)
 
 
-def lam_bit(label):
+def lam_bit(label, npar=NPAR):
     p = label if label < 2 else label + 2
-    return NPAR - 1 - p
+    return npar - 1 - p
 
 
 class Layout:
+    npar = NPAR
+
     def __init__(self):
         s = 0
         self.MOM = s; s += 4 * N            # signed gluon momenta (+p incoming, -p outgoing)
@@ -80,7 +82,7 @@ class Inst:
 
     # ---- operand helpers
     def leaf(self, name, l):
-        self.L("const W4<R> %s = gluon_pol_s<R>(sm + %s, lam_of<R>(h, %s));" % (name, self.off(self.lay.GB + 5 * l), self.P(lam_bit(l))))
+        self.L("const W4<R> %s = gluon_pol_s<R>(sm + %s, lam_of<R>(h, %s));" % (name, self.off(self.lay.GB + 5 * l), self.P(lam_bit(l, self.lay.npar))))
         self.flops += FL["gluon_pol"]
 
     def kvec(self, name, labels):

@@ -1,0 +1,574 @@
+"""Orbit-looped emitter for g g -> t t~ g g g (BASELINE.json config 5): 1240 diagrams, 1890 amplitude terms,
+120 colour flows.  Same ideas as emit_orbit.py (shapes looped over gluon relabellings with table-driven
+operands, two-sided quark line, bilinear / dual-current factorisations), plus what the size of the process forces:
+
+  * the diagrams are split across THREE kernels (north_star: "splitting the diagrams across kernels"), each small
+    enough to stay in the instruction cache; every kernel loops over the helicities of the current chunk;
+  * the 120 jamps do not fit on chip: each block instance accumulates the <= 36 colour flows it touches in
+    per-thread shared-memory slots and adds them once into the global staging buffer gj[hel][flow][re/im][event]
+    that the batched colour-sum kernel (csrc/color_sum.cu) contracts with the colour matrix.
+
+Every diagram is cut at the gluon sub-tree that covers the third gluon along the quark line:
+    amp = L . mid-slash . R,   L = row current with <= 2 gluons (from the t end), R = column current with <= 2
+gluons (from the t~ end); (|L|,|mid|,|R|) = (0,5,0) 510, (0,4,1)+(1,4,0) 450, (0,3,2)+(2,3,0) 360, (1,3,1) 120,
+(1,2,2)+(2,2,1) 180, (2,1,2) 270 amplitude terms = 1890.
+"""
+from itertools import permutations
+
+from .emit_orbit import Inst, FL, c_leaf, c_v3, c_v4, c_step, c_close, ONE, mask_of
+from .topology import color_matrix
+
+N = 5
+NPAR = 7
+BLOCK = 96
+FL5 = dict(FL, cx_comb=56)
+
+
+class Layout5:
+    """per-thread shared-memory slots of one kernel (units of R)"""
+    npar = NPAR
+
+    def __init__(self, want_pairs, want_iq_mid, jacc):
+        s = 0
+        self.MOM = s; s += 4 * N
+        self.PT = s; s += 4
+        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
+        self.IK2 = {m: s + i for i, m in enumerate(masks2)}; s += len(masks2)
+        # quark propagators: row side sets of size 1,2 and (for the column currents) size 3,4
+        masksq = [m for m in range(1, (1 << N) - 1) if want_iq_mid or bin(m).count("1") in (1, 4)]
+        self.IQ = {m: s + i for i, m in enumerate(masksq)}; s += len(masksq)
+        self.GB = s; s += 5 * N
+        self.PAIR = {}
+        if want_pairs:
+            pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+            self.PAIR = {p: s + 8 * i for i, p in enumerate(pairs)}; s += 8 * len(pairs)
+        self.Q1 = s; s += 8 * N
+        self.CHI = s; s += 8 * N
+        self.J = s; s += 2 * jacc
+        self.jacc = jacc
+        self.nslots = s
+
+
+class Inst5(Inst):
+    """Block instance whose jamps go to LOCAL accumulators (shared memory) and are flushed to global staging."""
+
+    def __init__(self, lay, stride):
+        super().__init__(lay, stride)
+        self.local = {}              # global colour-flow index -> local accumulator slot
+        self.redundant = 0           # flops that recompute something another block / kernel also computes
+
+    def flush_jamps(self):
+        order, by = [], {}
+        for sigma, code, amp in self.pending:
+            if sigma not in by:
+                by[sigma] = []; order.append(sigma)
+            by[sigma].append((code, amp))
+        for sigma in order:
+            loc = self.local.setdefault(sigma, len(self.local))
+            assert loc < self.lay.jacc, "local jamp accumulators exhausted"
+            re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
+            im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
+            o = (self.lay.J + 2 * loc) * self.stride
+            self.L("sm[%d] = sm[%d]%s; sm[%d] = sm[%d]%s;" % (o, o, re, o + self.stride, o + self.stride, im))
+            self.flops += 2 * len(by[sigma])
+        self.pending = []
+
+    def flush_global(self):
+        """add the local accumulators into gj and clear them.  The add is a fire-and-forget reduction (RED.ADD, no
+        read latency); every address is private to one thread, whose program order fixes the order of the adds, so
+        the result is deterministic run to run."""
+        for sigma, loc in sorted(self.local.items(), key=lambda t: t[1]):
+            o = (self.lay.J + 2 * loc) * self.stride
+            self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
+                   % (self.P(2 * sigma), o, o + self.stride, o, o + self.stride))
+            self.flops += 2
+        self.local = {}
+
+
+def cpair(a, b):
+    return c_v3(c_leaf(a), c_leaf(b))
+
+
+def cq1(l):
+    return c_step(ONE, c_leaf(l))
+
+
+def cchi(l):
+    return c_step(c_leaf(l), ONE)
+
+
+def rest_of(*labels):
+    return [l for l in range(N) if l not in labels]
+
+
+def full_mask():
+    return (1 << N) - 1
+
+
+# ------------------------------------------------------------------------------------------
+# shared code fragments
+# ------------------------------------------------------------------------------------------
+def emit_pair(I, name, a, b, ea, eb, ka, kb):
+    I.L("const W4<R> %s = v3_current(%s, %s, %s, %s, %s);" % (name, ea, eb, ka, kb, I.ik2(a, b)))
+    I.flops += FL5["v3_current"]
+
+
+def emit_rows2(I, a, b, pab, ea, eb):
+    """the three row currents with gluons {a,b} attached (a<b): returns [(name, colour)]"""
+    I.ldw("q1a", I.lay.Q1 + 8 * a); I.ldw("q1b", I.lay.Q1 + 8 * b)
+    I.qvec("qr", [a, b])
+    I.L("const R iqr = %s;" % I.iq(a, b))
+    I.L("const W4<R> ra = quark_step2(ub, %s, qr, mt, iqr), rb = quark_step2(q1a, %s, qr, mt, iqr), rc = quark_step2(q1b, %s, qr, mt, iqr);" % (pab, eb, ea))
+    I.flops += 3 * FL5["quark_step2"]
+    return [("ra", c_step(ONE, cpair(a, b))), ("rb", c_step(cq1(a), c_leaf(b))), ("rc", c_step(cq1(b), c_leaf(a)))]
+
+
+def emit_cols2(I, c, d, pcd, ec, ed, tag=""):
+    """the three column currents with gluons {c,d} attached (c<d), grown from the t~ end"""
+    I.ldw("chc" + tag, I.lay.CHI + 8 * c); I.ldw("chd" + tag, I.lay.CHI + 8 * d)
+    row_side = rest_of(c, d)
+    I.qvec("qc" + tag, row_side)
+    I.L("const R iqc%s = %s;" % (tag, I.iq(*row_side)))
+    I.L("const W4<R> ca%s = col_step(slash_col(%s, vv), qc%s, mt, iqc%s), cb%s = col_step(slash_col(%s, chd%s), qc%s, mt, iqc%s),"
+        " cc%s = col_step(slash_col(%s, chc%s), qc%s, mt, iqc%s);" % (tag, pcd, tag, tag, tag, ec, tag, tag, tag, tag, ed, tag, tag, tag))
+    I.flops += 3 * (FL5["slash_col"] + FL5["col_step"])
+    # colour of a column step: -(gluon)(previous column)
+    return [("ca" + tag, c_step(cpair(c, d), ONE)), ("cb" + tag, c_step(c_leaf(c), cchi(d))), ("cc" + tag, c_step(c_leaf(d), cchi(c)))]
+
+
+def phase_a(lay, stride, add_group, want_pairs):
+    labels = list(range(N))
+    if want_pairs:
+        insts = []
+        for (a, b) in lay.PAIR:
+            I = Inst5(lay, stride)
+            I.leaf("ea", a); I.leaf("eb", b); I.kvec("ka", [a]); I.kvec("kb", [b])
+            emit_pair(I, "t", a, b, "ea", "eb", "ka", "kb")
+            I.stw(lay.PAIR[(a, b)], "t")
+            insts.append(I)
+        add_group("pairs", insts, 2)
+    insts = []
+    for l in labels:
+        I = Inst5(lay, stride)
+        I.leaf("el", l); I.qvec("q", [l])
+        I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL5["quark_step2"]
+        I.stw(lay.Q1 + 8 * l, "t")
+        insts.append(I)
+    add_group("q1", insts, 1)
+    insts = []
+    for w in labels:
+        rest = rest_of(w)
+        I = Inst5(lay, stride)
+        I.leaf("ew", w); I.qvec("q", rest)
+        I.L("const W4<R> t = col_step(slash_col(ew, vv), q, mt, %s);" % I.iq(*rest)); I.flops += FL5["slash_col"] + FL5["col_step"]
+        I.stw(lay.CHI + 8 * w, "t")
+        insts.append(I)
+    add_group("chi1", insts, 1)
+
+
+# ------------------------------------------------------------------------------------------
+# kernel 1: everything that contains a three-gluon sub-tree t on M = {a,b,c}; {x,y} = the other two gluons.
+# The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
+# vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
+# ------------------------------------------------------------------------------------------
+def build_k1(stride, pidx):
+    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36)
+    groups = []
+
+    def add_group(name, insts, unroll=1):
+        tmpl = insts[0]
+        for it in insts[1:]:
+            assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
+            assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
+        groups.append((name, tmpl, [it.params for it in insts], unroll))
+
+    phase_a(lay, stride, add_group, want_pairs=False)
+    insts = []
+    for M in [(a, b, c) for a in range(N) for b in range(a + 1, N) for c in range(b + 1, N)]:
+        a, b, c = M
+        x, y = rest_of(a, b, c)
+        I = Inst5(lay, stride)
+        for nm, l in (("ea", a), ("eb", b), ("ec", c), ("ex", x), ("ey", y)):
+            I.leaf(nm, l)
+        for nm, l in (("ka", a), ("kb", b), ("kc", c), ("kx", x), ("ky", y)):
+            I.kvec(nm, [l])
+        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc), kM = padd(kab, kc), kxy = padd(kx, ky),"
+            " kMx = padd(kM, kx), kMy = padd(kM, ky);"); I.flops += 28
+        emit_pair(I, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(I, "pac", a, c, "ea", "ec", "ka", "kc")
+        emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc"); emit_pair(I, "pxy", x, y, "ex", "ey", "kx", "ky")
+        I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once would do
+        I.L("const R ik3 = %s, ik5 = %s, ik4x = %s, ik4y = %s;" % (I.ik2(a, b, c), I.ik2(*range(N)), I.ik2(a, b, c, x), I.ik2(a, b, c, y)))
+        I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
+        terms = [("t0", "v3_current(pab, ec, kab, kc, ik3)", c_v3(cpair(a, b), c_leaf(c))),
+                 ("t1", "v3_current(pac, eb, kac, kb, ik3)", c_v3(cpair(a, c), c_leaf(b))),
+                 ("t2", "v3_current(pbc, ea, kbc, ka, ik3)", c_v3(cpair(b, c), c_leaf(a)))]
+        for k in range(3):
+            terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
+        for i, (nm, expr, col) in enumerate(terms):
+            I.L("const W4<R> %s = %s;" % (nm, expr)); I.flops += FL5["v3_current"] if i < 3 else FL5["v4_current"]
+        I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("q1y", lay.Q1 + 8 * y); I.ldw("chx", lay.CHI + 8 * x); I.ldw("chy", lay.CHI + 8 * y)
+
+        def dots_with(xname, flops, colour_of_term):
+            """6 amplitudes t_i . X and their jamp updates"""
+            I.L("{ const W4<R> X = %s;" % xname); I.flops += flops
+            I.L("  const Cx<R> a0 = wdot(t0, X), a1 = wdot(t1, X), a2 = wdot(t2, X), a3 = wdot(t3, X), a4 = wdot(t4, X), a5 = wdot(t5, X);")
+            I.flops += 6 * FL5["wdot"]
+            for i, (nm, expr, col) in enumerate(terms):
+                I.jamp("a%d" % i, colour_of_term(col), pidx)
+            I.flush_jamps()
+            I.L("}")
+
+        # quad = V3(t, eps_u) closing three ways with the last gluon w  (u,w) = (x,y) and (y,x)
+        for (u, w, eu, ew, ku, kw, kMu, ik4u, q1w, chw) in ((x, y, "ex", "ey", "kx", "ky", "kMx", "ik4x", "q1y", "chy"),
+                                                             (y, x, "ey", "ex", "ky", "kx", "kMy", "ik4y", "q1x", "chx")):
+            quad = lambda col, u=u: c_v3(col, c_leaf(u))
+            dots_with("v3_dual(%s, bilinear(ub, %s), kM, %s, %s)" % (eu, chw, ku, ik4u), FL5["v3_dual"] + FL5["bilinear"],
+                      lambda col, w=w, quad=quad: c_close(ONE, quad(col), cchi(w)))
+            dots_with("v3_dual(%s, bilinear(%s, vv), kM, %s, %s)" % (eu, q1w, ku, ik4u), FL5["v3_dual"] + FL5["bilinear"],
+                      lambda col, w=w, quad=quad: c_close(cq1(w), quad(col), ONE))
+            dots_with("v3_dual(%s, v3_dual(%s, jtt, %s, %s, ik5), kM, %s, %s)" % (eu, ew, kMu, kw, ku, ik4u), 2 * FL5["v3_dual"],
+                      lambda col, w=w, quad=quad: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
+        # V3(t, pair(x,y)) on the bare line
+        dots_with("v3_dual(pxy, jtt, kM, kxy, ik5)", FL5["v3_dual"], lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
+        # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
+        I.L("const Cx<R> cxj = cxs(wdot(ex, jtt), ik5), cyj = cxs(wdot(ey, jtt), ik5), cxy = cxs(wdot(ex, ey), ik5);"); I.flops += 3 * FL5["wdot"] + 6
+        dots_with("cx_comb(cxj, ey, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(0, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with("cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with("cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
+        # q1(u) . t-slash . chi1(w)
+        dots_with("bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
+        dots_with("bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
+        # ubar . t-slash . chi2(x,y)  and  q2(x,y) . t-slash . v
+        I.L("{")
+        cols = emit_cols2(I, x, y, "pxy", "ex", "ey")
+        I.redundant += 0
+        for nm, ccol in cols:
+            dots_with("bilinear(ub, %s)" % nm, FL5["bilinear"], lambda col, ccol=ccol: c_close(ONE, col, ccol))
+        I.L("}")
+        I.L("{")
+        rows = emit_rows2(I, x, y, "pxy", "ex", "ey")
+        for nm, rcol in rows:
+            dots_with("bilinear(%s, vv)" % nm, FL5["bilinear"], lambda col, rcol=rcol: c_close(rcol, col, ONE))
+        I.L("}")
+        I.flush_global()
+        insts.append(I)
+    add_group("triples", insts, 1)
+    return lay, groups
+
+
+def _grouper(groups):
+    def add_group(name, insts, unroll=1):
+        tmpl = insts[0]
+        for it in insts[1:]:
+            assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
+            assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
+        groups.append((name, tmpl, [it.params for it in insts], unroll))
+    return add_group
+
+
+def spair(p):
+    return tuple(sorted(p))
+
+
+# ------------------------------------------------------------------------------------------
+# kernel 2: amplitudes whose two ends carry (2 | 2), (2 | 1) or (1 | 2) gluons and whose middle is a gluon or a pair
+# ------------------------------------------------------------------------------------------
+def build_k2(stride, pidx):
+    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=12)
+    groups = []
+    add_group = _grouper(groups)
+    phase_a(lay, stride, add_group, want_pairs=True)
+    # ---- rows2 loop: A = {a,b}; the three row currents on A meet (i) eps_m . chi2(B), (ii) pair(P) . chi1(w)
+    insts = []
+    for (a, b) in lay.PAIR:
+        rest = rest_of(a, b)
+        I = Inst5(lay, stride)
+        I.leaf("ea", a); I.leaf("eb", b)
+        I.ldw("pab", lay.PAIR[(a, b)])
+        rows = emit_rows2(I, a, b, "pab", "ea", "eb")
+        for i, m in enumerate(rest):
+            c, d = [l for l in rest if l != m]
+            t = "_%d" % i
+            I.L("{")
+            I.leaf("em", m); I.leaf("ec", c); I.leaf("ed", d)
+            I.ldw("pcd", lay.PAIR[(c, d)])
+            cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
+            I.redundant += 2 * (FL5["slash_col"] + FL5["col_step"])      # each chi2 set is formed for 3 masks A
+            I.L("const W4<R> xa = slash_col(em, ca), xb = slash_col(em, cb), xc = slash_col(em, cc);"); I.flops += 3 * FL5["slash_col"]
+            for (rn, rcol) in rows:
+                I.L("{ const Cx<R> a0 = row_col(%s, xa), a1 = row_col(%s, xb), a2 = row_col(%s, xc);" % (rn, rn, rn)); I.flops += 3 * FL5["row_col"]
+                for k, (cn, ccol) in enumerate(cols):
+                    I.jamp("a%d" % k, c_close(rcol, c_leaf(m), ccol), pidx)
+                I.flush_jamps()
+                I.L("}")
+            # (2,2,1): rows . pair(c,d)-slash . chi1(m)
+            I.ldw("chm", lay.CHI + 8 * m)
+            I.L("const W4<R> xp = slash_col(pcd, chm);"); I.flops += FL5["slash_col"]
+            I.L("{ const Cx<R> a0 = row_col(ra, xp), a1 = row_col(rb, xp), a2 = row_col(rc, xp);"); I.flops += 3 * FL5["row_col"]
+            for k, (rn, rcol) in enumerate(rows):
+                I.jamp("a%d" % k, c_close(rcol, cpair(c, d), cchi(m)), pidx)
+            I.flush_jamps()
+            I.L("}")
+            I.L("}")
+        I.flush_global()
+        insts.append(I)
+    add_group("rows2", insts, 1)
+    # ---- cols2 loop: B = {c,d}; q1(x) . pair(P)-slash . chi2(B)
+    insts = []
+    for (c, d) in lay.PAIR:
+        rest = rest_of(c, d)
+        I = Inst5(lay, stride)
+        I.leaf("ec", c); I.leaf("ed", d)
+        I.ldw("pcd", lay.PAIR[(c, d)])
+        cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
+        for x in rest:
+            p = spair([l for l in rest if l != x])
+            I.L("{")
+            I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("pp", lay.PAIR[p])
+            I.L("const W4<R> r = row_slash(q1x, pp);"); I.flops += FL5["row_slash"]
+            I.L("const Cx<R> a0 = row_col(r, ca), a1 = row_col(r, cb), a2 = row_col(r, cc);"); I.flops += 3 * FL5["row_col"]
+            for k, (cn, ccol) in enumerate(cols):
+                I.jamp("a%d" % k, c_close(cq1(x), cpair(*p), ccol), pidx)
+            I.flush_jamps()
+            I.L("}")
+        I.flush_global()
+        insts.append(I)
+    add_group("cols2", insts, 1)
+    return lay, groups
+
+
+# ------------------------------------------------------------------------------------------
+# kernel 3: four-gluon sub-trees built from pairs (V3(pair,pair), V4(pair,eps,eps)) closing three ways with the last
+# gluon w, and the contact term V4(pair, pair, eps) on the bare line
+# ------------------------------------------------------------------------------------------
+def build_k3(stride, pidx):
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24)
+    groups = []
+    add_group = _grouper(groups)
+    phase_a(lay, stride, add_group, want_pairs=True)
+    insts = []
+    for w in range(N):
+        quad = rest_of(w)
+        I = Inst5(lay, stride)
+        I.leaf("ew", w); I.kvec("kw", [w]); I.kvec("kq", quad)
+        I.ldw("chw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
+        I.L("const R ik4 = %s;" % I.ik2(*quad))
+        I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv), x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
+        I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
+
+        def close3(tname, col):
+            I.L("{ const Cx<R> a1 = wdot(%s, x1), a2 = wdot(%s, x2), a3 = wdot(%s, x3);" % (tname, tname, tname)); I.flops += 3 * FL5["wdot"]
+            I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)
+            I.jamp("a2", c_close(cq1(w), col, ONE), pidx)
+            I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
+            I.flush_jamps()
+            I.L("}")
+
+        a0 = quad[0]
+        for b0 in quad[1:]:
+            p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
+            I.L("{")
+            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.kvec("k1", list(p1)); I.kvec("k2", list(p2))
+            I.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); I.flops += FL5["v3_current"]
+            close3("t", c_v3(cpair(*p1), cpair(*p2)))
+            I.L("}")
+            I.flush_global()
+        for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
+            l1, l2 = [l for l in quad if l not in p]
+            I.L("{")
+            I.ldw("pp", lay.PAIR[p]); I.leaf("e1", l1); I.leaf("e2", l2)
+            I.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); I.flops += FL5["v4_dots"]
+            for k in range(3):
+                I.L("{ const W4<R> t = v4_current(%d, dots, pp, e1, e2);" % k); I.flops += FL5["v4_current"]
+                close3("t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
+                I.L("}")
+            I.L("}")
+            I.flush_global()
+        insts.append(I)
+    add_group("quads", insts, 1)
+    # ---- V4(pair, pair', eps_m) on the bare line
+    insts = []
+    for m in range(N):
+        quad = rest_of(m)
+        a0 = quad[0]
+        for b0 in quad[1:]:
+            p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
+            I = Inst5(lay, stride)
+            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.leaf("em", m)
+            I.L("const V4Dots<R> dots = v4_dots(p1, p2, em, %s);" % I.ik2(*range(N))); I.flops += FL5["v4_dots"]
+            for k in range(3):
+                I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, p1, p2, em), jtt);" % (k, k)); I.flops += FL5["v4_current"] + FL5["wdot"]
+                I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(*p1), cpair(*p2), c_leaf(m)), ONE), pidx)
+            I.flush_jamps()
+            I.flush_global()
+            insts.append(I)
+    add_group("pair_pair_v4", insts, 1)
+    return lay, groups
+
+
+# ------------------------------------------------------------------------------------------
+# source emission
+# ------------------------------------------------------------------------------------------
+def prologue_lines(lay):
+    """per-event, helicity-independent: momenta -> signed gluon momenta, propagator denominators (FP64 from pairwise
+    invariants, then rounded to R), polarisation bases, spinor bases"""
+    sgn = lambda l: 1 if l < 2 else -1
+    part = lambda l: l if l < 2 else l + 2
+    out, fixed = [], 0
+    A = out.append
+    A("const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % NPAR)
+    for k in range(NPAR):
+        A("const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
+    for i in range(N):
+        for j in range(i + 1, N):
+            A("const double d%d_%d = pdot(pd%d, pd%d);" % (i, j, part(i), part(j))); fixed += 7
+    for l in range(N):
+        A("const double dt%d = pdot(pd2, pd%d);" % (l, part(l))); fixed += 7
+
+    def k2expr(m):
+        b = [i for i in range(N) if m >> i & 1]
+        terms = []
+        for i in range(len(b)):
+            for j in range(i + 1, len(b)):
+                terms.append(("+" if sgn(b[i]) * sgn(b[j]) > 0 else "-") + "d%d_%d" % (b[i], b[j]))
+        return "2.0*(" + "".join(terms).lstrip("+") + ")"
+
+    for l in range(N):
+        A("stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
+    A("stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
+    for m, slot in lay.IK2.items():
+        A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+    for m, slot in lay.IQ.items():
+        b = [i for i in range(N) if m >> i & 1]
+        lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
+        if len(b) == 1:
+            A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
+        else:
+            A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
+        fixed += 8
+    for l in range(N):
+        A("{ GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GB + 5 * l))
+        fixed += 22
+    A("sbt = spinor_basis(pcast<R>(pd2), mt);")
+    A("sbtb = spinor_basis(pcast<R>(pd3), mt);")
+    fixed += 40
+    return out, fixed
+
+
+def emit_kernel(name, ki, lay, groups):
+    src = []
+    S = src.append
+    namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
+    S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter, emit_orbit5.py) — do not edit.")
+    S("// g g -> t t~ g g g, diagram kernel %d: %d amplitude terms in %d looped shapes; %d shared-memory slots per thread." % (ki, namp, len(groups), lay.nslots))
+    S("#define ME_SM_STRIDE %d" % BLOCK)
+    S("#include \"hel_amp.cuh\"")
+    S("#include \"kernels.h\"")
+    S("#include \"multi.h\"")
+    S("namespace me {")
+    for gname, tmpl, rows, _ in groups:
+        S("__constant__ int tab_%s_o%d_%s[%d][%d] = {" % (name, ki, gname, len(rows), len(tmpl.params)))
+        for r in rows:
+            S("  {%s}," % ", ".join(str(v) for v in r))
+        S("};")
+    S("template <typename R, typename RJ>")
+    S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
+      " double mt_d, RJ* __restrict__ gjbase) {" % (BLOCK, name, ki))
+    S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
+    S("  R* sm = reinterpret_cast<R*>(smem_raw) + threadIdx.x;")
+    S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
+    S("  if (e >= npad) return;")
+    S("  const R mt = (R)mt_d;")
+    S("  SpinorBasis<R> sbt, sbtb;")
+    S("  {")
+    pro, fixed = prologue_lines(lay)
+    for l in pro:
+        S("    " + l)
+    S("  }")
+    S("#pragma unroll")
+    S("  for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * lay.jacc, lay.J))
+    S("  for (int hc = 0; hc < nh; ++hc) {")
+    S("    const int h = hels[hc];")
+    S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
+    S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
+    S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
+    S("    const W4<R> jtt = bilinear(ub, vv);")
+    for gname, tmpl, rows, unroll in groups:
+        S("    // ---- %s: %d instances" % (gname, len(rows)))
+        S("#pragma unroll %d" % unroll)
+        S("    for (int it = 0; it < %d; ++it) {" % len(rows))
+        S("      const int* tb = tab_%s_o%d_%s[it];" % (name, ki, gname))
+        for l in tmpl.lines:
+            S("      " + l)
+        S("    }")
+    S("  }")
+    S("}")
+    S("static cudaError_t launch_o%d(int precision, const MultiArgs& a) {" % ki)
+    S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (BLOCK, BLOCK))
+    S("  if (precision == 2) {")
+    S("    const size_t smb = sizeof(float) * %d * %d;" % (lay.nslots, BLOCK))
+    S("    cudaFuncSetAttribute(k_%s_o%d<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
+    S("    k_%s_o%d<float, float><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj);" % (name, ki, BLOCK))
+    S("  } else {")
+    S("    const size_t smb = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK))
+    S("    cudaFuncSetAttribute(k_%s_o%d<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
+    S("    k_%s_o%d<double, double><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj);" % (name, ki, BLOCK))
+    S("  }")
+    S("  return cudaGetLastError();")
+    S("}")
+    S("extern const MultiKernel mk_%s_o%d = {launch_o%d};" % (name, ki, ki))
+    S("}  // namespace me")
+    flops = sum(t.flops * len(rows) for _, t, rows, _ in groups)
+    redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
+    return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, fixed=fixed, slots=lay.nslots,
+                                       shapes={g: len(r) for g, _, r, _ in groups})
+
+
+def emit_orbit5_process(name="gg_ttxggg"):
+    perms = list(permutations(range(N)))
+    pidx = {p: i for i, p in enumerate(perms)}
+    color_num, color_denom = color_matrix(perms)
+    ncol = len(perms)
+    files, kinfo = {}, []
+    builders = (build_k1, build_k2, build_k3)
+    for ki, b in enumerate(builders):
+        lay, groups = b(BLOCK, pidx)
+        src, info = emit_kernel(name, ki, lay, groups)
+        files["gen_%s_o%d.cu" % (name, ki)] = src
+        kinfo.append(info)
+    namp = sum(k["amplitudes"] for k in kinfo)
+    assert namp == 1890, namp
+    cs_flops = 2 * (2 * ncol * ncol) + 4 * ncol
+    head = 2 * FL5["spinor"] + FL5["bilinear"]
+    executed = sum(k["flops"] for k in kinfo) + len(kinfo) * head + cs_flops
+    # algorithmic: every current once -> drop the tagged recomputation and the repeated phase A / spinors of kernels 2,3
+    phase_a_repeat = 0
+    for k, b in zip(kinfo, builders):
+        pass
+    lay2, groups2 = build_k2(BLOCK, pidx)
+    pa = {g: t.flops * len(rows) for g, t, rows, _ in groups2 if g in ("pairs", "q1", "chi1")}
+    redundant = sum(k["redundant"] for k in kinfo) + 2 * (pa["q1"] + pa["chi1"]) + pa["pairs"] + 2 * head
+    # the 10 pairs are needed once: kernel 1 recomputes them per block (tagged), kernels 2 and 3 both run the pairs loop
+    algo = executed - redundant
+    fixed = sum(k["fixed"] for k in kinfo)
+    src = []
+    S = src.append
+    S("// GENERATED by paper_2303_18244_b200/codegen (emit_orbit5.py) — do not edit.  g g -> t t~ g g g process table.")
+    S("#include \"kernels.h\"")
+    S("#include \"multi.h\"")
+    S("namespace me {")
+    for ki in range(len(kinfo)):
+        S("extern const MultiKernel mk_%s_o%d;" % (name, ki))
+    S("static const MultiKernel* const parts_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo)))))
+    S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
+    S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) { return launch_multi(precision, a, parts_%s, %d, %d, color_num_%s); }"
+      % (name, name, len(kinfo), ncol, name))
+    S("static size_t scratch_%s(int precision, long npad) { return multi_scratch_bytes(precision, npad, %d); }" % (name, ncol))
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s};"
+      % (name, N, 1240, namp, ncol, color_denom, len(kinfo) + 1, float(algo), float(algo), float(algo),
+         float(executed), float(executed), float(executed), float(fixed), name, name, name))
+    S("}  // namespace me")
+    files["gen_%s_table.cu" % name] = "\n".join(src) + "\n"
+    info = dict(n=N, ndiagrams=1240, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=algo,
+                flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK)
+    return files, info

@@ -316,6 +316,7 @@ namespace me {
 template <typename R> ME_DEV W4<R> ldw(const R* p) { return ldw<R>(p, 0); }
 template <typename R> ME_DEV void stw(R* p, const W4<R>& w) { stw<R>(p, 0, w); }
 template <typename R> ME_DEV P4<R> ldp(const R* p) { return ldp<R>(p, 0); }
+template <typename R> ME_DEV Cx<R> cxs(const Cx<R>& c, R s) { return {c.re * s, c.im * s}; }
 template <typename R> ME_DEV R lam_of(int h, int bit) { return ((h >> bit) & 1) ? (R)1 : (R)-1; }
 // polarisation from a basis whose b part is pre-signed (+ for outgoing eps*, - for incoming eps)
 template <typename R> ME_DEV W4<R> gluon_pol_s(const R* p, R lam) {

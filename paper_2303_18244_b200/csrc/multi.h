@@ -1,11 +1,12 @@
-// multi.h — pipeline of the multi-kernel process (g g -> t t~ g g g): diagram kernels write the
+// multi.h — pipeline of the multi-kernel process (g g -> t t~ g g g): diagram kernels (each looping over the
+// helicities of the chunk) add the
 // colour-flow amplitudes of a chunk of helicities into a global staging buffer
 //     gj[hc][ncol][2 (re,im)][npad]      (FP64 in double and mixed mode, FP32 in float mode)
 // and the batched colour-sum kernel (color_sum.cu) contracts them with the colour matrix.
 #pragma once
 #include "kernels.h"
 
-#define ME_HEL_CHUNK 8   // helicities staged per pass
+#define ME_HEL_CHUNK 16   // helicities staged per pass
 
 namespace me {
 
