@@ -28,8 +28,11 @@ class Layout5:
     """per-thread shared-memory slots of one kernel (units of R)"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False):
         s = 0
+        self.FERM = None
+        if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
+            self.FERM = dict(ub=s, vv=s + 8, jtt=s + 16, sbt=s + 24, sbtb=s + 29); s += 34
         self.MOM = s; s += 4 * N
         self.PT = s; s += 4
         masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
@@ -56,6 +59,26 @@ class Inst5(Inst):
         super().__init__(lay, stride)
         self.local = {}              # global colour-flow index -> local accumulator slot
         self.redundant = 0           # flops that recompute something another block / kernel also computes
+        self.scopes = [set()]        # names of fermion values loaded in each open brace scope
+
+    def L(self, s):
+        super().L(s)
+        for ch in s:
+            if ch == "{":
+                self.scopes.append(set())
+            elif ch == "}":
+                self.scopes.pop()
+
+    def fv(self, *names):
+        """make ub / vv / jtt usable here: registers of the kernel scope, or (kernels that keep them in shared
+        memory to relieve register pressure) loaded into the current brace scope"""
+        if self.lay.FERM is None:
+            return
+        for name in names:
+            if any(name in sc for sc in self.scopes):
+                continue
+            self.L("const W4<R> %s = ldw<R>(sm + %d);" % (name, self.lay.FERM[name] * self.stride))
+            self.scopes[-1].add(name)
 
     def flush_jamps(self):
         order, by = [], {}
@@ -118,6 +141,7 @@ def emit_rows2(I, a, b, pab, ea, eb):
     I.ldw("q1a", I.lay.Q1 + 8 * a); I.ldw("q1b", I.lay.Q1 + 8 * b)
     I.qvec("qr", [a, b])
     I.L("const R iqr = %s;" % I.iq(a, b))
+    I.fv("ub")
     I.L("const W4<R> ra = quark_step2(ub, %s, qr, mt, iqr), rb = quark_step2(q1a, %s, qr, mt, iqr), rc = quark_step2(q1b, %s, qr, mt, iqr);" % (pab, eb, ea))
     I.flops += 3 * FL5["quark_step2"]
     return [("ra", c_step(ONE, cpair(a, b))), ("rb", c_step(cq1(a), c_leaf(b))), ("rc", c_step(cq1(b), c_leaf(a)))]
@@ -129,6 +153,7 @@ def emit_cols2(I, c, d, pcd, ec, ed, tag=""):
     row_side = rest_of(c, d)
     I.qvec("qc" + tag, row_side)
     I.L("const R iqc%s = %s;" % (tag, I.iq(*row_side)))
+    I.fv("vv")
     I.L("const W4<R> ca%s = col_step(slash_col(%s, vv), qc%s, mt, iqc%s), cb%s = col_step(slash_col(%s, chd%s), qc%s, mt, iqc%s),"
         " cc%s = col_step(slash_col(%s, chc%s), qc%s, mt, iqc%s);" % (tag, pcd, tag, tag, tag, ec, tag, tag, tag, tag, ed, tag, tag, tag))
     I.flops += 3 * (FL5["slash_col"] + FL5["col_step"])
@@ -150,7 +175,7 @@ def phase_a(lay, stride, add_group, want_pairs):
     insts = []
     for l in labels:
         I = Inst5(lay, stride)
-        I.leaf("el", l); I.qvec("q", [l])
+        I.leaf("el", l); I.qvec("q", [l]); I.fv("ub")
         I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL5["quark_step2"]
         I.stw(lay.Q1 + 8 * l, "t")
         insts.append(I)
@@ -159,7 +184,7 @@ def phase_a(lay, stride, add_group, want_pairs):
     for w in labels:
         rest = rest_of(w)
         I = Inst5(lay, stride)
-        I.leaf("ew", w); I.qvec("q", rest)
+        I.leaf("ew", w); I.qvec("q", rest); I.fv("vv")
         I.L("const W4<R> t = col_step(slash_col(ew, vv), q, mt, %s);" % I.iq(*rest)); I.flops += FL5["slash_col"] + FL5["col_step"]
         I.stw(lay.CHI + 8 * w, "t")
         insts.append(I)
@@ -172,7 +197,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
 def build_k1(stride, pidx):
-    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36)
+    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True)
     groups = []
 
     def add_group(name, insts, unroll=1):
@@ -188,68 +213,82 @@ def build_k1(stride, pidx):
         a, b, c = M
         x, y = rest_of(a, b, c)
         I = Inst5(lay, stride)
-        for nm, l in (("ea", a), ("eb", b), ("ec", c), ("ex", x), ("ey", y)):
+        I.leaf("ex", x); I.leaf("ey", y); I.kvec("kx", [x]); I.kvec("ky", [y])
+        I.L("const R ik5 = %s;" % I.ik2(*range(N)))
+        emit_pair(I, "pxy", x, y, "ex", "ey", "kx", "ky")
+        # the six three-gluon terms on M (registers for the whole block); their inputs die in this scope
+        tcol = [c_v3(cpair(a, b), c_leaf(c)), c_v3(cpair(a, c), c_leaf(b)), c_v3(cpair(b, c), c_leaf(a))] + \
+               [c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c)) for k in range(3)]
+        I.L("W4<R> t0, t1, t2, t3, t4, t5; P4<R> kM;")
+        I.L("{")
+        for nm, l in (("ea", a), ("eb", b), ("ec", c)):
             I.leaf(nm, l)
-        for nm, l in (("ka", a), ("kb", b), ("kc", c), ("kx", x), ("ky", y)):
+        for nm, l in (("ka", a), ("kb", b), ("kc", c)):
             I.kvec(nm, [l])
-        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc), kM = padd(kab, kc), kxy = padd(kx, ky),"
-            " kMx = padd(kM, kx), kMy = padd(kM, ky);"); I.flops += 28
+        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc);"); I.flops += 12
+        I.L("kM = padd(kab, kc);"); I.flops += 4
         emit_pair(I, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(I, "pac", a, c, "ea", "ec", "ka", "kc")
-        emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc"); emit_pair(I, "pxy", x, y, "ex", "ey", "kx", "ky")
+        emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc")
         I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once would do
-        I.L("const R ik3 = %s, ik5 = %s, ik4x = %s, ik4y = %s;" % (I.ik2(a, b, c), I.ik2(*range(N)), I.ik2(a, b, c, x), I.ik2(a, b, c, y)))
+        I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
-        terms = [("t0", "v3_current(pab, ec, kab, kc, ik3)", c_v3(cpair(a, b), c_leaf(c))),
-                 ("t1", "v3_current(pac, eb, kac, kb, ik3)", c_v3(cpair(a, c), c_leaf(b))),
-                 ("t2", "v3_current(pbc, ea, kbc, ka, ik3)", c_v3(cpair(b, c), c_leaf(a)))]
-        for k in range(3):
-            terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
-        for i, (nm, expr, col) in enumerate(terms):
-            I.L("const W4<R> %s = %s;" % (nm, expr)); I.flops += FL5["v3_current"] if i < 3 else FL5["v4_current"]
-        I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("q1y", lay.Q1 + 8 * y); I.ldw("chx", lay.CHI + 8 * x); I.ldw("chy", lay.CHI + 8 * y)
+        I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
+        I.L("t3 = v4_current(0, dots, ea, eb, ec); t4 = v4_current(1, dots, ea, eb, ec); t5 = v4_current(2, dots, ea, eb, ec);")
+        I.flops += 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
+        I.L("}")
 
-        def dots_with(xname, flops, colour_of_term):
-            """6 amplitudes t_i . X and their jamp updates"""
-            I.L("{ const W4<R> X = %s;" % xname); I.flops += flops
+        def dots_with(prelude, xexpr, flops, colour_of_term):
+            """6 amplitudes t_i . X and their jamp updates; operands of X are loaded inside the scope"""
+            I.L("{")
+            for fn in prelude:
+                fn()
+            I.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])
+            I.L("  const W4<R> X = %s;" % xexpr); I.flops += flops
             I.L("  const Cx<R> a0 = wdot(t0, X), a1 = wdot(t1, X), a2 = wdot(t2, X), a3 = wdot(t3, X), a4 = wdot(t4, X), a5 = wdot(t5, X);")
             I.flops += 6 * FL5["wdot"]
-            for i, (nm, expr, col) in enumerate(terms):
+            for i, col in enumerate(tcol):
                 I.jamp("a%d" % i, colour_of_term(col), pidx)
             I.flush_jamps()
             I.L("}")
 
+        ld = lambda nm, slot: (lambda: I.ldw(nm, slot))
         # quad = V3(t, eps_u) closing three ways with the last gluon w  (u,w) = (x,y) and (y,x)
-        for (u, w, eu, ew, ku, kw, kMu, ik4u, q1w, chw) in ((x, y, "ex", "ey", "kx", "ky", "kMx", "ik4x", "q1y", "chy"),
-                                                             (y, x, "ey", "ex", "ky", "kx", "kMy", "ik4y", "q1x", "chx")):
+        for (u, w, eu, ew, ku, kw) in ((x, y, "ex", "ey", "kx", "ky"), (y, x, "ey", "ex", "ky", "kx")):
             quad = lambda col, u=u: c_v3(col, c_leaf(u))
-            dots_with("v3_dual(%s, bilinear(ub, %s), kM, %s, %s)" % (eu, chw, ku, ik4u), FL5["v3_dual"] + FL5["bilinear"],
+            ik4 = lambda u=u: I.L("const R ik4 = %s;" % I.ik2(a, b, c, u))
+            dots_with([ld("chw", lay.CHI + 8 * w), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
                       lambda col, w=w, quad=quad: c_close(ONE, quad(col), cchi(w)))
-            dots_with("v3_dual(%s, bilinear(%s, vv), kM, %s, %s)" % (eu, q1w, ku, ik4u), FL5["v3_dual"] + FL5["bilinear"],
+            dots_with([ld("q1w", lay.Q1 + 8 * w), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
                       lambda col, w=w, quad=quad: c_close(cq1(w), quad(col), ONE))
-            dots_with("v3_dual(%s, v3_dual(%s, jtt, %s, %s, ik5), kM, %s, %s)" % (eu, ew, kMu, kw, ku, ik4u), 2 * FL5["v3_dual"],
+            dots_with([ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
                       lambda col, w=w, quad=quad: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
         # V3(t, pair(x,y)) on the bare line
-        dots_with("v3_dual(pxy, jtt, kM, kxy, ik5)", FL5["v3_dual"], lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
+        dots_with([], "v3_dual(pxy, jtt, kM, padd(kx, ky), ik5)", FL5["v3_dual"] + 4, lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
         # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
-        I.L("const Cx<R> cxj = cxs(wdot(ex, jtt), ik5), cyj = cxs(wdot(ey, jtt), ik5), cxy = cxs(wdot(ex, ey), ik5);"); I.flops += 3 * FL5["wdot"] + 6
-        dots_with("cx_comb(cxj, ey, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(0, col, c_leaf(x), c_leaf(y)), ONE))
-        dots_with("cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
-        dots_with("cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
+        cdots = lambda: (I.fv("jtt"), I.L("const Cx<R> cxj = cxs(wdot(ex, jtt), ik5), cyj = cxs(wdot(ey, jtt), ik5), cxy = cxs(wdot(ex, ey), ik5);"))
+        dots_with([cdots], "cx_comb(cxj, ey, cxy, jtt)", FL5["cx_comb"] + 3 * FL5["wdot"] + 6, lambda col: c_close(ONE, c_v4(0, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with([cdots], "cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with([cdots], "cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
         # q1(u) . t-slash . chi1(w)
-        dots_with("bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
-        dots_with("bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
+        dots_with([ld("q1x", lay.Q1 + 8 * x), ld("chy", lay.CHI + 8 * y)], "bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
+        dots_with([ld("q1y", lay.Q1 + 8 * y), ld("chx", lay.CHI + 8 * x)], "bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
         # ubar . t-slash . chi2(x,y)  and  q2(x,y) . t-slash . v
-        I.L("{")
-        cols = emit_cols2(I, x, y, "pxy", "ex", "ey")
-        I.redundant += 0
-        for nm, ccol in cols:
-            dots_with("bilinear(ub, %s)" % nm, FL5["bilinear"], lambda col, ccol=ccol: c_close(ONE, col, ccol))
-        I.L("}")
-        I.L("{")
-        rows = emit_rows2(I, x, y, "pxy", "ex", "ey")
-        for nm, rcol in rows:
-            dots_with("bilinear(%s, vv)" % nm, FL5["bilinear"], lambda col, rcol=rcol: c_close(rcol, col, ONE))
-        I.L("}")
+        # (one current at a time: three live two-gluon currents next to t0..t5 would spill)
+        row_side = rest_of(x, y)
+        qc = lambda: (I.qvec("qc", row_side), I.L("const R iqc = %s;" % I.iq(*row_side)))
+        qr = lambda: (I.qvec("qr", [x, y]), I.L("const R iqr = %s;" % I.iq(x, y)))
+        st = FL5["slash_col"] + FL5["col_step"] + FL5["bilinear"]
+        dots_with([qc], "bilinear(ub, col_step(slash_col(pxy, vv), qc, mt, iqc))", st, lambda col: c_close(ONE, col, c_step(cpair(x, y), ONE)))
+        dots_with([qc, ld("chy", lay.CHI + 8 * y)], "bilinear(ub, col_step(slash_col(ex, chy), qc, mt, iqc))", st,
+                  lambda col: c_close(ONE, col, c_step(c_leaf(x), cchi(y))))
+        dots_with([qc, ld("chx", lay.CHI + 8 * x)], "bilinear(ub, col_step(slash_col(ey, chx), qc, mt, iqc))", st,
+                  lambda col: c_close(ONE, col, c_step(c_leaf(y), cchi(x))))
+        st = FL5["quark_step2"] + FL5["bilinear"]
+        dots_with([qr], "bilinear(quark_step2(ub, pxy, qr, mt, iqr), vv)", st, lambda col: c_close(c_step(ONE, cpair(x, y)), col, ONE))
+        dots_with([qr, ld("q1x", lay.Q1 + 8 * x)], "bilinear(quark_step2(q1x, ey, qr, mt, iqr), vv)", st,
+                  lambda col: c_close(c_step(cq1(x), c_leaf(y)), col, ONE))
+        dots_with([qr, ld("q1y", lay.Q1 + 8 * y)], "bilinear(quark_step2(q1y, ex, qr, mt, iqr), vv)", st,
+                  lambda col: c_close(c_step(cq1(y), c_leaf(x)), col, ONE))
         I.flush_global()
         insts.append(I)
     add_group("triples", insts, 1)
@@ -484,15 +523,24 @@ def emit_kernel(name, ki, lay, groups):
     pro, fixed = prologue_lines(lay)
     for l in pro:
         S("    " + l)
+    if lay.FERM is not None:
+        S("    stsb<R>(sm, %d, sbt); stsb<R>(sm, %d, sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
     S("  }")
     S("#pragma unroll")
     S("  for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * lay.jacc, lay.J))
     S("  for (int hc = 0; hc < nh; ++hc) {")
     S("    const int h = hels[hc];")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
-    S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
-    S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
-    S("    const W4<R> jtt = bilinear(ub, vv);")
+    if lay.FERM is not None:
+        S("    {")
+        S("      const W4<R> ub = spinor_ubar(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbt"], NPAR - 1 - 2))
+        S("      const W4<R> vv = spinor_v(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbtb"], NPAR - 1 - 3))
+        S("      stw<R>(sm, %d, ub); stw<R>(sm, %d, vv); stw<R>(sm, %d, bilinear(ub, vv));" % (lay.FERM["ub"], lay.FERM["vv"], lay.FERM["jtt"]))
+        S("    }")
+    else:
+        S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
+        S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
+        S("    const W4<R> jtt = bilinear(ub, vv);")
     for gname, tmpl, rows, unroll in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
         S("#pragma unroll %d" % unroll)
