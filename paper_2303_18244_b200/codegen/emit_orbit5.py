@@ -239,7 +239,7 @@ def build_k1(stride, pidx):
 
         def dots_with(prelude, xexpr, flops, colour_of_term):
             """6 amplitudes t_i . X and their jamp updates; operands of X are loaded inside the scope"""
-            I.L("{")
+            I.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
                 fn()
             I.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])

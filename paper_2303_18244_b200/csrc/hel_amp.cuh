@@ -21,6 +21,8 @@
 namespace me {
 
 #define ME_DEV __device__ __forceinline__
+// compiler-only fence: memory operations are not moved across it (bounds load hoisting, hence register pressure)
+#define ME_FENCE asm volatile("" ::: "memory")
 
 template <typename R> struct P4 { R e, x, y, z; };            // real four-vector (E,px,py,pz)
 template <typename R> struct Cx { R re, im; };
