@@ -7,6 +7,8 @@
 // C operand is a warp-uniform (broadcast) load.
 #include "multi.h"
 
+#include <cstdlib>
+
 namespace me {
 
 #define CS_NCOL 120
@@ -76,6 +78,8 @@ size_t multi_scratch_bytes(int precision, long npad, int ncol) {
 }
 
 static bool g_color_loaded = false;
+// FP64: tensor-core (DMMA) colour sum; ME_COLOR_FMA=1 in the environment selects the plain-FMA kernel (A/B timing)
+static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
 
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host) {
@@ -111,7 +115,12 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
     const int first = base == 0;
     const size_t smd = sizeof(double) * (2 * CS_NCOL + CS_WARPS) * 32, smf = sizeof(float) * (2 * CS_NCOL + CS_WARPS) * 32;
     cudaFuncSetAttribute(k_color_sum<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);
-    if (precision == 0)
+    if (precision == 0 && g_use_dmma) {
+      const double* cm = nullptr;
+      cudaError_t e2 = cudaGetSymbolAddress((void**)&cm, c_color_d);
+      if (e2 == cudaSuccess) e2 = launch_color_sum_dmma(cm, (const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      if (e2 != cudaSuccess) return e2;
+    } else if (precision == 0)
       k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     else if (precision == 1)
       k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);

@@ -1,0 +1,126 @@
+// color_sum_dmma.cu — FP64 colour sum of the 120-flow process on the tensor cores (SURVEY.md §8(a) step a7,
+// BASELINE.json north_star: "the colour sum is batched as a genuine dense contraction over events, on FP64 DMMA").
+//
+//     Y = C X,   C [120 x 120] colour-matrix numerators,  X [120 x (2 * events)] = (Re J, Im J) of one helicity,
+//     ME_h(evt) = sum_i  X[i][evt,re] Y[i][evt,re] + X[i][evt,im] Y[i][evt,im]
+//
+// mma.sync.m8n8k4.f64 (DMMA): M = 8 colour rows, N = 8 events, K = 4 colour columns.  A warp owns 8 events and both
+// their Re and Im columns (two N-tiles) for ALL 15 row blocks: 30 accumulator tiles (60 doubles) in registers, so each
+// A fragment (from shared memory, stored in fragment order -> conflict-free) feeds two DMMAs and each B fragment
+// (read straight from the global staging buffer, 64-byte segments) feeds fifteen.  The epilogue multiplies Y with X in
+// the accumulator layout and reduces over the 8 lanes that share a column with shuffles.  Persistent CTAs (one per
+// SM, 8 warps) keep the 115 KB of C fragments resident.
+#include "multi.h"
+
+namespace me {
+
+#define CD_NCOL 120
+#define CD_RB (CD_NCOL / 8)     // 15 row blocks
+#define CD_KS (CD_NCOL / 4)     // 30 k-steps
+#define CD_WARPS 8
+#define CD_PF 6                 // k-steps of B fragments prefetched per batch
+
+__device__ __forceinline__ void dmma8x8x4(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const double* __restrict__ cmat, const double* __restrict__ gj, long npad, long n, int nh,
+                                                                    const unsigned char* __restrict__ hels, int first,
+                                                                    double norm_hel, double inv_avg,
+                                                                    double* __restrict__ me_out, double* __restrict__ me_hel) {
+  extern __shared__ __align__(16) double cfrag[];          // [CD_RB][CD_KS][32] in A-fragment order
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < CD_RB * CD_KS * 32; i += blockDim.x) {
+    const int l = i & 31, ks = (i >> 5) % CD_KS, rb = (i >> 5) / CD_KS;
+    cfrag[i] = cmat[(rb * 8 + (l >> 2)) * CD_NCOL + ks * 4 + (l & 3)];
+  }
+  __syncthreads();
+  const long ntiles = (npad + 8 * CD_WARPS - 1) / (8 * CD_WARPS);
+  const int kr = lane & 3, ec = lane >> 2;                 // B fragment: row kr of the k-step, event column ec
+  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const long e0 = (tile * CD_WARPS + w) * 8;
+    if (e0 >= npad) continue;                              // npad is a multiple of 32: a warp is either fully in or out
+    double me_acc0 = 0, me_acc1 = 0;
+    for (int hc = 0; hc < nh; ++hc) {
+      const double* g = gj + (long)hc * (2 * CD_NCOL) * npad + e0;
+      double acc[CD_RB][2][2];
+#pragma unroll
+      for (int rb = 0; rb < CD_RB; ++rb) { acc[rb][0][0] = acc[rb][0][1] = acc[rb][1][0] = acc[rb][1][1] = 0; }
+      double bre[CD_PF], bim[CD_PF];
+#pragma unroll
+      for (int j = 0; j < CD_PF; ++j) {
+        const double* p = g + (long)(2 * (4 * j + kr)) * npad + ec;
+        bre[j] = p[0]; bim[j] = p[npad];
+      }
+#pragma unroll 1
+      for (int kb = 0; kb < CD_KS; kb += CD_PF) {
+        double nre[CD_PF], nim[CD_PF];
+        if (kb + CD_PF < CD_KS) {
+#pragma unroll
+          for (int j = 0; j < CD_PF; ++j) {
+            const double* p = g + (long)(2 * (4 * (kb + CD_PF + j) + kr)) * npad + ec;
+            nre[j] = p[0]; nim[j] = p[npad];
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < CD_PF; ++j) {
+          const double* af = cfrag + (kb + j) * 32 + lane;
+#pragma unroll
+          for (int rb = 0; rb < CD_RB; ++rb) {
+            const double a = af[rb * CD_KS * 32];
+            dmma8x8x4(acc[rb][0][0], acc[rb][0][1], a, bre[j]);
+            dmma8x8x4(acc[rb][1][0], acc[rb][1][1], a, bim[j]);
+          }
+        }
+        if (kb + CD_PF < CD_KS) {
+#pragma unroll
+          for (int j = 0; j < CD_PF; ++j) { bre[j] = nre[j]; bim[j] = nim[j]; }
+        }
+      }
+      // epilogue: accumulator element (row = rb*8 + lane/4, column = 2*(lane%4) + {0,1})
+      double p0 = 0, p1 = 0;
+#pragma unroll
+      for (int rb = 0; rb < CD_RB; ++rb) {
+        const double* x = g + (long)(2 * (rb * 8 + ec)) * npad + 2 * kr;
+        const double2 xr = *reinterpret_cast<const double2*>(x), xi = *reinterpret_cast<const double2*>(x + npad);
+        p0 += acc[rb][0][0] * xr.x + acc[rb][1][0] * xi.x;
+        p1 += acc[rb][0][1] * xr.y + acc[rb][1][1] * xi.y;
+      }
+#pragma unroll
+      for (int o = 4; o < 32; o <<= 1) { p0 += __shfl_xor_sync(0xffffffffu, p0, o); p1 += __shfl_xor_sync(0xffffffffu, p1, o); }
+      if (lane < 4) {
+        const long e = e0 + 2 * lane;
+        if (me_hel != nullptr) {
+          if (e < n) me_hel[(long)hels[hc] * n + e] = p0 * norm_hel * 0.5;
+          if (e + 1 < n) me_hel[(long)hels[hc] * n + e + 1] = p1 * norm_hel * 0.5;
+        }
+        me_acc0 += p0; me_acc1 += p1;
+      }
+    }
+    if (lane < 4 && me_out != nullptr) {
+      const long e = e0 + 2 * lane;
+      const double s = norm_hel * 0.5 * inv_avg;
+      if (e < n) me_out[e] = first ? me_acc0 * s : me_out[e] + me_acc0 * s;
+      if (e + 1 < n) me_out[e + 1] = first ? me_acc1 * s : me_out[e + 1] + me_acc1 * s;
+    }
+  }
+}
+
+cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, int nh, const unsigned char* hels, int first,
+                                  double norm_hel, double inv_avg, double* me_out, double* me_hel, cudaStream_t stream) {
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  }
+  const size_t smem = sizeof(double) * CD_RB * CD_KS * 32;
+  cudaError_t e = cudaFuncSetAttribute(k_color_sum_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  const long ntiles = (npad + 8 * CD_WARPS - 1) / (8 * CD_WARPS);
+  const unsigned grid = (unsigned)(ntiles < sms ? ntiles : sms);
+  k_color_sum_dmma<<<grid, 32 * CD_WARPS, smem, stream>>>(cmat, gj, npad, n, nh, hels, first, norm_hel, inv_avg, me_out, me_hel);
+  return cudaGetLastError();
+}
+
+}  // namespace me
