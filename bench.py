@@ -83,7 +83,7 @@ def oracle_rate(proc, p, target_seconds=15.0):
     import oracle
     oracle.build()
     cores = oracle.max_threads()
-    n0 = min(len(p), 8 * cores)
+    n0 = min(len(p), 256 * cores)
     t0 = time.perf_counter(); oracle.me(proc, p[:n0]); dt = time.perf_counter() - t0
     n = int(min(len(p), max(n0, target_seconds * n0 / max(dt, 1e-6))))
     t0 = time.perf_counter(); oracle.me(proc, p[:n]); dt = time.perf_counter() - t0
@@ -128,6 +128,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="headline workload only (no other processes, no oracle leg)")
     ap.add_argument("--events", type=int, default=0, help="override events per GPU (default: the config's)")
+    ap.add_argument("--config", type=int, default=HEADLINE, choices=[1, 2, 3, 4],
+                    help="index into inputs.CONFIGS of the timed workload (default 3 = g g -> t t~ g g, the BASELINE.json metric; "
+                         "others are for profiling a single process, e.g. --quick --config 4)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -154,7 +157,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = inputs.CONFIGS[HEADLINE]
+    HL = args.config
+    cfg = inputs.CONFIGS[HL]
     per_gpu = args.events or cfg["events"]
     first, n = shard_range(per_gpu * world, rank, world)
     stream = torch.cuda.current_stream()
@@ -198,7 +202,7 @@ def main():
         return float(t.item())
 
     # ------------------------------------------------------------------ headline: g g -> t t~ g g
-    ctx, mom = setup(HEADLINE, n, first)
+    ctx, mom = setup(HL, n, first)
     info = ctx.info
     ngood = bin(ctx.me_filter_helicities(mom, 32)[0]).count("1")
     flops_alg = info.flops_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
@@ -210,21 +214,22 @@ def main():
     total_ms = allmax(total_ms)
     value = per_gpu * world * args.steps / (total_ms * 1e-3)
     ms_kernel = statistics.mean(per)
-    launches = args.steps * info.nkernels
+    per_step_launches = info.nkernels * ((ngood + 15) // 16 if HL == 4 else 1)    # cfg 5: 3 diagram kernels + colour sum per 16-helicity chunk
+    launches = args.steps * per_step_launches
     results[cfg["name"]] = {"fp64": {"MEs_per_s": n * args.steps / (sum(per) * 1e-3), "ms_per_step": ms_kernel}}
     # measured FMA-chain peaks (register-resident microkernel, same box, same run)
     peak_meas = {"fp64": me.me_fma_peak(1), "fp32": me.me_fma_peak(0)}
     ach = flops_alg * n / (ms_kernel * 1e-3) * 1e-12
-    roofline = {"bound": "alu", "kernel": "k_gg_ttxgg<double,double>", "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "k_%s<double,double>" % cfg["name"] + (" (+ colour sum)" if HL == 4 else ""), "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
                 "frac": ach / PEAK_TFLOPS["fp64"], "traffic": None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md clocks; no FP64 entry in MEASURED_PEAKS.json)",
                 "peak_measured_fma_chain": peak_meas["fp64"], "frac_of_measured": ach / peak_meas["fp64"],
                 "flops_per_event_algorithmic": flops_alg, "flops_per_event_executed": flops_exe,
                 "achieved_executed": flops_exe * n / (ms_kernel * 1e-3) * 1e-12}
     # other precisions of the headline workload
-    for pname in ("mixed", "fp32"):
+    for pname in [q for q in ("mixed", "fp32") if q in cfg["precisions"]]:
         t, pp = timed(ctx, mom, n, me.PRECISIONS[pname], args.steps, args.warmup)
-        launches += args.steps * info.nkernels
+        launches += args.steps * per_step_launches
         ms = statistics.mean(pp)
         results[cfg["name"]][pname] = {"MEs_per_s": n / (ms * 1e-3), "ms_per_step": ms}
     a32 = flops_alg * n / (results[cfg["name"]]["fp32"]["ms_per_step"] * 1e-3) * 1e-12
@@ -236,9 +241,9 @@ def main():
     e2e_ms = allmax(e2e_ms)
     e2e = {"value": per_gpu * world * args.steps / (e2e_ms * 1e-3), "unit": "MEs/s", "h2d_bytes_per_step": host.numel() * 8,
            "d2h_bytes_per_step": n * 8, "api": "MEContext.me_compute_host (pinned host momenta -> me_compute -> pinned host MEs)"}
-    launches += args.steps * info.nkernels
+    launches += args.steps * per_step_launches
     line = {
-        "metric": "matrix elements/sec (g g -> t t~ g g, FP64)", "value": value, "unit": "MEs/s", "n_gpus": world, "steps": args.steps,
+        "metric": "matrix elements/sec (%s, FP64)" % cfg["label"], "value": value, "unit": "MEs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s, %d RAMBO events per GPU, sqrt(s)=1500 GeV, Philox seed %d, %d good helicities" % (cfg["label"], per_gpu, cfg["seed"], ngood),
@@ -256,7 +261,7 @@ def main():
     ctx.close(); del mom, host
     # ------------------------------------------------------------------ the other processes (context numbers; not the headline)
     if world == 1 and not args.quick:
-        for proc in (1, 2, 4):
+        for proc in [q for q in (1, 2, 3, 4) if q != HL]:
             c = inputs.CONFIGS[proc]
             cx, mm = setup(proc, c["events"], 0)
             ng = bin(cx.me_filter_helicities(mm, 32)[0]).count("1")
