@@ -196,7 +196,9 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx):
+def build_k1(stride, pidx, part=None):
+    """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
+    instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True)
     groups = []
 
@@ -230,6 +232,8 @@ def build_k1(stride, pidx):
         emit_pair(I, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(I, "pac", a, c, "ea", "ec", "ka", "kc")
         emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc")
         I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once would do
+        if part is not None and part > 0:             # the split kernels each rebuild the six terms
+            I.redundant += 6 * FL5["v3_current"] + FL5["v4_dots"] + 3 * FL5["v4_current"]
         I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
         I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
@@ -237,8 +241,13 @@ def build_k1(stride, pidx):
         I.flops += 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
         I.L("}")
 
+        counter = [0]
+
         def dots_with(prelude, xexpr, flops, colour_of_term):
             """6 amplitudes t_i . X and their jamp updates; operands of X are loaded inside the scope"""
+            idx = counter[0]; counter[0] += 1
+            if part is not None and idx // 6 != part:
+                return
             I.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
                 fn()
@@ -289,6 +298,7 @@ def build_k1(stride, pidx):
                   lambda col: c_close(c_step(cq1(x), c_leaf(y)), col, ONE))
         dots_with([qr, ld("q1y", lay.Q1 + 8 * y)], "bilinear(quark_step2(q1y, ex, qr, mt, iqr), vv)", st,
                   lambda col: c_close(c_step(cq1(y), c_leaf(x)), col, ONE))
+        assert counter[0] == 18
         I.flush_global()
         insts.append(I)
     add_group("triples", insts, 1)
@@ -385,46 +395,55 @@ def build_k3(stride, pidx):
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
-    insts = []
-    for w in range(N):
-        quad = rest_of(w)
-        I = Inst5(lay, stride)
+    def ends(I, w, quad):
+        """the three four-vectors a quad term is dotted with: bilinears of the fermion ends and the dual of V3(quad, eps_w)"""
         I.leaf("ew", w); I.kvec("kw", [w]); I.kvec("kq", quad)
         I.ldw("chw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
         I.L("const R ik4 = %s;" % I.ik2(*quad))
         I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv), x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
         I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
 
-        def close3(tname, col):
-            I.L("{ const Cx<R> a1 = wdot(%s, x1), a2 = wdot(%s, x2), a3 = wdot(%s, x3);" % (tname, tname, tname)); I.flops += 3 * FL5["wdot"]
-            I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)
-            I.jamp("a2", c_close(cq1(w), col, ONE), pidx)
-            I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
-            I.flush_jamps()
-            I.L("}")
+    def close3(I, w, tname, col):
+        I.L("{ const Cx<R> a1 = wdot(%s, x1), a2 = wdot(%s, x2), a3 = wdot(%s, x3);" % (tname, tname, tname)); I.flops += 3 * FL5["wdot"]
+        I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)
+        I.jamp("a2", c_close(cq1(w), col, ONE), pidx)
+        I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
+        I.flush_jamps()
+        I.L("}")
 
+    # (small instances: a per-w instance with all 21 quad terms unrolled was ~8 k instructions and instruction-fetch bound)
+    insts = []
+    for w in range(N):
+        quad = rest_of(w)
         a0 = quad[0]
         for b0 in quad[1:]:
             p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
-            I.L("{")
+            I = Inst5(lay, stride)
+            ends(I, w, quad)
+            I.redundant += (2 * FL5["bilinear"] + FL5["v3_dual"]) * 8 // 9      # 5 distinct end triples, formed 45 times
             I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.kvec("k1", list(p1)); I.kvec("k2", list(p2))
             I.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); I.flops += FL5["v3_current"]
-            close3("t", c_v3(cpair(*p1), cpair(*p2)))
-            I.L("}")
+            close3(I, w, "t", c_v3(cpair(*p1), cpair(*p2)))
             I.flush_global()
+            insts.append(I)
+    add_group("quad_v3", insts, 1)
+    insts = []
+    for w in range(N):
+        quad = rest_of(w)
         for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
             l1, l2 = [l for l in quad if l not in p]
-            I.L("{")
+            I = Inst5(lay, stride)
+            ends(I, w, quad)
+            I.redundant += (2 * FL5["bilinear"] + FL5["v3_dual"]) * 8 // 9
             I.ldw("pp", lay.PAIR[p]); I.leaf("e1", l1); I.leaf("e2", l2)
             I.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); I.flops += FL5["v4_dots"]
             for k in range(3):
                 I.L("{ const W4<R> t = v4_current(%d, dots, pp, e1, e2);" % k); I.flops += FL5["v4_current"]
-                close3("t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
+                close3(I, w, "t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
                 I.L("}")
-            I.L("}")
             I.flush_global()
-        insts.append(I)
-    add_group("quads", insts, 1)
+            insts.append(I)
+    add_group("quad_v4", insts, 1)
     # ---- V4(pair, pair', eps_m) on the bare line
     insts = []
     for m in range(N):
@@ -578,7 +597,8 @@ def emit_orbit5_process(name="gg_ttxggg"):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     files, kinfo = {}, []
-    builders = (build_k1, build_k2, build_k3)
+    builders = (lambda st, px: build_k1(st, px, 0), lambda st, px: build_k1(st, px, 1), lambda st, px: build_k1(st, px, 2),
+                build_k2, build_k3)
     for ki, b in enumerate(builders):
         lay, groups = b(BLOCK, pidx)
         src, info = emit_kernel(name, ki, lay, groups)
@@ -595,7 +615,7 @@ def emit_orbit5_process(name="gg_ttxggg"):
         pass
     lay2, groups2 = build_k2(BLOCK, pidx)
     pa = {g: t.flops * len(rows) for g, t, rows, _ in groups2 if g in ("pairs", "q1", "chi1")}
-    redundant = sum(k["redundant"] for k in kinfo) + 2 * (pa["q1"] + pa["chi1"]) + pa["pairs"] + 2 * head
+    redundant = sum(k["redundant"] for k in kinfo) + (len(kinfo) - 1) * (pa["q1"] + pa["chi1"] + head) + pa["pairs"]
     # the 10 pairs are needed once: kernel 1 recomputes them per block (tagged), kernels 2 and 3 both run the pairs loop
     algo = executed - redundant
     fixed = sum(k["fixed"] for k in kinfo)
