@@ -34,24 +34,52 @@ def lam_bit(label, npar=NPAR):
     return npar - 1 - p
 
 
+class SlotAlloc:
+    """Slot allocator for the paired shared-memory layout (hel_amp.cuh): vectors start on even slots; the odd
+    slot left behind by a 5-real basis (and any alignment gap) is handed out to scalars first."""
+
+    def __init__(self):
+        self.n, self.holes = 0, []
+
+    def vec(self, size):
+        if self.n & 1:
+            self.holes.append(self.n); self.n += 1
+        s = self.n
+        self.n += size
+        if size & 1:
+            self.holes.append(self.n); self.n += 1
+        return s
+
+    def scalar(self):
+        if self.holes:
+            return self.holes.pop(0)
+        s = self.n; self.n += 1
+        return s
+
+
+def eo(slot, stride):
+    """element offset of a slot in the per-thread R array (ME_EO of hel_amp.cuh)"""
+    return (slot >> 1) * 2 * stride + (slot & 1)
+
+
 class Layout:
     npar = NPAR
 
     def __init__(self):
-        s = 0
-        self.MOM = s; s += 4 * N            # signed gluon momenta (+p incoming, -p outgoing)
-        self.PT = s; s += 4                 # p_t
-        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
-        self.IK2 = {m: s + i for i, m in enumerate(masks2)}; s += len(masks2)
-        masksq = [m for m in range(1, (1 << N) - 1)]
-        self.IQ = {m: s + i for i, m in enumerate(masksq)}; s += len(masksq)
-        self.GB = s; s += 5 * N
+        A = SlotAlloc()
+        self.MOM = A.vec(4 * N)            # signed gluon momenta (+p incoming, -p outgoing)
+        self.PT = A.vec(4)                 # p_t
+        self.GBS = [A.vec(5) for _ in range(N)]
         pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
-        self.PAIR = {p: s + 8 * i for i, p in enumerate(pairs)}; s += 8 * len(pairs)
-        self.Q1 = s; s += 8 * N
-        self.CHI = s; s += 8 * N
-        self.J = s; s += 2 * 24
-        self.nslots = s
+        self.PAIR = {p: A.vec(8) for p in pairs}
+        self.Q1 = A.vec(8 * N)
+        self.CHI = A.vec(8 * N)
+        self.J = A.vec(2 * 24)
+        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
+        self.IK2 = {m: A.scalar() for m in masks2}
+        masksq = [m for m in range(1, (1 << N) - 1)]
+        self.IQ = {m: A.scalar() for m in masksq}
+        self.nslots = A.n + (A.n & 1)
 
 
 def mask_of(*labels):
@@ -59,6 +87,16 @@ def mask_of(*labels):
     for l in labels:
         m |= 1 << l
     return m
+
+
+def sum_expr(terms):
+    """' + a.re - b.im' -> 'a.re - b.im' (no leading zero: 0 + x is not an identity for x = -0)"""
+    t = terms.strip()
+    if t.startswith("+ "):
+        return t[2:]
+    if t.startswith("- "):
+        return "-" + t[2:]
+    return t
 
 
 class Inst:
@@ -75,14 +113,14 @@ class Inst:
         return "tb[%d]" % (len(self.params) - 1)
 
     def off(self, slot):                       # shared-memory element offset of a slot
-        return self.P(slot * self.stride)
+        return self.P(eo(slot, self.stride))
 
     def L(self, s):
         self.lines.append(s)
 
     # ---- operand helpers
     def leaf(self, name, l):
-        self.L("const W4<R> %s = gluon_pol_s<R>(sm + %s, lam_of<R>(h, %s));" % (name, self.off(self.lay.GB + 5 * l), self.P(lam_bit(l, self.lay.npar))))
+        self.L("const W4<R> %s = gluon_pol_s<R>(sm + %s, lam_of<R>(h, %s));" % (name, self.off(self.lay.GBS[l]), self.P(lam_bit(l, self.lay.npar))))
         self.flops += FL["gluon_pol"]
 
     def kvec(self, name, labels):
@@ -94,7 +132,7 @@ class Inst:
         self.L("const P4<R> %s = %s;" % (name, expr))
 
     def qvec(self, name, labels):
-        expr = "ldp<R>(sm + %d)" % (self.lay.PT * self.stride)
+        expr = "ldp<R>(sm + %d)" % eo(self.lay.PT, self.stride)
         for l in labels:
             expr = "psub(%s, ldp<R>(sm + %s))" % (expr, self.off(self.lay.MOM + 4 * l))
             self.flops += 4
@@ -133,7 +171,7 @@ class Inst:
         for sigma in order:
             re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
             im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
-            self.L("{ R* j = sm + %s; j[0] = j[0]%s; j[ME_SM_STRIDE] = j[ME_SM_STRIDE]%s; }" % (self.off(self.lay.J + 2 * sigma), re, im))
+            self.L("cacc<R>(sm + %s, %s, %s);" % (self.off(self.lay.J + 2 * sigma), sum_expr(re), sum_expr(im)))
             self.flops += 2 * len(by[sigma])
         self.pending = []
 
@@ -338,7 +376,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
       " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out) {" % (block, name))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
-    S("  R* sm = reinterpret_cast<R*>(smem_raw) + threadIdx.x;")
+    S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
     S("  const R mt = (R)mt_d;")
@@ -366,17 +404,17 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         S("    stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
     S("    stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
     for m, slot in lay.IK2.items():
-        S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+        S("    sm[ME_EO(%d)] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
     for m, slot in lay.IQ.items():
         b = [i for i in range(N) if m >> i & 1]
         lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
         if len(b) == 1:
-            S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
+            S("    sm[ME_EO(%d)] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
         else:
-            S("    sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
+            S("    sm[ME_EO(%d)] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
         fixed += 8
     for l in range(N):
-        S("    { GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GB + 5 * l))
+        S("    { GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GBS[l]))
         fixed += 22
     S("    sbt = spinor_basis(pcast<R>(pd2), mt);")
     S("    sbtb = spinor_basis(pcast<R>(pd3), mt);")
@@ -389,7 +427,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * ncol, lay.J))
+    S("    for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * ncol, lay.J))
     for gname, tmpl, rows in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
         S("#pragma unroll %d" % UNROLL.get(gname, 1))
@@ -400,11 +438,11 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         S("    }")
     S("    if (jamp_out != nullptr && e < n) {")
     S("#pragma unroll")
-    S("      for (int s = 0; s < %d; ++s) jamp_out[(long)s * n + e] = (double)sm[(%d + s) * ME_SM_STRIDE];" % (2 * ncol, lay.J))
+    S("      for (int s = 0; s < %d; ++s) jamp_out[(long)s * n + e] = (double)sm[ME_EO(%d + s)];" % (2 * ncol, lay.J))
     S("    }")
     S("    RC cr[%d], ci[%d];" % (ncol, ncol))
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) { cr[s] = (RC)sm[(%d + 2 * s) * ME_SM_STRIDE]; ci[s] = (RC)sm[(%d + 2 * s + 1) * ME_SM_STRIDE]; }" % (ncol, lay.J, lay.J))
+    S("    for (int s = 0; s < %d; ++s) { cr[s] = (RC)sm[ME_EO(%d + 2 * s)]; ci[s] = (RC)sm[ME_EO(%d + 2 * s) + 1]; }" % (ncol, lay.J, lay.J))
     for l in cs_lines:
         S("    " + l)
     S("    const double meh = (double)cs;")

@@ -15,7 +15,7 @@ gluons (from the t~ end); (|L|,|mid|,|R|) = (0,5,0) 510, (0,4,1)+(1,4,0) 450, (0
 """
 from itertools import permutations
 
-from .emit_orbit import Inst, FL, c_leaf, c_v3, c_v4, c_step, c_close, ONE, mask_of
+from .emit_orbit import Inst, FL, c_leaf, c_v3, c_v4, c_step, c_close, ONE, mask_of, SlotAlloc, eo, sum_expr
 from .topology import color_matrix
 
 N = 5
@@ -25,31 +25,31 @@ FL5 = dict(FL, cx_comb=56)
 
 
 class Layout5:
-    """per-thread shared-memory slots of one kernel (units of R)"""
+    """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
     def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False):
-        s = 0
+        A = SlotAlloc()
         self.FERM = None
         if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
-            self.FERM = dict(ub=s, vv=s + 8, jtt=s + 16, sbt=s + 24, sbtb=s + 29); s += 34
-        self.MOM = s; s += 4 * N
-        self.PT = s; s += 4
-        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
-        self.IK2 = {m: s + i for i, m in enumerate(masks2)}; s += len(masks2)
-        # quark propagators: row side sets of size 1,2 and (for the column currents) size 3,4
-        masksq = [m for m in range(1, (1 << N) - 1) if want_iq_mid or bin(m).count("1") in (1, 4)]
-        self.IQ = {m: s + i for i, m in enumerate(masksq)}; s += len(masksq)
-        self.GB = s; s += 5 * N
+            self.FERM = dict(ub=A.vec(8), vv=A.vec(8), jtt=A.vec(8), sbt=A.vec(5), sbtb=A.vec(5))
+        self.MOM = A.vec(4 * N)
+        self.PT = A.vec(4)
+        self.GBS = [A.vec(5) for _ in range(N)]
         self.PAIR = {}
         if want_pairs:
             pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
-            self.PAIR = {p: s + 8 * i for i, p in enumerate(pairs)}; s += 8 * len(pairs)
-        self.Q1 = s; s += 8 * N
-        self.CHI = s; s += 8 * N
-        self.J = s; s += 2 * jacc
+            self.PAIR = {p: A.vec(8) for p in pairs}
+        self.Q1 = A.vec(8 * N)
+        self.CHI = A.vec(8 * N)
+        self.J = A.vec(2 * jacc)
         self.jacc = jacc
-        self.nslots = s
+        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
+        self.IK2 = {m: A.scalar() for m in masks2}
+        # quark propagators: row side sets of size 1,2 and (for the column currents) size 3,4
+        masksq = [m for m in range(1, (1 << N) - 1) if want_iq_mid or bin(m).count("1") in (1, 4)]
+        self.IQ = {m: A.scalar() for m in masksq}
+        self.nslots = A.n + (A.n & 1)
 
 
 class Inst5(Inst):
@@ -77,7 +77,7 @@ class Inst5(Inst):
         for name in names:
             if any(name in sc for sc in self.scopes):
                 continue
-            self.L("const W4<R> %s = ldw<R>(sm + %d);" % (name, self.lay.FERM[name] * self.stride))
+            self.L("const W4<R> %s = ldw<R>(sm + %d);" % (name, eo(self.lay.FERM[name], self.stride)))
             self.scopes[-1].add(name)
 
     def flush_jamps(self):
@@ -91,8 +91,7 @@ class Inst5(Inst):
             assert loc < self.lay.jacc, "local jamp accumulators exhausted"
             re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
             im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
-            o = (self.lay.J + 2 * loc) * self.stride
-            self.L("sm[%d] = sm[%d]%s; sm[%d] = sm[%d]%s;" % (o, o, re, o + self.stride, o + self.stride, im))
+            self.L("cacc<R>(sm + %d, %s, %s);" % (eo(self.lay.J + 2 * loc, self.stride), sum_expr(re), sum_expr(im)))
             self.flops += 2 * len(by[sigma])
         self.pending = []
 
@@ -101,9 +100,9 @@ class Inst5(Inst):
         read latency); every address is private to one thread, whose program order fixes the order of the adds, so
         the result is deterministic run to run."""
         for sigma, loc in sorted(self.local.items(), key=lambda t: t[1]):
-            o = (self.lay.J + 2 * loc) * self.stride
+            o = eo(self.lay.J + 2 * loc, self.stride)
             self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
-                   % (self.P(2 * sigma), o, o + self.stride, o, o + self.stride))
+                   % (self.P(2 * sigma), o, o + 1, o, o + 1))
             self.flops += 2
         self.local = {}
 
@@ -495,17 +494,17 @@ def prologue_lines(lay):
         A("stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
     A("stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
     for m, slot in lay.IK2.items():
-        A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+        A("sm[ME_EO(%d)] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
     for m, slot in lay.IQ.items():
         b = [i for i in range(N) if m >> i & 1]
         lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
         if len(b) == 1:
-            A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
+            A("sm[ME_EO(%d)] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
         else:
-            A("sm[%d * ME_SM_STRIDE] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
+            A("sm[ME_EO(%d)] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
         fixed += 8
     for l in range(N):
-        A("{ GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GB + 5 * l))
+        A("{ GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GBS[l]))
         fixed += 22
     A("sbt = spinor_basis(pcast<R>(pd2), mt);")
     A("sbtb = spinor_basis(pcast<R>(pd3), mt);")
@@ -533,7 +532,7 @@ def emit_kernel(name, ki, lay, groups):
     S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
       " double mt_d, RJ* __restrict__ gjbase) {" % (BLOCK, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
-    S("  R* sm = reinterpret_cast<R*>(smem_raw) + threadIdx.x;")
+    S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
     S("  const R mt = (R)mt_d;")
@@ -546,7 +545,7 @@ def emit_kernel(name, ki, lay, groups):
         S("    stsb<R>(sm, %d, sbt); stsb<R>(sm, %d, sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
     S("  }")
     S("#pragma unroll")
-    S("  for (int s = 0; s < %d; ++s) sm[(%d + s) * ME_SM_STRIDE] = 0;" % (2 * lay.jacc, lay.J))
+    S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
     S("  for (int hc = 0; hc < nh; ++hc) {")
     S("    const int h = hels[hc];")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))

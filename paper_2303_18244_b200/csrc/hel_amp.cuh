@@ -275,38 +275,77 @@ template <typename R> ME_DEV W4<R> bilinear(const W4<R>& r, const W4<R>& c) {
 }  // namespace me
 
 // ------------------------------------------------------------------------------------
-// Per-thread shared-memory slots (blocked kernels): slot i of this thread lives at
-// sm[i * ME_SM_STRIDE] with sm already offset by threadIdx.x -> conflict-free, static offsets.
+// Per-thread shared-memory slots.  Slots are stored in PAIRS: slot s of thread t is element
+//     2 * ((s >> 1) * ME_SM_STRIDE + t) + (s & 1)        (ME_SM_STRIDE = threads per CTA)
+// of an R array, so two consecutive slots (an even one and its successor: re/im of a complex number,
+// half of a four-vector) are one 16-byte (FP64) / 8-byte (FP32) access per thread, conflict-free
+// across the warp, and a complex current is 4 loads instead of 8.  `sm` below is the R pointer already
+// offset by 2*threadIdx.x; ME_EO(s) is the element offset of slot s.  Vector types start on even slots.
 // ------------------------------------------------------------------------------------
 #ifndef ME_SM_STRIDE
 #define ME_SM_STRIDE 128
 #endif
+#define ME_EO(s) ((((s) >> 1) * 2 * ME_SM_STRIDE) + ((s) & 1))
 namespace me {
-template <typename R> ME_DEV W4<R> ldw(const R* sm, int s) {
-  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE],
-          sm[(s + 4) * ME_SM_STRIDE], sm[(s + 5) * ME_SM_STRIDE], sm[(s + 6) * ME_SM_STRIDE], sm[(s + 7) * ME_SM_STRIDE]};
+template <typename R> struct Pair2;
+template <> struct Pair2<double> { typedef double2 T; };
+template <> struct Pair2<float> { typedef float2 T; };
+// pointer-based forms: p = sm + ME_EO(even slot)
+template <typename R> ME_DEV W4<R> ldw(const R* p) {
+  typedef typename Pair2<R>::T R2;
+  const R2* q = reinterpret_cast<const R2*>(p);
+  const R2 a = q[0], b = q[ME_SM_STRIDE], c = q[2 * ME_SM_STRIDE], d = q[3 * ME_SM_STRIDE];
+  return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
 }
-template <typename R> ME_DEV void stw(R* sm, int s, const W4<R>& w) {
-  sm[(s + 0) * ME_SM_STRIDE] = w.r0; sm[(s + 1) * ME_SM_STRIDE] = w.i0; sm[(s + 2) * ME_SM_STRIDE] = w.r1; sm[(s + 3) * ME_SM_STRIDE] = w.i1;
-  sm[(s + 4) * ME_SM_STRIDE] = w.r2; sm[(s + 5) * ME_SM_STRIDE] = w.i2; sm[(s + 6) * ME_SM_STRIDE] = w.r3; sm[(s + 7) * ME_SM_STRIDE] = w.i3;
+template <typename R> ME_DEV void stw(R* p, const W4<R>& w) {
+  typedef typename Pair2<R>::T R2;
+  R2* q = reinterpret_cast<R2*>(p);
+  R2 a, b, c, d; a.x = w.r0; a.y = w.i0; b.x = w.r1; b.y = w.i1; c.x = w.r2; c.y = w.i2; d.x = w.r3; d.y = w.i3;
+  q[0] = a; q[ME_SM_STRIDE] = b; q[2 * ME_SM_STRIDE] = c; q[3 * ME_SM_STRIDE] = d;
 }
-template <typename R> ME_DEV P4<R> ldp(const R* sm, int s) {
-  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE]};
+template <typename R> ME_DEV P4<R> ldp(const R* p) {
+  typedef typename Pair2<R>::T R2;
+  const R2* q = reinterpret_cast<const R2*>(p);
+  const R2 a = q[0], b = q[ME_SM_STRIDE];
+  return {a.x, a.y, b.x, b.y};
 }
-template <typename R> ME_DEV void stp(R* sm, int s, const P4<R>& p) {
-  sm[(s + 0) * ME_SM_STRIDE] = p.e; sm[(s + 1) * ME_SM_STRIDE] = p.x; sm[(s + 2) * ME_SM_STRIDE] = p.y; sm[(s + 3) * ME_SM_STRIDE] = p.z;
+template <typename R> ME_DEV void stp(R* p, const P4<R>& v) {
+  typedef typename Pair2<R>::T R2;
+  R2* q = reinterpret_cast<R2*>(p);
+  R2 a, b; a.x = v.e; a.y = v.x; b.x = v.y; b.y = v.z;
+  q[0] = a; q[ME_SM_STRIDE] = b;
 }
-template <typename R> ME_DEV GluonBasis<R> ldgb(const R* sm, int s) {
-  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE], sm[(s + 4) * ME_SM_STRIDE]};
+// five reals (polarisation basis, spinor basis): two pairs + one single (the sixth slot is free for a scalar)
+template <typename R> ME_DEV void ld5(const R* p, R& v0, R& v1, R& v2, R& v3, R& v4) {
+  typedef typename Pair2<R>::T R2;
+  const R2* q = reinterpret_cast<const R2*>(p);
+  const R2 a = q[0], b = q[ME_SM_STRIDE];
+  v0 = a.x; v1 = a.y; v2 = b.x; v3 = b.y; v4 = p[4 * ME_SM_STRIDE];
 }
-template <typename R> ME_DEV void stgb(R* sm, int s, const GluonBasis<R>& g) {
-  sm[(s + 0) * ME_SM_STRIDE] = g.ax; sm[(s + 1) * ME_SM_STRIDE] = g.ay; sm[(s + 2) * ME_SM_STRIDE] = g.az; sm[(s + 3) * ME_SM_STRIDE] = g.bx; sm[(s + 4) * ME_SM_STRIDE] = g.by;
+template <typename R> ME_DEV void st5(R* p, R v0, R v1, R v2, R v3, R v4) {
+  typedef typename Pair2<R>::T R2;
+  R2* q = reinterpret_cast<R2*>(p);
+  R2 a, b; a.x = v0; a.y = v1; b.x = v2; b.y = v3;
+  q[0] = a; q[ME_SM_STRIDE] = b; p[4 * ME_SM_STRIDE] = v4;
 }
-template <typename R> ME_DEV SpinorBasis<R> ldsb(const R* sm, int s) {
-  return {sm[(s + 0) * ME_SM_STRIDE], sm[(s + 1) * ME_SM_STRIDE], sm[(s + 2) * ME_SM_STRIDE], sm[(s + 3) * ME_SM_STRIDE], sm[(s + 4) * ME_SM_STRIDE]};
-}
-template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) {
-  sm[(s + 0) * ME_SM_STRIDE] = g.a; sm[(s + 1) * ME_SM_STRIDE] = g.b; sm[(s + 2) * ME_SM_STRIDE] = g.c; sm[(s + 3) * ME_SM_STRIDE] = g.wp; sm[(s + 4) * ME_SM_STRIDE] = g.wm;
+template <typename R> ME_DEV GluonBasis<R> ldgb(const R* p) { GluonBasis<R> g; ld5<R>(p, g.ax, g.ay, g.az, g.bx, g.by); return g; }
+template <typename R> ME_DEV void stgb(R* p, const GluonBasis<R>& g) { st5<R>(p, g.ax, g.ay, g.az, g.bx, g.by); }
+template <typename R> ME_DEV SpinorBasis<R> ldsb(const R* p) { SpinorBasis<R> g; ld5<R>(p, g.a, g.b, g.c, g.wp, g.wm); return g; }
+template <typename R> ME_DEV void stsb(R* p, const SpinorBasis<R>& g) { st5<R>(p, g.a, g.b, g.c, g.wp, g.wm); }
+// slot-index forms (static slot numbers)
+template <typename R> ME_DEV W4<R> ldw(const R* sm, int s) { return ldw<R>(sm + ME_EO(s)); }
+template <typename R> ME_DEV void stw(R* sm, int s, const W4<R>& w) { stw<R>(sm + ME_EO(s), w); }
+template <typename R> ME_DEV P4<R> ldp(const R* sm, int s) { return ldp<R>(sm + ME_EO(s)); }
+template <typename R> ME_DEV void stp(R* sm, int s, const P4<R>& v) { stp<R>(sm + ME_EO(s), v); }
+template <typename R> ME_DEV GluonBasis<R> ldgb(const R* sm, int s) { return ldgb<R>(sm + ME_EO(s)); }
+template <typename R> ME_DEV void stgb(R* sm, int s, const GluonBasis<R>& g) { stgb<R>(sm + ME_EO(s), g); }
+template <typename R> ME_DEV SpinorBasis<R> ldsb(const R* sm, int s) { return ldsb<R>(sm + ME_EO(s)); }
+template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) { stsb<R>(sm + ME_EO(s), g); }
+// complex accumulator in a slot pair: one vector load, one vector store
+template <typename R> ME_DEV void cacc(R* p, R dre, R dim) {
+  typedef typename Pair2<R>::T R2;
+  R2* q = reinterpret_cast<R2*>(p);
+  R2 v = *q; v.x += dre; v.y += dim; *q = v;
 }
 }  // namespace me
 
@@ -315,14 +354,11 @@ template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) {
 // per-instance table of shared-memory offsets, two-sided quark line, dual currents.
 // ------------------------------------------------------------------------------------
 namespace me {
-template <typename R> ME_DEV W4<R> ldw(const R* p) { return ldw<R>(p, 0); }
-template <typename R> ME_DEV void stw(R* p, const W4<R>& w) { stw<R>(p, 0, w); }
-template <typename R> ME_DEV P4<R> ldp(const R* p) { return ldp<R>(p, 0); }
 template <typename R> ME_DEV Cx<R> cxs(const Cx<R>& c, R s) { return {c.re * s, c.im * s}; }
 template <typename R> ME_DEV R lam_of(int h, int bit) { return ((h >> bit) & 1) ? (R)1 : (R)-1; }
 // polarisation from a basis whose b part is pre-signed (+ for outgoing eps*, - for incoming eps)
 template <typename R> ME_DEV W4<R> gluon_pol_s(const R* p, R lam) {
-  const GluonBasis<R> g = ldgb<R>(p, 0);
+  const GluonBasis<R> g = ldgb<R>(p);
   return {(R)0, (R)0, -lam * g.ax, g.bx, -lam * g.ay, g.by, -lam * g.az, (R)0};
 }
 // column current grown from the t~ end: chi' = (q-slash + m) X * iden  (X = V-slash chi already formed)
