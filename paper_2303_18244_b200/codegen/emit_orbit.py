@@ -26,7 +26,8 @@ N = 4
 NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
-UNROLL = dict(pairs=2, q1=2, chi1=2, triples=1, rows2=1, q1_pair_chi=4, pair_pair=3, pair_v4=2)
+UNROLL = dict(pairs=2, q1=2, chi1=2, triples=1, rows2=1, q1_pair_chi=4, pair_pair=3, pair_v4=2)      # FP64 (255 registers, 4 warps/SM)
+UNROLL32 = dict(pairs=3, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=6, pair_pair=3, pair_v4=3)    # FP32 (8 warps/SM, registers to spare)
 
 
 def lam_bit(label, npar=NPAR):
@@ -427,10 +428,10 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * ncol, lay.J))
+    S("    for (int s = 0; s < %d; ++s) cset<R>(sm + ME_EO(%d + 2 * s), (R)0, (R)0);" % (ncol, lay.J))
     for gname, tmpl, rows in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
-        S("#pragma unroll %d" % UNROLL.get(gname, 1))
+        S("#pragma unroll(sizeof(R) == 8 ? %d : %d)" % (UNROLL.get(gname, 1), UNROLL32.get(gname, 1)))
         S("    for (int it = 0; it < %d; ++it) {" % len(rows))
         S("      const int* tb = tab_%s_%s[it];" % (name, gname))
         for l in tmpl.lines:
@@ -442,7 +443,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    }")
     S("    RC cr[%d], ci[%d];" % (ncol, ncol))
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) { cr[s] = (RC)sm[ME_EO(%d + 2 * s)]; ci[s] = (RC)sm[ME_EO(%d + 2 * s) + 1]; }" % (ncol, lay.J, lay.J))
+    S("    for (int s = 0; s < %d; ++s) { R jr, ji; cget<R>(sm + ME_EO(%d + 2 * s), jr, ji); cr[s] = (RC)jr; ci[s] = (RC)ji; }" % (ncol, lay.J))
     for l in cs_lines:
         S("    " + l)
     S("    const double meh = (double)cs;")

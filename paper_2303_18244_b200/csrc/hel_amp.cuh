@@ -341,6 +341,14 @@ template <typename R> ME_DEV GluonBasis<R> ldgb(const R* sm, int s) { return ldg
 template <typename R> ME_DEV void stgb(R* sm, int s, const GluonBasis<R>& g) { stgb<R>(sm + ME_EO(s), g); }
 template <typename R> ME_DEV SpinorBasis<R> ldsb(const R* sm, int s) { return ldsb<R>(sm + ME_EO(s)); }
 template <typename R> ME_DEV void stsb(R* sm, int s, const SpinorBasis<R>& g) { stsb<R>(sm + ME_EO(s), g); }
+template <typename R> ME_DEV void cset(R* p, R re, R im) {
+  typedef typename Pair2<R>::T R2;
+  R2 v; v.x = re; v.y = im; *reinterpret_cast<R2*>(p) = v;
+}
+template <typename R> ME_DEV void cget(const R* p, R& re, R& im) {
+  typedef typename Pair2<R>::T R2;
+  const R2 v = *reinterpret_cast<const R2*>(p); re = v.x; im = v.y;
+}
 // complex accumulator in a slot pair: one vector load, one vector store
 template <typename R> ME_DEV void cacc(R* p, R dre, R dim) {
   typedef typename Pair2<R>::T R2;
