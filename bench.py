@@ -235,6 +235,12 @@ def main():
     a32 = flops_alg * n / (results[cfg["name"]]["fp32"]["ms_per_step"] * 1e-3) * 1e-12
     roofline["fp32"] = {"achieved": a32, "peak": PEAK_TFLOPS["fp32"], "frac": a32 / PEAK_TFLOPS["fp32"],
                         "peak_measured_fma_chain": peak_meas["fp32"], "frac_of_measured": a32 / peak_meas["fp32"]}
+    # optional exact symmetry (include/me.h ME_OPT_PARITY_PAIRING): half the helicities, same number; NOT the headline
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
+    t, pp = timed(ctx, mom, n, me.ME_FP64, args.steps, args.warmup)
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
+    launches += args.steps * info.nkernels * ((ngood // 2 + 15) // 16 if HL == 4 else 1)
+    results[cfg["name"]]["fp64_parity_pairing"] = {"MEs_per_s": n / (statistics.mean(pp) * 1e-3), "ms_per_step": statistics.mean(pp)}
     # ------------------------------------------------------------------ end to end: HOST buffers through the public call
     host = mom.cpu().pin_memory()
     e2e_ms, _ = timed(ctx, mom, n, me.ME_FP64, args.steps, 1, host=host)

@@ -96,6 +96,14 @@ me_status me_get_info(const me_ctx* ctx, me_info* out);
 me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
                                uint64_t mask_out[2], int* ngood_out, void* stream);
 
+/* Options (default 0 = off).
+ * ME_OPT_PARITY_PAIRING: for the pure-QCD processes |M_h|^2 = |M_{~h}|^2 where ~h flips
+ * every helicity (parity invariance, tree level, real momenta), so me_compute evaluates one helicity of every good
+ * pair and counts it twice: half the work, same number up to rounding (~1e-14).  Ignored for e+ e- -> mu+ mu- and
+ * whenever the installed mask is not closed under h -> ~h.  me_compute_helicities is unaffected. */
+typedef enum { ME_OPT_PARITY_PAIRING = 0 } me_option;
+me_status me_set_option(me_ctx* ctx, me_option option, int value);
+
 /* Install a helicity mask without filtering (e.g. one returned by an earlier context). */
 me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
 

@@ -14,10 +14,11 @@ LIB_PATH = os.path.join(_PKG, "libme_b200.so")
 ME_OK, ME_EINVAL, ME_EPROCESS, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA = range(7)
 ME_EPEM_MUPMUM, ME_GG_TTX, ME_GG_TTXG, ME_GG_TTXGG, ME_GG_TTXGGG = range(5)
 ME_FP64, ME_MIXED, ME_FP32 = range(3)
+ME_OPT_PARITY_PAIRING = 0
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
 EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute",
-           "me_compute_helicities", "me_compute_jamps", "me_color_matrix", "me_philox_uniform", "me_rambo",
+           "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_color_matrix", "me_philox_uniform", "me_rambo",
            "me_fma_peak", "me_strerror")
 
 
@@ -54,6 +55,7 @@ def lib():
         L.me_get_info.argtypes = [vp, ctypes.POINTER(me_info)]
         L.me_filter_helicities.argtypes = [vp, vp, i64, ctypes.POINTER(u64), ctypes.POINTER(cint), vp]
         L.me_set_helicities.argtypes = [vp, ctypes.POINTER(u64)]
+        L.me_set_option.argtypes = [vp, cint, cint]
         L.me_compute.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_helicities.argtypes = [vp, vp, i64, cint, vp, vp, vp]
         L.me_compute_jamps.argtypes = [vp, vp, i64, cint, vp, vp]
@@ -162,6 +164,9 @@ class MEContext:
     def me_set_helicities(self, mask):
         m = (ctypes.c_uint64 * 2)(mask & ((1 << 64) - 1), mask >> 64)
         _check(lib().me_set_helicities(self._h, m))
+
+    def me_set_option(self, option, value):
+        _check(lib().me_set_option(self._h, int(option), int(value)))
 
     def me_compute(self, momenta, n, precision=ME_FP64, out=None, stream=None):
         import torch

@@ -21,6 +21,9 @@ struct me_ctx {
   unsigned char* d_hels_all;     // [ncomb] 0..ncomb-1
   unsigned char* d_hels_good;    // [ngood]
   int ngood;
+  unsigned char* d_hels_half;    // parity pairing: one helicity of every good pair {h, ~h}
+  int nhalf;                     // 0 = pairing not applicable to the current mask
+  bool pairing;                  // option ME_OPT_PARITY_PAIRING
   uint64_t mask[2];
   bool filtered;
   void* scratch; size_t scratch_bytes;
@@ -62,7 +65,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
   me_ctx* c = new (std::nothrow) me_ctx();
   if (c == nullptr) return ME_ENOMEM;
   c->process = process; c->prm = *prm; c->filtered = false; c->ngood = 0; c->mask[0] = c->mask[1] = 0;
-  c->scratch = nullptr; c->scratch_bytes = 0; c->d_hels_all = c->d_hels_good = nullptr;
+  c->scratch = nullptr; c->scratch_bytes = 0; c->d_hels_all = c->d_hels_good = c->d_hels_half = nullptr; c->nhalf = 0; c->pairing = false;
   me_info& I = c->info; memset(&I, 0, sizeof(I));
   I.page = ME_PAGE; I.ninitial = 2;
   const double PI = 3.14159265358979323846;
@@ -93,11 +96,12 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
   cudaError_t e = cudaGetDevice(&c->device);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_hels_all, 128);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_hels_good, 128);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_hels_half, 128);
   if (e == cudaSuccess) {
     unsigned char all[128]; for (int i = 0; i < 128; ++i) all[i] = (unsigned char)i;
     e = cudaMemcpy(c->d_hels_all, all, 128, cudaMemcpyHostToDevice);
   }
-  if (e != cudaSuccess) { cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); delete c; return cuda_fail(e, "me_create"); }
+  if (e != cudaSuccess) { cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); cudaFree(c->d_hels_half); delete c; return cuda_fail(e, "me_create"); }
   *out = c;
   return ME_OK;
 }
@@ -105,7 +109,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
 extern "C" me_status me_destroy(me_ctx* c) {
   if (c == nullptr) return ME_EINVAL;
   cudaDeviceSynchronize();
-  cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); cudaFree(c->scratch);
+  cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); cudaFree(c->d_hels_half); cudaFree(c->scratch);
   delete c;
   return ME_OK;
 }
@@ -156,7 +160,31 @@ extern "C" me_status me_set_helicities(me_ctx* c, const uint64_t mask[2]) {
   if (ng == 0) return ME_EINVAL;
   ME_CUDA(cudaMemcpy(c->d_hels_good, good, ng, cudaMemcpyHostToDevice), "me_set_helicities");
   c->ngood = ng; c->mask[0] = mask[0]; c->mask[1] = c->info.ncomb > 64 ? mask[1] : 0; c->filtered = true;
+  // parity pairing (pure-QCD processes): ME_h = ME_{~h}, ~h = all helicities flipped.  Usable only if the mask is
+  // closed under h -> ~h; then the helicities with particle 0 at -1 represent every pair.
+  c->nhalf = 0;
+  if (c->tab != nullptr) {
+    const int full = c->info.ncomb - 1, top = c->info.ncomb >> 1;
+    unsigned char half[64]; int nh = 0; bool closed = true;
+    for (int i = 0; i < ng && closed; ++i) {
+      const int h = good[i], hb = full ^ h;
+      if (!(mask[hb >> 6] >> (hb & 63) & 1)) closed = false;
+      else if (!(h & top)) half[nh++] = (unsigned char)h;
+    }
+    if (closed && 2 * nh == ng) {
+      ME_CUDA(cudaMemcpy(c->d_hels_half, half, nh, cudaMemcpyHostToDevice), "me_set_helicities");
+      c->nhalf = nh;
+    }
+  }
   return ME_OK;
+}
+
+extern "C" me_status me_set_option(me_ctx* c, me_option opt, int value) {
+  if (c == nullptr) return ME_EINVAL;
+  switch (opt) {
+    case ME_OPT_PARITY_PAIRING: c->pairing = value != 0; return ME_OK;
+  }
+  return ME_EINVAL;
 }
 
 extern "C" me_status me_filter_helicities(me_ctx* c, const double* d_mom, int64_t n, uint64_t mask_out[2], int* ngood_out, void* stream) {
@@ -194,6 +222,13 @@ extern "C" me_status me_compute(me_ctx* c, const double* d_mom, int64_t n, me_pr
   if (n == 0) return ME_OK;
   if (d_mom == nullptr || d_me == nullptr) return ME_EINVAL;
   if (!c->filtered) return ME_ENOTFILTERED;
+  if (c->pairing && c->nhalf > 0) {           // half the helicities, each counted twice
+    const double keep = c->inv_avg;
+    c->inv_avg = 2.0 * keep;
+    const me_status st = run(c, d_mom, n, prec, c->d_hels_half, c->nhalf, d_me, nullptr, nullptr, stream);
+    c->inv_avg = keep;
+    return st;
+  }
   return run(c, d_mom, n, prec, c->d_hels_good, c->ngood, d_me, nullptr, nullptr, stream);
 }
 

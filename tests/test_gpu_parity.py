@@ -282,3 +282,33 @@ def test_full_size_sampled_parity_and_properties(me, orc, proc):
         print("%s: MC sigma = %.6e +- %.1e GeV^-2, closed form %.6e" % (cfg["name"], sigma, err, target))
         assert abs(sigma - target) < 4 * err
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- option: parity pairing
+@pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
+def test_parity_pairing_option(me, orc, proc):
+    """|M_h|^2 = |M_{~h}|^2 for the pure-QCD processes; with the option on, me_compute evaluates half the good
+    helicities and must reproduce the full sum (and the oracle) to rounding.  No-op for e+ e- -> mu+ mu-."""
+    cfg = inputs.CONFIGS[proc]
+    n = 150 if proc == 4 else 400
+    ctx = me.MEContext(proc)
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    ctx.me_filter_helicities(mom, 32)
+    full = ctx.me_compute(mom, n).cpu().numpy()
+    if proc > 0:
+        _, mh = ctx.me_compute_helicities(mom, n)
+        mh = mh.cpu().numpy()
+        flipped = mh[::-1]                                   # ~h = ncomb-1-h
+        assert (np.abs(mh - flipped) / mh.max(axis=0)).max() < 1e-10
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
+    for name, tol in (("fp64", 1e-12), ("mixed", 1e-6), ("fp32", 1e-4)):
+        paired = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
+        assert np.abs(paired / full - 1).max() < tol
+    if proc == 0:
+        assert np.array_equal(ctx.me_compute(mom, n).cpu().numpy(), full)
+    p = to_aos(mom, n, cfg)
+    ref_ld = orc.me(proc, p[:100], long_double=True)
+    check_fp64(ctx.me_compute(mom, n).cpu().numpy()[:100], ref_ld, p[:100], cfg["name"] + " parity-paired")
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
+    assert np.array_equal(ctx.me_compute(mom, n).cpu().numpy(), full)
+    ctx.close()
