@@ -108,6 +108,7 @@ class Inst:
         self.params, self.lines, self.flops, self.namp = [], [], 0, 0
         self.jamp_codes = []
         self.pending = []          # (sigma, code, amp) waiting for flush_jamps()
+        self.zcount = 0
 
     def P(self, v):
         self.params.append(int(v))
@@ -161,20 +162,52 @@ class Inst:
             self.jamp_codes.append(code)
             self.pending.append((perm_index[st], code, amp))
 
-    def flush_jamps(self):
-        """one shared-memory read-modify-write per colour flow touched since the last flush: amplitudes that
-        feed the same flow are combined in registers first"""
+    # ---- jamp updates.  code: 0 -> +1, 1 -> -1, 2 -> +i, 3 -> -i
+    _MUL = {(0, 0): 0, (0, 1): 1, (0, 2): 2, (0, 3): 3, (1, 0): 1, (1, 1): 0, (1, 2): 3, (1, 3): 2,
+            (2, 0): 2, (2, 1): 3, (2, 2): 1, (2, 3): 0, (3, 0): 3, (3, 1): 2, (3, 2): 0, (3, 3): 1}
+    _INV = {0: 0, 1: 1, 2: 3, 3: 2}
+
+    def grouped_updates(self):
+        """pending (sigma, code, amp) -> [(sigma, unit code u, name of combination z)] with J_sigma += u * z; every
+        distinct combination z = sum_k c_k a_k (up to a unit factor) is formed ONCE in registers"""
         order, by = [], {}
         for sigma, code, amp in self.pending:
             if sigma not in by:
                 by[sigma] = []; order.append(sigma)
             by[sigma].append((code, amp))
-        for sigma in order:
-            re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
-            im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
-            self.L("cacc<R>(sm + %s, %s, %s);" % (self.off(self.lay.J + 2 * sigma), sum_expr(re), sum_expr(im)))
-            self.flops += 2 * len(by[sigma])
         self.pending = []
+        combos, out = {}, []
+        for sigma in order:
+            L = by[sigma]
+            u = L[0][0]
+            key = tuple((self._MUL[(self._INV[u], c)], a) for c, a in L)
+            if len(key) == 1:
+                out.append((sigma, u, key[0][1]))
+                continue
+            if key not in combos:
+                name = "z%d_%d" % (self.zcount, len(combos))
+                re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in key)
+                im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in key)
+                self.L("const Cx<R> %s = {%s, %s};" % (name, sum_expr(re), sum_expr(im)))
+                self.flops += 2 * (len(key) - 1)
+                combos[key] = name
+            out.append((sigma, u, combos[key]))
+        self.zcount += 1
+        return out
+
+    @staticmethod
+    def unit_times(u, z):
+        """(re, im) expressions of u * z"""
+        return {0: ("%s.re" % z, "%s.im" % z), 1: ("-%s.re" % z, "-%s.im" % z),
+                2: ("-%s.im" % z, "%s.re" % z), 3: ("%s.im" % z, "-%s.re" % z)}[u]
+
+    def flush_jamps(self):
+        """one shared-memory read-modify-write (a single 128-bit load and store) per colour flow touched since the
+        last flush; amplitudes that feed the same flow are combined in registers first"""
+        for sigma, u, z in self.grouped_updates():
+            re, im = self.unit_times(u, z)
+            self.L("cacc<R>(sm + %s, %s, %s);" % (self.off(self.lay.J + 2 * sigma), re, im))
+            self.flops += 2
 
 
 # colour polynomials (phases folded in, see topology.py): strings are tuples of gluon labels

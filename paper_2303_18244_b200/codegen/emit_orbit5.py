@@ -81,19 +81,12 @@ class Inst5(Inst):
             self.scopes[-1].add(name)
 
     def flush_jamps(self):
-        order, by = [], {}
-        for sigma, code, amp in self.pending:
-            if sigma not in by:
-                by[sigma] = []; order.append(sigma)
-            by[sigma].append((code, amp))
-        for sigma in order:
+        for sigma, u, z in self.grouped_updates():
             loc = self.local.setdefault(sigma, len(self.local))
             assert loc < self.lay.jacc, "local jamp accumulators exhausted"
-            re = "".join({0: " + %s.re", 1: " - %s.re", 2: " - %s.im", 3: " + %s.im"}[c] % a for c, a in by[sigma])
-            im = "".join({0: " + %s.im", 1: " - %s.im", 2: " + %s.re", 3: " - %s.re"}[c] % a for c, a in by[sigma])
-            self.L("cacc<R>(sm + %d, %s, %s);" % (eo(self.lay.J + 2 * loc, self.stride), sum_expr(re), sum_expr(im)))
-            self.flops += 2 * len(by[sigma])
-        self.pending = []
+            re, im = self.unit_times(u, z)
+            self.L("cacc<R>(sm + %d, %s, %s);" % (eo(self.lay.J + 2 * loc, self.stride), re, im))
+            self.flops += 2
 
     def flush_global(self):
         """add the local accumulators into gj and clear them.  The add is a fire-and-forget reduction (RED.ADD, no
