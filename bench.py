@@ -128,6 +128,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true", help="headline workload only (no other processes, no oracle leg)")
     ap.add_argument("--events", type=int, default=0, help="override events per GPU (default: the config's)")
+    ap.add_argument("--sweep", action="store_true", help="add throughput vs batch size (8192 .. config size) and 1/2/4 concurrent streams "
+                                                         "to the JSON line (PAPER.md line 65 / Fig. 1: plateau and GPU sharing)")
     ap.add_argument("--config", type=int, default=HEADLINE, choices=[1, 2, 3, 4],
                     help="index into inputs.CONFIGS of the timed workload (default 3 = g g -> t t~ g g, the BASELINE.json metric; "
                          "others are for profiling a single process, e.g. --quick --config 4)")
@@ -241,6 +243,35 @@ def main():
     ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
     launches += args.steps * info.nkernels * ((ngood // 2 + 15) // 16 if HL == 4 else 1)
     results[cfg["name"]]["fp64_parity_pairing"] = {"MEs_per_s": n / (statistics.mean(pp) * 1e-3), "ms_per_step": statistics.mean(pp)}
+    if args.sweep and world == 1:
+        sweep = {"batch": {}, "streams": {}}
+        nb = 8192
+        while nb <= n:
+            t, pp = timed(ctx, mom, nb, me.ME_FP64, 5, 2)
+            sweep["batch"][str(nb)] = nb / (min(pp) * 1e-3)
+            nb *= 2
+        # several streams sharing the GPU, each computing its own slice of the batch (the paper shares a V100 between processes)
+        for ns in (1, 2, 4, 8):
+            for nb in (8192, 32768):
+                if ns * nb > n:
+                    continue
+                streams = [torch.cuda.Stream() for _ in range(ns)]
+                ppages = ctx.momenta_numel(nb)
+                outs = [torch.empty(nb, dtype=torch.float64, device="cuda") for _ in range(ns)]
+                torch.cuda.synchronize()
+                best = 1e30
+                for rep in range(4):
+                    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    for k, st in enumerate(streams):
+                        st.wait_event(e0)
+                        ctx.me_compute(mom[k * ppages:(k + 1) * ppages], nb, me.ME_FP64, out=outs[k], stream=st)
+                    for st in streams:
+                        torch.cuda.current_stream().wait_stream(st)
+                    e1.record(); e1.synchronize()
+                    best = min(best, e0.elapsed_time(e1))
+                sweep["streams"]["%dx%d" % (ns, nb)] = ns * nb / (best * 1e-3)
+        results["sweep_fp64_MEs_per_s"] = sweep
     # ------------------------------------------------------------------ end to end: HOST buffers through the public call
     host = mom.cpu().pin_memory()
     e2e_ms, _ = timed(ctx, mom, n, me.ME_FP64, args.steps, 1, host=host)
