@@ -272,6 +272,13 @@ def main():
                     best = min(best, e0.elapsed_time(e1))
                 sweep["streams"]["%dx%d" % (ns, nb)] = ns * nb / (best * 1e-3)
         results["sweep_fp64_MEs_per_s"] = sweep
+        # helicity / leading-colour selection: per-helicity pass + per-event-helicity jamp pass, all in lockstep
+        ns = min(n, 131072)
+        ctx.me_select_helicity_color(mom, ns, seed=1)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        ctx.me_select_helicity_color(mom, ns, seed=1)
+        torch.cuda.synchronize()
+        results["select_helicity_color_events_per_s"] = ns / (time.perf_counter() - t0)
     # ------------------------------------------------------------------ end to end: HOST buffers through the public call
     host = mom.cpu().pin_memory()
     e2e_ms, _ = timed(ctx, mom, n, me.ME_FP64, args.steps, 1, host=host)

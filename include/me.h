@@ -128,6 +128,17 @@ me_status me_compute(me_ctx* ctx, const double* d_momenta, int64_t n, me_precisi
 me_status me_compute_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
                                 me_precision precision, double* d_me, double* d_me_hel, void* stream);
 
+/* Event-by-event random choice of a helicity and a leading-colour flow (section 5; SURVEY.md
+ * section 8(f) item 2).  Per event two uniforms come from Philox4x32-10 with key = seed and counter
+ * (event lo32, event hi32, 0x53454C45, 0), event = first_event + row: u1 = u53(w0,w1), u2 = u53(w2,w3) (mapping of
+ * me_philox_uniform).  d_ihel[e] = helicity index drawn with probability ME_h / sum_h ME_h over the installed good
+ * helicities; d_icol[e] = colour-flow index drawn with probability |J_s|^2 / sum_s |J_s|^2 at that helicity; both by
+ * inverse CDF in index order with FP64 left-to-right sums (first k with cum_k >= u * total).  FP64 throughout; every
+ * kernel stays in lockstep (the helicity enters as data).  d_ihel, d_icol: DEVICE int32 [n].  Allocates and frees a
+ * temporary buffer and synchronises `stream`.  Errors as me_compute. */
+me_status me_select_helicity_color(me_ctx* ctx, const double* d_momenta, int64_t n, uint64_t seed, uint64_t first_event,
+                                   int32_t* d_ihel, int32_t* d_icol, void* stream);
+
 /* Colour-flow amplitudes of one helicity (test hook for step a6): d_jamp is DEVICE FP64
  * [ncolor][2][n] (re, im), in units where the overall factor g_s^(npar-2) and a global
  * phase are stripped; QCD processes only. */

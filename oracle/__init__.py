@@ -98,6 +98,20 @@ def helicity_mask(me_hel, threshold=1e-12):
     return mask
 
 
+def select(process, p, seed, first_event, mask, params=DEFAULT_PARAMS):
+    """helicity / leading-colour choice per event (me_oracle.cpp orc_select) -> (ihel[n], icol[n]) int32"""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    n = p.shape[0]
+    prm = np.asarray(params, dtype=np.float64)
+    m = (ctypes.c_uint64 * 2)(mask & ((1 << 64) - 1), mask >> 64)
+    ihel = np.zeros(n, dtype=np.int32); icol = np.zeros(n, dtype=np.int32)
+    rc = lib().orc_select(int(process), _dp(prm), _dp(p), ctypes.c_long(n), ctypes.c_uint64(seed), ctypes.c_uint64(first_event), m,
+                          ihel.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), icol.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+    if rc:
+        raise ValueError("orc_select failed")
+    return ihel, icol
+
+
 def jamps(process, p_event, ihel, params=DEFAULT_PARAMS):
     p_event = np.ascontiguousarray(p_event, dtype=np.float64)
     nc = info(process)["ncol"]

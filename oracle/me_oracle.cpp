@@ -657,6 +657,51 @@ int orc_jamps(int process, const double* params, const double* p, int ihel, doub
   return 0;
 }
 
+// Event-by-event helicity / leading-colour choice (rule stated in include/me.h
+// me_select_helicity_color and DESIGN.md "Selection"): u1,u2 from Philox counter (event lo, event hi, 'SELE', 0);
+// inverse CDF in index order over ME_h of the good helicities, then over |J_s|^2 at the chosen helicity.
+static int orc_inverse_cdf(const std::vector<double>& w, double u) {
+  double tot = 0; for (double x : w) tot += x;
+  const double target = u * tot;
+  double cum = 0; int sel = -1, lastpos = 0;
+  for (size_t k = 0; k < w.size(); ++k) {
+    cum += w[k];
+    if (w[k] > 0) lastpos = (int)k;
+    if (sel < 0 && w[k] > 0 && cum >= target) sel = (int)k;
+  }
+  return sel < 0 ? lastpos : sel;
+}
+int orc_select(int process, const double* params, const double* p, long n, uint64_t seed, uint64_t first_event,
+               const uint64_t* mask, int* ihel, int* icol) {
+  orc::ProcInfo pi; if (!orc::proc_info(process, pi)) return 1;
+  orc::Params prm; std::memcpy(&prm, params, sizeof(prm));
+  if (process != 0) orc::topology(pi.nglu);
+  const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 4)
+#endif
+  for (long e = 0; e < n; ++e) {
+    const double* pe = p + (size_t)e * pi.npar * 4;
+    std::vector<double> mh(pi.ncomb); double tot;
+    orc::me_event<double>(process, prm, pe, -1, mh.data(), &tot);
+    for (int h = 0; h < pi.ncomb; ++h) if (!(mask[h >> 6] >> (h & 63) & 1)) mh[h] = 0;
+    const uint64_t ev = first_event + (uint64_t)e;
+    const uint32_t ctr[4] = {(uint32_t)ev, (uint32_t)(ev >> 32), 0x53454C45u, 0u};
+    uint32_t w[4]; orc::philox4x32_10(ctr, key, w);
+    const double u1 = orc::u53(w[0], w[1]), u2 = orc::u53(w[2], w[3]);
+    ihel[e] = orc_inverse_cdf(mh, u1);
+    if (process == 0) { icol[e] = 0; continue; }
+    const orc::Topology& T = orc::topology(pi.nglu);
+    orc::P4<double> pp[8]; int hel[8];
+    for (int k = 0; k < pi.npar; ++k) { for (int i = 0; i < 4; ++i) pp[k].c[i] = pe[4 * k + i]; hel[k] = (ihel[e] >> (pi.npar - 1 - k) & 1) ? 1 : -1; }
+    std::vector<orc::Cx<double>> J; orc::qcd_jamps<double>(T, prm, pp, hel, -1, J);
+    std::vector<double> wj(T.ncol);
+    for (int a = 0; a < T.ncol; ++a) wj[a] = std::norm(J[a]);
+    icol[e] = orc_inverse_cdf(wj, u2);
+  }
+  return 0;
+}
+
 int orc_max_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -18,7 +18,7 @@ ME_OPT_PARITY_PAIRING = 0
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
 EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute",
-           "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_color_matrix", "me_philox_uniform", "me_rambo",
+           "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_select_helicity_color", "me_color_matrix", "me_philox_uniform", "me_rambo",
            "me_fma_peak", "me_strerror")
 
 
@@ -56,6 +56,7 @@ def lib():
         L.me_filter_helicities.argtypes = [vp, vp, i64, ctypes.POINTER(u64), ctypes.POINTER(cint), vp]
         L.me_set_helicities.argtypes = [vp, ctypes.POINTER(u64)]
         L.me_set_option.argtypes = [vp, cint, cint]
+        L.me_select_helicity_color.argtypes = [vp, vp, i64, u64, u64, vp, vp, vp]
         L.me_compute.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_helicities.argtypes = [vp, vp, i64, cint, vp, vp, vp]
         L.me_compute_jamps.argtypes = [vp, vp, i64, cint, vp, vp]
@@ -183,6 +184,14 @@ class MEContext:
         mh = torch.empty((self.info.ncomb, n), dtype=torch.float64, device=momenta.device)
         _check(lib().me_compute_helicities(self._h, _ptr(momenta, torch.float64), n, int(precision), _ptr(me), _ptr(mh), _stream(stream)))
         return me, mh
+
+    def me_select_helicity_color(self, momenta, n, seed, first_event=0, stream=None):
+        """-> (ihel int32 [n], icol int32 [n]) (include/me.h me_select_helicity_color)"""
+        import torch
+        ihel = torch.empty(n, dtype=torch.int32, device=momenta.device)
+        icol = torch.empty(n, dtype=torch.int32, device=momenta.device)
+        _check(lib().me_select_helicity_color(self._h, _ptr(momenta, torch.float64), n, seed, first_event, _ptr(ihel), _ptr(icol), _stream(stream)))
+        return ihel, icol
 
     def me_compute_jamps(self, momenta, n, ihel, stream=None):
         import torch

@@ -259,7 +259,8 @@ def emit_single_kernel_process(n, name):
     S("#define JI(s) Ji[s]")
     S("template <typename R, typename RC>")
     S("__global__ void __launch_bounds__(ME_BLOCK) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
-      " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out) {" % name)
+      " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out,"
+      " const int* __restrict__ helpe) {" % name)
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
     S("  const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % npar)
@@ -269,7 +270,7 @@ def emit_single_kernel_process(n, name):
     src.extend(pro)
     S("  double acc = 0;")
     S("  for (int ih = 0; ih < nhel; ++ih) {")
-    S("    const int h = hels[ih];")
+    S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
     for k in range(npar):
         S("    const R lam%d = ((h >> %d) & 1) ? (R)1 : (R)-1;" % (k, npar - 1 - k))
     S("    const W4<R> ub = spinor_ubar(sbt, lam2);")
@@ -298,7 +299,7 @@ def emit_single_kernel_process(n, name):
     per_hel = K.flops + cs_flops + 2 * FLOPS["spinor"]
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + ME_BLOCK - 1) / ME_BLOCK);")
-    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out")
+    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event")
     S("  if (precision == 0) k_%s<double, double><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)
     S("  else if (precision == 1) k_%s<double, float><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)
     S("  else k_%s<float, float><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)

@@ -408,7 +408,8 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         S("};")
     S("template <typename R, typename RC>")
     S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
-      " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out) {" % (block, name))
+      " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out,"
+      " const int* __restrict__ helpe) {" % (block, name))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
@@ -456,7 +457,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  }")
     S("  double acc = 0;")
     S("  for (int ih = 0; ih < nhel; ++ih) {")
-    S("    const int h = hels[ih];")
+    S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
     S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
     S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
@@ -488,7 +489,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
     S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d;" % (lay.nslots, block, lay.nslots, block))
-    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out")
+    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event")
     S("  if (precision == 0) {")
     S("    cudaFuncSetAttribute(k_%s<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);" % name)
     S("    k_%s<double, double><<<grid, %d, smd, a.stream>>>(ME_ARGS);" % (name, block))

@@ -523,7 +523,7 @@ def emit_kernel(name, ki, lay, groups):
         S("};")
     S("template <typename R, typename RJ>")
     S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
-      " double mt_d, RJ* __restrict__ gjbase) {" % (BLOCK, name, ki))
+      " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n) {" % (BLOCK, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
@@ -540,7 +540,7 @@ def emit_kernel(name, ki, lay, groups):
     S("#pragma unroll")
     S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
     S("  for (int hc = 0; hc < nh; ++hc) {")
-    S("    const int h = hels[hc];")
+    S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
     if lay.FERM is not None:
         S("    {")
@@ -567,11 +567,11 @@ def emit_kernel(name, ki, lay, groups):
     S("  if (precision == 2) {")
     S("    const size_t smb = sizeof(float) * %d * %d;" % (lay.nslots, BLOCK))
     S("    cudaFuncSetAttribute(k_%s_o%d<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<float, float><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj);" % (name, ki, BLOCK))
+    S("    k_%s_o%d<float, float><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
     S("  } else {")
     S("    const size_t smb = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK))
     S("    cudaFuncSetAttribute(k_%s_o%d<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<double, double><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj);" % (name, ki, BLOCK))
+    S("    k_%s_o%d<double, double><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
     S("  }")
     S("  return cudaGetLastError();")
     S("}")

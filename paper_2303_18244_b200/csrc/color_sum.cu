@@ -95,7 +95,7 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
   const unsigned cgrid = (unsigned)(a.npad / 32);
   for (int base = 0; base < a.nhel; base += ME_HEL_CHUNK) {
     const int nh = a.nhel - base < ME_HEL_CHUNK ? a.nhel - base : ME_HEL_CHUNK;
-    MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream};
+    MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream, a.hel_per_event, a.n};
     {   // every diagram kernel ADDS its colour flows into the staging buffer
       const size_t esz = precision == 2 ? sizeof(float) : sizeof(double);
       cudaError_t e = cudaMemsetAsync(a.scratch, 0, (size_t)nh * ncol * 2 * a.npad * esz, a.stream);

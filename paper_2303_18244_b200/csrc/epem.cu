@@ -12,7 +12,7 @@ const double epem_flops_per_helicity = 4 * 8 + 4 * 72 + 16 + 2 * 30 + 20;
 template <typename R>
 __global__ void __launch_bounds__(ME_BLOCK) k_epem(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels,
                                                    int nhel, double gL_d, double gR_d, double mz, double wz, double norm_hel, double inv_avg,
-                                                   double* __restrict__ me_out, double* __restrict__ me_hel) {
+                                                   double* __restrict__ me_out, double* __restrict__ me_hel, const int* __restrict__ helpe) {
   const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= npad) return;
   const double* pm = mom + (e >> 5) * (4 * 4 * 32) + (e & 31);
@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(ME_BLOCK) k_epem(const double* __restrict__ mo
   for (int k = 0; k < 4; ++k) sb[k] = spinor_basis(pcast<R>(pd[k]), (R)0);
   double acc = 0;
   for (int ih = 0; ih < nhel; ++ih) {
-    const int h = hels[ih];
+    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];
     const R l0 = (h & 8) ? (R)1 : (R)-1, l1 = (h & 4) ? (R)1 : (R)-1, l2 = (h & 2) ? (R)1 : (R)-1, l3 = (h & 1) ? (R)1 : (R)-1;
     const W4<R> vb = dirac_bar(spinor_v(sb[0], l0));   // incoming e+
     const W4<R> u = spinor_u(sb[1], l1);               // incoming e-
@@ -58,9 +58,9 @@ __global__ void __launch_bounds__(ME_BLOCK) k_epem(const double* __restrict__ mo
 cudaError_t launch_epem(int precision, const LaunchArgs& a, const EpemCouplings& c) {
   const int grid = (int)((a.npad + ME_BLOCK - 1) / ME_BLOCK);
   if (precision == 2)
-    k_epem<float><<<grid, ME_BLOCK, 0, a.stream>>>(a.mom, a.n, a.npad, a.hels, a.nhel, c.gL, c.gR, c.mz, c.wz, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+    k_epem<float><<<grid, ME_BLOCK, 0, a.stream>>>(a.mom, a.n, a.npad, a.hels, a.nhel, c.gL, c.gR, c.mz, c.wz, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.hel_per_event);
   else
-    k_epem<double><<<grid, ME_BLOCK, 0, a.stream>>>(a.mom, a.n, a.npad, a.hels, a.nhel, c.gL, c.gR, c.mz, c.wz, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+    k_epem<double><<<grid, ME_BLOCK, 0, a.stream>>>(a.mom, a.n, a.npad, a.hels, a.nhel, c.gL, c.gR, c.mz, c.wz, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.hel_per_event);
   return cudaGetLastError();
 }
 

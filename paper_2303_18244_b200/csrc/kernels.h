@@ -15,6 +15,7 @@ struct LaunchArgs {
   long n, npad;               // events, events rounded up to a whole page
   const unsigned char* hels;  // device list of helicity indices to evaluate
   int nhel;
+  const int* hel_per_event;    // device [n] or null: if set, every event evaluates ITS OWN single helicity (nhel must be 1)
   double mt;                  // quark mass (QCD) — unused for e+e-
   double norm_hel;            // per-helicity normalisation (couplings, colour denominator)
   double inv_avg;             // 1 / averaging denominator
@@ -48,5 +49,7 @@ cudaError_t launch_philox(uint64_t seed, uint64_t first_event, long n, int per_e
 cudaError_t launch_rambo(int nfinal, const double* masses /*host, nfinal*/, double sqrt_s, const double* d_rnd, long n,
                          double* d_mom, double* d_wt, cudaStream_t s);
 cudaError_t run_fma_peak(int fp64, double* tflops);
+cudaError_t launch_select_hel(const double* me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* ihel, cudaStream_t s);
+cudaError_t launch_select_col(double* jamp, int ncol, long n, uint64_t seed, uint64_t first_event, int* icol, cudaStream_t s);
 
 }  // namespace me

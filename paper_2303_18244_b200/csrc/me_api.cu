@@ -128,14 +128,14 @@ extern "C" me_status me_color_matrix(const me_ctx* c, double* out) {
 }
 
 static me_status run(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, const unsigned char* hels, int nhel,
-                     double* d_me, double* d_me_hel, double* d_jamp, void* stream) {
+                     double* d_me, double* d_me_hel, double* d_jamp, void* stream, const int* hel_per_event = nullptr) {
   if ((int)prec < 0 || (int)prec > 2) return ME_EINVAL;
   if (((uintptr_t)d_mom & 15) || ((uintptr_t)d_me & 7) || ((uintptr_t)d_me_hel & 7)) return ME_EALIGN;
   me::LaunchArgs a;
   a.mom = d_mom; a.n = n; a.npad = (n + ME_PAGE - 1) / ME_PAGE * ME_PAGE; a.hels = hels; a.nhel = nhel;
   a.mt = c->prm.mt; a.norm_hel = c->norm_hel; a.inv_avg = c->inv_avg;
   a.me_out = d_me; a.me_hel = d_me_hel; a.jamp_out = d_jamp; a.stream = (cudaStream_t)stream;
-  a.scratch = nullptr; a.scratch_bytes = 0;
+  a.scratch = nullptr; a.scratch_bytes = 0; a.hel_per_event = hel_per_event;
   if (c->tab != nullptr && c->tab->scratch_bytes != nullptr) {
     const size_t need = c->tab->scratch_bytes((int)prec, a.npad);
     if (need > c->scratch_bytes) {
@@ -244,6 +244,38 @@ extern "C" me_status me_compute_jamps(me_ctx* c, const double* d_mom, int64_t n,
   if (c->tab == nullptr || ihel < 0 || ihel >= c->info.ncomb) return ME_EINVAL;
   if (n == 0) return ME_OK;
   return run(c, d_mom, n, ME_FP64, c->d_hels_all + ihel, 1, nullptr, nullptr, d_jamp, stream);
+}
+
+extern "C" me_status me_select_helicity_color(me_ctx* c, const double* d_mom, int64_t n, uint64_t seed, uint64_t first_event,
+                                              int32_t* d_ihel, int32_t* d_icol, void* stream) {
+  if (c == nullptr || n < 0) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  if (d_mom == nullptr || d_ihel == nullptr || d_icol == nullptr) return ME_EINVAL;
+  if (!c->filtered) return ME_ENOTFILTERED;
+  const int nc = c->info.ncomb, ncol = c->info.ncolor;
+  cudaStream_t st = (cudaStream_t)stream;
+  double* buf = nullptr;
+  const size_t words = (size_t)n * (nc > 2 * ncol ? nc : 2 * ncol);
+  cudaError_t e = cudaMalloc(&buf, sizeof(double) * words);
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return ME_ENOMEM; }
+  ME_CUDA(e, "select alloc");
+  me_status ms = ME_OK;
+  e = cudaMemsetAsync(buf, 0, sizeof(double) * (size_t)nc * n, st);                      // masked helicities weigh 0
+  if (e == cudaSuccess) ms = run(c, d_mom, n, ME_FP64, c->d_hels_good, c->ngood, nullptr, buf, nullptr, stream);
+  if (e == cudaSuccess && ms == ME_OK) e = me::launch_select_hel(buf, nc, n, seed, first_event, d_ihel, st);
+  if (e == cudaSuccess && ms == ME_OK) {
+    if (c->tab == nullptr) e = cudaMemsetAsync(d_icol, 0, sizeof(int32_t) * n, st);       // one colour structure
+    else {
+      ms = run(c, d_mom, n, ME_FP64, c->d_hels_all, 1, nullptr, nullptr, buf, stream, d_ihel);   // jamps of each event's own helicity
+      if (ms == ME_OK) e = me::launch_select_col(buf, ncol, n, seed, first_event, d_icol, st);
+    }
+  }
+  cudaError_t e2 = cudaStreamSynchronize(st);
+  cudaFree(buf);
+  if (ms != ME_OK) return ms;
+  if (e != cudaSuccess) return cuda_fail(e, "me_select_helicity_color");
+  if (e2 != cudaSuccess) return cuda_fail(e2, "me_select_helicity_color");
+  return ME_OK;
 }
 
 extern "C" me_status me_philox_uniform(uint64_t seed, uint64_t first_event, int64_t n, int per_event, double* d_rnd, void* stream) {

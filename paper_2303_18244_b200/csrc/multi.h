@@ -12,6 +12,7 @@ namespace me {
 
 struct MultiArgs {
   const double* mom; long npad; const unsigned char* hels; int nh; double mt; void* gj; cudaStream_t stream;
+  const int* hel_per_event; long n;
 };
 struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); };
 

@@ -46,6 +46,55 @@ cudaError_t launch_philox(uint64_t seed, uint64_t first_event, long n, int per_e
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------- helicity / colour selection
+// PAPER.md line 138 (section 5): "event-by-event random choice of leading colour and helicity".  Reading (DESIGN.md
+// "Selection"): two uniforms per event from Philox counter (event lo, event hi, 'SELE', 0); helicity h drawn with
+// probability ME_h / sum ME_h over the good helicities, colour flow s with probability |J_s(h)|^2 / sum |J|^2; inverse
+// CDF in index order, FP64, left-to-right sums: pick the first k with cum_k >= u * total.
+#define ME_SELECT_TAG 0x53454C45u
+__device__ __forceinline__ void select_uniforms(uint64_t seed, uint64_t ev, double& u1, double& u2) {
+  uint32_t w[4];
+  philox4x32_10((uint32_t)ev, (uint32_t)(ev >> 32), ME_SELECT_TAG, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+  u1 = u53(w[0], w[1]); u2 = u53(w[2], w[3]);
+}
+__device__ __forceinline__ int inverse_cdf(const double* __restrict__ w, int m, long stride, double u) {
+  double tot = 0;
+  for (int k = 0; k < m; ++k) tot += w[k * stride];
+  const double target = u * tot;
+  double cum = 0; int sel = -1, lastpos = 0;
+  for (int k = 0; k < m; ++k) {
+    const double x = w[k * stride];
+    cum += x;
+    if (x > 0) lastpos = k;
+    if (sel < 0 && x > 0 && cum >= target) sel = k;
+  }
+  return sel < 0 ? lastpos : sel;
+}
+__global__ void k_select_hel(const double* __restrict__ me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* __restrict__ ihel) {
+  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  double u1, u2; select_uniforms(seed, first_event + (uint64_t)e, u1, u2);
+  ihel[e] = inverse_cdf(me_hel + e, ncomb, n, u1);
+}
+__global__ void k_select_col(double* __restrict__ jamp, int ncol, long n, uint64_t seed, uint64_t first_event, int* __restrict__ icol) {
+  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  double u1, u2; select_uniforms(seed, first_event + (uint64_t)e, u1, u2);
+  for (int s = 0; s < ncol; ++s) {          // |J_s|^2 in place (re slot)
+    const double re = jamp[(2 * s) * n + e], im = jamp[(2 * s + 1) * n + e];
+    jamp[(2 * s) * n + e] = re * re + im * im;
+  }
+  icol[e] = inverse_cdf(jamp + e, ncol, 2 * n, u2);
+}
+cudaError_t launch_select_hel(const double* me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* ihel, cudaStream_t s) {
+  k_select_hel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(me_hel, ncomb, n, seed, first_event, ihel);
+  return cudaGetLastError();
+}
+cudaError_t launch_select_col(double* jamp, int ncol, long n, uint64_t seed, uint64_t first_event, int* icol, cudaStream_t s) {
+  k_select_col<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(jamp, ncol, n, seed, first_event, icol);
+  return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------- RAMBO
 struct RamboMasses { double m[6]; };
 

@@ -111,7 +111,8 @@ def test_generated_flop_counts_are_recorded(melib):
     import json
     s = json.load(open(os.path.join(ROOT, "paper_2303_18244_b200", "csrc", "generated", "gen_summary.json")))
     assert s["gg_ttxgg"]["ndiagrams"] == 123 and s["gg_ttxggg"]["ndiagrams"] == 1240
-    assert 2e4 < s["gg_ttxgg"]["flops_per_helicity"] < 6e4      # SURVEY §8(d) estimate 27-42 k + colour
+    # SURVEY §8(d) estimated 27-42 k + colour for the plain recursion; the two-sided scheme needs ~20 k
+    assert 1.5e4 < s["gg_ttxgg"]["flops_per_helicity"] < 6e4
 
 
 # ------------------------------------------------------------------ host logic
