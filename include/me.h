@@ -139,6 +139,18 @@ me_status me_compute_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
 me_status me_select_helicity_color(me_ctx* ctx, const double* d_momenta, int64_t n, uint64_t seed, uint64_t first_event,
                                    int32_t* d_ihel, int32_t* d_icol, void* stream);
 
+/* Device-side cross-section sums and hit-or-miss unweighting ("hit-or-miss unweighting,
+ * cross-section", line 45 the idea of offloading them).
+ *   w_i = flux * d_weight[i] * d_me[i]   (flux = 1/(2 s) for a fixed-energy collision; d_weight from me_rambo)
+ *   sums_out (HOST) = { sum_i w_i, sum_i w_i^2, max_i w_i }: sigma = sums[0]/n, its standard error from sums[1]
+ *   d_accept[i] (DEVICE uint8 [n], nullable) = 1 iff u_i * wmax < w_i, with u_i = u53 of Philox4x32-10 at counter
+ *   (event lo32, event hi32, 0x554E5754, 0), key = seed, event = first_event + i; wmax <= 0 selects the batch maximum;
+ *   *naccept_out = number of accepted events.
+ * Reductions are fixed-order trees without atomics (bit-identical run to run).  Allocates temporaries and
+ * synchronises `stream`.  Errors: ME_EINVAL (n < 1, null, flux <= 0), ME_ENOMEM, ME_ECUDA. */
+me_status me_unweight(const double* d_weight, const double* d_me, int64_t n, double flux, uint64_t seed, uint64_t first_event,
+                      double wmax, double sums_out[3], uint8_t* d_accept, int64_t* naccept_out, void* stream);
+
 /* Colour-flow amplitudes of one helicity (test hook for step a6): d_jamp is DEVICE FP64
  * [ncolor][2][n] (re, im), in units where the overall factor g_s^(npar-2) and a global
  * phase are stripped; QCD processes only. */

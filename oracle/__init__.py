@@ -112,6 +112,18 @@ def select(process, p, seed, first_event, mask, params=DEFAULT_PARAMS):
     return ihel, icol
 
 
+def unweight(weight, me_values, flux, seed, first_event=0, wmax=0.0):
+    """Cross-section sums and hit-or-miss unweighting, the plain definition (include/me.h me_unweight):
+    w = flux * W * ME; returns (sum w, sum w^2, max w, accept[n] bool) with accept_i = u_i * wmax < w_i."""
+    import math
+    w = flux * np.asarray(weight, dtype=np.float64) * np.asarray(me_values, dtype=np.float64)
+    n = w.shape[0]
+    u = np.zeros(n)
+    lib().orc_tagged_uniform(ctypes.c_uint64(seed), ctypes.c_uint64(first_event), ctypes.c_long(n), ctypes.c_uint32(0x554E5754), _dp(u))
+    wm = float(w.max()) if wmax <= 0 else float(wmax)
+    return math.fsum(w), math.fsum(w * w), float(w.max()), (u * wm < w)
+
+
 def jamps(process, p_event, ihel, params=DEFAULT_PARAMS):
     p_event = np.ascontiguousarray(p_event, dtype=np.float64)
     nc = info(process)["ncol"]

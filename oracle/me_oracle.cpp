@@ -702,6 +702,18 @@ int orc_select(int process, const double* params, const double* p, long n, uint6
   return 0;
 }
 
+// first uniform of Philox counter (event lo, event hi, tag, 0), key = seed: the per-event random number of the
+// unweighting step (tag 'UNWT', include/me.h me_unweight)
+void orc_tagged_uniform(uint64_t seed, uint64_t first_event, long n, uint32_t tag, double* out) {
+  const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  for (long e = 0; e < n; ++e) {
+    const uint64_t ev = first_event + (uint64_t)e;
+    const uint32_t ctr[4] = {(uint32_t)ev, (uint32_t)(ev >> 32), tag, 0u};
+    uint32_t w[4]; orc::philox4x32_10(ctr, key, w);
+    out[e] = orc::u53(w[0], w[1]);
+  }
+}
+
 int orc_max_threads() {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -18,7 +18,7 @@ ME_OPT_PARITY_PAIRING = 0
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
 EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute",
-           "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_select_helicity_color", "me_color_matrix", "me_philox_uniform", "me_rambo",
+           "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_select_helicity_color", "me_unweight", "me_color_matrix", "me_philox_uniform", "me_rambo",
            "me_fma_peak", "me_strerror")
 
 
@@ -57,6 +57,7 @@ def lib():
         L.me_set_helicities.argtypes = [vp, ctypes.POINTER(u64)]
         L.me_set_option.argtypes = [vp, cint, cint]
         L.me_select_helicity_color.argtypes = [vp, vp, i64, u64, u64, vp, vp, vp]
+        L.me_unweight.argtypes = [vp, vp, i64, dbl, u64, u64, dbl, ctypes.POINTER(dbl), vp, ctypes.POINTER(i64), vp]
         L.me_compute.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_helicities.argtypes = [vp, vp, i64, cint, vp, vp, vp]
         L.me_compute_jamps.argtypes = [vp, vp, i64, cint, vp, vp]
@@ -104,6 +105,18 @@ def me_philox_uniform(seed, first_event, n, per_event, device="cuda", stream=Non
     out = torch.empty((n, per_event, 4), dtype=torch.float64, device=device)
     _check(lib().me_philox_uniform(seed, first_event, n, per_event, _ptr(out), _stream(stream)))
     return out
+
+
+def me_unweight(weight, me_values, flux, seed, first_event=0, wmax=0.0, want_accept=True, stream=None):
+    """-> (sum w, sum w^2, max w, accept uint8 [n] or None, n accepted)  (include/me.h me_unweight)"""
+    import torch
+    n = me_values.numel()
+    sums = (ctypes.c_double * 3)()
+    na = ctypes.c_int64(0)
+    acc = torch.empty(n, dtype=torch.uint8, device=me_values.device) if want_accept else None
+    _check(lib().me_unweight(_ptr(weight, torch.float64), _ptr(me_values, torch.float64), n, float(flux), seed, first_event, float(wmax),
+                             sums, _ptr(acc), ctypes.byref(na), _stream(stream)))
+    return sums[0], sums[1], sums[2], acc, na.value
 
 
 def me_fma_peak(fp64):

@@ -49,6 +49,8 @@ cudaError_t launch_philox(uint64_t seed, uint64_t first_event, long n, int per_e
 cudaError_t launch_rambo(int nfinal, const double* masses /*host, nfinal*/, double sqrt_s, const double* d_rnd, long n,
                          double* d_mom, double* d_wt, cudaStream_t s);
 cudaError_t run_fma_peak(int fp64, double* tflops);
+cudaError_t run_unweight(const double* d_wt, const double* d_me, long n, double flux, uint64_t seed, uint64_t first_event, double wmax_in,
+                         double sums[3], unsigned char* d_accept, long long* naccept, cudaStream_t st);
 cudaError_t launch_select_hel(const double* me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* ihel, cudaStream_t s);
 cudaError_t launch_select_col(double* jamp, int ncol, long n, uint64_t seed, uint64_t first_event, int* icol, cudaStream_t s);
 

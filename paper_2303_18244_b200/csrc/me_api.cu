@@ -278,6 +278,17 @@ extern "C" me_status me_select_helicity_color(me_ctx* c, const double* d_mom, in
   return ME_OK;
 }
 
+extern "C" me_status me_unweight(const double* d_weight, const double* d_me, int64_t n, double flux, uint64_t seed, uint64_t first_event,
+                                 double wmax, double sums_out[3], uint8_t* d_accept, int64_t* naccept_out, void* stream) {
+  if (n < 1 || d_weight == nullptr || d_me == nullptr || sums_out == nullptr || !(flux > 0)) return ME_EINVAL;
+  long long na = 0;
+  cudaError_t e = me::run_unweight(d_weight, d_me, n, flux, seed, first_event, wmax, sums_out, d_accept, &na, (cudaStream_t)stream);
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return ME_ENOMEM; }
+  if (e != cudaSuccess) return cuda_fail(e, "me_unweight");
+  if (naccept_out != nullptr) *naccept_out = na;
+  return ME_OK;
+}
+
 extern "C" me_status me_philox_uniform(uint64_t seed, uint64_t first_event, int64_t n, int per_event, double* d_rnd, void* stream) {
   if (n < 0 || per_event < 1 || (n > 0 && d_rnd == nullptr)) return ME_EINVAL;
   if ((uintptr_t)d_rnd & 15) return ME_EALIGN;

@@ -95,6 +95,88 @@ cudaError_t launch_select_col(double* jamp, int ncol, long n, uint64_t seed, uin
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------- cross section + unweighting
+// PAPER.md line 24 (section 2): "hit-or-miss unweighting, cross-section"; line 45: idea of offloading it.  Reading (DESIGN.md
+// "Unweighting"): w_i = flux * W_i * ME_i; sigma = mean w; event i is kept iff u_i * wmax < w_i with u_i from Philox counter
+// (event lo, event hi, 'UNWT', 0).  Reductions are fixed-order trees (no atomics): bit-identical run to run.
+#define ME_UNWT_TAG 0x554E5754u
+#define ME_RED_THREADS 256
+__device__ __forceinline__ void block_reduce3(double& s, double& q, double& m, double* sh) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s += __shfl_down_sync(0xffffffffu, s, o); q += __shfl_down_sync(0xffffffffu, q, o);
+    m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+  }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { sh[3 * w] = s; sh[3 * w + 1] = q; sh[3 * w + 2] = m; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < ME_RED_THREADS / 32; ++k) { s += sh[3 * k]; q += sh[3 * k + 1]; m = fmax(m, sh[3 * k + 2]); }
+  }
+}
+__global__ void __launch_bounds__(ME_RED_THREADS) k_weight_partials(const double* __restrict__ wt, const double* __restrict__ me_, long n,
+                                                                    double flux, double* __restrict__ w_out, double* __restrict__ part) {
+  __shared__ double sh[3 * ME_RED_THREADS / 32];
+  const long e = (long)blockIdx.x * ME_RED_THREADS + threadIdx.x;
+  double w = 0;
+  if (e < n) { w = flux * wt[e] * me_[e]; w_out[e] = w; }
+  double s = w, q = w * w, m = w;
+  block_reduce3(s, q, m, sh);
+  if (threadIdx.x == 0) { part[3 * blockIdx.x] = s; part[3 * blockIdx.x + 1] = q; part[3 * blockIdx.x + 2] = m; }
+}
+__global__ void __launch_bounds__(ME_RED_THREADS) k_weight_final(const double* __restrict__ part, long nblocks, double* __restrict__ out) {
+  __shared__ double sh[3 * ME_RED_THREADS / 32];
+  double s = 0, q = 0, m = 0;
+  for (long b = threadIdx.x; b < nblocks; b += ME_RED_THREADS) { s += part[3 * b]; q += part[3 * b + 1]; m = fmax(m, part[3 * b + 2]); }
+  block_reduce3(s, q, m, sh);
+  if (threadIdx.x == 0) { out[0] = s; out[1] = q; out[2] = m; }
+}
+__global__ void __launch_bounds__(ME_RED_THREADS) k_accept(const double* __restrict__ w, long n, double wmax, uint64_t seed, uint64_t first_event,
+                                                           unsigned char* __restrict__ accept, unsigned long long* __restrict__ part) {
+  __shared__ int sh[ME_RED_THREADS / 32];
+  const long e = (long)blockIdx.x * ME_RED_THREADS + threadIdx.x;
+  int a = 0;
+  if (e < n) {
+    const uint64_t ev = first_event + (uint64_t)e;
+    uint32_t r[4];
+    philox4x32_10((uint32_t)ev, (uint32_t)(ev >> 32), ME_UNWT_TAG, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), r);
+    a = u53(r[0], r[1]) * wmax < w[e] ? 1 : 0;
+    accept[e] = (unsigned char)a;
+  }
+  const unsigned b = __ballot_sync(0xffffffffu, a);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = __popc(b);
+  __syncthreads();
+  if (threadIdx.x == 0) { int c = 0; for (int k = 0; k < ME_RED_THREADS / 32; ++k) c += sh[k]; part[blockIdx.x] = (unsigned long long)c; }
+}
+cudaError_t run_unweight(const double* d_wt, const double* d_me, long n, double flux, uint64_t seed, uint64_t first_event, double wmax_in,
+                         double sums[3], unsigned char* d_accept, long long* naccept, cudaStream_t st) {
+  const long nb = (n + ME_RED_THREADS - 1) / ME_RED_THREADS;
+  double *d_w = nullptr, *d_part = nullptr, *d_out = nullptr; unsigned long long* d_cnt = nullptr;
+  cudaError_t e = cudaMalloc(&d_w, sizeof(double) * n);
+  if (e == cudaSuccess) e = cudaMalloc(&d_part, sizeof(double) * 3 * nb);
+  if (e == cudaSuccess) e = cudaMalloc(&d_out, sizeof(double) * 3);
+  if (e == cudaSuccess) e = cudaMalloc(&d_cnt, sizeof(unsigned long long) * nb);
+  if (e == cudaSuccess) {
+    k_weight_partials<<<(unsigned)nb, ME_RED_THREADS, 0, st>>>(d_wt, d_me, n, flux, d_w, d_part);
+    k_weight_final<<<1, ME_RED_THREADS, 0, st>>>(d_part, nb, d_out);
+    e = cudaMemcpyAsync(sums, d_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  if (e == cudaSuccess && d_accept != nullptr) {
+    const double wmax = wmax_in > 0 ? wmax_in : sums[2];
+    k_accept<<<(unsigned)nb, ME_RED_THREADS, 0, st>>>(d_w, n, wmax, seed, first_event, d_accept, d_cnt);
+    unsigned long long* h = new unsigned long long[nb];
+    e = cudaMemcpyAsync(h, d_cnt, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    long long c = 0; for (long b = 0; b < nb; ++b) c += (long long)h[b];
+    delete[] h;
+    if (naccept != nullptr) *naccept = c;
+  }
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d_w); cudaFree(d_part); cudaFree(d_out); cudaFree(d_cnt);
+  return e;
+}
+
 // ---------------------------------------------------------------------------------- RAMBO
 struct RamboMasses { double m[6]; };
 

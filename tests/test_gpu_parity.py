@@ -344,3 +344,34 @@ def test_select_helicity_color_matches_oracle(me, orc, proc):
     ih3, _ = ctx.me_select_helicity_color(mom, n, seed=7, first_event=first)
     assert not np.array_equal(ih3.cpu().numpy(), ihel)
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- cross section + unweighting
+@pytest.mark.parametrize("proc,n", [(0, 16384), (1, 50000), (3, 3001)])
+def test_unweight_matches_oracle(me, orc, proc, n):
+    """sums within rounding of the exactly rounded host sums; accept flags (bytes) equal the oracle's except where
+    u*wmax and w agree to 1e-9 (the oracle's w uses the oracle's ME, the GPU's the GPU's: they differ by ~1e-13)."""
+    cfg = inputs.CONFIGS[proc]
+    ctx = me.MEContext(proc)
+    rnd, mom, wt = gen_events(me, ctx, cfg, n)
+    ctx.me_filter_helicities(mom, 32)
+    me_dev = ctx.me_compute(mom, n)
+    flux = 1.0 / (2 * SQRT_S ** 2)
+    s1, s2, wmax, acc, nacc = me.me_unweight(wt, me_dev, flux, seed=31337, first_event=17)
+    acc = acc.cpu().numpy().astype(bool)
+    assert nacc == int(acc.sum())
+    p = to_aos(mom, n, cfg)
+    ref_me = orc.me(proc, p)
+    r1, r2, rmax, racc = orc.unweight(wt.cpu().numpy(), ref_me, flux, seed=31337, first_event=17)
+    assert abs(s1 / r1 - 1) < 1e-11 and abs(s2 / r2 - 1) < 1e-11 and abs(wmax / rmax - 1) < 1e-11
+    assert (acc != racc).sum() <= 1
+    # deterministic reductions: bit-identical on a second call
+    t1, t2, tmax, acc2, _ = me.me_unweight(wt, me_dev, flux, seed=31337, first_event=17)
+    assert (t1, t2, tmax) == (s1, s2, wmax) and np.array_equal(acc2.cpu().numpy().astype(bool), acc)
+    # fixed wmax: subset of the batch-max selection's uniforms scaled
+    _, _, _, acc3, n3 = me.me_unweight(wt, me_dev, flux, seed=31337, first_event=17, wmax=2 * wmax)
+    assert n3 <= nacc and not (acc3.cpu().numpy().astype(bool) & ~acc).any()
+    if proc in (0, 1):
+        sigma, err = s1 / n, math.sqrt(max(s2 / n - (s1 / n) ** 2, 0) / n)
+        assert abs(sigma - (SIGMA_EPEM if proc == 0 else SIGMA_GGTT)) < 4 * err
+    ctx.close()
