@@ -26,8 +26,8 @@ N = 4
 NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
-UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
-UNROLL32 = dict(pairs=3, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=6, pair_pair=3, pair_v4=3)    # FP32 (8 warps/SM, registers to spare)
+UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
+UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)    # FP32 (8 warps/SM, registers to spare)
 
 
 def lam_bit(label, npar=NPAR):
