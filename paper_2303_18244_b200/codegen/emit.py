@@ -6,9 +6,9 @@ Emitted structure, per kernel:
               dot products), gluon polarisation bases and spinor bases
   per helicity: external wavefunctions -> gluon sub-tree currents (by subset size) -> quark-line
               currents (by subset size) -> one amplitude per closure -> jamp accumulation
-  flush     : single-kernel processes: colour sum J^dagger C J in-register, helicity accumulate;
-              multi-kernel process (g g -> t t~ g g g): add the segment's jamps into the global
-              staging buffer consumed by the batched colour-sum kernel.
+  flush     : colour sum J^dagger C J in-register, helicity accumulate.
+Used for g g -> t t~ and g g -> t t~ g (everything fits the register file); the larger processes use the
+orbit-looped emitters emit_orbit.py / emit_orbit5.py, which import the flop table and the colour-sum emitter from here.
 
 Flop counting rule: add = mul = div = sqrt = 1, fma = 2, counted on the routines
 of csrc/hel_amp.cuh as written.
@@ -227,18 +227,6 @@ def colour_sum_lines(C, ncol, denom):
     return out, flops
 
 
-def algorithmic_flops(T):
-    """Single-pass count: every gluon term, quark term, Vslash.v product and amplitude exactly once, jamp adds,
-    triangular colour sum (ncol <= 24) or dense contraction (ncol = 120), external spinors."""
-    K = KernelEmitter(T)
-    K.emit_segment([c.id for c in T.Cl], {s: s for s in range(T.ncol)})
-    if T.ncol <= 24:
-        cs = colour_sum_lines(T.color_num, T.ncol, T.color_denom)[1]
-    else:
-        cs = 2 * (2 * T.ncol * T.ncol) + 4 * T.ncol
-    return K.flops + cs + 2 * FLOPS["spinor"]
-
-
 def emit_single_kernel_process(n, name):
     """g g -> t t~ + (n-2) g evaluated by ONE kernel (n = 2,3,4): jamps in registers/local, in-kernel colour sum."""
     T = Topology(n)
@@ -316,154 +304,3 @@ def emit_single_kernel_process(n, name):
                 n_gterms=len(K.done_g), n_qterms=len(K.done_q), color_num=T.color_num)
     return "\n".join(src) + "\n", info
 
-
-# ==========================================================================================
-# g g -> t t~ g g g: diagrams split across kernels (BASELINE.json north_star: "Register-pressure
-# control for the 1240-diagram case comes from splitting the diagrams across kernels"), jamps
-# staged in global memory and summed by the batched colour kernel (csrc/color_sum.cu).
-# ==========================================================================================
-JMAX = 48            # local jamp accumulators per segment (shared memory, [2*JMAX][ME_BLOCK])
-KERNEL_CLOSURES = 60
-
-
-def _chain_key(T, c):
-    """Gluon-subset masks along the quark line from the t end; bare-line closures are keyed by the top-level split."""
-    if c.q < 0:
-        g = T.G[c.g]
-        return (tuple(sorted(T.G[x].mask for x in g.ch)), (g.mask,))
-    ms = [T.G[c.g].mask]
-    q = c.q
-    while q >= 0:
-        ms.append(T.G[T.Q[q].g].mask)
-        q = T.Q[q].prev
-    return ((), tuple(reversed(ms)))
-
-
-def partition(T, jmax=None, kernel_closures=None):
-    """-> list of kernels, each a list of segments (closure ids, sorted support)."""
-    jmax = jmax or JMAX
-    kernel_closures = kernel_closures or KERNEL_CLOSURES
-    cl = sorted(T.Cl, key=lambda c: (_chain_key(T, c), c.q, c.g))
-    segs, cur, sup = [], [], set()
-    for c in cl:
-        s = set(j for j, _ in c.jamp)
-        if cur and (len(sup | s) > jmax or len(cur) >= kernel_closures):
-            segs.append((cur, sorted(sup))); cur, sup = [], set()
-        cur.append(c.id); sup |= s
-    segs.append((cur, sorted(sup)))
-    kernels, curk, cnt = [], [], 0
-    for sg in segs:
-        if curk and cnt + len(sg[0]) > kernel_closures:
-            kernels.append(curk); curk, cnt = [], 0
-        curk.append(sg); cnt += len(sg[0])
-    kernels.append(curk)
-    return kernels
-
-
-def emit_multi_kernel_process(n, name):
-    T = Topology(n)
-    kernels = partition(T)
-    npar = n + 2
-    files = {}
-    touched = set()
-    total_flops, total_namp, fixed_max = 0, 0, 0
-    kinfo = []
-    for ki, segs in enumerate(kernels):
-        K = KernelEmitter(T)
-        body = []
-        for (cids, sup) in segs:
-            jmap = {sigma: slot for slot, sigma in enumerate(sup)}
-            K.lines = []
-            K.emit_segment(cids, jmap)
-            body.extend(K.lines)
-            # flush this segment's jamps into the global staging buffer, then clear the slots
-            for sigma in sup:
-                op = "+=" if sigma in touched else "="
-                touched.add(sigma)
-                body.append("      gj[%dL * npad] %s (RJ)JR(%d); gj[%dL * npad] %s (RJ)JI(%d); JR(%d) = 0; JI(%d) = 0;"
-                            % (2 * sigma, op, jmap[sigma], 2 * sigma + 1, op, jmap[sigma], jmap[sigma], jmap[sigma]))
-                if op == "+=":
-                    K.flops += 2
-        pro = K.prologue()
-        src = []
-        S = src.append
-        S("// GENERATED by paper_2303_18244_b200/codegen — do not edit.  g g -> t t~ g g g, diagram kernel %d of %d:" % (ki, len(kernels)))
-        S("// %d amplitudes in %d segments; %d gluon terms, %d quark terms evaluated here." % (K.namp, len(segs), len(K.done_g), len(K.done_q)))
-        S("#include \"hel_amp.cuh\"")
-        S("#include \"kernels.h\"")
-        S("#include \"multi.h\"")
-        S("namespace me {")
-        S("#define JR(s) sj[(2 * (s)) * ME_BLOCK]")
-        S("#define JI(s) sj[(2 * (s) + 1) * ME_BLOCK]")
-        S("template <typename R, typename RJ>")
-        S("__global__ void __launch_bounds__(ME_BLOCK) k_%s_p%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels,"
-          " double mt_d, RJ* __restrict__ gjbase) {" % (name, ki))
-        S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
-        S("  R* sj = reinterpret_cast<R*>(smem_raw) + threadIdx.x;")
-        S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
-        S("  if (e >= npad) return;")
-        S("  const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % npar)
-        for k in range(npar):
-            S("  const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
-        S("  const R mt = (R)mt_d;")
-        src.extend(pro)
-        S("  {")
-        S("    const int h = hels[blockIdx.y];")
-        S("    RJ* gj = gjbase + (long)blockIdx.y * (%d * 2) * npad + e;" % T.ncol)
-        for k in range(npar):
-            S("    const R lam%d = ((h >> %d) & 1) ? (R)1 : (R)-1;" % (k, npar - 1 - k))
-        S("    const W4<R> ub = spinor_ubar(sbt, lam2);")
-        S("    const W4<R> vv = spinor_v(sbtb, lam3);")
-        S("#pragma unroll")
-        S("    for (int s = 0; s < %d; ++s) { JR(s) = 0; JI(s) = 0; }" % JMAX)
-        S("    {")
-        src.extend(body)
-        S("    }")
-        S("  }")
-        S("}")
-        S("static cudaError_t launch_p%d(int precision, const MultiArgs& a) {" % ki)
-        S("  const dim3 grid((unsigned)((a.npad + ME_BLOCK - 1) / ME_BLOCK), (unsigned)a.nh);")
-        S("  if (precision == 2) {")
-        S("    const size_t sm = sizeof(float) * 2 * %d * ME_BLOCK;" % JMAX)
-        S("    cudaFuncSetAttribute(k_%s_p%d<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);" % (name, ki))
-        S("    k_%s_p%d<float, float><<<grid, ME_BLOCK, sm, a.stream>>>(a.mom, a.npad, a.hels, a.mt, (float*)a.gj);" % (name, ki))
-        S("  } else {")
-        S("    const size_t sm = sizeof(double) * 2 * %d * ME_BLOCK;" % JMAX)
-        S("    cudaFuncSetAttribute(k_%s_p%d<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);" % (name, ki))
-        S("    k_%s_p%d<double, double><<<grid, ME_BLOCK, sm, a.stream>>>(a.mom, a.npad, a.hels, a.mt, (double*)a.gj);" % (name, ki))
-        S("  }")
-        S("  return cudaGetLastError();")
-        S("}")
-        S("extern const MultiKernel mk_%s_p%d = {launch_p%d};" % (name, ki, ki))
-        S("}  // namespace me")
-        files["gen_%s_p%d.cu" % (name, ki)] = "\n".join(src) + "\n"
-        total_flops += K.flops + 2 * FLOPS["spinor"]
-        total_namp += K.namp
-        fixed_max += K.fixed_flops
-        kinfo.append(dict(amplitudes=K.namp, segments=len(segs), gterms=len(K.done_g), qterms=len(K.done_q), flops=K.flops))
-    assert touched == set(range(T.ncol))
-    # colour sum as a dense contraction: 2 * ncol * (2 ncol) FMA-flops + 4 ncol for the final dot
-    cs_flops = 2 * (2 * T.ncol * T.ncol) + 4 * T.ncol
-    per_hel = total_flops + cs_flops
-    src = []
-    S = src.append
-    S("// GENERATED by paper_2303_18244_b200/codegen — do not edit.  g g -> t t~ g g g process table.")
-    S("#include \"kernels.h\"")
-    S("#include \"multi.h\"")
-    S("namespace me {")
-    for ki in range(len(kernels)):
-        S("extern const MultiKernel mk_%s_p%d;" % (name, ki))
-    S("static const MultiKernel* const parts_%s[%d] = {%s};" % (name, len(kernels), ", ".join("&mk_%s_p%d" % (name, ki) for ki in range(len(kernels)))))
-    S("static const double color_num_%s[%d] = {%s};" % (name, T.ncol * T.ncol, ", ".join(str(float(x)) for row in T.color_num for x in row)))
-    S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) { return launch_multi(precision, a, parts_%s, %d, %d, color_num_%s); }"
-      % (name, name, len(kernels), T.ncol, name))
-    S("static size_t scratch_%s(int precision, long npad) { return multi_scratch_bytes(precision, npad, %d); }" % (name, T.ncol))
-    algo = algorithmic_flops(T)
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s};"
-      % (name, n, T.ndiagrams, total_namp, T.ncol, T.color_denom, len(kernels) + 1, float(algo), float(algo), float(algo),
-         float(per_hel), float(per_hel), float(per_hel), float(fixed_max), name, name, name))
-    S("}  // namespace me")
-    files["gen_%s_table.cu" % name] = "\n".join(src) + "\n"
-    info = dict(n=n, ndiagrams=T.ndiagrams, namp=total_namp, ncol=T.ncol, color_denom=T.color_denom,
-                flops_per_helicity=algo, flops_executed_per_helicity=per_hel, fixed_flops=fixed_max, colour_flops=cs_flops, kernels=kinfo)
-    return files, info

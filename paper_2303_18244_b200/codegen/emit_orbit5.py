@@ -2,7 +2,8 @@
 120 colour flows.  Same ideas as emit_orbit.py (shapes looped over gluon relabellings with table-driven
 operands, two-sided quark line, bilinear / dual-current factorisations), plus what the size of the process forces:
 
-  * the diagrams are split across THREE kernels (north_star: "splitting the diagrams across kernels"), each small
+  * the diagrams are split across FIVE kernels (north_star: "splitting the diagrams across kernels"; three for the
+    three-gluon sub-trees, one for the 2+2 / 2+1 quark ends, one for four-gluon sub-trees made of pairs), each small
     enough to stay in the instruction cache; every kernel loops over the helicities of the current chunk;
   * the 120 jamps do not fit on chip: each block instance accumulates the <= 36 colour flows it touches in
     per-thread shared-memory slots and adds them once into the global staging buffer gj[hel][flow][re/im][event]
