@@ -99,8 +99,8 @@ def run_reference(args):
     oracle.build()
     cfg = inputs.CONFIGS[HEADLINE]
     cores = oracle.max_threads()
-    # bounded sample per step: the first 64*cores events of the seeded config (host Philox + RAMBO of the oracle)
-    nsample = 64 * cores
+    # bounded sample per step: the first 1024*cores events of the seeded config (host Philox + RAMBO of the oracle)
+    nsample = 1024 * cores
     p, _ = oracle.events(cfg["process"], nsample, cfg["seed"])
     for _ in range(args.warmup):
         oracle.me(cfg["process"], p[:8 * cores])
@@ -297,7 +297,7 @@ def main():
     }
     # ------------------------------------------------------------------ the oracle timed beside it (rank 0, N = 1)
     if rank == 0 and world == 1 and not args.quick:
-        nb = min(n, 262144)
+        nb = n
         p = inputs.aosoa_to_aos(mom[: ctx.momenta_numel(nb)].cpu().numpy(), nb, cfg["npar"], info.page)
         rate, cores, ns, dt = oracle_rate(cfg["process"], p)
         line["cpu_baseline"] = {"value": rate, "unit": "MEs/s", "cores": cores, "kind": "oracle",
