@@ -375,3 +375,21 @@ def test_unweight_matches_oracle(me, orc, proc, n):
         sigma, err = s1 / n, math.sqrt(max(s2 / n - (s1 / n) ** 2, 0) / n)
         assert abs(sigma - (SIGMA_EPEM if proc == 0 else SIGMA_GGTT)) < 4 * err
     ctx.close()
+
+
+@pytest.mark.parametrize("proc", [3, 4])
+def test_ragged_sizes_and_determinism_large_processes(me, proc):
+    """n = 1, a partial page, a partial CTA and a partial colour-sum tile reproduce the prefix of a larger batch bit for
+    bit, in every precision, and repeated calls are bit-identical (fixed reduction orders; the staging REDs of cfg 5 are
+    per-thread private)."""
+    cfg = inputs.CONFIGS[proc]
+    nmax = 200
+    ctx = me.MEContext(proc)
+    _, mom, _ = gen_events(me, ctx, cfg, nmax)
+    ctx.me_set_helicities(EXPECTED_MASK[proc])
+    for name in ("fp64", "mixed", "fp32"):
+        full = ctx.me_compute(mom, nmax, me.PRECISIONS[name]).cpu().numpy()
+        assert np.array_equal(ctx.me_compute(mom, nmax, me.PRECISIONS[name]).cpu().numpy(), full)
+        for n in (1, 31, 65, 129):
+            assert np.array_equal(ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy(), full[:n]), (name, n)
+    ctx.close()
