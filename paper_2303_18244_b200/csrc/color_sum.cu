@@ -25,7 +25,7 @@ template <> __device__ __forceinline__ float cmat<float>(int i) { return __ldg(&
 
 // RJ: staging type, RC: arithmetic type of the contraction
 template <typename RJ, typename RC>
-__global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restrict__ gj, long npad, long n, int nh,
+__global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restrict__ gj, long npad, long n, long hs, int nh,
                                                              const unsigned char* __restrict__ hels, int first,
                                                              double norm_hel, double inv_avg,
                                                              double* __restrict__ me_out, double* __restrict__ me_hel) {
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restric
 #pragma unroll
       for (int k = 0; k < CS_WARPS; ++k) s += red[k][lane];
       const double meh = (double)s;
-      if (me_hel != nullptr && e < n) me_hel[(long)hels[hc] * n + e] = meh * norm_hel * 0.5;
+      if (me_hel != nullptr && e < n) me_hel[(long)hels[hc] * hs + e] = meh * norm_hel * 0.5;
       acc += meh;
     }
   }
@@ -73,16 +73,40 @@ __global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restric
   }
 }
 
+// events are processed in slices so that the staging buffer stays bounded (3.8 GB in FP64) whatever n is
+#define ME_EVENT_SLICE 131072L
 size_t multi_scratch_bytes(int precision, long npad, int ncol) {
-  return (size_t)ME_HEL_CHUNK * ncol * 2 * npad * (precision == 2 ? sizeof(float) : sizeof(double));
+  const long np = npad < ME_EVENT_SLICE ? npad : ME_EVENT_SLICE;
+  return (size_t)ME_HEL_CHUNK * ncol * 2 * np * (precision == 2 ? sizeof(float) : sizeof(double));
 }
 
 static bool g_color_loaded = false;
 // FP64: tensor-core (DMMA) colour sum; ME_COLOR_FMA=1 in the environment selects the plain-FMA kernel (A/B timing)
 static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
 
+static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
+                                      const double* color_num_host);
+
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host) {
+  const int npar = 7;   // g g -> t t~ g g g
+  for (long start = 0; start < a.n; start += ME_EVENT_SLICE) {
+    LaunchArgs s = a;
+    s.n = a.n - start < ME_EVENT_SLICE ? a.n - start : ME_EVENT_SLICE;
+    s.npad = (s.n + ME_PAGE - 1) / ME_PAGE * ME_PAGE;
+    s.mom = a.mom + (start / ME_PAGE) * (npar * 4 * ME_PAGE);
+    if (a.me_out != nullptr) s.me_out = a.me_out + start;
+    if (a.me_hel != nullptr) s.me_hel = a.me_hel + start;
+    if (a.jamp_out != nullptr) s.jamp_out = a.jamp_out + start;
+    if (a.hel_per_event != nullptr) s.hel_per_event = a.hel_per_event + start;
+    cudaError_t e = launch_multi_slice(precision, s, a.n, parts, nparts, ncol, color_num_host);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
+                                      const double* color_num_host) {
   if (ncol != CS_NCOL) return cudaErrorInvalidValue;
   if (!g_color_loaded) {
     static float cf[CS_NCOL * CS_NCOL];
@@ -108,7 +132,7 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
     if (a.jamp_out != nullptr && base == 0) {
       const size_t esz = precision == 2 ? sizeof(float) : sizeof(double);
       if (esz != sizeof(double)) return cudaErrorInvalidValue;   // jamp hook is FP64 only
-      cudaError_t e = cudaMemcpy2DAsync(a.jamp_out, a.n * sizeof(double), a.scratch, a.npad * sizeof(double), a.n * sizeof(double),
+      cudaError_t e = cudaMemcpy2DAsync(a.jamp_out, hs * sizeof(double), a.scratch, a.npad * sizeof(double), a.n * sizeof(double),
                                         2 * ncol, cudaMemcpyDeviceToDevice, a.stream);
       if (e != cudaSuccess) return e;
     }
@@ -118,14 +142,14 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
     if (precision == 0 && g_use_dmma) {
       const double* cm = nullptr;
       cudaError_t e2 = cudaGetSymbolAddress((void**)&cm, c_color_d);
-      if (e2 == cudaSuccess) e2 = launch_color_sum_dmma(cm, (const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      if (e2 == cudaSuccess) e2 = launch_color_sum_dmma(cm, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
       if (e2 != cudaSuccess) return e2;
     } else if (precision == 0)
-      k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     else if (precision == 1)
-      k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const double*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     else
-      k_color_sum<float, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const float*)a.scratch, a.npad, a.n, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<float, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const float*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }

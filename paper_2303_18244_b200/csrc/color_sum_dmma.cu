@@ -24,7 +24,7 @@ __device__ __forceinline__ void dmma8x8x4(double& d0, double& d1, double a, doub
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-__global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const double* __restrict__ cmat, const double* __restrict__ gj, long npad, long n, int nh,
+__global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const double* __restrict__ cmat, const double* __restrict__ gj, long npad, long n, long hs, int nh,
                                                                     const unsigned char* __restrict__ hels, int first,
                                                                     double norm_hel, double inv_avg,
                                                                     double* __restrict__ me_out, double* __restrict__ me_hel) {
@@ -91,8 +91,8 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
       if (lane < 4) {
         const long e = e0 + 2 * lane;
         if (me_hel != nullptr) {
-          if (e < n) me_hel[(long)hels[hc] * n + e] = p0 * norm_hel * 0.5;
-          if (e + 1 < n) me_hel[(long)hels[hc] * n + e + 1] = p1 * norm_hel * 0.5;
+          if (e < n) me_hel[(long)hels[hc] * hs + e] = p0 * norm_hel * 0.5;
+          if (e + 1 < n) me_hel[(long)hels[hc] * hs + e + 1] = p1 * norm_hel * 0.5;
         }
         me_acc0 += p0; me_acc1 += p1;
       }
@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
   }
 }
 
-cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, int nh, const unsigned char* hels, int first,
+cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
                                   double norm_hel, double inv_avg, double* me_out, double* me_hel, cudaStream_t stream) {
   static int sms = 0;
   if (sms == 0) {
@@ -119,7 +119,7 @@ cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npa
   if (e != cudaSuccess) return e;
   const long ntiles = (npad + 8 * CD_WARPS - 1) / (8 * CD_WARPS);
   const unsigned grid = (unsigned)(ntiles < sms ? ntiles : sms);
-  k_color_sum_dmma<<<grid, 32 * CD_WARPS, smem, stream>>>(cmat, gj, npad, n, nh, hels, first, norm_hel, inv_avg, me_out, me_hel);
+  k_color_sum_dmma<<<grid, 32 * CD_WARPS, smem, stream>>>(cmat, gj, npad, n, hs, nh, hels, first, norm_hel, inv_avg, me_out, me_hel);
   return cudaGetLastError();
 }
 

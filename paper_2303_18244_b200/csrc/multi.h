@@ -20,7 +20,7 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
                          const double* color_num_host);
 size_t multi_scratch_bytes(int precision, long npad, int ncol);
 // FP64 colour sum on the tensor cores (color_sum_dmma.cu); cmat = device pointer to the [ncol*ncol] numerators
-cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, int nh, const unsigned char* hels, int first,
+cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
                                   double norm_hel, double inv_avg, double* me_out, double* me_hel, cudaStream_t stream);
 
 }  // namespace me

@@ -393,3 +393,20 @@ def test_ragged_sizes_and_determinism_large_processes(me, proc):
         for n in (1, 31, 65, 129):
             assert np.array_equal(ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy(), full[:n]), (name, n)
     ctx.close()
+
+
+def test_event_slicing_of_the_staged_pipeline(me):
+    """g g -> t t~ g g g processes more than 131072 events in slices (bounded staging buffer): one call over 140000 events
+    equals two calls on the two slices bit for bit."""
+    cfg = inputs.CONFIGS[4]
+    n, cut = 140000, 131072
+    ctx = me.MEContext(4)
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    ctx.me_set_helicities(EXPECTED_MASK[4])
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)             # half the helicities: keeps the test short
+    whole = ctx.me_compute(mom, n, me.ME_FP32).cpu().numpy()
+    head = ctx.me_compute(mom, cut, me.ME_FP32).cpu().numpy()
+    tail = ctx.me_compute(mom[ctx.momenta_numel(cut):], n - cut, me.ME_FP32).cpu().numpy()
+    assert np.array_equal(whole[:cut], head) and np.array_equal(whole[cut:], tail)
+    assert np.isfinite(whole).all() and (whole > 0).all()
+    ctx.close()
