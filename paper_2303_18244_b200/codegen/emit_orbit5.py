@@ -540,7 +540,8 @@ def emit_kernel(name, ki, lay, groups):
     S("  }")
     S("#pragma unroll")
     S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
-    S("  for (int hc = 0; hc < nh; ++hc) {")
+    S("  const int hc_end = (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
+    S("  for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
     if lay.FERM is not None:
@@ -564,7 +565,8 @@ def emit_kernel(name, ki, lay, groups):
     S("  }")
     S("}")
     S("static cudaError_t launch_o%d(int precision, const MultiArgs& a) {" % ki)
-    S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (BLOCK, BLOCK))
+    S("  // few helicities per CTA: many short CTAs, so the last partial wave costs little (65536 events are only 4.6 waves of 96-thread CTAs)")
+    S("  const dim3 grid((unsigned)((a.npad + %d - 1) / %d), (unsigned)((a.nh + ME_HEL_PER_CTA - 1) / ME_HEL_PER_CTA));" % (BLOCK, BLOCK))
     S("  if (precision == 2) {")
     S("    const size_t smb = sizeof(float) * %d * %d;" % (lay.nslots, BLOCK))
     S("    cudaFuncSetAttribute(k_%s_o%d<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))

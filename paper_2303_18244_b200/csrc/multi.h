@@ -7,6 +7,9 @@
 #include "kernels.h"
 
 #define ME_HEL_CHUNK 16   // helicities staged per pass
+#ifndef ME_HEL_PER_CTA
+#define ME_HEL_PER_CTA 2   // helicities looped inside one CTA of a diagram kernel (grid.y covers the chunk)
+#endif
 
 namespace me {
 
