@@ -181,3 +181,18 @@ def test_two_rank_gloo_sharding_reproduces_single_rank(orc):
     assert cnt == n
     assert np.array_equal(me_sharded, me_all)            # bit-identical: same events, same arithmetic
     assert abs(tot / float((w_all * me_all).sum()) - 1) < 1e-13
+
+
+def test_orbit_emitters_cover_every_diagram_term():
+    """the orbit-looped emitters enumerate shapes x relabellings on their own; their amplitude-term counts must equal the
+    closure counts of the generic diagram enumeration (159 for 4 gluons, 1890 for 5), their colour-flow count n!"""
+    from paper_2303_18244_b200.codegen import emit_orbit, emit_orbit5
+    from paper_2303_18244_b200.codegen.topology import Topology
+    _, info4 = emit_orbit.emit_orbit_process()
+    assert info4["namp"] == len(Topology(4).Cl) == 159 and info4["ncol"] == 24
+    assert sum(info4["shapes"].values()) == 6 + 4 + 4 + 4 + 6 + 12 + 3 + 6
+    _, info5 = emit_orbit5.emit_orbit5_process()
+    assert info5["namp"] == len(Topology(5).Cl) == 1890 and info5["ncol"] == 120
+    # shared-memory budgets: one 128-thread CTA (FP64) for cfg 4, 96-thread CTAs for cfg 5 must fit 227 KB
+    assert info4["smem_slots"] * 8 * 128 <= 227 * 1024
+    assert all(k["slots"] * 8 * 96 <= 227 * 1024 for k in info5["kernels"])
