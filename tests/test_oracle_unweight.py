@@ -38,3 +38,19 @@ def test_unweighted_sample_reproduces_closed_form_asymmetry_and_cross_section(or
     _, _, _, acc2 = orc.unweight(w, me, 1.0 / (2 * sqs * sqs), seed=99, wmax=2 * wmax)
     assert abs(acc2.mean() - eff / 2) < 5 * math.sqrt(eff / 2 / n)
     assert (acc2 <= acc).all()                                 # same uniforms: a subset
+
+
+def test_unweighting_uniforms_are_the_stated_philox_words(orc):
+    """u_i = u53(w0, w1) of Philox4x32-10 at counter (event lo, event hi, 'UNWT', 0): recomputed here word by word from the
+    known-answer-tested block function; a rejected event has u * wmax >= w, an accepted one u * wmax < w."""
+    n, seed, first = 300, 0x1234567890, (1 << 32) - 100            # crosses the 32-bit boundary of the event counter
+    rng = np.random.default_rng(1)
+    w, me = rng.uniform(0.5, 1.5, n), rng.uniform(0.0, 1.0, n)
+    s1, s2, wmax, acc = orc.unweight(w, me, 2.0, seed=seed, first_event=first)
+    ww = 2.0 * w * me
+    assert wmax == ww.max() and abs(s1 - ww.sum()) < 1e-12 * s1 and abs(s2 - (ww * ww).sum()) < 1e-12 * s2
+    for i in range(n):
+        ev = first + i
+        wd = orc.philox4x32_10([ev & 0xFFFFFFFF, ev >> 32, 0x554E5754, 0], [seed & 0xFFFFFFFF, seed >> 32])
+        u = ((wd[0] >> 5) * 67108864.0 + (wd[1] >> 6) + 0.5) / 9007199254740992.0
+        assert bool(acc[i]) == (u * wmax < ww[i])
