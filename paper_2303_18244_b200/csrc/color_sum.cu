@@ -81,7 +81,7 @@ size_t multi_scratch_bytes(int precision, long npad, int ncol) {
 }
 
 static bool g_color_loaded = false;
-// FP64: tensor-core (DMMA) colour sum; ME_COLOR_FMA=1 in the environment selects the plain-FMA kernel (A/B timing)
+// tensor-core colour sums (FP64: DMMA, FP32: TF32 split); ME_COLOR_FMA=1 in the environment selects the plain-FMA kernels (A/B timing)
 static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
 
 static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
@@ -143,6 +143,11 @@ static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long h
       const double* cm = nullptr;
       cudaError_t e2 = cudaGetSymbolAddress((void**)&cm, c_color_d);
       if (e2 == cudaSuccess) e2 = launch_color_sum_dmma(cm, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      if (e2 != cudaSuccess) return e2;
+    } else if (precision != 0 && g_use_dmma) {      // FP32 colour sum (float and mixed mode) on the tensor cores, TF32 hi/lo split
+      const float* cf = nullptr;
+      cudaError_t e2 = cudaGetSymbolAddress((void**)&cf, c_color_f);
+      if (e2 == cudaSuccess) e2 = launch_color_sum_tf32(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
       if (e2 != cudaSuccess) return e2;
     } else if (precision == 0)
       k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
