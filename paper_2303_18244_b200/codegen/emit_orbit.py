@@ -110,9 +110,11 @@ class Inst:
         self.pending = []          # (sigma, code, amp) waiting for flush_jamps()
         self.zcount = 0
 
+    tbname = "tb"          # name of the parameter-table row pointer in the emitted loop body
+
     def P(self, v):
         self.params.append(int(v))
-        return "tb[%d]" % (len(self.params) - 1)
+        return "%s[%d]" % (self.tbname, len(self.params) - 1)
 
     def off(self, slot):                       # shared-memory element offset of a slot
         return self.P(eo(slot, self.stride))

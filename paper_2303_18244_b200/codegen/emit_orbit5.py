@@ -56,8 +56,11 @@ class Layout5:
 class Inst5(Inst):
     """Block instance whose jamps go to LOCAL accumulators (shared memory) and are flushed to global staging."""
 
-    def __init__(self, lay, stride):
+    def __init__(self, lay, stride, inner=False):
         super().__init__(lay, stride)
+        self.subtables = []          # (name, [param rows]) of nested loops
+        if inner:                    # body of a nested loop: own table row `tb2`, may use the variables of the outer instance
+            self.tbname = "tb2"
         self.local = {}              # global colour-flow index -> local accumulator slot
         self.redundant = 0           # flops that recompute something another block / kernel also computes
         self.scopes = [set()]        # names of fermion values loaded in each open brace scope
@@ -88,6 +91,23 @@ class Inst5(Inst):
             re, im = self.unit_times(u, z)
             self.L("cacc<R>(sm + %d, %s, %s);" % (eo(self.lay.J + 2 * loc, self.stride), re, im))
             self.flops += 2
+
+    def inner_loop(self, name, inners):
+        """nested table-driven loop over `inners` (Inst5(inner=True) objects of identical shape) inside this instance"""
+        t = inners[0]
+        for it in inners[1:]:
+            assert it.lines == t.lines and it.jamp_codes == t.jamp_codes, "inner instances of %s differ" % name
+        self.L("#pragma unroll 1")
+        self.L("for (int i2 = 0; i2 < %d; ++i2) {" % len(inners))
+        self.L("  const int* tb2 = &@SUB:%s@[it * %d + i2][0];" % (name, len(inners)))
+        for l in t.lines:
+            self.L("  " + l)
+        self.L("}")
+        self.subtables.append((name, [it.params for it in inners]))
+        self.flops += sum(it.flops for it in inners)
+        self.namp += sum(it.namp for it in inners)
+        self.redundant += sum(it.redundant for it in inners)
+        self.jamp_codes.extend(t.jamp_codes)
 
     def flush_global(self):
         """add the local accumulators into gj and clear them.  The add is a fire-and-forget reduction (RED.ADD, no
@@ -305,6 +325,8 @@ def _grouper(groups):
             assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
             assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
         groups.append((name, tmpl, [it.params for it in insts], unroll))
+        for si, (sname, _) in enumerate(tmpl.subtables):
+            tmpl.subtables[si] = (sname, [r for it in insts for r in it.subtables[si][1]])
     return add_group
 
 
@@ -404,39 +426,40 @@ def build_k3(stride, pidx):
         I.flush_jamps()
         I.L("}")
 
-    # (small instances: a per-w instance with all 21 quad terms unrolled was ~8 k instructions and instruction-fetch bound)
+    # one instance per last gluon w: the three end vectors are formed once, then two nested table-driven loops run over the
+    # 3 + 6 four-gluon sub-trees (unrolled they were ~8 k instructions and instruction-fetch bound; as 45 independent small
+    # instances they rebuilt the end vectors 45 times: 38 % of this kernel's flops)
     insts = []
     for w in range(N):
         quad = rest_of(w)
+        I = Inst5(lay, stride)
+        ends(I, w, quad)
         a0 = quad[0]
+        inners = []
         for b0 in quad[1:]:
             p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
-            I = Inst5(lay, stride)
-            ends(I, w, quad)
-            I.redundant += (2 * FL5["bilinear"] + FL5["v3_dual"]) * 8 // 9      # 5 distinct end triples, formed 45 times
-            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.kvec("k1", list(p1)); I.kvec("k2", list(p2))
-            I.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); I.flops += FL5["v3_current"]
-            close3(I, w, "t", c_v3(cpair(*p1), cpair(*p2)))
-            I.flush_global()
-            insts.append(I)
-    add_group("quad_v3", insts, 1)
-    insts = []
-    for w in range(N):
-        quad = rest_of(w)
+            J = Inst5(lay, stride, inner=True)
+            J.ldw("p1", lay.PAIR[p1]); J.ldw("p2", lay.PAIR[p2]); J.kvec("k1", list(p1)); J.kvec("k2", list(p2))
+            J.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); J.flops += FL5["v3_current"]
+            close3(J, w, "t", c_v3(cpair(*p1), cpair(*p2)))
+            J.flush_global()
+            inners.append(J)
+        I.inner_loop("v3", inners)
+        inners = []
         for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
             l1, l2 = [l for l in quad if l not in p]
-            I = Inst5(lay, stride)
-            ends(I, w, quad)
-            I.redundant += (2 * FL5["bilinear"] + FL5["v3_dual"]) * 8 // 9
-            I.ldw("pp", lay.PAIR[p]); I.leaf("e1", l1); I.leaf("e2", l2)
-            I.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); I.flops += FL5["v4_dots"]
+            J = Inst5(lay, stride, inner=True)
+            J.ldw("pp", lay.PAIR[p]); J.leaf("e1", l1); J.leaf("e2", l2)
+            J.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); J.flops += FL5["v4_dots"]
             for k in range(3):
-                I.L("{ const W4<R> t = v4_current(%d, dots, pp, e1, e2);" % k); I.flops += FL5["v4_current"]
-                close3(I, w, "t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
-                I.L("}")
-            I.flush_global()
-            insts.append(I)
-    add_group("quad_v4", insts, 1)
+                J.L("{ const W4<R> t = v4_current(%d, dots, pp, e1, e2);" % k); J.flops += FL5["v4_current"]
+                close3(J, w, "t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
+                J.L("}")
+            J.flush_global()
+            inners.append(J)
+        I.inner_loop("v4", inners)
+        insts.append(I)
+    add_group("quads", insts, 1)
     # ---- V4(pair, pair', eps_m) on the bare line
     insts = []
     for m in range(N):
@@ -522,6 +545,11 @@ def emit_kernel(name, ki, lay, groups):
         for r in rows:
             S("  {%s}," % ", ".join(str(v) for v in r))
         S("};")
+        for sname, srows in getattr(tmpl, "subtables", []):
+            S("__constant__ int tab_%s_o%d_%s_%s[%d][%d] = {" % (name, ki, gname, sname, len(srows), len(srows[0])))
+            for r in srows:
+                S("  {%s}," % ", ".join(str(v) for v in r))
+            S("};")
     S("template <typename R, typename RJ>")
     S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
       " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n) {" % (BLOCK, name, ki))
@@ -560,6 +588,9 @@ def emit_kernel(name, ki, lay, groups):
         S("    for (int it = 0; it < %d; ++it) {" % len(rows))
         S("      const int* tb = tab_%s_o%d_%s[it];" % (name, ki, gname))
         for l in tmpl.lines:
+            if "@SUB:" in l:
+                sname = l.split("@SUB:")[1].split("@")[0]
+                l = l.replace("@SUB:%s@" % sname, "tab_%s_o%d_%s_%s" % (name, ki, gname, sname))
             S("      " + l)
         S("    }")
     S("  }")
