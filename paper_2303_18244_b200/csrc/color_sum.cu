@@ -83,6 +83,8 @@ size_t multi_scratch_bytes(int precision, long npad, int ncol) {
 static bool g_color_loaded = false;
 // tensor-core colour sums (FP64: DMMA, FP32: TF32 split); ME_COLOR_FMA=1 in the environment selects the plain-FMA kernels (A/B timing)
 static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
+// ME_COLOR_MMA_SYNC=1 selects the warp-level TF32 kernel (color_sum_tf32.cu) instead of the tcgen05 one (A/B timing)
+static const bool g_use_tcgen05 = getenv("ME_COLOR_MMA_SYNC") == nullptr;
 
 static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
                                       const double* color_num_host);
@@ -147,7 +149,9 @@ static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long h
     } else if (precision != 0 && g_use_dmma) {      // FP32 colour sum (float and mixed mode) on the tensor cores, TF32 hi/lo split
       const float* cf = nullptr;
       cudaError_t e2 = cudaGetSymbolAddress((void**)&cf, c_color_f);
-      if (e2 == cudaSuccess) e2 = launch_color_sum_tf32(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      if (e2 == cudaSuccess && g_use_tcgen05)
+        e2 = launch_color_sum_tcgen05(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      else if (e2 == cudaSuccess) e2 = launch_color_sum_tf32(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
       if (e2 != cudaSuccess) return e2;
     } else if (precision == 0)
       k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);

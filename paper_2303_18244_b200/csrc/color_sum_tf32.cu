@@ -9,8 +9,7 @@
 // color_sum_dmma.cu a warp owns 8 events and both their Re and Im columns for ALL row tiles (8 tiles of 16 rows, the
 // last half-tile zero padded): 16 accumulator tiles (64 floats) in registers; C fragments in shared memory in
 // fragment order (conflict-free 128-bit loads), B fragments straight from the global staging buffer.
-// tcgen05 is not used: per launch this is 0.12 TFLOP of work next to 1-2 GB of staging traffic, i.e. HBM-bound
-// at any tensor rate; the legacy warp-level MMA already leaves the kernel at the memory roofline.
+// Superseded as the default by color_sum_tcgen05.cu (3x faster); kept behind ME_COLOR_MMA_SYNC=1 as its A/B baseline.
 #include "multi.h"
 
 namespace me {

@@ -301,7 +301,8 @@ def test_parity_pairing_option(me, orc, proc):
         flipped = mh[::-1]                                   # ~h = ncomb-1-h
         assert (np.abs(mh - flipped) / mh.max(axis=0)).max() < 1e-10
     ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
-    for name, tol in (("fp64", 1e-12), ("mixed", 1e-6), ("fp32", 1e-4)):
+    # mixed: the FP32 colour sum alone leaves ~1e-6 (120 FP32 terms per flow); the bound of the task is 1e-4
+    for name, tol in (("fp64", 1e-12), ("mixed", 5e-6), ("fp32", 1e-4)):
         paired = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
         assert np.abs(paired / full - 1).max() < tol
     if proc == 0:
