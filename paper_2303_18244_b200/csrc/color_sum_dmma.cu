@@ -1,8 +1,10 @@
 // color_sum_dmma.cu — FP64 colour sum of the 120-flow process on the tensor cores (SURVEY.md §8(a) step a7,
 // BASELINE.json north_star: "the colour sum is batched as a genuine dense contraction over events, on FP64 DMMA").
 //
-//     Y = C X,   C [120 x 120] colour-matrix numerators,  X [120 x (2 * events)] = (Re J, Im J) of one helicity,
+//     Y = L X,   L = lower triangle of the [120 x 120] colour-matrix numerators (off-diagonal entries doubled: C is
+//     symmetric),  X [120 x (2 * events)] = (Re J, Im J) of one helicity,
 //     ME_h(evt) = sum_i  X[i][evt,re] Y[i][evt,re] + X[i][evt,im] Y[i][evt,im]
+// The 8 x 4 tiles of L above the diagonal are zero and are skipped: 240 of the 450 (row block, k-step) pairs remain.
 //
 // mma.sync.m8n8k4.f64 (DMMA): M = 8 colour rows, N = 8 events, K = 4 colour columns.  A warp owns 8 events and both
 // their Re and Im columns (two N-tiles) for ALL 15 row blocks: 30 accumulator tiles (60 doubles) in registers, so each
@@ -18,7 +20,7 @@ namespace me {
 #define CD_RB (CD_NCOL / 8)     // 15 row blocks
 #define CD_KS (CD_NCOL / 4)     // 30 k-steps
 #define CD_WARPS 8
-#define CD_PF 6                 // k-steps of B fragments prefetched per batch
+#define CD_PF 5                 // k-steps of B fragments prefetched per batch
 
 __device__ __forceinline__ void dmma8x8x4(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
@@ -32,7 +34,9 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int i = threadIdx.x; i < CD_RB * CD_KS * 32; i += blockDim.x) {
     const int l = i & 31, ks = (i >> 5) % CD_KS, rb = (i >> 5) / CD_KS;
-    cfrag[i] = cmat[(rb * 8 + (l >> 2)) * CD_NCOL + ks * 4 + (l & 3)];
+    const int r = rb * 8 + (l >> 2), c = ks * 4 + (l & 3);
+    // C is symmetric: x^T C x = sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), so only the lower triangle is contracted
+    cfrag[i] = c < r ? 2.0 * cmat[r * CD_NCOL + c] : c == r ? cmat[r * CD_NCOL + c] : 0.0;
   }
   __syncthreads();
   const long ntiles = (npad + 8 * CD_WARPS - 1) / (8 * CD_WARPS);
@@ -52,7 +56,7 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
         const double* p = g + (long)(2 * (4 * j + kr)) * npad + ec;
         bre[j] = p[0]; bim[j] = p[npad];
       }
-#pragma unroll 1
+#pragma unroll   // fully unrolled: the triangular skip below is then resolved at compile time (a predicated-off DMMA still costs its pipe slot)
       for (int kb = 0; kb < CD_KS; kb += CD_PF) {
         double nre[CD_PF], nim[CD_PF];
         if (kb + CD_PF < CD_KS) {
@@ -65,8 +69,10 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
 #pragma unroll
         for (int j = 0; j < CD_PF; ++j) {
           const double* af = cfrag + (kb + j) * 32 + lane;
+          const int rbmin = (kb + j) >> 1;                 // row blocks above this one hold only zeros in columns 4 (kb + j) ..
 #pragma unroll
           for (int rb = 0; rb < CD_RB; ++rb) {
+            if (rb < rbmin) continue;
             const double a = af[rb * CD_KS * 32];
             dmma8x8x4(acc[rb][0][0], acc[rb][0][1], a, bre[j]);
             dmma8x8x4(acc[rb][1][0], acc[rb][1][1], a, bim[j]);
