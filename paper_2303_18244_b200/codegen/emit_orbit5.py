@@ -21,7 +21,8 @@ from .topology import color_matrix
 
 N = 5
 NPAR = 7
-BLOCK = 96
+BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56)
 
 
@@ -29,7 +30,7 @@ class Layout5:
     """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True):
         A = SlotAlloc()
         self.FERM = None
         if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
@@ -41,8 +42,10 @@ class Layout5:
         if want_pairs:
             pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
             self.PAIR = {p: A.vec(8) for p in pairs}
-        self.Q1 = A.vec(8 * N)
-        self.CHI = A.vec(8 * N)
+        self.Q1 = self.CHI = None             # one-gluon currents of both quark ends (kernel 1 rebuilds them at each use instead)
+        if want_q1chi:
+            self.Q1 = A.vec(8 * N)
+            self.CHI = A.vec(8 * N)
         self.J = A.vec(2 * jacc)
         self.jacc = jacc
         masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
@@ -185,6 +188,8 @@ def phase_a(lay, stride, add_group, want_pairs):
             I.stw(lay.PAIR[(a, b)], "t")
             insts.append(I)
         add_group("pairs", insts, 2)
+    if lay.Q1 is None:
+        return
     insts = []
     for l in labels:
         I = Inst5(lay, stride)
@@ -212,7 +217,9 @@ def phase_a(lay, stride, add_group, want_pairs):
 def build_k1(stride, pidx, part=None):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
-    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True)
+    # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
+    # brings the kernel from 292 to 212 slots per thread, i.e. from 96 to 128 threads per CTA (all four schedulers busy)
+    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True, want_q1chi=False)
     groups = []
 
     def add_group(name, insts, unroll=1):
@@ -273,14 +280,33 @@ def build_k1(stride, pidx, part=None):
             I.flush_jamps()
             I.L("}")
 
-        ld = lambda nm, slot: (lambda: I.ldw(nm, slot))
+        leafname = {x: "ex", y: "ey"}
+
+        def mk_q1(nm, l):
+            """q1(l) = ubar with gluon l attached, rebuilt in the current scope"""
+            def f():
+                f0 = I.flops
+                I.qvec("qk_" + nm, [l]); I.fv("ub")
+                I.L("const W4<R> %s = quark_step2(ub, %s, qk_%s, mt, %s);" % (nm, leafname[l], nm, I.iq(l)))
+                I.flops += FL5["quark_step2"]; I.redundant += I.flops - f0
+            return f
+
+        def mk_chi(nm, w):
+            """chi1(w) = v with gluon w attached, rebuilt in the current scope"""
+            def f():
+                rest = rest_of(w)
+                f0 = I.flops
+                I.qvec("qk_" + nm, rest); I.fv("vv")
+                I.L("const W4<R> %s = col_step(slash_col(%s, vv), qk_%s, mt, %s);" % (nm, leafname[w], nm, I.iq(*rest)))
+                I.flops += FL5["slash_col"] + FL5["col_step"]; I.redundant += I.flops - f0
+            return f
         # quad = V3(t, eps_u) closing three ways with the last gluon w  (u,w) = (x,y) and (y,x)
         for (u, w, eu, ew, ku, kw) in ((x, y, "ex", "ey", "kx", "ky"), (y, x, "ey", "ex", "ky", "kx")):
             quad = lambda col, u=u: c_v3(col, c_leaf(u))
             ik4 = lambda u=u: I.L("const R ik4 = %s;" % I.ik2(a, b, c, u))
-            dots_with([ld("chw", lay.CHI + 8 * w), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+            dots_with([mk_chi("chw", w), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
                       lambda col, w=w, quad=quad: c_close(ONE, quad(col), cchi(w)))
-            dots_with([ld("q1w", lay.Q1 + 8 * w), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+            dots_with([mk_q1("q1w", w), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
                       lambda col, w=w, quad=quad: c_close(cq1(w), quad(col), ONE))
             dots_with([ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
                       lambda col, w=w, quad=quad: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
@@ -292,8 +318,8 @@ def build_k1(stride, pidx, part=None):
         dots_with([cdots], "cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
         dots_with([cdots], "cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
         # q1(u) . t-slash . chi1(w)
-        dots_with([ld("q1x", lay.Q1 + 8 * x), ld("chy", lay.CHI + 8 * y)], "bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
-        dots_with([ld("q1y", lay.Q1 + 8 * y), ld("chx", lay.CHI + 8 * x)], "bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
+        dots_with([mk_q1("q1x", x), mk_chi("chy", y)], "bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
+        dots_with([mk_q1("q1y", y), mk_chi("chx", x)], "bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
         # ubar . t-slash . chi2(x,y)  and  q2(x,y) . t-slash . v
         # (one current at a time: three live two-gluon currents next to t0..t5 would spill)
         row_side = rest_of(x, y)
@@ -301,15 +327,15 @@ def build_k1(stride, pidx, part=None):
         qr = lambda: (I.qvec("qr", [x, y]), I.L("const R iqr = %s;" % I.iq(x, y)))
         st = FL5["slash_col"] + FL5["col_step"] + FL5["bilinear"]
         dots_with([qc], "bilinear(ub, col_step(slash_col(pxy, vv), qc, mt, iqc))", st, lambda col: c_close(ONE, col, c_step(cpair(x, y), ONE)))
-        dots_with([qc, ld("chy", lay.CHI + 8 * y)], "bilinear(ub, col_step(slash_col(ex, chy), qc, mt, iqc))", st,
+        dots_with([qc, mk_chi("chy", y)], "bilinear(ub, col_step(slash_col(ex, chy), qc, mt, iqc))", st,
                   lambda col: c_close(ONE, col, c_step(c_leaf(x), cchi(y))))
-        dots_with([qc, ld("chx", lay.CHI + 8 * x)], "bilinear(ub, col_step(slash_col(ey, chx), qc, mt, iqc))", st,
+        dots_with([qc, mk_chi("chx", x)], "bilinear(ub, col_step(slash_col(ey, chx), qc, mt, iqc))", st,
                   lambda col: c_close(ONE, col, c_step(c_leaf(y), cchi(x))))
         st = FL5["quark_step2"] + FL5["bilinear"]
         dots_with([qr], "bilinear(quark_step2(ub, pxy, qr, mt, iqr), vv)", st, lambda col: c_close(c_step(ONE, cpair(x, y)), col, ONE))
-        dots_with([qr, ld("q1x", lay.Q1 + 8 * x)], "bilinear(quark_step2(q1x, ey, qr, mt, iqr), vv)", st,
+        dots_with([qr, mk_q1("q1x", x)], "bilinear(quark_step2(q1x, ey, qr, mt, iqr), vv)", st,
                   lambda col: c_close(c_step(cq1(x), c_leaf(y)), col, ONE))
-        dots_with([qr, ld("q1y", lay.Q1 + 8 * y)], "bilinear(quark_step2(q1y, ex, qr, mt, iqr), vv)", st,
+        dots_with([qr, mk_q1("q1y", y)], "bilinear(quark_step2(q1y, ex, qr, mt, iqr), vv)", st,
                   lambda col: c_close(c_step(cq1(y), c_leaf(x)), col, ONE))
         assert counter[0] == 18
         I.flush_global()
@@ -406,14 +432,20 @@ def build_k2(stride, pidx):
 # gluon w, and the contact term V4(pair, pair, eps) on the bare line
 # ------------------------------------------------------------------------------------------
 def build_k3(stride, pidx):
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24)
+    # no Q1 / CHI slots: the one-gluon quark currents are needed exactly once each (in `ends`) and are formed there:
+    # 214 slots per thread -> 128 threads per CTA
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
     def ends(I, w, quad):
         """the three four-vectors a quad term is dotted with: bilinears of the fermion ends and the dual of V3(quad, eps_w)"""
         I.leaf("ew", w); I.kvec("kw", [w]); I.kvec("kq", quad)
-        I.ldw("chw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
+        f0 = I.flops
+        I.qvec("qw", [w]); I.qvec("qq", quad)
+        I.L("const W4<R> q1w = quark_step2(ub, ew, qw, mt, %s), chw = col_step(slash_col(ew, vv), qq, mt, %s);" % (I.iq(w), I.iq(*quad)))
+        I.flops += FL5["quark_step2"] + FL5["slash_col"] + FL5["col_step"]
+        I.redundant += I.flops - f0                    # kernel 2 forms the same ten currents
         I.L("const R ik4 = %s;" % I.ik2(*quad))
         I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv), x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
         I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
@@ -529,7 +561,7 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups):
+def emit_kernel(name, ki, lay, groups, BLOCK):
     src = []
     S = src.append
     namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
@@ -625,9 +657,10 @@ def emit_orbit5_process(name="gg_ttxggg"):
     files, kinfo = {}, []
     builders = (lambda st, px: build_k1(st, px, 0), lambda st, px: build_k1(st, px, 1), lambda st, px: build_k1(st, px, 2),
                 build_k2, build_k3)
+    blocks = (BLOCK1, BLOCK1, BLOCK1, BLOCK, BLOCK1)
     for ki, b in enumerate(builders):
-        lay, groups = b(BLOCK, pidx)
-        src, info = emit_kernel(name, ki, lay, groups)
+        lay, groups = b(blocks[ki], pidx)
+        src, info = emit_kernel(name, ki, lay, groups, blocks[ki])
         files["gen_%s_o%d.cu" % (name, ki)] = src
         kinfo.append(info)
     namp = sum(k["amplitudes"] for k in kinfo)
@@ -644,7 +677,9 @@ def emit_orbit5_process(name="gg_ttxggg"):
         pass
     lay2, groups2 = build_k2(BLOCK, pidx)
     pa = {g: t.flops * len(rows) for g, t, rows, _ in groups2 if g in ("pairs", "q1", "chi1")}
-    redundant = sum(k["redundant"] for k in kinfo) + (len(kinfo) - 1) * (pa["q1"] + pa["chi1"] + head) + pa["pairs"]
+    # q1 / chi1 are needed once: kernel 2 runs those loops (kernels 1 and 3 rebuild them in place, tagged); the spinors
+    # and their bilinear once, not once per kernel
+    redundant = sum(k["redundant"] for k in kinfo) + (len(kinfo) - 1) * head + pa["pairs"]
     # the 10 pairs are needed once: kernel 1 recomputes them per block (tagged), kernels 2 and 3 both run the pairs loop
     algo = executed - redundant - (cs_executed - cs_flops)
     fixed = sum(k["fixed"] for k in kinfo)
