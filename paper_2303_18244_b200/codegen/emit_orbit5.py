@@ -22,6 +22,7 @@ from .topology import color_matrix
 N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56)
 
@@ -30,7 +31,7 @@ class Layout5:
     """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5)):
         A = SlotAlloc()
         self.FERM = None
         if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
@@ -46,9 +47,11 @@ class Layout5:
         if want_q1chi:
             self.Q1 = A.vec(8 * N)
             self.CHI = A.vec(8 * N)
+        elif want_chi:
+            self.CHI = A.vec(8 * N)
         self.J = A.vec(2 * jacc)
         self.jacc = jacc
-        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
+        masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") in ik2_sizes]
         self.IK2 = {m: A.scalar() for m in masks2}
         # quark propagators: row side sets of size 1,2 and (for the column currents) size 3,4
         masksq = [m for m in range(1, (1 << N) - 1) if want_iq_mid or bin(m).count("1") in (1, 4)]
@@ -120,7 +123,7 @@ class Inst5(Inst):
             o = eo(self.lay.J + 2 * loc, self.stride)
             self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
                    % (self.P(2 * sigma), o, o + 1, o, o + 1))
-            self.flops += 2
+            self.flops += 2; self.redundant += 2     # staging adds are overhead of the multi-kernel split, not of the method
         self.local = {}
 
 
@@ -154,7 +157,13 @@ def emit_pair(I, name, a, b, ea, eb, ka, kb):
 
 def emit_rows2(I, a, b, pab, ea, eb):
     """the three row currents with gluons {a,b} attached (a<b): returns [(name, colour)]"""
-    I.ldw("q1a", I.lay.Q1 + 8 * a); I.ldw("q1b", I.lay.Q1 + 8 * b)
+    if I.lay.Q1 is not None:
+        I.ldw("q1a", I.lay.Q1 + 8 * a); I.ldw("q1b", I.lay.Q1 + 8 * b)
+    else:                                 # no Q1 slots: the two one-gluon row currents are formed here
+        f0 = I.flops
+        I.qvec("qa1", [a]); I.qvec("qb1", [b]); I.fv("ub")
+        I.L("const W4<R> q1a = quark_step2(ub, %s, qa1, mt, %s), q1b = quark_step2(ub, %s, qb1, mt, %s);" % (ea, I.iq(a), eb, I.iq(b)))
+        I.flops += 2 * FL5["quark_step2"]; I.redundant += I.flops - f0
     I.qvec("qr", [a, b])
     I.L("const R iqr = %s;" % I.iq(a, b))
     I.fv("ub")
@@ -188,16 +197,17 @@ def phase_a(lay, stride, add_group, want_pairs):
             I.stw(lay.PAIR[(a, b)], "t")
             insts.append(I)
         add_group("pairs", insts, 2)
-    if lay.Q1 is None:
+    if lay.CHI is None:
         return
-    insts = []
-    for l in labels:
-        I = Inst5(lay, stride)
-        I.leaf("el", l); I.qvec("q", [l]); I.fv("ub")
-        I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL5["quark_step2"]
-        I.stw(lay.Q1 + 8 * l, "t")
-        insts.append(I)
-    add_group("q1", insts, 1)
+    if lay.Q1 is not None:
+        insts = []
+        for l in labels:
+            I = Inst5(lay, stride)
+            I.leaf("el", l); I.qvec("q", [l]); I.fv("ub")
+            I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL5["quark_step2"]
+            I.stw(lay.Q1 + 8 * l, "t")
+            insts.append(I)
+        add_group("q1", insts, 1)
     insts = []
     for w in labels:
         rest = rest_of(w)
@@ -214,7 +224,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None):
+def build_k1(stride, pidx, part=None, nparts=3):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
@@ -251,22 +261,22 @@ def build_k1(stride, pidx, part=None):
         I.L("kM = padd(kab, kc);"); I.flops += 4
         emit_pair(I, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(I, "pac", a, c, "ea", "ec", "ka", "kc")
         emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc")
-        I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once would do
-        if part is not None and part > 0:             # the split kernels each rebuild the six terms
-            I.redundant += 6 * FL5["v3_current"] + FL5["v4_dots"] + 3 * FL5["v4_current"]
+        I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once (as pxy of its own block) would do
         I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
         I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
         I.L("t3 = v4_current(0, dots, ea, eb, ec); t4 = v4_current(1, dots, ea, eb, ec); t5 = v4_current(2, dots, ea, eb, ec);")
         I.flops += 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
         I.L("}")
+        if part is not None and part > 0:             # the split kernels each rebuild pxy and the six terms: all of it overhead
+            I.redundant = I.flops
 
         counter = [0]
 
         def dots_with(prelude, xexpr, flops, colour_of_term):
             """6 amplitudes t_i . X and their jamp updates; operands of X are loaded inside the scope"""
             idx = counter[0]; counter[0] += 1
-            if part is not None and idx // 6 != part:
+            if part is not None and idx // (18 // nparts) != part:
                 return
             I.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
@@ -364,7 +374,9 @@ def spair(p):
 # kernel 2: amplitudes whose two ends carry (2 | 2), (2 | 1) or (1 | 2) gluons and whose middle is a gluon or a pair
 # ------------------------------------------------------------------------------------------
 def build_k2(stride, pidx):
-    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=12)
+    # 226 slots per thread -> 128 threads per CTA: no Q1 slots (the row-side one-gluon currents are formed where they are
+    # used: 5 per ten uses would do, +14 % flops), only the pair propagators, 8 local jamp accumulators flushed per sub-block
+    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=8, want_q1chi=False, want_chi=True, ik2_sizes=(2,))
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -400,7 +412,7 @@ def build_k2(stride, pidx):
             I.flush_jamps()
             I.L("}")
             I.L("}")
-        I.flush_global()
+            I.flush_global()
         insts.append(I)
     add_group("rows2", insts, 1)
     # ---- cols2 loop: B = {c,d}; q1(x) . pair(P)-slash . chi2(B)
@@ -414,14 +426,18 @@ def build_k2(stride, pidx):
         for x in rest:
             p = spair([l for l in rest if l != x])
             I.L("{")
-            I.ldw("q1x", lay.Q1 + 8 * x); I.ldw("pp", lay.PAIR[p])
+            f0 = I.flops
+            I.leaf("ex", x); I.qvec("qx", [x]); I.fv("ub")
+            I.L("const W4<R> q1x = quark_step2(ub, ex, qx, mt, %s);" % I.iq(x)); I.flops += FL5["quark_step2"]
+            I.redundant += I.flops - f0
+            I.ldw("pp", lay.PAIR[p])
             I.L("const W4<R> r = row_slash(q1x, pp);"); I.flops += FL5["row_slash"]
             I.L("const Cx<R> a0 = row_col(r, ca), a1 = row_col(r, cb), a2 = row_col(r, cc);"); I.flops += 3 * FL5["row_col"]
             for k, (cn, ccol) in enumerate(cols):
                 I.jamp("a%d" % k, c_close(cq1(x), cpair(*p), ccol), pidx)
             I.flush_jamps()
             I.L("}")
-        I.flush_global()
+            I.flush_global()
         insts.append(I)
     add_group("cols2", insts, 1)
     return lay, groups
@@ -655,9 +671,8 @@ def emit_orbit5_process(name="gg_ttxggg"):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     files, kinfo = {}, []
-    builders = (lambda st, px: build_k1(st, px, 0), lambda st, px: build_k1(st, px, 1), lambda st, px: build_k1(st, px, 2),
-                build_k2, build_k3)
-    blocks = (BLOCK1, BLOCK1, BLOCK1, BLOCK, BLOCK1)
+    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
+    blocks = (BLOCK1,) * len(builders)
     for ki, b in enumerate(builders):
         lay, groups = b(blocks[ki], pidx)
         src, info = emit_kernel(name, ki, lay, groups, blocks[ki])
@@ -675,12 +690,14 @@ def emit_orbit5_process(name="gg_ttxggg"):
     phase_a_repeat = 0
     for k, b in zip(kinfo, builders):
         pass
-    lay2, groups2 = build_k2(BLOCK, pidx)
-    pa = {g: t.flops * len(rows) for g, t, rows, _ in groups2 if g in ("pairs", "q1", "chi1")}
-    # q1 / chi1 are needed once: kernel 2 runs those loops (kernels 1 and 3 rebuild them in place, tagged); the spinors
-    # and their bilinear once, not once per kernel
-    redundant = sum(k["redundant"] for k in kinfo) + (len(kinfo) - 1) * head + pa["pairs"]
-    # the 10 pairs are needed once: kernel 1 recomputes them per block (tagged), kernels 2 and 3 both run the pairs loop
+    # the pairs, q1 and chi1 loops as they would run once (reference layout with all slots)
+    ref_groups = []
+    phase_a(Layout5(want_pairs=True, want_iq_mid=True, jacc=12), BLOCK, _grouper(ref_groups), want_pairs=True)
+    pa = {g: t.flops * len(rows) for g, t, rows, _ in ref_groups}
+    # needed once: the 10 pairs (untagged as pxy of the first kernel; kernels 2 and 3 both run the pairs loop again), the 5 + 5
+    # one-gluon quark currents (chi1: kernel 2's loop; q1: every use is a tagged rebuild, so one set is taken back out of the
+    # redundant count), the spinors and their bilinear (once, not once per kernel)
+    redundant = sum(k["redundant"] for k in kinfo) + (len(kinfo) - 1) * head + 2 * pa["pairs"] - pa["q1"]
     algo = executed - redundant - (cs_executed - cs_flops)
     fixed = sum(k["fixed"] for k in kinfo)
     src = []

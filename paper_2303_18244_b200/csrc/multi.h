@@ -8,7 +8,7 @@
 
 #define ME_HEL_CHUNK 16   // helicities staged per pass
 #ifndef ME_HEL_PER_CTA
-#define ME_HEL_PER_CTA 2   // helicities looped inside one CTA of a diagram kernel (grid.y covers the chunk)
+#define ME_HEL_PER_CTA 4   // helicities looped inside one CTA of a diagram kernel (grid.y covers the chunk)
 #endif
 
 namespace me {
