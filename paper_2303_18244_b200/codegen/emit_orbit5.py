@@ -31,7 +31,7 @@ class Layout5:
     """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5)):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5), scratch=False):
         A = SlotAlloc()
         self.FERM = None
         if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
@@ -49,6 +49,7 @@ class Layout5:
             self.CHI = A.vec(8 * N)
         elif want_chi:
             self.CHI = A.vec(8 * N)
+        self.TMP = A.vec(8) if scratch else None   # one parked current (kernel 1)
         self.J = A.vec(2 * jacc)
         self.jacc = jacc
         masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") in ik2_sizes]
@@ -62,9 +63,10 @@ class Layout5:
 class Inst5(Inst):
     """Block instance whose jamps go to LOCAL accumulators (shared memory) and are flushed to global staging."""
 
-    def __init__(self, lay, stride, inner=False):
+    def __init__(self, lay, stride, inner=False, parent=None):
         super().__init__(lay, stride)
         self.subtables = []          # (name, [param rows]) of nested loops
+        self.parent = parent         # inner instance that accumulates into the local jamp slots of its outer instance
         if inner:                    # body of a nested loop: own table row `tb2`, may use the variables of the outer instance
             self.tbname = "tb2"
         self.local = {}              # global colour-flow index -> local accumulator slot
@@ -92,10 +94,13 @@ class Inst5(Inst):
 
     def flush_jamps(self):
         for sigma, u, z in self.grouped_updates():
-            loc = self.local.setdefault(sigma, len(self.local))
+            owner = self.parent if self.parent is not None else self
+            loc = owner.local.setdefault(sigma, len(owner.local))
             assert loc < self.lay.jacc, "local jamp accumulators exhausted"
             re, im = self.unit_times(u, z)
-            self.L("cacc<R>(sm + %d, %s, %s);" % (eo(self.lay.J + 2 * loc, self.stride), re, im))
+            o = eo(self.lay.J + 2 * loc, self.stride)
+            # the slot of a flow differs between the iterations of a nested loop: table-driven there, immediate otherwise
+            self.L("cacc<R>(sm + %s, %s, %s);" % (self.P(o) if self.parent is not None else "%d" % o, re, im))
             self.flops += 2
 
     def inner_loop(self, name, inners):
@@ -224,21 +229,14 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None, nparts=3):
+def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
-    # brings the kernel from 292 to 212 slots per thread, i.e. from 96 to 128 threads per CTA (all four schedulers busy)
-    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True, want_q1chi=False)
+    # brings the kernel from 292 to 220 slots per thread (incl. one scratch vector that carries chi1(w) / q1(u) across scopes), i.e. from 96 to 128 threads per CTA (all four schedulers busy)
+    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True, want_q1chi=False, scratch=True)
     groups = []
-
-    def add_group(name, insts, unroll=1):
-        tmpl = insts[0]
-        for it in insts[1:]:
-            assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
-            assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
-        groups.append((name, tmpl, [it.params for it in insts], unroll))
-
+    add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=False)
     insts = []
     for M in [(a, b, c) for a in range(N) for b in range(a + 1, N) for c in range(b + 1, N)]:
@@ -273,80 +271,102 @@ def build_k1(stride, pidx, part=None, nparts=3):
 
         counter = [0]
 
-        def dots_with(prelude, xexpr, flops, colour_of_term):
-            """6 amplitudes t_i . X and their jamp updates; operands of X are loaded inside the scope"""
+        def dots_with(T, prelude, xexpr, flops, colour_of_term, post=None):
+            """6 amplitudes t_i . X and their jamp updates, emitted into instance T (the block, or the body of its nested
+            (u, w) loop); operands of X are loaded inside the scope"""
             idx = counter[0]; counter[0] += 1
             if part is not None and idx // (18 // nparts) != part:
                 return
-            I.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
+            T.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
-                fn()
-            I.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])
-            I.L("  const W4<R> X = %s;" % xexpr); I.flops += flops
-            I.L("  const Cx<R> a0 = wdot(t0, X), a1 = wdot(t1, X), a2 = wdot(t2, X), a3 = wdot(t3, X), a4 = wdot(t4, X), a5 = wdot(t5, X);")
-            I.flops += 6 * FL5["wdot"]
+                fn(T)
+            T.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])
+            T.L("  const W4<R> X = %s;" % xexpr); T.flops += flops
+            if post is not None:
+                post(T)
+            T.L("  const Cx<R> a0 = wdot(t0, X), a1 = wdot(t1, X), a2 = wdot(t2, X), a3 = wdot(t3, X), a4 = wdot(t4, X), a5 = wdot(t5, X);")
+            T.flops += 6 * FL5["wdot"]
             for i, col in enumerate(tcol):
-                I.jamp("a%d" % i, colour_of_term(col), pidx)
-            I.flush_jamps()
-            I.L("}")
+                T.jamp("a%d" % i, colour_of_term(col), pidx)
+            T.flush_jamps()
+            T.L("}")
 
-        leafname = {x: "ex", y: "ey"}
-
-        def mk_q1(nm, l):
-            """q1(l) = ubar with gluon l attached, rebuilt in the current scope"""
-            def f():
-                f0 = I.flops
-                I.qvec("qk_" + nm, [l]); I.fv("ub")
-                I.L("const W4<R> %s = quark_step2(ub, %s, qk_%s, mt, %s);" % (nm, leafname[l], nm, I.iq(l)))
-                I.flops += FL5["quark_step2"]; I.redundant += I.flops - f0
+        def mk_q1(nm, l, el):
+            """q1(l) = ubar with gluon l attached (polarisation vector el), rebuilt in the current scope"""
+            def f(T):
+                f0 = T.flops
+                T.qvec("qk_" + nm, [l]); T.fv("ub")
+                T.L("const W4<R> %s = quark_step2(ub, %s, qk_%s, mt, %s);" % (nm, el, nm, T.iq(l)))
+                T.flops += FL5["quark_step2"]; T.redundant += T.flops - f0
             return f
 
-        def mk_chi(nm, w):
-            """chi1(w) = v with gluon w attached, rebuilt in the current scope"""
-            def f():
+        def mk_chi(nm, w, ew):
+            """chi1(w) = v with gluon w attached (polarisation vector ew), rebuilt in the current scope"""
+            def f(T):
                 rest = rest_of(w)
-                f0 = I.flops
-                I.qvec("qk_" + nm, rest); I.fv("vv")
-                I.L("const W4<R> %s = col_step(slash_col(%s, vv), qk_%s, mt, %s);" % (nm, leafname[w], nm, I.iq(*rest)))
-                I.flops += FL5["slash_col"] + FL5["col_step"]; I.redundant += I.flops - f0
+                f0 = T.flops
+                T.qvec("qk_" + nm, rest); T.fv("vv")
+                T.L("const W4<R> %s = col_step(slash_col(%s, vv), qk_%s, mt, %s);" % (nm, ew, nm, T.iq(*rest)))
+                T.flops += FL5["slash_col"] + FL5["col_step"]; T.redundant += T.flops - f0
             return f
-        # quad = V3(t, eps_u) closing three ways with the last gluon w  (u,w) = (x,y) and (y,x)
-        for (u, w, eu, ew, ku, kw) in ((x, y, "ex", "ey", "kx", "ky"), (y, x, "ey", "ex", "ky", "kx")):
-            quad = lambda col, u=u: c_v3(col, c_leaf(u))
-            ik4 = lambda u=u: I.L("const R ik4 = %s;" % I.ik2(a, b, c, u))
-            dots_with([mk_chi("chw", w), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                      lambda col, w=w, quad=quad: c_close(ONE, quad(col), cchi(w)))
-            dots_with([mk_q1("q1w", w), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                      lambda col, w=w, quad=quad: c_close(cq1(w), quad(col), ONE))
-            dots_with([ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
-                      lambda col, w=w, quad=quad: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
-        # V3(t, pair(x,y)) on the bare line
-        dots_with([], "v3_dual(pxy, jtt, kM, padd(kx, ky), ik5)", FL5["v3_dual"] + 4, lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
-        # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
-        cdots = lambda: (I.fv("jtt"), I.L("const Cx<R> cxj = cxs(wdot(ex, jtt), ik5), cyj = cxs(wdot(ey, jtt), ik5), cxy = cxs(wdot(ex, ey), ik5);"))
-        dots_with([cdots], "cx_comb(cxj, ey, cxy, jtt)", FL5["cx_comb"] + 3 * FL5["wdot"] + 6, lambda col: c_close(ONE, c_v4(0, col, c_leaf(x), c_leaf(y)), ONE))
-        dots_with([cdots], "cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
-        dots_with([cdots], "cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
-        # q1(u) . t-slash . chi1(w)
-        dots_with([mk_q1("q1x", x), mk_chi("chy", y)], "bilinear(q1x, chy)", FL5["bilinear"], lambda col: c_close(cq1(x), col, cchi(y)))
-        dots_with([mk_q1("q1y", y), mk_chi("chx", x)], "bilinear(q1y, chx)", FL5["bilinear"], lambda col: c_close(cq1(y), col, cchi(x)))
-        # ubar . t-slash . chi2(x,y)  and  q2(x,y) . t-slash . v
-        # (one current at a time: three live two-gluon currents next to t0..t5 would spill)
+
         row_side = rest_of(x, y)
-        qc = lambda: (I.qvec("qc", row_side), I.L("const R iqc = %s;" % I.iq(*row_side)))
-        qr = lambda: (I.qvec("qr", [x, y]), I.L("const R iqr = %s;" % I.iq(x, y)))
-        st = FL5["slash_col"] + FL5["col_step"] + FL5["bilinear"]
-        dots_with([qc], "bilinear(ub, col_step(slash_col(pxy, vv), qc, mt, iqc))", st, lambda col: c_close(ONE, col, c_step(cpair(x, y), ONE)))
-        dots_with([qc, mk_chi("chy", y)], "bilinear(ub, col_step(slash_col(ex, chy), qc, mt, iqc))", st,
-                  lambda col: c_close(ONE, col, c_step(c_leaf(x), cchi(y))))
-        dots_with([qc, mk_chi("chx", x)], "bilinear(ub, col_step(slash_col(ey, chx), qc, mt, iqc))", st,
-                  lambda col: c_close(ONE, col, c_step(c_leaf(y), cchi(x))))
-        st = FL5["quark_step2"] + FL5["bilinear"]
-        dots_with([qr], "bilinear(quark_step2(ub, pxy, qr, mt, iqr), vv)", st, lambda col: c_close(c_step(ONE, cpair(x, y)), col, ONE))
-        dots_with([qr, mk_q1("q1x", x)], "bilinear(quark_step2(q1x, ey, qr, mt, iqr), vv)", st,
-                  lambda col: c_close(c_step(cq1(x), c_leaf(y)), col, ONE))
-        dots_with([qr, mk_q1("q1y", y)], "bilinear(quark_step2(q1y, ex, qr, mt, iqr), vv)", st,
-                  lambda col: c_close(c_step(cq1(y), c_leaf(x)), col, ONE))
+        qc = lambda T: (T.qvec("qc", row_side), T.L("const R iqc = %s;" % T.iq(*row_side)))
+        qr = lambda T: (T.qvec("qr", [x, y]), T.L("const R iqr = %s;" % T.iq(x, y)))
+        stc = FL5["slash_col"] + FL5["col_step"] + FL5["bilinear"]
+        str_ = FL5["quark_step2"] + FL5["bilinear"]
+
+        def uw_vectors(T, u, w, eu, ew, ku, kw):
+            """the six closing vectors that come in a (u, w) = (x, y), (y, x) pair"""
+            quad = lambda col: c_v3(col, c_leaf(u))
+            ik4 = lambda T_: T_.L("const R ik4 = %s;" % T_.ik2(a, b, c, u))
+            # chi1(w) is formed once and parked in the scratch vector for its three scopes; q1(u) takes the slot over for its second
+            park = lambda nm: (lambda T_: T_.stw(lay.TMP, nm))
+            fetch = lambda nm: (lambda T_: T_.ldw(nm, lay.TMP))
+            T.L("{"); mk_chi("chw", w, ew)(T); park("chw")(T); T.L("}")
+            # quad = V3(t, eps_u) closing three ways with the last gluon w
+            dots_with(T, [fetch("chw"), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+                      lambda col: c_close(ONE, quad(col), cchi(w)))
+            dots_with(T, [mk_q1("q1w", w, ew), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+                      lambda col: c_close(cq1(w), quad(col), ONE))
+            dots_with(T, [ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
+                      lambda col: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
+            # ubar . t-slash . chi2: eps_u attached to chi1(w)
+            dots_with(T, [qc, fetch("chw")], "bilinear(ub, col_step(slash_col(%s, chw), qc, mt, iqc))" % eu, stc,
+                      lambda col: c_close(ONE, col, c_step(c_leaf(u), cchi(w))))
+            # q1(u) . t-slash . chi1(w)
+            dots_with(T, [mk_q1("q1u", u, eu), fetch("chw")], "bilinear(q1u, chw)", FL5["bilinear"], lambda col: c_close(cq1(u), col, cchi(w)),
+                      post=park("q1u"))
+            # q2 . t-slash . v: eps_w attached to q1(u)
+            dots_with(T, [qr, fetch("q1u")], "bilinear(quark_step2(q1u, %s, qr, mt, iqr), vv)" % ew, str_,
+                      lambda col: c_close(c_step(cq1(u), c_leaf(w)), col, ONE))
+
+        if share_uw:
+            # one nested table-driven loop of two iterations instead of two copies of six scopes; its jamp updates go to the
+            # block's accumulators.  Measured: 10.6 k -> 8.5 k SASS instructions, but the table-driven operand and accumulator
+            # offsets cost more than the instruction fetch they save (FP64 150 ms vs 144 ms per 65536 events): off by default
+            inners = []
+            for (u, w) in ((x, y), (y, x)):
+                J = Inst5(lay, stride, inner=True, parent=I)
+                J.leaf("eu", u); J.leaf("ew", w); J.kvec("ku", [u]); J.kvec("kw", [w])
+                J.redundant += J.flops                # ex, ey, kx, ky exist in the block
+                uw_vectors(J, u, w, "eu", "ew", "ku", "kw")
+                inners.append(J)
+            I.inner_loop("uw", inners)
+        else:
+            uw_vectors(I, x, y, "ex", "ey", "kx", "ky")
+            uw_vectors(I, y, x, "ey", "ex", "ky", "kx")
+        # V3(t, pair(x,y)) on the bare line
+        dots_with(I, [], "v3_dual(pxy, jtt, kM, padd(kx, ky), ik5)", FL5["v3_dual"] + 4, lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
+        # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
+        cdots = lambda T: (T.fv("jtt"), T.L("const Cx<R> cxj = cxs(wdot(ex, jtt), ik5), cyj = cxs(wdot(ey, jtt), ik5), cxy = cxs(wdot(ex, ey), ik5);"))
+        dots_with(I, [cdots], "cx_comb(cxj, ey, cxy, jtt)", FL5["cx_comb"] + 3 * FL5["wdot"] + 6, lambda col: c_close(ONE, c_v4(0, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with(I, [cdots], "cx_comb(cyj, ex, cxy, jtt)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(1, col, c_leaf(x), c_leaf(y)), ONE))
+        dots_with(I, [cdots], "cx_comb(cyj, ex, cxj, ey)", FL5["cx_comb"], lambda col: c_close(ONE, c_v4(2, col, c_leaf(x), c_leaf(y)), ONE))
+        # ubar . t-slash . chi2(pair)  and  q2(pair) . t-slash . v
+        # (one current at a time: three live two-gluon currents next to t0..t5 would spill)
+        dots_with(I, [qc], "bilinear(ub, col_step(slash_col(pxy, vv), qc, mt, iqc))", stc, lambda col: c_close(ONE, col, c_step(cpair(x, y), ONE)))
+        dots_with(I, [qr], "bilinear(quark_step2(ub, pxy, qr, mt, iqr), vv)", str_, lambda col: c_close(c_step(ONE, cpair(x, y)), col, ONE))
         assert counter[0] == 18
         I.flush_global()
         insts.append(I)
