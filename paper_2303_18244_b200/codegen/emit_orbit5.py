@@ -103,6 +103,15 @@ class Inst5(Inst):
             self.L("cacc<R>(sm + %s, %s, %s);" % (self.P(o) if self.parent is not None else "%d" % o, re, im))
             self.flops += 2
 
+    def flush_direct(self):
+        """pending jamp updates go straight into the global staging buffer, one fire-and-forget reduction per colour flow
+        (all amplitudes that feed a flow are combined in registers first).  For blocks in which a flow is touched once: a
+        shared-memory accumulator there is a read-modify-write plus a flush for nothing."""
+        for sigma, u, z in self.grouped_updates():
+            re, im = self.unit_times(u, z)
+            self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)(%s)); atomicAdd(g + npad, (RJ)(%s)); }" % (self.P(2 * sigma), re, im))
+            self.flops += 2
+
     def inner_loop(self, name, inners):
         """nested table-driven loop over `inners` (Inst5(inner=True) objects of identical shape) inside this instance"""
         t = inners[0]
@@ -470,7 +479,7 @@ def build_k2(stride, pidx):
 def build_k3(stride, pidx):
     # no Q1 / CHI slots: the one-gluon quark currents are needed exactly once each (in `ends`) and are formed there:
     # 214 slots per thread -> 128 threads per CTA
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False)
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=0, want_q1chi=False)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -486,13 +495,12 @@ def build_k3(stride, pidx):
         I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv), x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
         I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
 
-    def close3(I, w, tname, col):
-        I.L("{ const Cx<R> a1 = wdot(%s, x1), a2 = wdot(%s, x2), a3 = wdot(%s, x3);" % (tname, tname, tname)); I.flops += 3 * FL5["wdot"]
-        I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)
-        I.jamp("a2", c_close(cq1(w), col, ONE), pidx)
-        I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
-        I.flush_jamps()
-        I.L("}")
+    def close3(I, w, tname, col, k=""):
+        """amplitudes of one four-gluon sub-tree term with the three ends; the caller flushes"""
+        I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2), a3%s = wdot(%s, x3);" % (k, tname, k, tname, k, tname)); I.flops += 3 * FL5["wdot"]
+        I.jamp("a1%s" % k, c_close(ONE, col, cchi(w)), pidx)
+        I.jamp("a2%s" % k, c_close(cq1(w), col, ONE), pidx)
+        I.jamp("a3%s" % k, c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
 
     # one instance per last gluon w: the three end vectors are formed once, then two nested table-driven loops run over the
     # 3 + 6 four-gluon sub-trees (unrolled they were ~8 k instructions and instruction-fetch bound; as 45 independent small
@@ -510,7 +518,7 @@ def build_k3(stride, pidx):
             J.ldw("p1", lay.PAIR[p1]); J.ldw("p2", lay.PAIR[p2]); J.kvec("k1", list(p1)); J.kvec("k2", list(p2))
             J.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); J.flops += FL5["v3_current"]
             close3(J, w, "t", c_v3(cpair(*p1), cpair(*p2)))
-            J.flush_global()
+            J.flush_direct()
             inners.append(J)
         I.inner_loop("v3", inners)
         inners = []
@@ -519,11 +527,10 @@ def build_k3(stride, pidx):
             J = Inst5(lay, stride, inner=True)
             J.ldw("pp", lay.PAIR[p]); J.leaf("e1", l1); J.leaf("e2", l2)
             J.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); J.flops += FL5["v4_dots"]
-            for k in range(3):
-                J.L("{ const W4<R> t = v4_current(%d, dots, pp, e1, e2);" % k); J.flops += FL5["v4_current"]
-                close3(J, w, "t", c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
-                J.L("}")
-            J.flush_global()
+            for k in range(3):          # the three contact structures share colour flows: their nine amplitudes are combined first
+                J.L("const W4<R> t%d = v4_current(%d, dots, pp, e1, e2);" % (k, k)); J.flops += FL5["v4_current"]
+                close3(J, w, "t%d" % k, c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)), "_%d" % k)
+            J.flush_direct()
             inners.append(J)
         I.inner_loop("v4", inners)
         insts.append(I)
@@ -541,8 +548,7 @@ def build_k3(stride, pidx):
             for k in range(3):
                 I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, p1, p2, em), jtt);" % (k, k)); I.flops += FL5["v4_current"] + FL5["wdot"]
                 I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(*p1), cpair(*p2), c_leaf(m)), ONE), pidx)
-            I.flush_jamps()
-            I.flush_global()
+            I.flush_direct()
             insts.append(I)
     add_group("pair_pair_v4", insts, 1)
     return lay, groups
