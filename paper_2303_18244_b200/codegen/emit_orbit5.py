@@ -109,7 +109,7 @@ class Inst5(Inst):
         shared-memory accumulator there is a read-modify-write plus a flush for nothing."""
         for sigma, u, z in self.grouped_updates():
             re, im = self.unit_times(u, z)
-            self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)(%s)); atomicAdd(g + npad, (RJ)(%s)); }" % (self.P(2 * sigma), re, im))
+            self.L("{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)(%s)); atomicAdd(g + npad32, (RJ)(%s)); }" % (self.P(2 * sigma), re, im))
             self.flops += 2
 
     def inner_loop(self, name, inners):
@@ -135,7 +135,7 @@ class Inst5(Inst):
         the result is deterministic run to run."""
         for sigma, loc in sorted(self.local.items(), key=lambda t: t[1]):
             o = eo(self.lay.J + 2 * loc, self.stride)
-            self.L("{ RJ* g = gj + (long)%s * npad; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
+            self.L("{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad32, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
                    % (self.P(2 * sigma), o, o + 1, o, o + 1))
             self.flops += 2; self.redundant += 2     # staging adds are overhead of the multi-kernel split, not of the method
         self.local = {}
@@ -632,6 +632,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
     S("  const R mt = (R)mt_d;")
+    S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 131072 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
     S("  {")
     pro, fixed = prologue_lines(lay)
