@@ -193,6 +193,24 @@ def test_orbit_emitters_cover_every_diagram_term():
     assert sum(info4["shapes"].values()) == 6 + 4 + 4 + 4 + 6 + 12 + 3 + 6
     _, info5 = emit_orbit5.emit_orbit5_process()
     assert info5["namp"] == len(Topology(5).Cl) == 1890 and info5["ncol"] == 120
-    # shared-memory budgets: one 128-thread CTA (FP64) for cfg 4, 96-thread CTAs for cfg 5 must fit 227 KB
+    # shared-memory budgets: one 128-thread CTA (FP64) per SM must fit 227 KB for cfg 4 and for every cfg 5 kernel
     assert info4["smem_slots"] * 8 * 128 <= 227 * 1024
-    assert all(k["slots"] * 8 * 96 <= 227 * 1024 for k in info5["kernels"])
+    assert all(k["slots"] * 8 * emit_orbit5.BLOCK1 <= 227 * 1024 for k in info5["kernels"])
+    assert sum(k["amplitudes"] for k in info5["kernels"]) == 1890
+
+
+def test_cfg5_flop_count_does_not_depend_on_the_kernel_split(monkeypatch):
+    """the algorithmic flop count of g g -> t t~ g g g (every current once, symmetric colour form, no staging adds) is a
+    property of the method: spreading the three-gluon sub-trees over 1, 2 or 3 kernels changes the executed count only"""
+    from paper_2303_18244_b200.codegen import emit_orbit5
+    seen = {}
+    for parts in (1, 2, 3):
+        monkeypatch.setattr(emit_orbit5, "K1_PARTS", parts)
+        _, info = emit_orbit5.emit_orbit5_process()
+        seen[parts] = (info["flops_per_helicity"], info["flops_executed_per_helicity"])
+        assert len(info["kernels"]) == parts + 2
+    assert len({v[0] for v in seen.values()}) == 1
+    assert seen[1][1] < seen[2][1] < seen[3][1]
+    ncol = 120
+    assert info["colour_flops"] == 2 * ncol * (ncol + 1) + 4 * ncol
+    assert 1.5e5 < seen[1][0] < seen[1][1] < 2.5e5

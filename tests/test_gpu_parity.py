@@ -411,3 +411,40 @@ def test_event_slicing_of_the_staged_pipeline(me):
     assert np.array_equal(whole[:cut], head) and np.array_equal(whole[cut:], tail)
     assert np.isfinite(whole).all() and (whole > 0).all()
     ctx.close()
+
+
+_AB_SCRIPT = """
+import sys, numpy as np
+sys.path.insert(0, {root!r})
+import inputs
+import paper_2303_18244_b200 as me
+cfg = inputs.CONFIGS[4]
+n = 200
+ctx = me.MEContext(4)
+rnd = me.me_philox_uniform(cfg["seed"], 0, n, cfg["nfinal"])
+mom, _ = ctx.me_rambo(1500.0, rnd)
+ctx.me_filter_helicities(mom, 32)
+np.save({out!r}, np.stack([ctx.me_compute(mom, n, p).cpu().numpy() for p in (me.ME_FP64, me.ME_MIXED, me.ME_FP32)]))
+"""
+
+
+@pytest.mark.parametrize("env", ["ME_COLOR_MMA_SYNC", "ME_COLOR_FMA"])
+def test_alternative_colour_sum_kernels_agree_with_the_default(me, tmp_path, env):
+    """the colour-sum kernels kept for A/B timing (warp-level TF32 MMA instead of tcgen05; plain FMA instead of the tensor
+    cores) are selected by an environment variable read at library load, so they run in a subprocess; they must agree with
+    the default kernels to the accuracy of the precision (FP64: rounding order only)"""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    outs = {}
+    for tag, extra in (("default", {}), ("alt", {env: "1"})):
+        out = str(tmp_path / (tag + ".npy"))
+        e = dict(os.environ, **extra)
+        e.pop("ME_COLOR_FMA" if env != "ME_COLOR_FMA" else "ME_COLOR_MMA_SYNC", None)
+        if tag == "default":
+            e.pop(env, None)
+        subprocess.run([sys.executable, "-c", _AB_SCRIPT.format(root=root, out=out)], check=True, env=e, timeout=600)
+        outs[tag] = np.load(out)
+    d, a = outs["default"], outs["alt"]
+    assert np.isfinite(a).all() and (a > 0).all()
+    for row, tol in ((0, 1e-12), (1, 5e-6), (2, 2e-5)):
+        assert np.abs(a[row] / d[row] - 1).max() < tol, (env, row)
