@@ -203,13 +203,34 @@ class Inst:
         return {0: ("%s.re" % z, "%s.im" % z), 1: ("-%s.re" % z, "-%s.im" % z),
                 2: ("-%s.im" % z, "%s.re" % z), 3: ("%s.im" % z, "-%s.re" % z)}[u]
 
+    JBATCH = 4     # accumulators read, updated and written back together
+
+    def emit_accumulate(self, ups):
+        """ups = [(shared-memory offset expression, re, im)]: J[offset] += (re, im).  The offsets are run-time values in the
+        looped shapes, so the compiler must assume that consecutive read-modify-writes alias and chains them (load -> add ->
+        store -> next load: one shared-memory latency per update, with one warp per scheduler to hide it).  The flows of one
+        flush are distinct by construction: all loads of a batch are issued first, then the adds, then the stores."""
+        for b0 in range(0, len(ups), self.JBATCH):
+            batch = ups[b0:b0 + self.JBATCH]
+            if len(batch) == 1:
+                self.L("cacc<R>(sm + %s, %s, %s);" % batch[0])
+                continue
+            self.L("{ R " + ", ".join("jr%d, ji%d" % (i, i) for i in range(len(batch))) + ";")
+            for i, (o, re, im) in enumerate(batch):
+                self.L("  cget<R>(sm + %s, jr%d, ji%d);" % (o, i, i))
+            for i, (o, re, im) in enumerate(batch):
+                self.L("  cset<R>(sm + %s, jr%d + (%s), ji%d + (%s));" % (o, i, re, i, im))
+            self.L("}")
+
     def flush_jamps(self):
         """one shared-memory read-modify-write (a single 128-bit load and store) per colour flow touched since the
         last flush; amplitudes that feed the same flow are combined in registers first"""
+        ups = []
         for sigma, u, z in self.grouped_updates():
             re, im = self.unit_times(u, z)
-            self.L("cacc<R>(sm + %s, %s, %s);" % (self.off(self.lay.J + 2 * sigma), re, im))
+            ups.append((self.off(self.lay.J + 2 * sigma), re, im))
             self.flops += 2
+        self.emit_accumulate(ups)
 
 
 # colour polynomials (phases folded in, see topology.py): strings are tuples of gluon labels

@@ -93,6 +93,7 @@ class Inst5(Inst):
             self.scopes[-1].add(name)
 
     def flush_jamps(self):
+        ups = []
         for sigma, u, z in self.grouped_updates():
             owner = self.parent if self.parent is not None else self
             loc = owner.local.setdefault(sigma, len(owner.local))
@@ -100,8 +101,9 @@ class Inst5(Inst):
             re, im = self.unit_times(u, z)
             o = eo(self.lay.J + 2 * loc, self.stride)
             # the slot of a flow differs between the iterations of a nested loop: table-driven there, immediate otherwise
-            self.L("cacc<R>(sm + %s, %s, %s);" % (self.P(o) if self.parent is not None else "%d" % o, re, im))
+            ups.append((self.P(o) if self.parent is not None else "%d" % o, re, im))
             self.flops += 2
+        self.emit_accumulate(ups)
 
     def flush_direct(self):
         """pending jamp updates go straight into the global staging buffer, one fire-and-forget reduction per colour flow
