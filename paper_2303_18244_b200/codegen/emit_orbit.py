@@ -26,7 +26,7 @@ N = 4
 NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
-UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
+UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
 UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)    # FP32 (8 warps/SM, registers to spare)
 
 
@@ -425,7 +425,10 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("namespace me {")
     for gname, tmpl, rows in groups:
         nf = len(tmpl.params)
-        S("static __device__ const int tab_%s_%s[%d][%d] = {" % (name, gname, len(rows), nf))
+        # fully unrolled shapes: `static const`, so that every entry folds into an immediate; looped shapes: __constant__
+        # (uniform-index reads through the constant cache instead of a global load in front of every shared-memory access)
+        looped = UNROLL.get(gname, 1) < len(rows)
+        S("%s int tab_%s_%s[%d][%d] = {" % ("__constant__" if looped else "static __device__ const", name, gname, len(rows), nf))
         for r in rows:
             S("  {%s}," % ", ".join(str(v) for v in r))
         S("};")
