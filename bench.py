@@ -226,7 +226,7 @@ def main():
                 "frac": ach / PEAK_TFLOPS["fp64"],
                 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel at the full config, from the committed
                 # ncu --set full capture (profiles/r1_ttxgg_fp64_orbit.md); algorithmic bytes = 200 B/event = 104.9 MB
-                "traffic": 113.6e6 if (HL == 3 and n == 524288) else None,
+                "traffic": 107.1e6 if (HL == 3 and n == 524288) else None,
                 "traffic_source": "profiles/r1_ttxgg_fp64_orbit.md" if (HL == 3 and n == 524288) else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md clocks; no FP64 entry in MEASURED_PEAKS.json)",
                 "peak_measured_fma_chain": peak_meas["fp64"], "frac_of_measured": ach / peak_meas["fp64"],
