@@ -22,6 +22,7 @@ from .topology import color_matrix
 N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
 K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56)
@@ -481,7 +482,7 @@ def build_k2(stride, pidx):
 def build_k3(stride, pidx):
     # no Q1 / CHI slots: the one-gluon quark currents are needed exactly once each (in `ends`) and are formed there:
     # 214 slots per thread -> 128 threads per CTA
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=0, want_q1chi=False)
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=K3_JACC, want_q1chi=False)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -516,25 +517,27 @@ def build_k3(stride, pidx):
         inners = []
         for b0 in quad[1:]:
             p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
-            J = Inst5(lay, stride, inner=True)
+            J = Inst5(lay, stride, inner=True, parent=I if K3_JACC else None)
             J.ldw("p1", lay.PAIR[p1]); J.ldw("p2", lay.PAIR[p2]); J.kvec("k1", list(p1)); J.kvec("k2", list(p2))
             J.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); J.flops += FL5["v3_current"]
             close3(J, w, "t", c_v3(cpair(*p1), cpair(*p2)))
-            J.flush_direct()
+            J.flush_jamps() if K3_JACC else J.flush_direct()
             inners.append(J)
         I.inner_loop("v3", inners)
         inners = []
         for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
             l1, l2 = [l for l in quad if l not in p]
-            J = Inst5(lay, stride, inner=True)
+            J = Inst5(lay, stride, inner=True, parent=I if K3_JACC else None)
             J.ldw("pp", lay.PAIR[p]); J.leaf("e1", l1); J.leaf("e2", l2)
             J.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); J.flops += FL5["v4_dots"]
             for k in range(3):          # the three contact structures share colour flows: their nine amplitudes are combined first
                 J.L("const W4<R> t%d = v4_current(%d, dots, pp, e1, e2);" % (k, k)); J.flops += FL5["v4_current"]
                 close3(J, w, "t%d" % k, c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)), "_%d" % k)
-            J.flush_direct()
+            J.flush_jamps() if K3_JACC else J.flush_direct()
             inners.append(J)
         I.inner_loop("v4", inners)
+        if K3_JACC:
+            I.flush_global()
         insts.append(I)
     add_group("quads", insts, 1)
     # ---- V4(pair, pair', eps_m) on the bare line
@@ -701,7 +704,7 @@ def emit_orbit5_process(name="gg_ttxggg"):
     ncol = len(perms)
     files, kinfo = {}, []
     builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
-    blocks = (BLOCK1,) * len(builders)
+    blocks = (BLOCK1,) * (len(builders) - 1) + (BLOCK if K3_JACC else BLOCK1,)
     for ki, b in enumerate(builders):
         lay, groups = b(blocks[ki], pidx)
         src, info = emit_kernel(name, ki, lay, groups, blocks[ki])
