@@ -110,7 +110,7 @@ me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
 /* The hot path.  Asynchronous on `stream`
  * (a cudaStream_t passed as void*; null = default stream).  No host<->device copy, no
  * synchronisation (except a one-off scratch allocation for ME_GG_TTXGGG the first time a
- * larger n is seen; that process is evaluated in slices of 131072 events so the scratch
+ * larger n is seen; that process is evaluated in slices of 65536 events so the scratch
  * never exceeds 3.8 GB).
  *   d_momenta : DEVICE, FP64 in every precision mode, AoSoA [ceil(n/P)][npar][4][P] with
  *               P = me_info.page and component order (E,px,py,pz); event e lives at page e/P,

@@ -637,7 +637,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
     S("  const R mt = (R)mt_d;")
-    S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 131072 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
+    S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 65536 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
     S("  {")
     pro, fixed = prologue_lines(lay)

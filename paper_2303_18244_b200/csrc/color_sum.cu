@@ -73,8 +73,8 @@ __global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restric
   }
 }
 
-// events are processed in slices so that the staging buffer stays bounded (3.8 GB in FP64) whatever n is
-#define ME_EVENT_SLICE 131072L
+// events are processed in slices so that the staging buffer stays bounded (32 helicities x 240 rows x 65536 events: 3.8 GB in FP64) whatever n is
+#define ME_EVENT_SLICE 65536L
 size_t multi_scratch_bytes(int precision, long npad, int ncol) {
   const long np = npad < ME_EVENT_SLICE ? npad : ME_EVENT_SLICE;
   return (size_t)ME_HEL_CHUNK * ncol * 2 * np * (precision == 2 ? sizeof(float) : sizeof(double));

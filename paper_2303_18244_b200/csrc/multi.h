@@ -6,7 +6,7 @@
 #pragma once
 #include "kernels.h"
 
-#define ME_HEL_CHUNK 16   // helicities staged per pass
+#define ME_HEL_CHUNK 32   // helicities staged per pass
 #ifndef ME_HEL_PER_CTA
 #define ME_HEL_PER_CTA 4   // helicities looped inside one CTA of a diagram kernel (grid.y covers the chunk)
 #endif

@@ -397,8 +397,8 @@ def test_ragged_sizes_and_determinism_large_processes(me, proc):
 
 
 def test_event_slicing_of_the_staged_pipeline(me):
-    """g g -> t t~ g g g processes more than 131072 events in slices (bounded staging buffer): one call over 140000 events
-    equals two calls on the two slices bit for bit."""
+    """g g -> t t~ g g g processes more than 65536 events in slices (bounded staging buffer): one call over 140000 events
+    (three slices) equals two calls on a head of 131072 and the tail, bit for bit."""
     cfg = inputs.CONFIGS[4]
     n, cut = 140000, 131072
     ctx = me.MEContext(4)
