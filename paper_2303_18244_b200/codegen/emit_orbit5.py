@@ -22,6 +22,7 @@ from .topology import color_matrix
 N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+K2_DIRECT = True  # kernel o1: amplitude combinations go straight to the staging buffer instead of through local accumulators
 K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
 K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
@@ -408,7 +409,7 @@ def spair(p):
 def build_k2(stride, pidx):
     # 226 slots per thread -> 128 threads per CTA: no Q1 slots (the row-side one-gluon currents are formed where they are
     # used: 5 per ten uses would do, +14 % flops), only the pair propagators, 8 local jamp accumulators flushed per sub-block
-    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=8, want_q1chi=False, want_chi=True, ik2_sizes=(2,))
+    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=0 if K2_DIRECT else 8, want_q1chi=False, want_chi=True, ik2_sizes=(2,))
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -429,7 +430,12 @@ def build_k2(stride, pidx):
             cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
             I.redundant += 2 * (FL5["slash_col"] + FL5["col_step"])      # each chi2 set is formed for 3 masks A
             I.L("const W4<R> xa = slash_col(em, ca), xb = slash_col(em, cb), xc = slash_col(em, cc);"); I.flops += 3 * FL5["slash_col"]
-            for (rn, rcol) in rows:
+            for ri, (rn, rcol) in enumerate(rows):
+                if K2_DIRECT:       # the twelve amplitudes of this sub-block are combined per colour flow and added once
+                    I.L("const Cx<R> a0_%d = row_col(%s, xa), a1_%d = row_col(%s, xb), a2_%d = row_col(%s, xc);" % (ri, rn, ri, rn, ri, rn)); I.flops += 3 * FL5["row_col"]
+                    for k, (cn, ccol) in enumerate(cols):
+                        I.jamp("a%d_%d" % (k, ri), c_close(rcol, c_leaf(m), ccol), pidx)
+                    continue
                 I.L("{ const Cx<R> a0 = row_col(%s, xa), a1 = row_col(%s, xb), a2 = row_col(%s, xc);" % (rn, rn, rn)); I.flops += 3 * FL5["row_col"]
                 for k, (cn, ccol) in enumerate(cols):
                     I.jamp("a%d" % k, c_close(rcol, c_leaf(m), ccol), pidx)
@@ -441,10 +447,11 @@ def build_k2(stride, pidx):
             I.L("{ const Cx<R> a0 = row_col(ra, xp), a1 = row_col(rb, xp), a2 = row_col(rc, xp);"); I.flops += 3 * FL5["row_col"]
             for k, (rn, rcol) in enumerate(rows):
                 I.jamp("a%d" % k, c_close(rcol, cpair(c, d), cchi(m)), pidx)
-            I.flush_jamps()
+            I.flush_direct() if K2_DIRECT else I.flush_jamps()
             I.L("}")
             I.L("}")
-            I.flush_global()
+            if not K2_DIRECT:
+                I.flush_global()
         insts.append(I)
     add_group("rows2", insts, 1)
     # ---- cols2 loop: B = {c,d}; q1(x) . pair(P)-slash . chi2(B)
@@ -467,9 +474,10 @@ def build_k2(stride, pidx):
             I.L("const Cx<R> a0 = row_col(r, ca), a1 = row_col(r, cb), a2 = row_col(r, cc);"); I.flops += 3 * FL5["row_col"]
             for k, (cn, ccol) in enumerate(cols):
                 I.jamp("a%d" % k, c_close(cq1(x), cpair(*p), ccol), pidx)
-            I.flush_jamps()
+            I.flush_direct() if K2_DIRECT else I.flush_jamps()
             I.L("}")
-            I.flush_global()
+            if not K2_DIRECT:
+                I.flush_global()
         insts.append(I)
     add_group("cols2", insts, 1)
     return lay, groups
