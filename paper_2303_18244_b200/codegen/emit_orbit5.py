@@ -22,11 +22,12 @@ from .topology import color_matrix
 N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: Q.w - w.Q)
 K2_DIRECT = True  # kernel o1: amplitude combinations go straight to the staging buffer instead of through local accumulators
 K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
 K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
-FL5 = dict(FL, cx_comb=56)
+FL5 = dict(FL, cx_comb=56, wadd=8)
 
 
 class Layout5:
@@ -337,13 +338,24 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             park = lambda nm: (lambda T_: T_.stw(lay.TMP, nm))
             fetch = lambda nm: (lambda T_: T_.ldw(nm, lay.TMP))
             T.L("{"); mk_chi("chw", w, ew)(T); park("chw")(T); T.L("}")
-            # quad = V3(t, eps_u) closing three ways with the last gluon w
-            dots_with(T, [fetch("chw"), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                      lambda col: c_close(ONE, quad(col), cchi(w)))
-            dots_with(T, [mk_q1("q1w", w, ew), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                      lambda col: c_close(cq1(w), quad(col), ONE))
-            dots_with(T, [ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
-                      lambda col: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
+            # quad = V3(t, eps_u) closing three ways with the last gluon w: on the t~ end (colour Q.w), on the t end (w.Q), or through a
+            # three-gluon vertex on the bare line (colour Q.w - w.Q).  MERGE_V3 folds the current of the third, y3, into the
+            # other two: two scopes instead of three
+            y3 = lambda T_: (T_.fv("jtt"), T_.L("const W4<R> y3 = v3_dual(%s, jtt, padd(kM, %s), %s, ik5);" % (ew, ku, kw)))
+            if MERGE_V3:
+                dots_with(T, [fetch("chw"), ik4, y3], "v3_dual(%s, wadd(bilinear(ub, chw), y3), kM, %s, ik4)" % (eu, ku),
+                          2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(ONE, quad(col), cchi(w)))
+                dots_with(T, [mk_q1("q1w", w, ew), ik4, y3], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
+                          2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(cq1(w), quad(col), ONE))
+                T.namp += 6; counter[0] += 1      # the six V3-closing terms are inside the twelve above
+                T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
+            else:
+                dots_with(T, [fetch("chw"), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+                          lambda col: c_close(ONE, quad(col), cchi(w)))
+                dots_with(T, [mk_q1("q1w", w, ew), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
+                          lambda col: c_close(cq1(w), quad(col), ONE))
+                dots_with(T, [ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
+                          lambda col: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
             # ubar . t-slash . chi2: eps_u attached to chi1(w)
             dots_with(T, [qc, fetch("chw")], "bilinear(ub, col_step(slash_col(%s, chw), qc, mt, iqc))" % eu, stc,
                       lambda col: c_close(ONE, col, c_step(c_leaf(u), cchi(w))))
@@ -503,15 +515,27 @@ def build_k3(stride, pidx):
         I.flops += FL5["quark_step2"] + FL5["slash_col"] + FL5["col_step"]
         I.redundant += I.flops - f0                    # kernel 2 forms the same ten currents
         I.L("const R ik4 = %s;" % I.ik2(*quad))
-        I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv), x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
+        # the last gluon w closes a sub-tree Q three ways: on the t~ end (colour Q.w), on the t end (w.Q), or through a three-gluon
+        # vertex on the bare line, whose colour is the commutator Q.w - w.Q: its current x3 is folded into the other two
+        # (MERGE_V3), which leaves two dot products and two jamp groups per sub-tree term instead of three
+        I.L("const W4<R> x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
+        if MERGE_V3:
+            I.L("const W4<R> x1 = wadd(bilinear(ub, chw), x3), x2 = wsub(bilinear(q1w, vv), x3);"); I.flops += 2 * FL5["wadd"]
+        else:
+            I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv);")
         I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
 
     def close3(I, w, tname, col, k=""):
         """amplitudes of one four-gluon sub-tree term with the three ends; the caller flushes"""
-        I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2), a3%s = wdot(%s, x3);" % (k, tname, k, tname, k, tname)); I.flops += 3 * FL5["wdot"]
+        if MERGE_V3:
+            I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2);" % (k, tname, k, tname)); I.flops += 2 * FL5["wdot"]
+            I.namp += 1                 # the V3 closing is inside a1 and a2
+        else:
+            I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2), a3%s = wdot(%s, x3);" % (k, tname, k, tname, k, tname)); I.flops += 3 * FL5["wdot"]
         I.jamp("a1%s" % k, c_close(ONE, col, cchi(w)), pidx)
         I.jamp("a2%s" % k, c_close(cq1(w), col, ONE), pidx)
-        I.jamp("a3%s" % k, c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
+        if not MERGE_V3:
+            I.jamp("a3%s" % k, c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
 
     # one instance per last gluon w: the three end vectors are formed once, then two nested table-driven loops run over the
     # 3 + 6 four-gluon sub-trees (unrolled they were ~8 k instructions and instruction-fetch bound; as 45 independent small

@@ -399,6 +399,12 @@ template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>&
   o.i1 = r.i3 * A + r.i2 * qx - r.r2 * qy + ms * r.i1;
   return o;
 }
+template <typename R> ME_DEV W4<R> wadd(const W4<R>& a, const W4<R>& b) {
+  return {a.r0 + b.r0, a.i0 + b.i0, a.r1 + b.r1, a.i1 + b.i1, a.r2 + b.r2, a.i2 + b.i2, a.r3 + b.r3, a.i3 + b.i3};
+}
+template <typename R> ME_DEV W4<R> wsub(const W4<R>& a, const W4<R>& b) {
+  return {a.r0 - b.r0, a.i0 - b.i0, a.r1 - b.r1, a.i1 - b.i1, a.r2 - b.r2, a.i2 - b.i2, a.r3 - b.r3, a.i3 - b.i3};
+}
 // dual of the three-gluon vertex:  v3_current(W1, W2, k1, k2, ik2) . J  ==  W1 . v3_dual(W2, J, k1, k2, ik2)
 //   D = [ W2 ((k1-k2).J) + (k1+2k2) (W2.J) - J ((2k1+k2).W2) ] * ik2
 template <typename R> ME_DEV W4<R> v3_dual(const W4<R>& W2, const W4<R>& J, const P4<R>& k1, const P4<R>& k2, R ik2) {
