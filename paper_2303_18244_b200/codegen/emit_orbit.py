@@ -25,6 +25,8 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 N = 4
 NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
+MERGE_ORDERED = True   # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
+MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: T.w - w.T)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
 UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
 UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)    # FP32 (8 warps/SM, registers to spare)
@@ -261,6 +263,15 @@ def c_close(left, mid, right):  # closing vertex: phase i
 ONE = {(): 1}
 
 
+def _cdiff(A, B, C):
+    """colour polynomial A - (B - C); empty when the colour-ordering identity A = B - C holds"""
+    out = dict(A)
+    for P, k in ((B, -1), (C, 1)):
+        for st, v in P.items():
+            out[st] = out.get(st, 0) + k * v
+    return {st: v for st, v in out.items() if abs(v) > 1e-12}
+
+
 def build_groups(stride):
     lay = Layout()
     perms = list(permutations(range(N)))
@@ -318,8 +329,14 @@ def build_groups(stride):
         I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc), kabc = padd(kab, kc);"); I.flops += 16
         I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pac", lay.PAIR[(a, c)]); I.ldw("pbc", lay.PAIR[(b, c)])
         I.ldw("chiw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
-        I.L("const W4<R> j1 = bilinear(ub, chiw);"); I.L("const W4<R> j2 = bilinear(q1w, vv);"); I.flops += 2 * FL["bilinear"]
+        # the last gluon w closes the sub-tree three ways: on the t~ end (colour T.w), on the t end (w.T), or through a
+        # three-gluon vertex on the bare line, whose colour is the commutator T.w - w.T.  MERGE_V3 folds the dual current dd of
+        # the third into the other two: two dot products and two jamp groups per term instead of three
         I.L("const W4<R> dd = v3_dual(ew, jtt, kabc, kw, %s);" % I.ik2(a, b, c, w)); I.flops += FL["v3_dual"]
+        if MERGE_V3:
+            I.L("const W4<R> j1 = wadd(bilinear(ub, chiw), dd), j2 = wsub(bilinear(q1w, vv), dd);"); I.flops += 2 * FL["bilinear"] + 16
+        else:
+            I.L("const W4<R> j1 = bilinear(ub, chiw);"); I.L("const W4<R> j2 = bilinear(q1w, vv);"); I.flops += 2 * FL["bilinear"]
         ik3 = I.ik2(a, b, c)
         I.L("const R ik3 = %s;" % ik3)
         terms = [("t0", "v3_current(pab, ec, kab, kc, ik3)", c_v3(cpair(a, b), c_leaf(c))),
@@ -330,10 +347,15 @@ def build_groups(stride):
             terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
         for i, (nm, expr, col) in enumerate(terms):
             I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["v3_current"] if i < 3 else FL["v4_current"]
-            I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2), a3 = wdot(%s, dd);" % (nm, nm, nm)); I.flops += 3 * FL["wdot"]
+            if MERGE_V3:
+                I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2);" % (nm, nm)); I.flops += 2 * FL["wdot"]
+                I.namp += 1                                                   # V3(t, eps_w) on the bare line is inside a1 and a2
+            else:
+                I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2), a3 = wdot(%s, dd);" % (nm, nm, nm)); I.flops += 3 * FL["wdot"]
             I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)                    # ubar . t-slash . chi_w
             I.jamp("a2", c_close(cq1(w), col, ONE), pidx)                     # q1(w) . t-slash . v
-            I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)       # V3(t, eps_w) on the bare line
+            if not MERGE_V3:
+                I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)   # V3(t, eps_w) on the bare line
             I.flush_jamps()
             I.L("}")
         insts.append(I)
@@ -349,18 +371,38 @@ def build_groups(stride):
         I.ldw("chic", lay.CHI + 8 * c); I.ldw("chid", lay.CHI + 8 * d)
         I.qvec("q", [a, b])
         I.L("const R iq2 = %s;" % I.iq(a, b))
-        I.L("const W4<R> xp = slash_col(pcd, vv), xcd = slash_col(ec, chid), xdc = slash_col(ed, chic);"); I.flops += 3 * FL["slash_col"]
-        rows = [("ra", "quark_step2(ub, pab, q, mt, iq2)", c_step(ONE, cpair(a, b))),
-                ("rb", "quark_step2(q1a, eb, q, mt, iq2)", c_step(cq1(a), c_leaf(b))),
-                ("rc", "quark_step2(q1b, ea, q, mt, iq2)", c_step(cq1(b), c_leaf(a)))]
-        for nm, expr, col in rows:
-            I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["quark_step2"]
-            I.L("  const Cx<R> a1 = row_col(%s, xp), a2 = row_col(%s, xcd), a3 = row_col(%s, xdc);" % (nm, nm, nm)); I.flops += 3 * FL["row_col"]
-            I.jamp("a1", c_close(col, cpair(c, d), ONE), pidx)
-            I.jamp("a2", c_close(col, c_leaf(c), cchi(d)), pidx)
-            I.jamp("a3", c_close(col, c_leaf(d), cchi(c)), pidx)
+        if MERGE_ORDERED:
+            # colour-ordered two-gluon currents: the pair current (a commutator, colour ab - ba) is folded into the two stepwise
+            # currents, on the row side before the common propagator and on the column side before the dot product; the nine
+            # diagram terms of this block become four colour-ordered amplitudes, one colour flow each
+            col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
+            assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
+            for col in (col_ab, col_ba):
+                assert not _cdiff(c_close(col, cpair(c, d), ONE), c_close(col, c_leaf(c), cchi(d)), c_close(col, c_leaf(d), cchi(c)))
+            I.L("const W4<R> sp = row_slash(ub, pab), xp = slash_col(pcd, vv);"); I.flops += FL["row_slash"] + FL["slash_col"]
+            I.L("const W4<R> rab = row_step(wadd(row_slash(q1a, eb), sp), q, mt, iq2), rba = row_step(wsub(row_slash(q1b, ea), sp), q, mt, iq2);")
+            I.flops += 2 * (FL["row_slash"] + 8 + FL["col_step"])
+            I.L("const W4<R> xcd = wadd(slash_col(ec, chid), xp), xdc = wsub(slash_col(ed, chic), xp);"); I.flops += 2 * (FL["slash_col"] + 8)
+            I.L("const Cx<R> a1 = row_col(rab, xcd), a2 = row_col(rab, xdc), a3 = row_col(rba, xcd), a4 = row_col(rba, xdc);"); I.flops += 4 * FL["row_col"]
+            I.jamp("a1", c_close(col_ab, c_leaf(c), cchi(d)), pidx)
+            I.jamp("a2", c_close(col_ab, c_leaf(d), cchi(c)), pidx)
+            I.jamp("a3", c_close(col_ba, c_leaf(c), cchi(d)), pidx)
+            I.jamp("a4", c_close(col_ba, c_leaf(d), cchi(c)), pidx)
+            I.namp += 5
             I.flush_jamps()
-            I.L("}")
+        else:
+            I.L("const W4<R> xp = slash_col(pcd, vv), xcd = slash_col(ec, chid), xdc = slash_col(ed, chic);"); I.flops += 3 * FL["slash_col"]
+            rows = [("ra", "quark_step2(ub, pab, q, mt, iq2)", c_step(ONE, cpair(a, b))),
+                    ("rb", "quark_step2(q1a, eb, q, mt, iq2)", c_step(cq1(a), c_leaf(b))),
+                    ("rc", "quark_step2(q1b, ea, q, mt, iq2)", c_step(cq1(b), c_leaf(a)))]
+            for nm, expr, col in rows:
+                I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["quark_step2"]
+                I.L("  const Cx<R> a1 = row_col(%s, xp), a2 = row_col(%s, xcd), a3 = row_col(%s, xdc);" % (nm, nm, nm)); I.flops += 3 * FL["row_col"]
+                I.jamp("a1", c_close(col, cpair(c, d), ONE), pidx)
+                I.jamp("a2", c_close(col, c_leaf(c), cchi(d)), pidx)
+                I.jamp("a3", c_close(col, c_leaf(d), cchi(c)), pidx)
+                I.flush_jamps()
+                I.L("}")
         insts.append(I)
     add_group("rows2", insts)
     # ---- B3: q1(x) . pair(y,z)-slash . chi_w

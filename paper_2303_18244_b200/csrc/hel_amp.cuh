@@ -384,9 +384,9 @@ template <typename R> ME_DEV W4<R> col_step(const W4<R>& X, const P4<R>& q, R m,
   o.i3 = A * X.i1 + qx * X.i0 + qy * X.r0 + ms * X.i3;
   return o;
 }
-// same arithmetic order for the row current (scale q once, then 4 products per component)
-template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden) {
-  const W4<R> r = row_slash(psibar, V);
+// row current grown from the t end: r' = r (q-slash + m) * iden  (r = psibar V-slash already formed); same arithmetic order
+// as col_step (scale q once, then 4 products per component)
+template <typename R> ME_DEV W4<R> row_step(const W4<R>& r, const P4<R>& q, R m, R iden) {
   const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;
   W4<R> o;
   o.r2 = r.r0 * A - r.r1 * qx + r.i1 * qy + ms * r.r2;
@@ -398,6 +398,9 @@ template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>&
   o.r1 = r.r3 * A + r.r2 * qx + r.i2 * qy + ms * r.r1;
   o.i1 = r.i3 * A + r.i2 * qx - r.r2 * qy + ms * r.i1;
   return o;
+}
+template <typename R> ME_DEV W4<R> quark_step2(const W4<R>& psibar, const W4<R>& V, const P4<R>& q, R m, R iden) {
+  return row_step(row_slash(psibar, V), q, m, iden);
 }
 template <typename R> ME_DEV W4<R> wadd(const W4<R>& a, const W4<R>& b) {
   return {a.r0 + b.r0, a.i0 + b.i0, a.r1 + b.r1, a.i1 + b.i1, a.r2 + b.r2, a.i2 + b.i2, a.r3 + b.r3, a.i3 + b.i3};
