@@ -22,12 +22,13 @@ from .topology import color_matrix
 N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
+MERGE_ORDERED = True  # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
 MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: Q.w - w.Q)
 K2_DIRECT = True  # kernel o1: amplitude combinations go straight to the staging buffer instead of through local accumulators
 K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
 K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
-FL5 = dict(FL, cx_comb=56, wadd=8)
+FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 
 
 class Layout5:
@@ -146,6 +147,15 @@ class Inst5(Inst):
         self.local = {}
 
 
+def _cdiff(A, B, C):
+    """colour polynomial A - (B - C); empty when the colour-ordering identity A = B - C holds"""
+    out = dict(A)
+    for P, k in ((B, -1), (C, 1)):
+        for st, v in P.items():
+            out[st] = out.get(st, 0) + k * v
+    return {st: v for st, v in out.items() if abs(v) > 1e-12}
+
+
 def cpair(a, b):
     return c_v3(c_leaf(a), c_leaf(b))
 
@@ -186,6 +196,15 @@ def emit_rows2(I, a, b, pab, ea, eb):
     I.qvec("qr", [a, b])
     I.L("const R iqr = %s;" % I.iq(a, b))
     I.fv("ub")
+    if MERGE_ORDERED:
+        # colour-ordered form: the pair current (a commutator, colour ab - ba) is folded into the two stepwise currents in
+        # front of their common propagator: two currents, one colour string each, instead of three
+        col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
+        assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
+        I.L("const W4<R> spr = row_slash(ub, %s);" % pab)
+        I.L("const W4<R> rb = row_step(wadd(row_slash(q1a, %s), spr), qr, mt, iqr), rc = row_step(wsub(row_slash(q1b, %s), spr), qr, mt, iqr);" % (eb, ea))
+        I.flops += 3 * FL5["row_slash"] + 2 * (FL5["wadd"] + FL5["col_step"])
+        return [("rb", col_ab), ("rc", col_ba)]
     I.L("const W4<R> ra = quark_step2(ub, %s, qr, mt, iqr), rb = quark_step2(q1a, %s, qr, mt, iqr), rc = quark_step2(q1b, %s, qr, mt, iqr);" % (pab, eb, ea))
     I.flops += 3 * FL5["quark_step2"]
     return [("ra", c_step(ONE, cpair(a, b))), ("rb", c_step(cq1(a), c_leaf(b))), ("rc", c_step(cq1(b), c_leaf(a)))]
@@ -198,6 +217,14 @@ def emit_cols2(I, c, d, pcd, ec, ed, tag=""):
     I.qvec("qc" + tag, row_side)
     I.L("const R iqc%s = %s;" % (tag, I.iq(*row_side)))
     I.fv("vv")
+    if MERGE_ORDERED:
+        col_cd, col_dc = c_step(c_leaf(c), cchi(d)), c_step(c_leaf(d), cchi(c))
+        assert not _cdiff(c_step(cpair(c, d), ONE), col_cd, col_dc)
+        I.L("const W4<R> spc%s = slash_col(%s, vv);" % (tag, pcd))
+        I.L("const W4<R> cb%s = col_step(wadd(slash_col(%s, chd%s), spc%s), qc%s, mt, iqc%s), cc%s = col_step(wsub(slash_col(%s, chc%s), spc%s), qc%s, mt, iqc%s);"
+            % (tag, ec, tag, tag, tag, tag, tag, ed, tag, tag, tag, tag))
+        I.flops += 3 * FL5["slash_col"] + 2 * (FL5["wadd"] + FL5["col_step"])
+        return [("cb" + tag, col_cd), ("cc" + tag, col_dc)]
     I.L("const W4<R> ca%s = col_step(slash_col(%s, vv), qc%s, mt, iqc%s), cb%s = col_step(slash_col(%s, chd%s), qc%s, mt, iqc%s),"
         " cc%s = col_step(slash_col(%s, chc%s), qc%s, mt, iqc%s);" % (tag, pcd, tag, tag, tag, ec, tag, tag, tag, tag, ed, tag, tag, tag))
     I.flops += 3 * (FL5["slash_col"] + FL5["col_step"])
@@ -347,8 +374,11 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
                           2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(ONE, quad(col), cchi(w)))
                 dots_with(T, [mk_q1("q1w", w, ew), ik4, y3], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
                           2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(cq1(w), quad(col), ONE))
-                T.namp += 6; counter[0] += 1      # the six V3-closing terms are inside the twelve above
-                T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
+                idx3 = counter[0]; counter[0] += 1
+                if part is None or idx3 // (18 // nparts) == part:
+                    T.namp += 6                   # the six V3-closing terms are inside the twelve above
+                if part is None or (idx3 - 1) // (18 // nparts) == part:
+                    T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
             else:
                 dots_with(T, [fetch("chw"), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
                           lambda col: c_close(ONE, quad(col), cchi(w)))
@@ -439,16 +469,19 @@ def build_k2(stride, pidx):
             I.L("{")
             I.leaf("em", m); I.leaf("ec", c); I.leaf("ed", d)
             I.ldw("pcd", lay.PAIR[(c, d)])
+            f0 = I.flops
             cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
-            I.redundant += 2 * (FL5["slash_col"] + FL5["col_step"])      # each chi2 set is formed for 3 masks A
-            I.L("const W4<R> xa = slash_col(em, ca), xb = slash_col(em, cb), xc = slash_col(em, cc);"); I.flops += 3 * FL5["slash_col"]
+            I.redundant += 2 * (I.flops - f0) // 3      # each chi2 set is formed for 3 masks A
+            I.namp += (9 - len(rows) * len(cols)) + (3 - len(rows))     # diagram terms folded into the colour-ordered currents
+            xs = ["x%d" % k for k in range(len(cols))]
+            I.L("const W4<R> " + ", ".join("%s = slash_col(em, %s)" % (xn, cn) for xn, (cn, _) in zip(xs, cols)) + ";"); I.flops += len(cols) * FL5["slash_col"]
             for ri, (rn, rcol) in enumerate(rows):
-                if K2_DIRECT:       # the twelve amplitudes of this sub-block are combined per colour flow and added once
-                    I.L("const Cx<R> a0_%d = row_col(%s, xa), a1_%d = row_col(%s, xb), a2_%d = row_col(%s, xc);" % (ri, rn, ri, rn, ri, rn)); I.flops += 3 * FL5["row_col"]
+                if K2_DIRECT:       # the amplitudes of this sub-block are combined per colour flow and added once
+                    I.L("const Cx<R> " + ", ".join("a%d_%d = row_col(%s, %s)" % (k, ri, rn, xn) for k, xn in enumerate(xs)) + ";"); I.flops += len(xs) * FL5["row_col"]
                     for k, (cn, ccol) in enumerate(cols):
                         I.jamp("a%d_%d" % (k, ri), c_close(rcol, c_leaf(m), ccol), pidx)
                     continue
-                I.L("{ const Cx<R> a0 = row_col(%s, xa), a1 = row_col(%s, xb), a2 = row_col(%s, xc);" % (rn, rn, rn)); I.flops += 3 * FL5["row_col"]
+                I.L("{ const Cx<R> " + ", ".join("a%d = row_col(%s, %s)" % (k, rn, xn) for k, xn in enumerate(xs)) + ";"); I.flops += len(xs) * FL5["row_col"]
                 for k, (cn, ccol) in enumerate(cols):
                     I.jamp("a%d" % k, c_close(rcol, c_leaf(m), ccol), pidx)
                 I.flush_jamps()
@@ -456,7 +489,7 @@ def build_k2(stride, pidx):
             # (2,2,1): rows . pair(c,d)-slash . chi1(m)
             I.ldw("chm", lay.CHI + 8 * m)
             I.L("const W4<R> xp = slash_col(pcd, chm);"); I.flops += FL5["slash_col"]
-            I.L("{ const Cx<R> a0 = row_col(ra, xp), a1 = row_col(rb, xp), a2 = row_col(rc, xp);"); I.flops += 3 * FL5["row_col"]
+            I.L("{ const Cx<R> " + ", ".join("a%d = row_col(%s, xp)" % (k, rn) for k, (rn, _) in enumerate(rows)) + ";"); I.flops += len(rows) * FL5["row_col"]
             for k, (rn, rcol) in enumerate(rows):
                 I.jamp("a%d" % k, c_close(rcol, cpair(c, d), cchi(m)), pidx)
             I.flush_direct() if K2_DIRECT else I.flush_jamps()
@@ -474,6 +507,7 @@ def build_k2(stride, pidx):
         I.leaf("ec", c); I.leaf("ed", d)
         I.ldw("pcd", lay.PAIR[(c, d)])
         cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
+        I.namp += 3 * (3 - len(cols))
         for x in rest:
             p = spair([l for l in rest if l != x])
             I.L("{")
@@ -483,7 +517,7 @@ def build_k2(stride, pidx):
             I.redundant += I.flops - f0
             I.ldw("pp", lay.PAIR[p])
             I.L("const W4<R> r = row_slash(q1x, pp);"); I.flops += FL5["row_slash"]
-            I.L("const Cx<R> a0 = row_col(r, ca), a1 = row_col(r, cb), a2 = row_col(r, cc);"); I.flops += 3 * FL5["row_col"]
+            I.L("const Cx<R> " + ", ".join("a%d = row_col(r, %s)" % (k, cn) for k, (cn, _) in enumerate(cols)) + ";"); I.flops += len(cols) * FL5["row_col"]
             for k, (cn, ccol) in enumerate(cols):
                 I.jamp("a%d" % k, c_close(cq1(x), cpair(*p), ccol), pidx)
             I.flush_direct() if K2_DIRECT else I.flush_jamps()
