@@ -27,6 +27,7 @@ NPAR = 6
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 MERGE_ORDERED = True   # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
 MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: T.w - w.T)
+MERGE_TRIPLE = True   # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
 UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
 UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)    # FP32 (8 warps/SM, registers to spare)
@@ -345,8 +346,21 @@ def build_groups(stride):
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL["v4_dots"]
         for k in range(3):
             terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
+        if MERGE_TRIPLE:
+            # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three
+            # channels, and the Jacobi identity col1 = col0 + col2 leaves two independent currents instead of six terms
+            cols = [t[2] for t in terms]
+            assert all(not _cdiff(cols[3 + k], cols[k], {}) for k in range(3)) and not _cdiff(cols[1], cols[0], _pscale(cols[2], -1))
+            I.L("const W4<R> t14 = wadd(%s, %s);" % (terms[1][1], terms[4][1]))
+            I.L("const W4<R> s0 = wadd(wadd(%s, %s), t14), s2 = wadd(wadd(%s, %s), t14);" % (terms[0][1], terms[3][1], terms[2][1], terms[5][1]))
+            I.flops += 3 * (FL["v3_current"] + FL["v4_current"]) + 5 * 8
+            I.namp += 4 * 3                              # diagram terms folded into the two ordered currents
+            terms = [("s0", None, cols[0]), ("s2", None, cols[2])]
         for i, (nm, expr, col) in enumerate(terms):
-            I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["v3_current"] if i < 3 else FL["v4_current"]
+            if expr is None:
+                I.L("{")
+            else:
+                I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["v3_current"] if i < 3 else FL["v4_current"]
             if MERGE_V3:
                 I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2);" % (nm, nm)); I.flops += 2 * FL["wdot"]
                 I.namp += 1                                                   # V3(t, eps_w) on the bare line is inside a1 and a2

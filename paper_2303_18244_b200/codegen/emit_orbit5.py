@@ -23,6 +23,7 @@ N = 5
 NPAR = 7
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
 MERGE_ORDERED = True  # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
+MERGE_TRIPLE = True  # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
 MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: Q.w - w.Q)
 K2_DIRECT = True  # kernel o1: amplitude combinations go straight to the staging buffer instead of through local accumulators
 K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
@@ -290,7 +291,15 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
         # the six three-gluon terms on M (registers for the whole block); their inputs die in this scope
         tcol = [c_v3(cpair(a, b), c_leaf(c)), c_v3(cpair(a, c), c_leaf(b)), c_v3(cpair(b, c), c_leaf(a))] + \
                [c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c)) for k in range(3)]
-        I.L("W4<R> t0, t1, t2, t3, t4, t5; P4<R> kM;")
+        if MERGE_TRIPLE:
+            # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three
+            # channels, and the Jacobi identity col1 = col0 + col2 leaves two independent currents instead of six terms
+            assert all(not _cdiff(tcol[3 + k], tcol[k], {}) for k in range(3)) and not _cdiff(tcol[1], tcol[0], {st: -v for st, v in tcol[2].items()})
+            tnames, tcol = ["s0", "s2"], [tcol[0], tcol[2]]
+            I.L("W4<R> s0, s2; P4<R> kM;")
+        else:
+            tnames = ["t%d" % k for k in range(6)]
+            I.L("W4<R> t0, t1, t2, t3, t4, t5; P4<R> kM;")
         I.L("{")
         for nm, l in (("ea", a), ("eb", b), ("ec", c)):
             I.leaf(nm, l)
@@ -303,8 +312,14 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
         I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once (as pxy of its own block) would do
         I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
-        I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
-        I.L("t3 = v4_current(0, dots, ea, eb, ec); t4 = v4_current(1, dots, ea, eb, ec); t5 = v4_current(2, dots, ea, eb, ec);")
+        if MERGE_TRIPLE:
+            I.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
+            I.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
+            I.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
+            I.flops += 5 * FL5["wadd"]
+        else:
+            I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
+            I.L("t3 = v4_current(0, dots, ea, eb, ec); t4 = v4_current(1, dots, ea, eb, ec); t5 = v4_current(2, dots, ea, eb, ec);")
         I.flops += 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
         I.L("}")
         if part is not None and part > 0:             # the split kernels each rebuild pxy and the six terms: all of it overhead
@@ -325,8 +340,9 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             T.L("  const W4<R> X = %s;" % xexpr); T.flops += flops
             if post is not None:
                 post(T)
-            T.L("  const Cx<R> a0 = wdot(t0, X), a1 = wdot(t1, X), a2 = wdot(t2, X), a3 = wdot(t3, X), a4 = wdot(t4, X), a5 = wdot(t5, X);")
-            T.flops += 6 * FL5["wdot"]
+            T.L("  const Cx<R> " + ", ".join("a%d = wdot(%s, X)" % (k, tn) for k, tn in enumerate(tnames)) + ";")
+            T.flops += len(tnames) * FL5["wdot"]
+            T.namp += 6 - len(tnames)                # diagram terms folded into the colour-ordered currents
             for i, col in enumerate(tcol):
                 T.jamp("a%d" % i, colour_of_term(col), pidx)
             T.flush_jamps()
