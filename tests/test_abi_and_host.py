@@ -213,4 +213,4 @@ def test_cfg5_flop_count_does_not_depend_on_the_kernel_split(monkeypatch):
     assert seen[1][1] < seen[2][1] < seen[3][1]
     ncol = 120
     assert info["colour_flops"] == 2 * ncol * (ncol + 1) + 4 * ncol
-    assert 1.5e5 < seen[1][0] < seen[1][1] < 2.5e5
+    assert 1.0e5 < seen[1][0] < seen[1][1] < 2.5e5
