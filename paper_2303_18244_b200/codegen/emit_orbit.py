@@ -70,20 +70,27 @@ class Layout:
     npar = NPAR
 
     def __init__(self):
+        # Slot order: what stays in shared memory in every precision first (momenta, bases, column currents, propagator
+        # denominators: TM0 = 98 slots), then the categories the FP64 kernels keep in tensor memory (hel_amp.cuh "Tensor memory
+        # as a per-thread scratchpad": 6 gluon-pair currents, 4 row currents, 24 jamps = 128 slots = 256 TMEM columns).  The FP32
+        # kernel keeps all 226 slots in shared memory (two CTAs per SM fit as it is).
         A = SlotAlloc()
         self.MOM = A.vec(4 * N)            # signed gluon momenta (+p incoming, -p outgoing)
         self.PT = A.vec(4)                 # p_t
         self.GBS = [A.vec(5) for _ in range(N)]
-        pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
-        self.PAIR = {p: A.vec(8) for p in pairs}
-        self.Q1 = A.vec(8 * N)
         self.CHI = A.vec(8 * N)
-        self.J = A.vec(2 * 24)
         masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") >= 2]
         self.IK2 = {m: A.scalar() for m in masks2}
         masksq = [m for m in range(1, (1 << N) - 1)]
         self.IQ = {m: A.scalar() for m in masksq}
+        self.TM0 = A.vec(0)                # first TMEM slot (even)
+        pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+        self.PAIR = {p: A.vec(8) for p in pairs}
+        self.Q1 = A.vec(8 * N)
+        self.J = A.vec(2 * 24)
         self.nslots = A.n + (A.n & 1)
+        self.tm_cols = 2 * (self.nslots - self.TM0)
+        assert self.tm_cols <= 256 and self.TM0 <= 113, (self.TM0, self.tm_cols)   # two CTAs per SM: 256 of 512 columns, 113 slots of smem each
 
 
 def mask_of(*labels):
@@ -112,6 +119,8 @@ class Inst:
         self.jamp_codes = []
         self.pending = []          # (sigma, code, amp) waiting for flush_jamps()
         self.zcount = 0
+        self.tm0 = getattr(lay, "TM0", None)      # slots >= tm0 live in tensor memory in the FP64 kernels (None: no TMEM)
+        self.inflight = []         # 4-vector loads issued, not yet converted (TMEM loads are asynchronous)
 
     tbname = "tb"          # name of the parameter-table row pointer in the emitted loop body
 
@@ -122,7 +131,13 @@ class Inst:
     def off(self, slot):                       # shared-memory element offset of a slot
         return self.P(eo(slot, self.stride))
 
+    def in_tm(self, slot):
+        return self.tm0 is not None and slot >= self.tm0
+
     def L(self, s):
+        for name in self.inflight:            # one tcgen05.wait::ld covers every load issued before it
+            self.lines.append("const W4<R> %s = xldw_get<R, TM>(%s_x);" % (name, name))
+        self.inflight = []
         self.lines.append(s)
 
     # ---- operand helpers
@@ -146,10 +161,17 @@ class Inst:
         self.L("const P4<R> %s = %s;" % (name, expr))
 
     def ldw(self, name, slot):
-        self.L("const W4<R> %s = ldw<R>(sm + %s);" % (name, self.off(slot)))
+        if self.in_tm(slot):
+            self.lines.append("XW<R, TM> %s_x; xldw_issue<R, TM>(%s_x, sm, tm, %s);" % (name, name, self.off(slot)))
+            self.inflight.append(name)
+        else:
+            self.lines.append("const W4<R> %s = ldw<R>(sm + %s);" % (name, self.off(slot)))     # does not end the in-flight group
 
     def stw(self, slot, name):
-        self.L("stw<R>(sm + %s, %s);" % (self.off(slot), name))
+        if self.in_tm(slot):
+            self.L("xstw<R, TM>(sm, tm, %s, %s); xwait_st<TM>();" % (self.off(slot), name))     # later loops read it with tcgen05.ld
+        else:
+            self.L("stw<R>(sm + %s, %s);" % (self.off(slot), name))
 
     def ik2(self, *labels):
         return "sm[%s]" % self.off(self.lay.IK2[mask_of(*labels)])
@@ -213,6 +235,20 @@ class Inst:
         looped shapes, so the compiler must assume that consecutive read-modify-writes alias and chains them (load -> add ->
         store -> next load: one shared-memory latency per update, with one warp per scheduler to hide it).  The flows of one
         flush are distinct by construction: all loads of a batch are issued first, then the adds, then the stores."""
+        if self.in_tm(self.lay.J):
+            # jamps in tensor memory: tcgen05.ld x4 / st x4 per flow; the stores of the previous batch must have completed first
+            for b0 in range(0, len(ups), self.JBATCH):
+                batch = ups[b0:b0 + self.JBATCH]
+                self.L("{ R " + ", ".join("jr%d, ji%d" % (i, i) for i in range(len(batch))) + "; XC<R, TM> "
+                       + ", ".join("jx%d" % i for i in range(len(batch))) + "; xwait_st<TM>();")
+                for i, (o, re, im) in enumerate(batch):
+                    self.L("  xcget_issue<R, TM>(jx%d, sm, tm, %s);" % (i, o))
+                for i, (o, re, im) in enumerate(batch):
+                    self.L("  xcget_get<R, TM>(jx%d, jr%d, ji%d);" % (i, i, i))
+                for i, (o, re, im) in enumerate(batch):
+                    self.L("  xcset<R, TM>(sm, tm, %s, jr%d + (%s), ji%d + (%s));" % (o, i, re, i, im))
+                self.L("}")
+            return
         for b0 in range(0, len(ups), self.JBATCH):
             batch = ups[b0:b0 + self.JBATCH]
             if len(batch) == 1:
@@ -476,8 +512,10 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter) — do not edit.")
     S("// g g -> t t~ g g: 123 diagrams, %d amplitudes in %d looped shapes, 24 colour flows; %d shared-memory slots per thread." % (namp, len(groups), lay.nslots))
     S("#define ME_SM_STRIDE %d" % block)
+    S("#define ME_TM_SLOT0 %d" % lay.TM0)
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
+    S("#include <stdlib.h>")
     S("namespace me {")
     for gname, tmpl, rows in groups:
         nf = len(tmpl.params)
@@ -488,14 +526,23 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         for r in rows:
             S("  {%s}," % ", ".join(str(v) for v in r))
         S("};")
-    S("template <typename R, typename RC>")
+    S("// TM: slots >= %d (gluon-pair currents, row currents, jamps) live in tensor memory, %d columns per CTA: two CTAs per SM in FP64" % (lay.TM0, lay.tm_cols))
+    S("template <typename R, typename RC, bool TM>")
     S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
       " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out,"
       " const int* __restrict__ helpe) {" % (block, name))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
-    S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
-    S("  if (e >= npad) return;")
+    S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
+    S("  if (!TM && e0 >= npad) return;")
+    S("  const long e = e0 < npad ? e0 : npad - 1;      // TMEM kernel: whole CTA stays (tcgen05 alloc / dealloc are CTA-wide); tail lanes repeat the last event")
+    S("  uint32_t tm = 0, tm_base = 0;")
+    S("  if constexpr (TM) {")
+    S("    static_assert(sizeof(R) == 8 && ME_SM_STRIDE == 128, \"TMEM scratchpad: FP64, 128 threads per CTA\");")
+    S("    __shared__ uint32_t tm_slot;")
+    S("    tm_base = tm_alloc(&tm_slot, %d);" % lay.tm_cols)
+    S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16);      // this warp's quarter of the 128 lanes")
+    S("  }")
     S("  const R mt = (R)mt_d;")
     S("  SpinorBasis<R> sbt, sbtb;")
     S("  {")
@@ -543,8 +590,14 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
     S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
+    S("    if constexpr (TM) {")
+    S("      const uint32_t zz[16] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};")
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) cset<R>(sm + ME_EO(%d + 2 * s), (R)0, (R)0);" % (ncol, lay.J))
+    S("      for (int s = 0; s < %d; ++s) tm_st16(tm + ME_TM_COL(ME_EO(%d)) + 16 * s, zz);" % (ncol // 4, lay.J))
+    S("    } else {")
+    S("#pragma unroll")
+    S("      for (int s = 0; s < %d; ++s) cset<R>(sm + ME_EO(%d + 2 * s), (R)0, (R)0);" % (ncol, lay.J))
+    S("    }")
     for gname, tmpl, rows in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
         S("#pragma unroll(sizeof(R) == 8 ? %d : %d)" % (UNROLL.get(gname, 1), UNROLL32.get(gname, 1)))
@@ -553,35 +606,57 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         for l in tmpl.lines:
             S("      " + l)
         S("    }")
-    S("    if (jamp_out != nullptr && e < n) {")
-    S("#pragma unroll")
-    S("      for (int s = 0; s < %d; ++s) jamp_out[(long)s * n + e] = (double)sm[ME_EO(%d + s)];" % (2 * ncol, lay.J))
-    S("    }")
     S("    RC cr[%d], ci[%d];" % (ncol, ncol))
+    S("    if constexpr (TM) {")
+    S("      XW<R, TM> jx[%d];" % (ncol // 4))
+    S("      xwait_st<TM>();")
     S("#pragma unroll")
-    S("    for (int s = 0; s < %d; ++s) { R jr, ji; cget<R>(sm + ME_EO(%d + 2 * s), jr, ji); cr[s] = (RC)jr; ci[s] = (RC)ji; }" % (ncol, lay.J))
+    S("      for (int s = 0; s < %d; ++s) xldw_issue<R, TM>(jx[s], sm, tm, ME_EO(%d + 8 * s));" % (ncol // 4, lay.J))
+    S("#pragma unroll")
+    S("      for (int s = 0; s < %d; ++s) {" % (ncol // 4))
+    S("        const W4<R> w = xldw_get<R, TM>(jx[s]);")
+    S("        if (jamp_out != nullptr && e0 < n) {")
+    S("          const R v[8] = {w.r0, w.i0, w.r1, w.i1, w.r2, w.i2, w.r3, w.i3};")
+    S("#pragma unroll")
+    S("          for (int k = 0; k < 8; ++k) jamp_out[(long)(8 * s + k) * n + e0] = (double)v[k];")
+    S("        }")
+    S("        cr[4 * s] = (RC)w.r0; ci[4 * s] = (RC)w.i0; cr[4 * s + 1] = (RC)w.r1; ci[4 * s + 1] = (RC)w.i1;")
+    S("        cr[4 * s + 2] = (RC)w.r2; ci[4 * s + 2] = (RC)w.i2; cr[4 * s + 3] = (RC)w.r3; ci[4 * s + 3] = (RC)w.i3;")
+    S("      }")
+    S("    } else {")
+    S("      if (jamp_out != nullptr && e0 < n) {")
+    S("#pragma unroll")
+    S("        for (int s = 0; s < %d; ++s) jamp_out[(long)s * n + e0] = (double)sm[ME_EO(%d + s)];" % (2 * ncol, lay.J))
+    S("      }")
+    S("#pragma unroll")
+    S("      for (int s = 0; s < %d; ++s) { R jr, ji; cget<R>(sm + ME_EO(%d + 2 * s), jr, ji); cr[s] = (RC)jr; ci[s] = (RC)ji; }" % (ncol, lay.J))
+    S("    }")
     for l in cs_lines:
         S("    " + l)
     S("    const double meh = (double)cs;")
-    S("    if (me_hel != nullptr && e < n) me_hel[(long)h * n + e] = meh * norm_hel;")
+    S("    if (me_hel != nullptr && e0 < n) me_hel[(long)h * n + e0] = meh * norm_hel;")
     S("    acc += meh;")
     S("  }")
-    S("  if (me_out != nullptr && e < n) me_out[e] = acc * norm_hel * inv_avg;")
+    S("  if (me_out != nullptr && e0 < n) me_out[e0] = acc * norm_hel * inv_avg;")
+    S("  if constexpr (TM) tm_free(tm_base, %d);" % lay.tm_cols)
     S("}")
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
-    S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d;" % (lay.nslots, block, lay.nslots, block))
+    S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.nslots, block, lay.TM0, block))
+    S("  // FP64 amplitudes (double and mixed): tensor-memory kernel, two CTAs per SM; ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
+    S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
     S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event")
+    S("#define ME_LAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
+    S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
+    S("    K<<<grid, %d, SMEM, a.stream>>>(ME_ARGS); } while (0)" % block)
     S("  if (precision == 0) {")
-    S("    cudaFuncSetAttribute(k_%s<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);" % name)
-    S("    k_%s<double, double><<<grid, %d, smd, a.stream>>>(ME_ARGS);" % (name, block))
+    S("    if (no_tmem) ME_LAUNCH((k_%s<double, double, false>), smd); else ME_LAUNCH((k_%s<double, double, true>), smt);" % (name, name))
     S("  } else if (precision == 1) {")
-    S("    cudaFuncSetAttribute(k_%s<double, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);" % name)
-    S("    k_%s<double, float><<<grid, %d, smd, a.stream>>>(ME_ARGS);" % (name, block))
+    S("    if (no_tmem) ME_LAUNCH((k_%s<double, float, false>), smd); else ME_LAUNCH((k_%s<double, float, true>), smt);" % (name, name))
     S("  } else {")
-    S("    cudaFuncSetAttribute(k_%s<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smf);" % name)
-    S("    k_%s<float, float><<<grid, %d, smf, a.stream>>>(ME_ARGS);" % (name, block))
+    S("    ME_LAUNCH((k_%s<float, float, false>), smf);" % name)
     S("  }")
+    S("#undef ME_LAUNCH")
     S("#undef ME_ARGS")
     S("  return cudaGetLastError();")
     S("}")

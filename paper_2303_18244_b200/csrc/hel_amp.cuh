@@ -17,6 +17,7 @@
 // =====================================================================================
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 namespace me {
 
@@ -354,6 +355,115 @@ template <typename R> ME_DEV void cacc(R* p, R dre, R dim) {
   typedef typename Pair2<R>::T R2;
   R2* q = reinterpret_cast<R2*>(p);
   R2 v = *q; v.x += dre; v.y += dim; *q = v;
+}
+}  // namespace me
+
+// ------------------------------------------------------------------------------------
+// Tensor memory as a per-thread scratchpad (FP64 kernels of g g -> t t~ g g).  The diagram kernels have no matrix
+// product to give to tcgen05.mma, but with 226 FP64 slots per thread shared memory admits only ONE 128-thread CTA per SM
+// (one warp per scheduler: every shared-memory and FP64 latency is exposed).  The 256 KB of TMEM are 128 lanes x 512
+// 32-bit columns; a thread that owns lane (warp % 4) * 32 + laneid can keep 128 more FP64 slots in 256 columns of it,
+// reached with tcgen05.ld / tcgen05.st (.32x32b: lane i of the warp <-> TMEM lane base + i, the column offset is
+// warp-uniform, which table-driven lockstep code satisfies by construction).  Two CTAs per SM then fit: 98 slots in
+// shared memory + 128 in TMEM each.  Slot s >= ME_TM_SLOT0 lives in TMEM at column 2 * (s - ME_TM_SLOT0); the emitter
+// keeps passing the shared-memory element offset of the slot (what the FP32 kernel uses) and ME_TM_COL converts it.
+// Loads are split into issue / get so that several are in flight before the one tcgen05.wait::ld; the loaded registers
+// are operands of the wait so that no use can be scheduled above it.
+// ------------------------------------------------------------------------------------
+#ifndef ME_TM_SLOT0
+#define ME_TM_SLOT0 0
+#endif
+// (assumes ME_SM_STRIDE == 128: the element offset of even slot s is 128 s; checked where the TMEM kernel is instantiated)
+#define ME_TM_COL(off) ((uint32_t)((off) >> 6) - (uint32_t)(2 * ME_TM_SLOT0))
+namespace me {
+ME_DEV void tm_ld16(uint32_t (&r)[16], uint32_t a) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(a));
+}
+ME_DEV void tm_wait_ld16(uint32_t (&r)[16]) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;"
+               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]), "+r"(r[9]),
+                 "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]));
+}
+ME_DEV void tm_ld4(uint32_t (&r)[4], uint32_t a) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
+}
+ME_DEV void tm_wait_ld4(uint32_t (&r)[4]) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]));
+}
+ME_DEV void tm_st16(uint32_t a, const uint32_t (&r)[16]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(a),
+               "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]),
+               "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]));
+}
+ME_DEV void tm_st4(uint32_t a, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(r0), "r"(r1), "r"(r2), "r"(r3));
+}
+// a 4-vector load in flight: from shared memory it is complete at issue; from TMEM it is 16 raw registers until xldw_get
+template <typename R, bool TM> struct XW { W4<R> w; };
+template <> struct XW<double, true> { uint32_t r[16]; };
+template <typename R, bool TM> struct XC { R re, im; };
+template <> struct XC<double, true> { uint32_t r[4]; };
+template <typename R, bool TM> ME_DEV void xldw_issue(XW<R, TM>& x, const R* sm, uint32_t tm, int off) {
+  if constexpr (TM) tm_ld16(x.r, tm + ME_TM_COL(off)); else x.w = ldw<R>(sm + off);
+}
+template <typename R, bool TM> ME_DEV W4<R> xldw_get(XW<R, TM>& x) {
+  if constexpr (TM) {
+    tm_wait_ld16(x.r);
+    return {__hiloint2double(x.r[1], x.r[0]), __hiloint2double(x.r[3], x.r[2]), __hiloint2double(x.r[5], x.r[4]), __hiloint2double(x.r[7], x.r[6]),
+            __hiloint2double(x.r[9], x.r[8]), __hiloint2double(x.r[11], x.r[10]), __hiloint2double(x.r[13], x.r[12]), __hiloint2double(x.r[15], x.r[14])};
+  } else {
+    return x.w;
+  }
+}
+template <typename R, bool TM> ME_DEV void xstw(R* sm, uint32_t tm, int off, const W4<R>& w) {
+  if constexpr (TM) {
+    const double v[8] = {w.r0, w.i0, w.r1, w.i1, w.r2, w.i2, w.r3, w.i3};
+    uint32_t r[16];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { r[2 * k] = (uint32_t)__double2loint(v[k]); r[2 * k + 1] = (uint32_t)__double2hiint(v[k]); }
+    tm_st16(tm + ME_TM_COL(off), r);
+  } else {
+    stw<R>(sm + off, w);
+  }
+}
+template <typename R, bool TM> ME_DEV void xcget_issue(XC<R, TM>& x, const R* sm, uint32_t tm, int off) {
+  if constexpr (TM) tm_ld4(x.r, tm + ME_TM_COL(off)); else cget<R>(sm + off, x.re, x.im);
+}
+template <typename R, bool TM> ME_DEV void xcget_get(XC<R, TM>& x, R& re, R& im) {
+  if constexpr (TM) {
+    tm_wait_ld4(x.r);
+    re = __hiloint2double(x.r[1], x.r[0]); im = __hiloint2double(x.r[3], x.r[2]);
+  } else {
+    re = x.re; im = x.im;
+  }
+}
+template <typename R, bool TM> ME_DEV void xcset(R* sm, uint32_t tm, int off, R re, R im) {
+  if constexpr (TM) tm_st4(tm + ME_TM_COL(off), (uint32_t)__double2loint(re), (uint32_t)__double2hiint(re), (uint32_t)__double2loint(im), (uint32_t)__double2hiint(im));
+  else cset<R>(sm + off, re, im);
+}
+// all earlier tcgen05.st of this thread are complete (needed before a tcgen05.ld that may read what they wrote)
+template <bool TM> ME_DEV void xwait_st() {
+  if constexpr (TM) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+// TMEM allocation for one CTA of 128 threads: ncols columns (power of two >= 32), address of the warp's lane quarter returned
+ME_DEV uint32_t tm_alloc(uint32_t* slot_in_smem, uint32_t ncols) {
+  const int warp = threadIdx.x >> 5;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(slot_in_smem)), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  return *slot_in_smem;
+}
+ME_DEV void tm_free(uint32_t base, uint32_t ncols) {
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if ((threadIdx.x >> 5) == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(ncols) : "memory");
 }
 }  // namespace me
 
