@@ -30,13 +30,18 @@ K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude comb
 K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
+# FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
+TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
+TM_K3 = ("PAIR",)         # kernel o2: 10 gluon-pair currents = 80 slots = 160 columns
 
 
 class Layout5:
     """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5), scratch=False):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5), scratch=False, tm=()):
+        # tm: categories ("PAIR", "CHI") that the FP64 kernel keeps in tensor memory (hel_amp.cuh "Tensor memory as a per-thread
+        # scratchpad"); they are allocated last, from the even slot TM0 on, so that the shared-memory part is contiguous
         A = SlotAlloc()
         self.FERM = None
         if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
@@ -45,14 +50,15 @@ class Layout5:
         self.PT = A.vec(4)
         self.GBS = [A.vec(5) for _ in range(N)]
         self.PAIR = {}
-        if want_pairs:
-            pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+        pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+        if want_pairs and "PAIR" not in tm:
             self.PAIR = {p: A.vec(8) for p in pairs}
         self.Q1 = self.CHI = None             # one-gluon currents of both quark ends (kernel 1 rebuilds them at each use instead)
         if want_q1chi:
+            assert "CHI" not in tm
             self.Q1 = A.vec(8 * N)
             self.CHI = A.vec(8 * N)
-        elif want_chi:
+        elif want_chi and "CHI" not in tm:
             self.CHI = A.vec(8 * N)
         self.TMP = A.vec(8) if scratch else None   # one parked current (kernel 1)
         self.J = A.vec(2 * jacc)
@@ -62,6 +68,16 @@ class Layout5:
         # quark propagators: row side sets of size 1,2 and (for the column currents) size 3,4
         masksq = [m for m in range(1, (1 << N) - 1) if want_iq_mid or bin(m).count("1") in (1, 4)]
         self.IQ = {m: A.scalar() for m in masksq}
+        if tm:
+            self.TM0 = A.vec(0)
+            if want_pairs and "PAIR" in tm:
+                self.PAIR = {p: A.vec(8) for p in pairs}
+            if want_chi and "CHI" in tm:
+                self.CHI = A.vec(8 * N)
+            self.tm_cols = 32
+            while self.tm_cols < 2 * (A.n - self.TM0):
+                self.tm_cols *= 2                      # tcgen05.alloc takes a power of two >= 32
+            assert self.tm_cols <= 256 and self.TM0 <= 113, (self.TM0, self.tm_cols)
         self.nslots = A.n + (A.n & 1)
 
 
@@ -467,7 +483,7 @@ def spair(p):
 def build_k2(stride, pidx):
     # 226 slots per thread -> 128 threads per CTA: no Q1 slots (the row-side one-gluon currents are formed where they are
     # used: 5 per ten uses would do, +14 % flops), only the pair propagators, 8 local jamp accumulators flushed per sub-block
-    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=0 if K2_DIRECT else 8, want_q1chi=False, want_chi=True, ik2_sizes=(2,))
+    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=0 if K2_DIRECT else 8, want_q1chi=False, want_chi=True, ik2_sizes=(2,), tm=TM_K2)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -552,7 +568,7 @@ def build_k2(stride, pidx):
 def build_k3(stride, pidx):
     # no Q1 / CHI slots: the one-gluon quark currents are needed exactly once each (in `ends`) and are formed there:
     # 214 slots per thread -> 128 threads per CTA
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=K3_JACC, want_q1chi=False)
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=K3_JACC, want_q1chi=False, tm=TM_K3)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -696,10 +712,15 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
     namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
     S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter, emit_orbit5.py) — do not edit.")
     S("// g g -> t t~ g g g, diagram kernel %d: %d amplitude terms in %d looped shapes; %d shared-memory slots per thread." % (ki, namp, len(groups), lay.nslots))
+    tm0 = getattr(lay, "TM0", None)
     S("#define ME_SM_STRIDE %d" % BLOCK)
+    if tm0 is not None:
+        assert BLOCK == 128
+        S("#define ME_TM_SLOT0 %d" % tm0)
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("#include \"multi.h\"")
+    S("#include <stdlib.h>")
     S("namespace me {")
     for gname, tmpl, rows, _ in groups:
         S("__constant__ int tab_%s_o%d_%s[%d][%d] = {" % (name, ki, gname, len(rows), len(tmpl.params)))
@@ -711,13 +732,23 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
             for r in srows:
                 S("  {%s}," % ", ".join(str(v) for v in r))
             S("};")
-    S("template <typename R, typename RJ>")
+    S("template <typename R, typename RJ, bool TM>")
     S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
       " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n) {" % (BLOCK, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
-    S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
-    S("  if (e >= npad) return;")
+    S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
+    S("  if (!TM && e0 >= npad) return;")
+    S("  const bool live = e0 < npad;                    // TMEM kernel: warps past the end stay for the CTA-wide alloc / dealloc and skip the helicity loop")
+    S("  const long e = live ? e0 : npad - 1;")
+    S("  uint32_t tm = 0, tm_base = 0;")
+    if tm0 is not None:
+        S("  if constexpr (TM) {")
+        S("    static_assert(sizeof(R) == 8 && ME_SM_STRIDE == 128, \"TMEM scratchpad: FP64, 128 threads per CTA\");")
+        S("    __shared__ uint32_t tm_slot;")
+        S("    tm_base = tm_alloc(&tm_slot, %d);" % lay.tm_cols)
+        S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16);      // this warp's quarter of the 128 lanes")
+        S("  }")
     S("  const R mt = (R)mt_d;")
     S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 65536 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
@@ -730,7 +761,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
     S("  }")
     S("#pragma unroll")
     S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
-    S("  const int hc_end = (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
+    S("  const int hc_end = !live ? 0 : (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
     S("  for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
@@ -756,18 +787,30 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
             S("      " + l)
         S("    }")
     S("  }")
+    if tm0 is not None:
+        S("  if constexpr (TM) tm_free(tm_base, %d);" % lay.tm_cols)
     S("}")
     S("static cudaError_t launch_o%d(int precision, const MultiArgs& a) {" % ki)
     S("  // few helicities per CTA: many short CTAs, so the last partial wave costs little (65536 events are only 4.6 waves of 96-thread CTAs)")
     S("  const dim3 grid((unsigned)((a.npad + %d - 1) / %d), (unsigned)((a.nh + ME_HEL_PER_CTA - 1) / ME_HEL_PER_CTA));" % (BLOCK, BLOCK))
     S("  if (precision == 2) {")
     S("    const size_t smb = sizeof(float) * %d * %d;" % (lay.nslots, BLOCK))
-    S("    cudaFuncSetAttribute(k_%s_o%d<float, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<float, float><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
+    S("    cudaFuncSetAttribute(k_%s_o%d<float, float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
+    S("    k_%s_o%d<float, float, false><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
     S("  } else {")
     S("    const size_t smb = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK))
-    S("    cudaFuncSetAttribute(k_%s_o%d<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<double, double><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
+    if tm0 is not None:
+        S("    // FP64 amplitudes: tensor-memory kernel (two CTAs per SM); ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
+        S("    static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
+        S("    if (!no_tmem) {")
+        S("      const size_t smt = sizeof(double) * %d * %d;" % (tm0, BLOCK))
+        S("      cudaFuncSetAttribute(k_%s_o%d<double, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smt);" % (name, ki))
+        S("      cudaFuncSetAttribute(k_%s_o%d<double, double, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);" % (name, ki))
+        S("      k_%s_o%d<double, double, true><<<grid, %d, smt, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
+        S("      return cudaGetLastError();")
+        S("    }")
+    S("    cudaFuncSetAttribute(k_%s_o%d<double, double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
+    S("    k_%s_o%d<double, double, false><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
     S("  }")
     S("  return cudaGetLastError();")
     S("}")
