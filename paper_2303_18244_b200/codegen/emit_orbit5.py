@@ -32,7 +32,9 @@ BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
-TM_K3 = ("PAIR",)         # kernel o2: 10 gluon-pair currents = 80 slots = 160 columns
+K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
+TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
+                          # K3_JACC = 0 gives two CTAs per SM but leaves the kernel bound by the L2 throughput of its 1320 RED pairs per helicity
 
 
 class Layout5:
@@ -61,7 +63,8 @@ class Layout5:
         elif want_chi and "CHI" not in tm:
             self.CHI = A.vec(8 * N)
         self.TMP = A.vec(8) if scratch else None   # one parked current (kernel 1)
-        self.J = A.vec(2 * jacc)
+        if "J" not in tm:
+            self.J = A.vec(2 * jacc)
         self.jacc = jacc
         masks2 = [m for m in range(1, 1 << N) if bin(m).count("1") in ik2_sizes]
         self.IK2 = {m: A.scalar() for m in masks2}
@@ -74,10 +77,13 @@ class Layout5:
                 self.PAIR = {p: A.vec(8) for p in pairs}
             if want_chi and "CHI" in tm:
                 self.CHI = A.vec(8 * N)
+            if "J" in tm:
+                assert jacc % 4 == 0
+                self.J = A.vec(2 * jacc)
             self.tm_cols = 32
             while self.tm_cols < 2 * (A.n - self.TM0):
                 self.tm_cols *= 2                      # tcgen05.alloc takes a power of two >= 32
-            assert self.tm_cols <= 256 and self.TM0 <= 113, (self.TM0, self.tm_cols)
+            assert self.tm_cols <= 512, (self.TM0, self.tm_cols)      # 256 columns and 113 slots: two CTAs per SM
         self.nslots = A.n + (A.n & 1)
 
 
@@ -156,6 +162,22 @@ class Inst5(Inst):
         """add the local accumulators into gj and clear them.  The add is a fire-and-forget reduction (RED.ADD, no
         read latency); every address is private to one thread, whose program order fixes the order of the adds, so
         the result is deterministic run to run."""
+        if self.in_tm(self.lay.J):
+            # accumulators in tensor memory: four flows per tcgen05.ld x16, reduced into gj, cleared with one tcgen05.st x16
+            items = sorted(self.local.items(), key=lambda t: t[1])
+            assert [loc for _, loc in items] == list(range(len(items)))
+            self.L("xwait_st<TM>();")
+            for g0 in range(0, len(items), 4):
+                grp = items[g0:g0 + 4]
+                o = eo(self.lay.J + 2 * g0, self.stride)
+                self.L("{ XW<R, TM> jx; xldw_issue<R, TM>(jx, sm, tm, %d);" % o)
+                self.L("  const W4<R> jw = xldw_get<R, TM>(jx);")
+                for k, (sigma, loc) in enumerate(grp):
+                    self.L("  { RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)jw.r%d); atomicAdd(g + npad32, (RJ)jw.i%d); }" % (self.P(2 * sigma), k, k))
+                    self.flops += 2; self.redundant += 2
+                self.L("  xstw<R, TM>(sm, tm, %d, W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0}); }" % o)
+            self.local = {}
+            return
         for sigma, loc in sorted(self.local.items(), key=lambda t: t[1]):
             o = eo(self.lay.J + 2 * loc, self.stride)
             self.L("{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad32, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
@@ -565,10 +587,10 @@ def build_k2(stride, pidx):
 # kernel 3: four-gluon sub-trees built from pairs (V3(pair,pair), V4(pair,eps,eps)) closing three ways with the last
 # gluon w, and the contact term V4(pair, pair, eps) on the bare line
 # ------------------------------------------------------------------------------------------
-def build_k3(stride, pidx):
+def build_k3(stride, pidx, jacc=0, tm=()):
     # no Q1 / CHI slots: the one-gluon quark currents are needed exactly once each (in `ends`) and are formed there:
     # 214 slots per thread -> 128 threads per CTA
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=K3_JACC, want_q1chi=False, tm=TM_K3)
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=jacc, want_q1chi=False, tm=tm)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -615,26 +637,26 @@ def build_k3(stride, pidx):
         inners = []
         for b0 in quad[1:]:
             p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
-            J = Inst5(lay, stride, inner=True, parent=I if K3_JACC else None)
+            J = Inst5(lay, stride, inner=True, parent=I if jacc else None)
             J.ldw("p1", lay.PAIR[p1]); J.ldw("p2", lay.PAIR[p2]); J.kvec("k1", list(p1)); J.kvec("k2", list(p2))
             J.L("const W4<R> t = v3_current(p1, p2, k1, k2, ik4);"); J.flops += FL5["v3_current"]
             close3(J, w, "t", c_v3(cpair(*p1), cpair(*p2)))
-            J.flush_jamps() if K3_JACC else J.flush_direct()
+            J.flush_jamps() if jacc else J.flush_direct()
             inners.append(J)
         I.inner_loop("v3", inners)
         inners = []
         for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
             l1, l2 = [l for l in quad if l not in p]
-            J = Inst5(lay, stride, inner=True, parent=I if K3_JACC else None)
+            J = Inst5(lay, stride, inner=True, parent=I if jacc else None)
             J.ldw("pp", lay.PAIR[p]); J.leaf("e1", l1); J.leaf("e2", l2)
             J.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); J.flops += FL5["v4_dots"]
             for k in range(3):          # the three contact structures share colour flows: their nine amplitudes are combined first
                 J.L("const W4<R> t%d = v4_current(%d, dots, pp, e1, e2);" % (k, k)); J.flops += FL5["v4_current"]
                 close3(J, w, "t%d" % k, c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)), "_%d" % k)
-            J.flush_jamps() if K3_JACC else J.flush_direct()
+            J.flush_jamps() if jacc else J.flush_direct()
             inners.append(J)
         I.inner_loop("v4", inners)
-        if K3_JACC:
+        if jacc:
             I.flush_global()
         insts.append(I)
     add_group("quads", insts, 1)
@@ -706,12 +728,14 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups, BLOCK):
+def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
+    """only: None (float and double instances of one template), 'double' (FP64-only variant; ki is then a tag like '2d');
+    delegate_double: tag of the FP64-only variant this kernel's launcher hands double / mixed precision to"""
     src = []
     S = src.append
     namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
     S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter, emit_orbit5.py) — do not edit.")
-    S("// g g -> t t~ g g g, diagram kernel %d: %d amplitude terms in %d looped shapes; %d shared-memory slots per thread." % (ki, namp, len(groups), lay.nslots))
+    S("// g g -> t t~ g g g, diagram kernel %s: %d amplitude terms in %d looped shapes; %d shared-memory slots per thread." % (ki, namp, len(groups), lay.nslots))
     tm0 = getattr(lay, "TM0", None)
     S("#define ME_SM_STRIDE %d" % BLOCK)
     if tm0 is not None:
@@ -723,17 +747,17 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
     S("#include <stdlib.h>")
     S("namespace me {")
     for gname, tmpl, rows, _ in groups:
-        S("__constant__ int tab_%s_o%d_%s[%d][%d] = {" % (name, ki, gname, len(rows), len(tmpl.params)))
+        S("__constant__ int tab_%s_o%s_%s[%d][%d] = {" % (name, ki, gname, len(rows), len(tmpl.params)))
         for r in rows:
             S("  {%s}," % ", ".join(str(v) for v in r))
         S("};")
         for sname, srows in getattr(tmpl, "subtables", []):
-            S("__constant__ int tab_%s_o%d_%s_%s[%d][%d] = {" % (name, ki, gname, sname, len(srows), len(srows[0])))
+            S("__constant__ int tab_%s_o%s_%s_%s[%d][%d] = {" % (name, ki, gname, sname, len(srows), len(srows[0])))
             for r in srows:
                 S("  {%s}," % ", ".join(str(v) for v in r))
             S("};")
     S("template <typename R, typename RJ, bool TM>")
-    S("__global__ void __launch_bounds__(%d) k_%s_o%d(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
+    S("__global__ void __launch_bounds__(%d) k_%s_o%s(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
       " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n) {" % (BLOCK, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
@@ -760,7 +784,10 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
         S("    stsb<R>(sm, %d, sbt); stsb<R>(sm, %d, sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
     S("  }")
     S("#pragma unroll")
-    S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
+    if tm0 is not None and lay.jacc and lay.J >= tm0:
+        S("  for (int s = 0; s < %d; ++s) xstw<R, TM>(sm, tm, ME_EO(%d) + s * 8 * ME_SM_STRIDE, W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0});" % (lay.jacc // 4, lay.J))
+    else:
+        S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
     S("  const int hc_end = !live ? 0 : (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
     S("  for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
@@ -779,42 +806,53 @@ def emit_kernel(name, ki, lay, groups, BLOCK):
         S("    // ---- %s: %d instances" % (gname, len(rows)))
         S("#pragma unroll %d" % unroll)
         S("    for (int it = 0; it < %d; ++it) {" % len(rows))
-        S("      const int* tb = tab_%s_o%d_%s[it];" % (name, ki, gname))
+        S("      const int* tb = tab_%s_o%s_%s[it];" % (name, ki, gname))
         for l in tmpl.lines:
             if "@SUB:" in l:
                 sname = l.split("@SUB:")[1].split("@")[0]
-                l = l.replace("@SUB:%s@" % sname, "tab_%s_o%d_%s_%s" % (name, ki, gname, sname))
+                l = l.replace("@SUB:%s@" % sname, "tab_%s_o%s_%s_%s" % (name, ki, gname, sname))
             S("      " + l)
         S("    }")
     S("  }")
     if tm0 is not None:
         S("  if constexpr (TM) tm_free(tm_base, %d);" % lay.tm_cols)
     S("}")
-    S("static cudaError_t launch_o%d(int precision, const MultiArgs& a) {" % ki)
+    if delegate_double is not None:
+        S("extern const MultiKernel mk_%s_o%s;" % (name, delegate_double))
+    S("static cudaError_t launch_o%s(int precision, const MultiArgs& a) {" % ki)
     S("  // few helicities per CTA: many short CTAs, so the last partial wave costs little (65536 events are only 4.6 waves of 96-thread CTAs)")
     S("  const dim3 grid((unsigned)((a.npad + %d - 1) / %d), (unsigned)((a.nh + ME_HEL_PER_CTA - 1) / ME_HEL_PER_CTA));" % (BLOCK, BLOCK))
-    S("  if (precision == 2) {")
-    S("    const size_t smb = sizeof(float) * %d * %d;" % (lay.nslots, BLOCK))
-    S("    cudaFuncSetAttribute(k_%s_o%d<float, float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<float, float, false><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (float*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
-    S("  } else {")
-    S("    const size_t smb = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK))
-    if tm0 is not None:
-        S("    // FP64 amplitudes: tensor-memory kernel (two CTAs per SM); ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
-        S("    static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
-        S("    if (!no_tmem) {")
-        S("      const size_t smt = sizeof(double) * %d * %d;" % (tm0, BLOCK))
-        S("      cudaFuncSetAttribute(k_%s_o%d<double, double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smt);" % (name, ki))
-        S("      cudaFuncSetAttribute(k_%s_o%d<double, double, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);" % (name, ki))
-        S("      k_%s_o%d<double, double, true><<<grid, %d, smt, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
-        S("      return cudaGetLastError();")
-        S("    }")
-    S("    cudaFuncSetAttribute(k_%s_o%d<double, double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);" % (name, ki))
-    S("    k_%s_o%d<double, double, false><<<grid, %d, smb, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (double*)a.gj, a.hel_per_event, a.n);" % (name, ki, BLOCK))
-    S("  }")
+    NO_TMEM = "    static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // A/B timing: shared-memory-only kernels"
+    def launch_line(inst, smem, cast):
+        S("      cudaFuncSetAttribute(k_%s_o%s<%s>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)%s);" % (name, ki, inst, smem))
+        S("      cudaFuncSetAttribute(k_%s_o%s<%s>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);" % (name, ki, inst))
+        S("      k_%s_o%s<%s><<<grid, %d, %s, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (%s*)a.gj, a.hel_per_event, a.n);" % (name, ki, inst, BLOCK, smem, cast))
+    S("  const size_t smf = sizeof(float) * %d * %d, smd = sizeof(double) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK, lay.nslots, BLOCK, tm0 or 0, BLOCK))
+    S("  (void)smf; (void)smd; (void)smt;")
+    if only == "double":
+        assert tm0 is not None
+        S("  if (precision == 2) return cudaErrorInvalidValue;")
+        S("  {")
+        launch_line("double, double, true", "smt", "double")
+        S("  }")
+    else:
+        if delegate_double is not None:
+            S(NO_TMEM)
+            S("  if (precision != 2 && !no_tmem) return mk_%s_o%s.launch(precision, a);     // FP64 amplitudes: the variant with local accumulators in tensor memory" % (name, delegate_double))
+        S("  if (precision == 2) {")
+        launch_line("float, float, false", "smf", "float")
+        S("  } else {")
+        if tm0 is not None:
+            S(NO_TMEM)
+            S("    if (!no_tmem) {         // FP64 amplitudes: tensor-memory kernel (two CTAs per SM)")
+            launch_line("double, double, true", "smt", "double")
+            S("      return cudaGetLastError();")
+            S("    }")
+        launch_line("double, double, false", "smd", "double")
+        S("  }")
     S("  return cudaGetLastError();")
     S("}")
-    S("extern const MultiKernel mk_%s_o%d = {launch_o%d};" % (name, ki, ki))
+    S("extern const MultiKernel mk_%s_o%s = {launch_o%s};" % (name, ki, ki))
     S("}  // namespace me")
     flops = sum(t.flops * len(rows) for _, t, rows, _ in groups)
     redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
@@ -829,12 +867,18 @@ def emit_orbit5_process(name="gg_ttxggg"):
     ncol = len(perms)
     files, kinfo = {}, []
     builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
-    blocks = (BLOCK1,) * (len(builders) - 1) + (BLOCK if K3_JACC else BLOCK1,)
+    blocks = (BLOCK1,) * (len(builders) - 1) + (BLOCK if (K3_JACC and not TM_K3) else BLOCK1,)
     for ki, b in enumerate(builders):
         lay, groups = b(blocks[ki], pidx)
-        src, info = emit_kernel(name, ki, lay, groups, blocks[ki])
+        last = ki == len(builders) - 1
+        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if (last and K3D_JACC) else None)
         files["gen_%s_o%d.cu" % (name, ki)] = src
         kinfo.append(info)
+        if last and K3D_JACC:      # FP64-only variant of the last kernel: local jamp accumulators in tensor memory (see TM_K3)
+            lay2, groups2 = build_k3(BLOCK1, pidx, jacc=K3D_JACC, tm=TM_K3)
+            src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="double")
+            files["gen_%s_o%dd.cu" % (name, ki)] = src2
+            info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, flops=info2["flops"], redundant=info2["redundant"])
     namp = sum(k["amplitudes"] for k in kinfo)
     assert namp == 1890, namp
     # colour sum in its symmetric form (S§8(d)): per part  sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), as for the smaller
