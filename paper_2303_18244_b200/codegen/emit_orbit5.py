@@ -31,6 +31,7 @@ K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees a
 BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
 FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
+TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
 K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
 TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
@@ -46,7 +47,7 @@ class Layout5:
         # scratchpad"); they are allocated last, from the even slot TM0 on, so that the shared-memory part is contiguous
         A = SlotAlloc()
         self.FERM = None
-        if ferm_smem:                         # ubar, v, ubar gamma v of the current helicity + the two spinor bases
+        if ferm_smem and "FERM" not in tm:    # ubar, v, ubar gamma v of the current helicity + the two spinor bases
             self.FERM = dict(ub=A.vec(8), vv=A.vec(8), jtt=A.vec(8), sbt=A.vec(5), sbtb=A.vec(5))
         self.MOM = A.vec(4 * N)
         self.PT = A.vec(4)
@@ -62,7 +63,7 @@ class Layout5:
             self.CHI = A.vec(8 * N)
         elif want_chi and "CHI" not in tm:
             self.CHI = A.vec(8 * N)
-        self.TMP = A.vec(8) if scratch else None   # one parked current (kernel 1)
+        self.TMP = A.vec(8) if (scratch and "TMP" not in tm) else None   # one parked current (kernel 1)
         if "J" not in tm:
             self.J = A.vec(2 * jacc)
         self.jacc = jacc
@@ -73,6 +74,10 @@ class Layout5:
         self.IQ = {m: A.scalar() for m in masksq}
         if tm:
             self.TM0 = A.vec(0)
+            if ferm_smem and "FERM" in tm:            # the spinor bases take a whole 8-slot vector each in TMEM (one tcgen05 x16 access)
+                self.FERM = dict(sbt=A.vec(8), sbtb=A.vec(8), ub=A.vec(8), vv=A.vec(8), jtt=A.vec(8))
+            if scratch and "TMP" in tm:
+                self.TMP = A.vec(8)
             if want_pairs and "PAIR" in tm:
                 self.PAIR = {p: A.vec(8) for p in pairs}
             if want_chi and "CHI" in tm:
@@ -116,7 +121,11 @@ class Inst5(Inst):
         for name in names:
             if any(name in sc for sc in self.scopes):
                 continue
-            self.L("const W4<R> %s = ldw<R>(sm + %d);" % (name, eo(self.lay.FERM[name], self.stride)))
+            if self.in_tm(self.lay.FERM[name]):
+                self.L("XW<R, TM> %s_x; xldw_issue<R, TM>(%s_x, sm, tm, %d);" % (name, name, eo(self.lay.FERM[name], self.stride)))
+                self.L("const W4<R> %s = xldw_get<R, TM>(%s_x);" % (name, name))
+            else:
+                self.L("const W4<R> %s = ldw<R>(sm + %d);" % (name, eo(self.lay.FERM[name], self.stride)))
             self.scopes[-1].add(name)
 
     def flush_jamps(self):
@@ -314,7 +323,7 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
     # brings the kernel from 292 to 220 slots per thread (incl. one scratch vector that carries chi1(w) / q1(u) across scopes), i.e. from 96 to 128 threads per CTA (all four schedulers busy)
-    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True, want_q1chi=False, scratch=True)
+    lay = Layout5(want_pairs=False, want_iq_mid=True, jacc=36, ferm_smem=True, want_q1chi=False, scratch=True, tm=TM_K1)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=False)
@@ -781,7 +790,10 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
     for l in pro:
         S("    " + l)
     if lay.FERM is not None:
-        S("    stsb<R>(sm, %d, sbt); stsb<R>(sm, %d, sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
+        if tm0 is not None and lay.FERM["sbt"] >= tm0:
+            S("    xstsb<R, TM>(sm, tm, ME_EO(%d), sbt); xstsb<R, TM>(sm, tm, ME_EO(%d), sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
+        else:
+            S("    stsb<R>(sm, %d, sbt); stsb<R>(sm, %d, sbtb);" % (lay.FERM["sbt"], lay.FERM["sbtb"]))
     S("  }")
     S("#pragma unroll")
     if tm0 is not None and lay.jacc and lay.J >= tm0:
@@ -794,9 +806,16 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
     if lay.FERM is not None:
         S("    {")
-        S("      const W4<R> ub = spinor_ubar(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbt"], NPAR - 1 - 2))
-        S("      const W4<R> vv = spinor_v(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbtb"], NPAR - 1 - 3))
-        S("      stw<R>(sm, %d, ub); stw<R>(sm, %d, vv); stw<R>(sm, %d, bilinear(ub, vv));" % (lay.FERM["ub"], lay.FERM["vv"], lay.FERM["jtt"]))
+        if tm0 is not None and lay.FERM["sbt"] >= tm0:
+            S("      xwait_st<TM>();")
+            S("      const W4<R> ub = spinor_ubar(xldsb<R, TM>(sm, tm, ME_EO(%d)), lam_of<R>(h, %d));" % (lay.FERM["sbt"], NPAR - 1 - 2))
+            S("      const W4<R> vv = spinor_v(xldsb<R, TM>(sm, tm, ME_EO(%d)), lam_of<R>(h, %d));" % (lay.FERM["sbtb"], NPAR - 1 - 3))
+            S("      xstw<R, TM>(sm, tm, ME_EO(%d), ub); xstw<R, TM>(sm, tm, ME_EO(%d), vv); xstw<R, TM>(sm, tm, ME_EO(%d), bilinear(ub, vv)); xwait_st<TM>();"
+              % (lay.FERM["ub"], lay.FERM["vv"], lay.FERM["jtt"]))
+        else:
+            S("      const W4<R> ub = spinor_ubar(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbt"], NPAR - 1 - 2))
+            S("      const W4<R> vv = spinor_v(ldsb<R>(sm, %d), lam_of<R>(h, %d));" % (lay.FERM["sbtb"], NPAR - 1 - 3))
+            S("      stw<R>(sm, %d, ub); stw<R>(sm, %d, vv); stw<R>(sm, %d, bilinear(ub, vv));" % (lay.FERM["ub"], lay.FERM["vv"], lay.FERM["jtt"]))
         S("    }")
     else:
         S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))

@@ -444,6 +444,20 @@ template <typename R, bool TM> ME_DEV void xcset(R* sm, uint32_t tm, int off, R 
   if constexpr (TM) tm_st4(tm + ME_TM_COL(off), (uint32_t)__double2loint(re), (uint32_t)__double2hiint(re), (uint32_t)__double2loint(im), (uint32_t)__double2hiint(im));
   else cset<R>(sm + off, re, im);
 }
+// spinor basis (five reals) in an 8-slot TMEM vector
+template <typename R, bool TM> ME_DEV SpinorBasis<R> xldsb(const R* sm, uint32_t tm, int off) {
+  if constexpr (TM) {
+    XW<R, TM> x; xldw_issue<R, TM>(x, sm, tm, off);
+    const W4<R> w = xldw_get<R, TM>(x);
+    SpinorBasis<R> g; g.a = w.r0; g.b = w.i0; g.c = w.r1; g.wp = w.i1; g.wm = w.r2; return g;
+  } else {
+    return ldsb<R>(sm + off);
+  }
+}
+template <typename R, bool TM> ME_DEV void xstsb(R* sm, uint32_t tm, int off, const SpinorBasis<R>& g) {
+  if constexpr (TM) xstw<R, TM>(sm, tm, off, W4<R>{g.a, g.b, g.c, g.wp, g.wm, (R)0, (R)0, (R)0});
+  else stsb<R>(sm + off, g);
+}
 // all earlier tcgen05.st of this thread are complete (needed before a tcgen05.ld that may read what they wrote)
 template <bool TM> ME_DEV void xwait_st() {
   if constexpr (TM) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
