@@ -216,18 +216,18 @@ def main():
     total_ms = allmax(total_ms)
     value = per_gpu * world * args.steps / (total_ms * 1e-3)
     ms_kernel = statistics.mean(per)
-    per_step_launches = info.nkernels * ((ngood + 15) // 16 if HL == 4 else 1)    # cfg 5: 3 diagram kernels + colour sum per 16-helicity chunk
+    per_step_launches = info.nkernels * ((ngood + 31) // 32 if HL == 4 else 1)    # cfg 5: 3 diagram kernels + colour sum per 32-helicity chunk (ME_HEL_CHUNK)
     launches = args.steps * per_step_launches
     results[cfg["name"]] = {"fp64": {"MEs_per_s": n * args.steps / (sum(per) * 1e-3), "ms_per_step": ms_kernel}}
     # measured FMA-chain peaks (register-resident microkernel, same box, same run)
     peak_meas = {"fp64": me.me_fma_peak(1), "fp32": me.me_fma_peak(0)}
     ach = flops_alg * n / (ms_kernel * 1e-3) * 1e-12
-    roofline = {"bound": "alu", "kernel": "k_%s<double,double>" % cfg["name"] + (" (+ colour sum)" if HL == 4 else ""), "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "k_%s<double,double,TM=true>" % cfg["name"] + (" (+ colour sum)" if HL == 4 else ""), "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
                 "frac": ach / PEAK_TFLOPS["fp64"],
                 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel at the full config, from the committed
-                # ncu --set full capture (profiles/r1_ttxgg_fp64_orbit.md); algorithmic bytes = 200 B/event = 104.9 MB
-                "traffic": 107.1e6 if (HL == 3 and n == 524288) else None,
-                "traffic_source": "profiles/r1_ttxgg_fp64_orbit.md" if (HL == 3 and n == 524288) else None,
+                # ncu --set full capture (profiles/r1_ttxgg_fp64_tmem.md: 101.8 MB read + 3.9 MB written); algorithmic bytes = 200 B/event = 104.9 MB
+                "traffic": 105.8e6 if (HL == 3 and n == 524288) else None,
+                "traffic_source": "profiles/r1_ttxgg_fp64_tmem.md" if (HL == 3 and n == 524288) else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md clocks; no FP64 entry in MEASURED_PEAKS.json)",
                 "peak_measured_fma_chain": peak_meas["fp64"], "frac_of_measured": ach / peak_meas["fp64"],
                 "flops_per_event_algorithmic": flops_alg, "flops_per_event_executed": flops_exe,
@@ -245,7 +245,7 @@ def main():
     ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
     t, pp = timed(ctx, mom, n, me.ME_FP64, args.steps, args.warmup)
     ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
-    launches += args.steps * info.nkernels * ((ngood // 2 + 15) // 16 if HL == 4 else 1)
+    launches += args.steps * info.nkernels * ((ngood // 2 + 31) // 32 if HL == 4 else 1)
     results[cfg["name"]]["fp64_parity_pairing"] = {"MEs_per_s": n / (statistics.mean(pp) * 1e-3), "ms_per_step": statistics.mean(pp)}
     if args.sweep and world == 1:
         sweep = {"batch": {}, "streams": {}}

@@ -666,6 +666,6 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
          float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name))
     S("}  // namespace me")
     info = dict(n=N, ndiagrams=123, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=per_hel,
-                flops_executed_per_helicity=per_hel, fixed_flops=fixed, colour_flops=cs_flops, smem_slots=lay.nslots, block=block,
+                flops_executed_per_helicity=per_hel, fixed_flops=fixed, colour_flops=cs_flops, smem_slots=lay.nslots, tm_slot0=lay.TM0, tm_cols=lay.tm_cols, block=block,
                 shapes={g: len(r) for g, _, r in groups}, color_num=color_num)
     return "\n".join(src) + "\n", info

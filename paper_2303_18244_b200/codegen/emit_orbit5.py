@@ -875,7 +875,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
     S("}  // namespace me")
     flops = sum(t.flops * len(rows) for _, t, rows, _ in groups)
     redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
-    return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, fixed=fixed, slots=lay.nslots,
+    return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, fixed=fixed, slots=lay.nslots, tm_slot0=tm0, tm_cols=getattr(lay, "tm_cols", 0),
                                        shapes={g: len(r) for g, _, r, _ in groups})
 
 

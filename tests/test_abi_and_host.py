@@ -197,6 +197,16 @@ def test_orbit_emitters_cover_every_diagram_term():
     assert info4["smem_slots"] * 8 * 128 <= 227 * 1024
     assert all(k["slots"] * 8 * emit_orbit5.BLOCK1 <= 227 * 1024 for k in info5["kernels"])
     assert sum(k["amplitudes"] for k in info5["kernels"]) == 1890
+    # FP64 kernels with a tensor-memory scratchpad: the slots below tm_slot0 stay in shared memory, the rest take two 32-bit TMEM
+    # columns each.  Two CTAs per SM need 2 x (dynamic + 16 B static + 1 KB reserved) <= 228 KB and 2 x tm_cols <= 512 columns.
+    def two_ctas(slot0, nslots, cols):
+        return 2 * (slot0 * 8 * 128 + 16 + 1024) <= 228 * 1024 and 2 * cols <= 512 and 2 * (nslots - slot0) <= cols
+    assert two_ctas(info4["tm_slot0"], info4["smem_slots"], info4["tm_cols"])
+    k0, k1, k2 = info5["kernels"]
+    assert two_ctas(k0["tm_slot0"], k0["slots"], k0["tm_cols"]) and two_ctas(k1["tm_slot0"], k1["slots"], k1["tm_cols"])
+    assert k2["tm_slot0"] is None                               # FP32 / fallback kernel: shared memory only
+    v = k2["fp64_variant"]                                      # FP64 variant: 48 accumulators in TMEM, one CTA per SM
+    assert v["tm_slot0"] * 8 * 128 + 16 <= 227 * 1024 and 2 * (v["slots"] - v["tm_slot0"]) <= v["tm_cols"] <= 512
 
 
 def test_cfg5_flop_count_does_not_depend_on_the_kernel_split(monkeypatch):

@@ -448,3 +448,40 @@ def test_alternative_colour_sum_kernels_agree_with_the_default(me, tmp_path, env
     assert np.isfinite(a).all() and (a > 0).all()
     for row, tol in ((0, 1e-12), (1, 5e-6), (2, 2e-5)):
         assert np.abs(a[row] / d[row] - 1).max() < tol, (env, row)
+
+
+_AB_TMEM_SCRIPT = """
+import sys, numpy as np
+sys.path.insert(0, {root!r})
+import inputs
+import paper_2303_18244_b200 as me
+proc, n = {proc}, {n}
+cfg = inputs.CONFIGS[proc]
+ctx = me.MEContext(proc)
+rnd = me.me_philox_uniform(cfg["seed"], 0, n, cfg["nfinal"])
+mom, _ = ctx.me_rambo(1500.0, rnd)
+ctx.me_filter_helicities(mom, 32)
+np.save({out!r}, np.stack([ctx.me_compute(mom, n, p).cpu().numpy() for p in (me.ME_FP64, me.ME_MIXED)]))
+"""
+
+
+@pytest.mark.parametrize("proc,n", [(3, 333), (4, 161)])
+def test_tensor_memory_kernels_agree_with_the_shared_memory_kernels(me, tmp_path, proc, n):
+    """FP64 / mixed diagram kernels of the two large processes keep part of their per-thread state in tensor memory
+    (tcgen05.ld / st, two CTAs per SM); ME_NO_TMEM=1 (read once per process) selects the shared-memory-only kernels that
+    the other parity tests do not reach.  Same arithmetic, so the two agree to rounding order (ragged n: the tail warps of the
+    last CTA take the stay-for-dealloc path of the TMEM kernels)."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    outs = {}
+    for tag, extra in (("tmem", {}), ("smem", {"ME_NO_TMEM": "1"})):
+        out = str(tmp_path / (tag + ".npy"))
+        e = dict(os.environ, **extra)
+        if tag == "tmem":
+            e.pop("ME_NO_TMEM", None)
+        subprocess.run([sys.executable, "-c", _AB_TMEM_SCRIPT.format(root=root, out=out, proc=proc, n=n)], check=True, env=e, timeout=600)
+        outs[tag] = np.load(out)
+    t, s = outs["tmem"], outs["smem"]
+    assert np.isfinite(t).all() and (t > 0).all()
+    assert np.abs(t[0] / s[0] - 1).max() < 1e-12
+    assert np.abs(t[1] / s[1] - 1).max() < 5e-6
