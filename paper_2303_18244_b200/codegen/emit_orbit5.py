@@ -33,6 +33,8 @@ FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
+K1_SYNC = False          # FP64 variant of kernel o0 (k_..._o0d): one 256-thread CTA, named barrier at every scope so that the eight warps fetch the
+                         # same instructions; measured 9.55 ms per chunk against 9.40 ms for two free-running 128-thread CTAs: off
 K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
 TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
                           # K3_JACC = 0 gives two CTAs per SM but leaves the kernel bound by the L2 throughput of its 1320 RED pairs per helicity
@@ -380,7 +382,7 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             idx = counter[0]; counter[0] += 1
             if part is not None and idx // (18 // nparts) != part:
                 return
-            T.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
+            T.L("{ if (sizeof(R) == 8) ME_FENCE; ME_SCOPE_SYNC;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
                 fn(T)
             T.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])
@@ -737,9 +739,11 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
+def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, sync=False):
     """only: None (float and double instances of one template), 'double' (FP64-only variant; ki is then a tag like '2d');
-    delegate_double: tag of the FP64-only variant this kernel's launcher hands double / mixed precision to"""
+    delegate_double: tag of the FP64-only variant this kernel's launcher hands double / mixed precision to;
+    sync: one 256-thread CTA per SM whose eight warps meet at a named barrier at every scope of the loop bodies, so that they
+    fetch the same instructions (two independent 128-thread CTAs drift apart and thrash the instruction cache)"""
     src = []
     S = src.append
     namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
@@ -748,8 +752,9 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
     tm0 = getattr(lay, "TM0", None)
     S("#define ME_SM_STRIDE %d" % BLOCK)
     if tm0 is not None:
-        assert BLOCK == 128
+        assert BLOCK in (128, 256)
         S("#define ME_TM_SLOT0 %d" % tm0)
+    S("#define ME_SCOPE_SYNC %s" % ('asm volatile("bar.sync 1, %0;" ::"r"(nlive) : "memory")' if sync else ""))
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("#include \"multi.h\"")
@@ -777,11 +782,14 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
     S("  uint32_t tm = 0, tm_base = 0;")
     if tm0 is not None:
         S("  if constexpr (TM) {")
-        S("    static_assert(sizeof(R) == 8 && ME_SM_STRIDE == 128, \"TMEM scratchpad: FP64, 128 threads per CTA\");")
+        S("    static_assert(sizeof(R) == 8, \"TMEM scratchpad: FP64\");")
         S("    __shared__ uint32_t tm_slot;")
-        S("    tm_base = tm_alloc(&tm_slot, %d);" % lay.tm_cols)
-        S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16);      // this warp's quarter of the 128 lanes")
+        S("    tm_base = tm_alloc(&tm_slot, %d);" % (lay.tm_cols * (BLOCK // 128)))
+        S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16) + (threadIdx.x >> 7) * %du;      // this warp's quarter of the 128 lanes (and half of the columns)" % lay.tm_cols)
         S("  }")
+    if sync:
+        S("  const long left = npad - (long)blockIdx.x * blockDim.x;")
+        S("  const unsigned nlive = (unsigned)(left < (long)blockDim.x ? left : (long)blockDim.x);      // threads of the live warps (npad is a multiple of 32)")
     S("  const R mt = (R)mt_d;")
     S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 65536 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
@@ -834,7 +842,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None):
         S("    }")
     S("  }")
     if tm0 is not None:
-        S("  if constexpr (TM) tm_free(tm_base, %d);" % lay.tm_cols)
+        S("  if constexpr (TM) tm_free(tm_base, %d);" % (lay.tm_cols * (BLOCK // 128)))
     S("}")
     if delegate_double is not None:
         S("extern const MultiKernel mk_%s_o%s;" % (name, delegate_double))
@@ -890,9 +898,15 @@ def emit_orbit5_process(name="gg_ttxggg"):
     for ki, b in enumerate(builders):
         lay, groups = b(blocks[ki], pidx)
         last = ki == len(builders) - 1
-        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if (last and K3D_JACC) else None)
+        k1_sync = K1_SYNC and K1_PARTS == 1 and ki == 0
+        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if ((last and K3D_JACC) or k1_sync) else None)
         files["gen_%s_o%d.cu" % (name, ki)] = src
         kinfo.append(info)
+        if k1_sync:                # FP64-only variant of kernel o0: one 256-thread CTA per SM, warps kept in step by scope barriers
+            lay2, groups2 = build_k1(256, pidx, 0, 1)
+            src2, info2 = emit_kernel(name, "0d", lay2, groups2, 256, only="double", sync=True)
+            files["gen_%s_o0d.cu" % name] = src2
+            info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, block=256)
         if last and K3D_JACC:      # FP64-only variant of the last kernel: local jamp accumulators in tensor memory (see TM_K3)
             lay2, groups2 = build_k3(BLOCK1, pidx, jacc=K3D_JACC, tm=TM_K3)
             src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="double")

@@ -373,8 +373,9 @@ template <typename R> ME_DEV void cacc(R* p, R dre, R dim) {
 #ifndef ME_TM_SLOT0
 #define ME_TM_SLOT0 0
 #endif
-// (assumes ME_SM_STRIDE == 128: the element offset of even slot s is 128 s; checked where the TMEM kernel is instantiated)
-#define ME_TM_COL(off) ((uint32_t)((off) >> 6) - (uint32_t)(2 * ME_TM_SLOT0))
+// (the element offset of even slot s is ME_SM_STRIDE * s; ME_SM_STRIDE is a power of two: 128 threads per CTA, or 256 in the kernels
+// whose two groups of four warps share the TMEM lanes and take half of the columns each)
+#define ME_TM_COL(off) (((uint32_t)(off) * 2u) / (uint32_t)ME_SM_STRIDE - (uint32_t)(2 * ME_TM_SLOT0))
 namespace me {
 ME_DEV void tm_ld16(uint32_t (&r)[16], uint32_t a) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
