@@ -288,7 +288,7 @@ def main():
     e2e_ms, _ = timed(ctx, mom, n, me.ME_FP64, args.steps, 1, host=host)
     e2e_ms = allmax(e2e_ms)
     e2e = {"value": per_gpu * world * args.steps / (e2e_ms * 1e-3), "unit": "MEs/s", "h2d_bytes_per_step": host.numel() * 8,
-           "d2h_bytes_per_step": n * 8, "api": "MEContext.me_compute_host (pinned host momenta -> me_compute -> pinned host MEs)"}
+           "d2h_bytes_per_step": n * 8, "api": "C-ABI me_compute_host (pinned host momenta -> sliced H2D overlapped with the kernels -> pinned host MEs)"}
     launches += args.steps * per_step_launches
     line = {
         "metric": "matrix elements/sec (%s, FP64)" % cfg["label"], "value": value, "unit": "MEs/s", "n_gpus": world, "steps": args.steps,

@@ -123,6 +123,22 @@ me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
 me_status me_compute(me_ctx* ctx, const double* d_momenta, int64_t n, me_precision precision,
                      double* d_me, void* stream);
 
+/* The same computation with HOST buffers: the end-to-end call ("e2e"; the paper's
+ * data flow "momenta in, matrix elements out", section 2, as seen from a host-side event generator).
+ *   h_momenta : HOST, same AoSoA layout and padding rule as d_momenta; page-locked memory lets the
+ *               copies overlap the computation (pageable memory is accepted, the copies then serialise).
+ *   h_me      : HOST, FP64 [n].
+ * The batch is cut in slices (the first of 6 x 128 events per SM, the others four times that: whole waves
+ * of CTAs); slice k + 1 is copied to the device on an internal copy stream while slice k is computed, the
+ * MEs of slice k return on a second copy stream; odd slices are computed on an internal stream so that
+ * consecutive kernels overlap.  Two slice buffers per direction are owned by the context (allocated on
+ * first use, freed by me_destroy).  Asynchronous like me_compute: work is ordered after what `stream` already holds,
+ * and `stream` waits for the last device -> host copy, so synchronising `stream` makes h_me valid.
+ * The buffers must stay untouched until then.  One call at a time per context.
+ * Errors: as me_compute. */
+me_status me_compute_host(me_ctx* ctx, const double* h_momenta, int64_t n, me_precision precision,
+                          double* h_me, void* stream);
+
 /* Same pass, but also returns the per-helicity colour-summed |M_h|^2 (not averaged) for ALL
  * ncomb helicities (masked ones evaluate too): d_me_hel is DEVICE FP64 [ncomb][n].
  * Used by the filter and by the parity tests.  d_me may be null. */

@@ -17,7 +17,7 @@ ME_FP64, ME_MIXED, ME_FP32 = range(3)
 ME_OPT_PARITY_PAIRING = 0
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
-EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute",
+EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute", "me_compute_host",
            "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_select_helicity_color", "me_unweight", "me_color_matrix", "me_philox_uniform", "me_rambo",
            "me_fma_peak", "me_strerror")
 
@@ -59,6 +59,7 @@ def lib():
         L.me_select_helicity_color.argtypes = [vp, vp, i64, u64, u64, vp, vp, vp]
         L.me_unweight.argtypes = [vp, vp, i64, dbl, u64, u64, dbl, ctypes.POINTER(dbl), vp, ctypes.POINTER(i64), vp]
         L.me_compute.argtypes = [vp, vp, i64, cint, vp, vp]
+        L.me_compute_host.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_helicities.argtypes = [vp, vp, i64, cint, vp, vp, vp]
         L.me_compute_jamps.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_color_matrix.argtypes = [vp, ctypes.POINTER(dbl)]
@@ -219,15 +220,15 @@ class MEContext:
         _check(lib().me_color_matrix(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
         return out
 
-    def me_compute_host(self, momenta_host, n, precision=ME_FP64, stream=None):
-        """End-to-end call with HOST buffers (pinned torch tensors): H2D copy of the momenta, me_compute,
-        D2H copy of the MEs, all on `stream`; returns the host tensor after synchronising."""
+    def me_compute_host(self, momenta_host, n, precision=ME_FP64, stream=None, out=None):
+        """End-to-end call with HOST buffers (pinned torch tensors) through the C-ABI me_compute_host: sliced H2D copies of the
+        momenta overlapped with the computation, D2H copies of the MEs; returns the (pinned) host tensor after synchronising."""
         import torch
+        assert not momenta_host.is_cuda and momenta_host.dtype == torch.float64 and momenta_host.is_contiguous()
+        assert momenta_host.numel() >= self.momenta_numel(n)
         s = stream if stream is not None else torch.cuda.current_stream()
-        with torch.cuda.stream(s):
-            d = momenta_host.to("cuda", non_blocking=True)
-            me = self.me_compute(d, n, precision, stream=s)
+        if out is None:
             out = torch.empty(n, dtype=torch.float64, pin_memory=True)
-            out.copy_(me, non_blocking=True)
+        _check(lib().me_compute_host(self._h, ctypes.c_void_p(momenta_host.data_ptr()), n, int(precision), ctypes.c_void_p(out.data_ptr()), _stream(s)))
         s.synchronize()
         return out

@@ -27,6 +27,10 @@ struct me_ctx {
   uint64_t mask[2];
   bool filtered;
   void* scratch; size_t scratch_bytes;
+  // me_compute_host: two device slices of momenta / MEs, a stream per copy direction, events (all created on first use)
+  double* h_mom[2]; double* h_me[2]; size_t h_slice;     // h_slice = events a slice buffer holds (0: nothing allocated)
+  cudaStream_t s_h2d, s_d2h, s_comp;
+  cudaEvent_t ev_start, ev_h2d[2], ev_comp[2], ev_d2h[2];
 };
 
 static thread_local char g_errbuf[256] = "CUDA error (none recorded)";
@@ -65,7 +69,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
   me_ctx* c = new (std::nothrow) me_ctx();
   if (c == nullptr) return ME_ENOMEM;
   c->process = process; c->prm = *prm; c->filtered = false; c->ngood = 0; c->mask[0] = c->mask[1] = 0;
-  c->scratch = nullptr; c->scratch_bytes = 0; c->d_hels_all = c->d_hels_good = c->d_hels_half = nullptr; c->nhalf = 0; c->pairing = false;
+  c->scratch = nullptr; c->scratch_bytes = 0; c->h_slice = 0; c->h_mom[0] = c->h_mom[1] = c->h_me[0] = c->h_me[1] = nullptr; c->s_h2d = c->s_d2h = nullptr; c->d_hels_all = c->d_hels_good = c->d_hels_half = nullptr; c->nhalf = 0; c->pairing = false;
   me_info& I = c->info; memset(&I, 0, sizeof(I));
   I.page = ME_PAGE; I.ninitial = 2;
   const double PI = 3.14159265358979323846;
@@ -110,6 +114,10 @@ extern "C" me_status me_destroy(me_ctx* c) {
   if (c == nullptr) return ME_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(c->d_hels_all); cudaFree(c->d_hels_good); cudaFree(c->d_hels_half); cudaFree(c->scratch);
+  if (c->s_h2d != nullptr) {
+    for (int b = 0; b < 2; ++b) { cudaFree(c->h_mom[b]); cudaFree(c->h_me[b]); cudaEventDestroy(c->ev_h2d[b]); cudaEventDestroy(c->ev_comp[b]); cudaEventDestroy(c->ev_d2h[b]); }
+    cudaEventDestroy(c->ev_start); cudaStreamDestroy(c->s_h2d); cudaStreamDestroy(c->s_d2h); cudaStreamDestroy(c->s_comp);
+  }
   delete c;
   return ME_OK;
 }
@@ -230,6 +238,77 @@ extern "C" me_status me_compute(me_ctx* c, const double* d_mom, int64_t n, me_pr
     return st;
   }
   return run(c, d_mom, n, prec, c->d_hels_good, c->ngood, d_me, nullptr, nullptr, stream);
+}
+
+// Host-buffer entry (include/me.h): the batch is cut in slices of whole waves of CTAs; slice k + 1 travels host -> device on a
+// copy stream while slice k is computed on the caller's stream, and the MEs of slice k travel back on a second copy stream.
+extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, me_precision prec, double* h_me, void* stream) {
+  if (c == nullptr || n < 0) return ME_EINVAL;
+  if (n == 0) return ME_OK;
+  if (h_mom == nullptr || h_me == nullptr || (int)prec < 0 || (int)prec > 2) return ME_EINVAL;
+  if (!c->filtered) return ME_ENOTFILTERED;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (c->s_h2d == nullptr) {
+    ME_CUDA(cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking), "host stream");
+    ME_CUDA(cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking), "host stream");
+    ME_CUDA(cudaStreamCreateWithFlags(&c->s_comp, cudaStreamNonBlocking), "host stream");
+    ME_CUDA(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming), "host event");
+    for (int b = 0; b < 2; ++b) {
+      ME_CUDA(cudaEventCreateWithFlags(&c->ev_h2d[b], cudaEventDisableTiming), "host event");
+      ME_CUDA(cudaEventCreateWithFlags(&c->ev_comp[b], cudaEventDisableTiming), "host event");
+      ME_CUDA(cudaEventCreateWithFlags(&c->ev_d2h[b], cudaEventDisableTiming), "host event");
+    }
+  }
+  // slice unit = 6 CTAs of ME_BLOCK events on every SM (whole waves for 1, 2, 3 or 6 resident CTAs per SM), a multiple of the page.
+  // The first slice is one unit, so that the computation starts after a short copy; the others are four units (every kernel ends with
+  // a drain phase in which SMs idle, so few, large slices).  Odd slices are computed on a second stream: the CTAs of slice k + 1 fill
+  // the drain of slice k.  Processes with a library-owned staging buffer (g g -> t t~ g g g) keep all slices on one stream.
+  int dev = 0, nsm = 0;
+  ME_CUDA(cudaGetDevice(&dev), "device");
+  ME_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "device");
+  const int64_t unit = (int64_t)nsm * ME_BLOCK * 6, slice = 4 * unit;
+  const bool one_stream = c->tab != nullptr && c->tab->scratch_bytes != nullptr;
+  const size_t ev_words = (size_t)c->info.npar * 4;            // doubles per event
+  if (c->h_slice < (size_t)slice) {
+    ME_CUDA(cudaStreamSynchronize(c->s_h2d), "host sync"); ME_CUDA(cudaStreamSynchronize(c->s_d2h), "host sync");
+    for (int b = 0; b < 2; ++b) {
+      cudaFree(c->h_mom[b]); cudaFree(c->h_me[b]); c->h_mom[b] = c->h_me[b] = nullptr;
+    }
+    c->h_slice = 0;
+    for (int b = 0; b < 2; ++b) {
+      cudaError_t e = cudaMalloc(&c->h_mom[b], sizeof(double) * ev_words * slice);
+      if (e == cudaSuccess) e = cudaMalloc(&c->h_me[b], sizeof(double) * slice);
+      if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return ME_ENOMEM; }
+      ME_CUDA(e, "host slice alloc");
+    }
+    c->h_slice = (size_t)slice;
+  }
+  ME_CUDA(cudaEventRecord(c->ev_start, st), "host start");
+  ME_CUDA(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0), "host start");
+  ME_CUDA(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0), "host start");
+  ME_CUDA(cudaStreamWaitEvent(c->s_comp, c->ev_start, 0), "host start");
+  int k = 0;
+  for (int64_t first = 0; first < n; ++k) {
+    const int b = k & 1;
+    const int64_t cap = k == 0 ? unit : slice;
+    const int64_t m = n - first < cap ? n - first : cap;
+    const int64_t mpad = (m + ME_PAGE - 1) / ME_PAGE * ME_PAGE;
+    cudaStream_t cs = (b == 1 && !one_stream) ? c->s_comp : st;
+    if (k >= 2) ME_CUDA(cudaStreamWaitEvent(c->s_h2d, c->ev_comp[b], 0), "host wait");      // slice k - 2 no longer reads this buffer
+    ME_CUDA(cudaMemcpyAsync(c->h_mom[b], h_mom + (size_t)first * ev_words, sizeof(double) * ev_words * mpad, cudaMemcpyHostToDevice, c->s_h2d), "host h2d");
+    ME_CUDA(cudaEventRecord(c->ev_h2d[b], c->s_h2d), "host h2d");
+    ME_CUDA(cudaStreamWaitEvent(cs, c->ev_h2d[b], 0), "host wait");
+    if (k >= 2) ME_CUDA(cudaStreamWaitEvent(cs, c->ev_d2h[b], 0), "host wait");             // the MEs of slice k - 2 have left
+    const me_status ms = me_compute(c, c->h_mom[b], m, prec, c->h_me[b], (void*)cs);
+    if (ms != ME_OK) return ms;
+    ME_CUDA(cudaEventRecord(c->ev_comp[b], cs), "host compute");
+    ME_CUDA(cudaStreamWaitEvent(c->s_d2h, c->ev_comp[b], 0), "host wait");
+    ME_CUDA(cudaMemcpyAsync(h_me + first, c->h_me[b], sizeof(double) * m, cudaMemcpyDeviceToHost, c->s_d2h), "host d2h");
+    ME_CUDA(cudaEventRecord(c->ev_d2h[b], c->s_d2h), "host d2h");
+    first += m;
+  }
+  for (int b = 0; b < (k < 2 ? k : 2); ++b) ME_CUDA(cudaStreamWaitEvent(st, c->ev_d2h[b], 0), "host end");
+  return ME_OK;
 }
 
 extern "C" me_status me_compute_helicities(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, double* d_me, double* d_me_hel, void* stream) {

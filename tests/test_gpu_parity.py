@@ -485,3 +485,23 @@ def test_tensor_memory_kernels_agree_with_the_shared_memory_kernels(me, tmp_path
     assert np.isfinite(t).all() and (t > 0).all()
     assert np.abs(t[0] / s[0] - 1).max() < 1e-12
     assert np.abs(t[1] / s[1] - 1).max() < 5e-6
+
+
+@pytest.mark.parametrize("proc,n", [(1, 1200001), (1, 100), (3, 1000), (4, 300)])
+def test_host_buffer_entry_equals_device_entry(me, proc, n):
+    """me_compute_host (include/me.h): host momenta in, host MEs out, sliced and overlapped copies.  Slicing changes nothing per
+    event, so the result is bit-identical to me_compute on the same momenta; 1200001 events span four slices (113664, then 454656 each on a B200) with a ragged last page, and a second call reuses the slice buffers."""
+    import torch
+    cfg = inputs.CONFIGS[proc]
+    ctx = me.MEContext(proc)
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    ctx.me_filter_helicities(mom, min(n, 32))
+    ref = ctx.me_compute(mom, n, me.ME_FP64).cpu()
+    host = mom.cpu().pin_memory()
+    for prec in (me.ME_FP64, me.ME_FP32, me.ME_FP64):
+        got = ctx.me_compute_host(host, n, prec)
+        want = ref if prec == me.ME_FP64 else ctx.me_compute(mom, n, prec).cpu()
+        assert not got.is_cuda and torch.equal(got, want)
+    pageable = mom.cpu()                                     # not page-locked: accepted, copies serialise
+    assert torch.equal(ctx.me_compute_host(pageable, n, me.ME_FP64), ref)
+    ctx.close()
