@@ -33,6 +33,8 @@ FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
+K1_SHARE_UW = False      # kernel o0: nested table-driven loop over the (u, w) halves of the closing vectors (8.5 k instead of 10.6 k SASS instructions);
+                         # re-measured with the tensor-memory kernels: FP64 94.0 vs 91.6 ms per pass, FP32 48.7 vs 46.5 ms: off
 K1_SYNC = False          # FP64 variant of kernel o0 (k_..._o0d): one 256-thread CTA, named barrier at every scope so that the eight warps fetch the
                          # same instructions; measured 9.55 ms per chunk against 9.40 ms for two free-running 128-thread CTAs: off
 K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
@@ -893,7 +895,7 @@ def emit_orbit5_process(name="gg_ttxggg"):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     files, kinfo = {}, []
-    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
+    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS, share_uw=K1_SHARE_UW)) for i in range(K1_PARTS)) + (build_k2, build_k3)
     blocks = (BLOCK1,) * (len(builders) - 1) + (BLOCK if (K3_JACC and not TM_K3) else BLOCK1,)
     for ki, b in enumerate(builders):
         lay, groups = b(blocks[ki], pidx)
