@@ -239,8 +239,9 @@ class Inst:
             # jamps in tensor memory: tcgen05.ld x4 / st x4 per flow; the stores of the previous batch must have completed first
             for b0 in range(0, len(ups), self.JBATCH):
                 batch = ups[b0:b0 + self.JBATCH]
+                # (the flows of one flush are distinct: only its first batch can read what an earlier flush stored)
                 self.L("{ R " + ", ".join("jr%d, ji%d" % (i, i) for i in range(len(batch))) + "; XC<R, TM> "
-                       + ", ".join("jx%d" % i for i in range(len(batch))) + "; xwait_st<TM>();")
+                       + ", ".join("jx%d" % i for i in range(len(batch))) + ";" + (" xwait_st<TM>();" if b0 == 0 else ""))
                 for i, (o, re, im) in enumerate(batch):
                     self.L("  xcget_issue<R, TM>(jx%d, sm, tm, %s);" % (i, o))
                 for i, (o, re, im) in enumerate(batch):
@@ -593,7 +594,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    if constexpr (TM) {")
     S("      const uint32_t zz[16] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};")
     S("#pragma unroll")
-    S("      for (int s = 0; s < %d; ++s) tm_st16(tm + ME_TM_COL(ME_EO(%d)) + 16 * s, zz);" % (ncol // 4, lay.J))
+    S("      for (int s = 0; s < %d; ++s) tm_st16(tm + ME_TM_COL(R, ME_EO(%d)) + 16 * s, zz);" % (ncol // 4, lay.J))
     S("    } else {")
     S("#pragma unroll")
     S("      for (int s = 0; s < %d; ++s) cset<R>(sm + ME_EO(%d + 2 * s), (R)0, (R)0);" % (ncol, lay.J))

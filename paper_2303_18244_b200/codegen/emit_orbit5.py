@@ -37,6 +37,7 @@ K1_SHARE_UW = False      # kernel o0: nested table-driven loop over the (u, w) h
                          # re-measured with the tensor-memory kernels: FP64 94.0 vs 91.6 ms per pass, FP32 48.7 vs 46.5 ms: off
 K1_SYNC = False          # FP64 variant of kernel o0 (k_..._o0d): one 256-thread CTA, named barrier at every scope so that the eight warps fetch the
                          # same instructions; measured 9.55 ms per chunk against 9.40 ms for two free-running 128-thread CTAs: off
+K3D_FLOAT = True          # the accumulator variant of kernel o2 also serves FP32 (96 TMEM columns, shared memory as before: two CTAs per SM)
 K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
 TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
                           # K3_JACC = 0 gives two CTAs per SM but leaves the kernel bound by the L2 throughput of its 1320 RED pairs per helicity
@@ -741,7 +742,7 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, sync=False):
+def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, sync=False, delegate_all=False):
     """only: None (float and double instances of one template), 'double' (FP64-only variant; ki is then a tag like '2d');
     delegate_double: tag of the FP64-only variant this kernel's launcher hands double / mixed precision to;
     sync: one 256-thread CTA per SM whose eight warps meet at a named barrier at every scope of the loop bodies, so that they
@@ -784,10 +785,10 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
     S("  uint32_t tm = 0, tm_base = 0;")
     if tm0 is not None:
         S("  if constexpr (TM) {")
-        S("    static_assert(sizeof(R) == 8, \"TMEM scratchpad: FP64\");")
+        S("    constexpr uint32_t tm_cols = sizeof(R) == 8 ? %du : %du;      // FP32 slots take one column" % (lay.tm_cols, max(32, lay.tm_cols // 2)))
         S("    __shared__ uint32_t tm_slot;")
-        S("    tm_base = tm_alloc(&tm_slot, %d);" % (lay.tm_cols * (BLOCK // 128)))
-        S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16) + (threadIdx.x >> 7) * %du;      // this warp's quarter of the 128 lanes (and half of the columns)" % lay.tm_cols)
+        S("    tm_base = tm_alloc(&tm_slot, tm_cols * %d);" % (BLOCK // 128))
+        S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16) + (threadIdx.x >> 7) * tm_cols;      // this warp's quarter of the 128 lanes (and half of the columns)")
         S("  }")
     if sync:
         S("  const long left = npad - (long)blockIdx.x * blockDim.x;")
@@ -844,7 +845,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("    }")
     S("  }")
     if tm0 is not None:
-        S("  if constexpr (TM) tm_free(tm_base, %d);" % (lay.tm_cols * (BLOCK // 128)))
+        S("  if constexpr (TM) tm_free(tm_base, (sizeof(R) == 8 ? %du : %du) * %d);" % (lay.tm_cols, max(32, lay.tm_cols // 2), BLOCK // 128))
     S("}")
     if delegate_double is not None:
         S("extern const MultiKernel mk_%s_o%s;" % (name, delegate_double))
@@ -864,10 +865,18 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("  {")
         launch_line("double, double, true", "smt", "double")
         S("  }")
+    elif only == "tm":
+        assert tm0 is not None
+        S("  const size_t smtf = sizeof(float) * %d * %d;" % (tm0, BLOCK))
+        S("  if (precision == 2) {")
+        launch_line("float, float, true", "smtf", "float")
+        S("  } else {")
+        launch_line("double, double, true", "smt", "double")
+        S("  }")
     else:
         if delegate_double is not None:
             S(NO_TMEM)
-            S("  if (precision != 2 && !no_tmem) return mk_%s_o%s.launch(precision, a);     // FP64 amplitudes: the variant with local accumulators in tensor memory" % (name, delegate_double))
+            S("  if (%s!no_tmem) return mk_%s_o%s.launch(precision, a);     // the variant with local accumulators in tensor memory" % ("" if delegate_all else "precision != 2 && ", name, delegate_double))
         S("  if (precision == 2) {")
         launch_line("float, float, false", "smf", "float")
         S("  } else {")
@@ -901,7 +910,8 @@ def emit_orbit5_process(name="gg_ttxggg"):
         lay, groups = b(blocks[ki], pidx)
         last = ki == len(builders) - 1
         k1_sync = K1_SYNC and K1_PARTS == 1 and ki == 0
-        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if ((last and K3D_JACC) or k1_sync) else None)
+        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if ((last and K3D_JACC) or k1_sync) else None,
+                                delegate_all=last and K3D_JACC and K3D_FLOAT)
         files["gen_%s_o%d.cu" % (name, ki)] = src
         kinfo.append(info)
         if k1_sync:                # FP64-only variant of kernel o0: one 256-thread CTA per SM, warps kept in step by scope barriers
@@ -911,7 +921,7 @@ def emit_orbit5_process(name="gg_ttxggg"):
             info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, block=256)
         if last and K3D_JACC:      # FP64-only variant of the last kernel: local jamp accumulators in tensor memory (see TM_K3)
             lay2, groups2 = build_k3(BLOCK1, pidx, jacc=K3D_JACC, tm=TM_K3)
-            src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="double")
+            src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="tm" if K3D_FLOAT else "double")
             files["gen_%s_o%dd.cu" % (name, ki)] = src2
             info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, flops=info2["flops"], redundant=info2["redundant"])
     namp = sum(k["amplitudes"] for k in kinfo)

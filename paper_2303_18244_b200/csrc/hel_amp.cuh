@@ -375,7 +375,8 @@ template <typename R> ME_DEV void cacc(R* p, R dre, R dim) {
 #endif
 // (the element offset of even slot s is ME_SM_STRIDE * s; ME_SM_STRIDE is a power of two: 128 threads per CTA, or 256 in the kernels
 // whose two groups of four warps share the TMEM lanes and take half of the columns each)
-#define ME_TM_COL(off) (((uint32_t)(off) * 2u) / (uint32_t)ME_SM_STRIDE - (uint32_t)(2 * ME_TM_SLOT0))
+// columns per slot: 2 for FP64, 1 for FP32
+#define ME_TM_COL(R, off) (((uint32_t)(off) * (uint32_t)(sizeof(R) / 4)) / (uint32_t)ME_SM_STRIDE - (uint32_t)((sizeof(R) / 4) * ME_TM_SLOT0))
 namespace me {
 ME_DEV void tm_ld16(uint32_t (&r)[16], uint32_t a) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
@@ -388,61 +389,99 @@ ME_DEV void tm_wait_ld16(uint32_t (&r)[16]) {
                : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]), "+r"(r[9]),
                  "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]));
 }
+ME_DEV void tm_ld8(uint32_t (&r)[8], uint32_t a) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(a));
+}
+ME_DEV void tm_wait_ld8(uint32_t (&r)[8]) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]));
+}
 ME_DEV void tm_ld4(uint32_t (&r)[4], uint32_t a) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
 }
 ME_DEV void tm_wait_ld4(uint32_t (&r)[4]) {
   asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]));
 }
+ME_DEV void tm_ld2(uint32_t (&r)[2], uint32_t a) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(a));
+}
+ME_DEV void tm_wait_ld2(uint32_t (&r)[2]) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]));
+}
 ME_DEV void tm_st16(uint32_t a, const uint32_t (&r)[16]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(a),
                "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]),
                "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]));
 }
+ME_DEV void tm_st8(uint32_t a, const uint32_t (&r)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(a),
+               "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]));
+}
 ME_DEV void tm_st4(uint32_t a, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(r0), "r"(r1), "r"(r2), "r"(r3));
 }
-// a 4-vector load in flight: from shared memory it is complete at issue; from TMEM it is 16 raw registers until xldw_get
+ME_DEV void tm_st2(uint32_t a, uint32_t r0, uint32_t r1) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(a), "r"(r0), "r"(r1));
+}
+// a 4-vector load in flight: from shared memory it is complete at issue; from TMEM it is 16 (FP64) or 8 (FP32) raw registers until xldw_get
 template <typename R, bool TM> struct XW { W4<R> w; };
 template <> struct XW<double, true> { uint32_t r[16]; };
+template <> struct XW<float, true> { uint32_t r[8]; };
 template <typename R, bool TM> struct XC { R re, im; };
 template <> struct XC<double, true> { uint32_t r[4]; };
+template <> struct XC<float, true> { uint32_t r[2]; };
 template <typename R, bool TM> ME_DEV void xldw_issue(XW<R, TM>& x, const R* sm, uint32_t tm, int off) {
-  if constexpr (TM) tm_ld16(x.r, tm + ME_TM_COL(off)); else x.w = ldw<R>(sm + off);
+  if constexpr (TM && sizeof(R) == 8) tm_ld16(x.r, tm + ME_TM_COL(R, off));
+  else if constexpr (TM) tm_ld8(x.r, tm + ME_TM_COL(R, off));
+  else x.w = ldw<R>(sm + off);
 }
 template <typename R, bool TM> ME_DEV W4<R> xldw_get(XW<R, TM>& x) {
-  if constexpr (TM) {
+  if constexpr (TM && sizeof(R) == 8) {
     tm_wait_ld16(x.r);
     return {__hiloint2double(x.r[1], x.r[0]), __hiloint2double(x.r[3], x.r[2]), __hiloint2double(x.r[5], x.r[4]), __hiloint2double(x.r[7], x.r[6]),
             __hiloint2double(x.r[9], x.r[8]), __hiloint2double(x.r[11], x.r[10]), __hiloint2double(x.r[13], x.r[12]), __hiloint2double(x.r[15], x.r[14])};
+  } else if constexpr (TM) {
+    tm_wait_ld8(x.r);
+    return {__uint_as_float(x.r[0]), __uint_as_float(x.r[1]), __uint_as_float(x.r[2]), __uint_as_float(x.r[3]),
+            __uint_as_float(x.r[4]), __uint_as_float(x.r[5]), __uint_as_float(x.r[6]), __uint_as_float(x.r[7])};
   } else {
     return x.w;
   }
 }
 template <typename R, bool TM> ME_DEV void xstw(R* sm, uint32_t tm, int off, const W4<R>& w) {
-  if constexpr (TM) {
+  if constexpr (TM && sizeof(R) == 8) {
     const double v[8] = {w.r0, w.i0, w.r1, w.i1, w.r2, w.i2, w.r3, w.i3};
     uint32_t r[16];
 #pragma unroll
     for (int k = 0; k < 8; ++k) { r[2 * k] = (uint32_t)__double2loint(v[k]); r[2 * k + 1] = (uint32_t)__double2hiint(v[k]); }
-    tm_st16(tm + ME_TM_COL(off), r);
+    tm_st16(tm + ME_TM_COL(R, off), r);
+  } else if constexpr (TM) {
+    const uint32_t r[8] = {__float_as_uint(w.r0), __float_as_uint(w.i0), __float_as_uint(w.r1), __float_as_uint(w.i1),
+                           __float_as_uint(w.r2), __float_as_uint(w.i2), __float_as_uint(w.r3), __float_as_uint(w.i3)};
+    tm_st8(tm + ME_TM_COL(R, off), r);
   } else {
     stw<R>(sm + off, w);
   }
 }
 template <typename R, bool TM> ME_DEV void xcget_issue(XC<R, TM>& x, const R* sm, uint32_t tm, int off) {
-  if constexpr (TM) tm_ld4(x.r, tm + ME_TM_COL(off)); else cget<R>(sm + off, x.re, x.im);
+  if constexpr (TM && sizeof(R) == 8) tm_ld4(x.r, tm + ME_TM_COL(R, off));
+  else if constexpr (TM) tm_ld2(x.r, tm + ME_TM_COL(R, off));
+  else cget<R>(sm + off, x.re, x.im);
 }
 template <typename R, bool TM> ME_DEV void xcget_get(XC<R, TM>& x, R& re, R& im) {
-  if constexpr (TM) {
+  if constexpr (TM && sizeof(R) == 8) {
     tm_wait_ld4(x.r);
     re = __hiloint2double(x.r[1], x.r[0]); im = __hiloint2double(x.r[3], x.r[2]);
+  } else if constexpr (TM) {
+    tm_wait_ld2(x.r);
+    re = __uint_as_float(x.r[0]); im = __uint_as_float(x.r[1]);
   } else {
     re = x.re; im = x.im;
   }
 }
 template <typename R, bool TM> ME_DEV void xcset(R* sm, uint32_t tm, int off, R re, R im) {
-  if constexpr (TM) tm_st4(tm + ME_TM_COL(off), (uint32_t)__double2loint(re), (uint32_t)__double2hiint(re), (uint32_t)__double2loint(im), (uint32_t)__double2hiint(im));
+  if constexpr (TM && sizeof(R) == 8) tm_st4(tm + ME_TM_COL(R, off), (uint32_t)__double2loint(re), (uint32_t)__double2hiint(re), (uint32_t)__double2loint(im), (uint32_t)__double2hiint(im));
+  else if constexpr (TM) tm_st2(tm + ME_TM_COL(R, off), __float_as_uint(re), __float_as_uint(im));
   else cset<R>(sm + off, re, im);
 }
 // spinor basis (five reals) in an 8-slot TMEM vector
