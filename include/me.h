@@ -128,8 +128,7 @@ me_status me_compute(me_ctx* ctx, const double* d_momenta, int64_t n, me_precisi
  *   h_momenta : HOST, same AoSoA layout and padding rule as d_momenta; page-locked memory lets the
  *               copies overlap the computation (pageable memory is accepted, the copies then serialise).
  *   h_me      : HOST, FP64 [n].
- * The batch is cut in slices (the first of 6 x 128 events per SM, the others four times that: whole waves
- * of CTAs); slice k + 1 is copied to the device on an internal copy stream while slice k is computed, the
+ * The batch is cut in slices of 6 x 128 events per SM (whole waves of CTAs); slice k + 1 is copied to the device on an internal copy stream while slice k is computed, the
  * MEs of slice k return on a second copy stream; odd slices are computed on an internal stream so that
  * consecutive kernels overlap.  Two slice buffers per direction are owned by the context (allocated on
  * first use, freed by me_destroy).  Asynchronous like me_compute: work is ordered after what `stream` already holds,

@@ -1,6 +1,7 @@
 // me_api.cu — the C-ABI boundary declared in include/me.h: context, helicity filtering, dispatch.
 // Host logic only; every arithmetic step of the path runs in the kernels (hel_amp.cuh, epem.cu,
 // gen_*.cu, rng_rambo.cu).  No CPU fallback: without a CUDA device every entry point returns ME_ECUDA.
+#include <stdlib.h>
 #include "../../include/me.h"
 #include "kernels.h"
 
@@ -259,14 +260,16 @@ extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, 
       ME_CUDA(cudaEventCreateWithFlags(&c->ev_d2h[b], cudaEventDisableTiming), "host event");
     }
   }
-  // slice unit = 6 CTAs of ME_BLOCK events on every SM (whole waves for 1, 2, 3 or 6 resident CTAs per SM), a multiple of the page.
-  // The first slice is one unit, so that the computation starts after a short copy; the others are four units (every kernel ends with
-  // a drain phase in which SMs idle, so few, large slices).  Odd slices are computed on a second stream: the CTAs of slice k + 1 fill
-  // the drain of slice k.  Processes with a library-owned staging buffer (g g -> t t~ g g g) keep all slices on one stream.
+  // slice = 6 CTAs of ME_BLOCK events on every SM (whole waves for 1, 2, 3 or 6 resident CTAs per SM), a multiple of the page
+  // (ME_HOST_SLICE_UNITS = k: k times that; measured equal for 1, 2 and 4 on the headline workload, 1 needs the least copy bandwidth:
+  // a slice of g g -> t t~ g g is 22 MB against 5.5 ms of kernel).  Every kernel ends with a drain phase in which SMs idle, so odd slices are
+  // computed on a second stream: the CTAs of slice k + 1 fill the drain of slice k.  Processes with a library-owned staging buffer
+  // (g g -> t t~ g g g) keep all slices on one stream.
   int dev = 0, nsm = 0;
   ME_CUDA(cudaGetDevice(&dev), "device");
   ME_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "device");
-  const int64_t unit = (int64_t)nsm * ME_BLOCK * 6, slice = 4 * unit;
+  static const int slice_units = getenv("ME_HOST_SLICE_UNITS") != nullptr ? atoi(getenv("ME_HOST_SLICE_UNITS")) : 1;
+  const int64_t unit = (int64_t)nsm * ME_BLOCK * 6, slice = (slice_units > 0 ? slice_units : 1) * unit;
   const bool one_stream = c->tab != nullptr && c->tab->scratch_bytes != nullptr;
   const size_t ev_words = (size_t)c->info.npar * 4;            // doubles per event
   if (c->h_slice < (size_t)slice) {
@@ -290,7 +293,7 @@ extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, 
   int k = 0;
   for (int64_t first = 0; first < n; ++k) {
     const int b = k & 1;
-    const int64_t cap = k == 0 ? unit : slice;
+    const int64_t cap = slice;
     const int64_t m = n - first < cap ? n - first : cap;
     const int64_t mpad = (m + ME_PAGE - 1) / ME_PAGE * ME_PAGE;
     cudaStream_t cs = (b == 1 && !one_stream) ? c->s_comp : st;

@@ -490,7 +490,7 @@ def test_tensor_memory_kernels_agree_with_the_shared_memory_kernels(me, tmp_path
 @pytest.mark.parametrize("proc,n", [(1, 1200001), (1, 100), (3, 1000), (4, 300)])
 def test_host_buffer_entry_equals_device_entry(me, proc, n):
     """me_compute_host (include/me.h): host momenta in, host MEs out, sliced and overlapped copies.  Slicing changes nothing per
-    event, so the result is bit-identical to me_compute on the same momenta; 1200001 events span four slices (113664, then 454656 each on a B200) with a ragged last page, and a second call reuses the slice buffers."""
+    event, so the result is bit-identical to me_compute on the same momenta; 1200001 events span eleven slices (113664 events each on a B200) with a ragged last page, and a second call reuses the slice buffers."""
     import torch
     cfg = inputs.CONFIGS[proc]
     ctx = me.MEContext(proc)
