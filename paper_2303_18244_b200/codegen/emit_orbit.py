@@ -228,7 +228,8 @@ class Inst:
         return {0: ("%s.re" % z, "%s.im" % z), 1: ("-%s.re" % z, "-%s.im" % z),
                 2: ("-%s.im" % z, "%s.re" % z), 3: ("%s.im" % z, "-%s.re" % z)}[u]
 
-    JBATCH = 4     # accumulators read, updated and written back together
+    JBATCH = 4     # accumulators read, updated and written back together (shared memory)
+    JBATCH_TM = 8  # the same in tensor memory: more tcgen05.ld in flight per wait (FP64 -1 %; 8 in shared memory costs FP32 +1 %)
 
     def emit_accumulate(self, ups):
         """ups = [(shared-memory offset expression, re, im)]: J[offset] += (re, im).  The offsets are run-time values in the
@@ -237,18 +238,23 @@ class Inst:
         flush are distinct by construction: all loads of a batch are issued first, then the adds, then the stores."""
         if self.in_tm(self.lay.J):
             # jamps in tensor memory: tcgen05.ld x4 / st x4 per flow; the stores of the previous batch must have completed first
-            for b0 in range(0, len(ups), self.JBATCH):
-                batch = ups[b0:b0 + self.JBATCH]
-                # (the flows of one flush are distinct: only its first batch can read what an earlier flush stored)
-                self.L("{ R " + ", ".join("jr%d, ji%d" % (i, i) for i in range(len(batch))) + "; XC<R, TM> "
-                       + ", ".join("jx%d" % i for i in range(len(batch))) + ";" + (" xwait_st<TM>();" if b0 == 0 else ""))
-                for i, (o, re, im) in enumerate(batch):
-                    self.L("  xcget_issue<R, TM>(jx%d, sm, tm, %s);" % (i, o))
-                for i, (o, re, im) in enumerate(batch):
-                    self.L("  xcget_get<R, TM>(jx%d, jr%d, ji%d);" % (i, i, i))
-                for i, (o, re, im) in enumerate(batch):
-                    self.L("  xcset<R, TM>(sm, tm, %s, jr%d + (%s), ji%d + (%s));" % (o, i, re, i, im))
-                self.L("}")
+            def emit(jb):
+                for b0 in range(0, len(ups), jb):
+                    batch = ups[b0:b0 + jb]
+                    # (the flows of one flush are distinct: only its first batch can read what an earlier flush stored)
+                    self.L("{ R " + ", ".join("jr%d, ji%d" % (i, i) for i in range(len(batch))) + "; XC<R, TM> "
+                           + ", ".join("jx%d" % i for i in range(len(batch))) + ";" + (" xwait_st<TM>();" if b0 == 0 else ""))
+                    for i, (o, re, im) in enumerate(batch):
+                        self.L("  xcget_issue<R, TM>(jx%d, sm, tm, %s);" % (i, o))
+                    for i, (o, re, im) in enumerate(batch):
+                        self.L("  xcget_get<R, TM>(jx%d, jr%d, ji%d);" % (i, i, i))
+                    for i, (o, re, im) in enumerate(batch):
+                        self.L("  xcset<R, TM>(sm, tm, %s, jr%d + (%s), ji%d + (%s));" % (o, i, re, i, im))
+                    self.L("}")
+            if len(ups) > self.JBATCH:          # batch size by instantiation: the shared-memory instance of the same template keeps 4
+                self.L("if constexpr (TM) {"); emit(self.JBATCH_TM); self.L("} else {"); emit(self.JBATCH); self.L("}")
+            else:
+                emit(self.JBATCH)
             return
         for b0 in range(0, len(ups), self.JBATCH):
             batch = ups[b0:b0 + self.JBATCH]
