@@ -228,8 +228,8 @@ def main():
     roofline = {"bound": "alu", "kernel": "k_%s<double,double,TM=true>" % cfg["name"] + (" (+ colour sum)" if HL == 4 else ""), "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
                 "frac": ach / PEAK_TFLOPS["fp64"],
                 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel at the full config, from the committed
-                # ncu --set full capture (profiles/r1_ttxgg_fp64_tmem.md: 101.8 MB read + 3.9 MB written); algorithmic bytes = 200 B/event = 104.9 MB
-                "traffic": 105.8e6 if (HL == 3 and n == 524288) else None,
+                # ncu --set full capture (profiles/r1_ttxgg_fp64_tmem.md: 101.6 MB read + 5.5 MB written); algorithmic bytes = 200 B/event = 104.9 MB
+                "traffic": 107.1e6 if (HL == 3 and n == 524288) else None,
                 "traffic_source": "profiles/r1_ttxgg_fp64_tmem.md" if (HL == 3 and n == 524288) else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md clocks; no FP64 entry in MEASURED_PEAKS.json)",
                 "peak_measured_fma_chain": peak_meas["fp64"], "frac_of_measured": ach / peak_meas["fp64"],
