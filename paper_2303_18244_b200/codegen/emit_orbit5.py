@@ -37,6 +37,8 @@ K1_SHARE_UW = False      # kernel o0: nested table-driven loop over the (u, w) h
                          # re-measured with the tensor-memory kernels: FP64 94.0 vs 91.6 ms per pass, FP32 48.7 vs 46.5 ms: off
 K1_SYNC = False          # FP64 variant of kernel o0 (k_..._o0d): one 256-thread CTA, named barrier at every scope so that the eight warps fetch the
                          # same instructions; measured 9.55 ms per chunk against 9.40 ms for two free-running 128-thread CTAs: off
+TM_FLOAT = False          # kernels o0 and o1 with their tensor-memory layout in FP32 as well (three CTAs per SM instead of two; the FP32 kernels need
+                          # only 128 - 160 registers): measured slower, o0 5.49 vs 4.57 ms and o1 2.86 vs 2.66 ms per chunk (FP32 pass 49.0 vs 44.6 ms): off
 K3D_FLOAT = True          # the accumulator variant of kernel o2 also serves FP32 (96 TMEM columns, shared memory as before: two CTAs per SM)
 K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
 TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
@@ -877,11 +879,20 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         if delegate_double is not None:
             S(NO_TMEM)
             S("  if (%s!no_tmem) return mk_%s_o%s.launch(precision, a);     // the variant with local accumulators in tensor memory" % ("" if delegate_all else "precision != 2 && ", name, delegate_double))
+        if tm0 is not None and delegate_double is None:
+            S(NO_TMEM)
         S("  if (precision == 2) {")
+        if tm0 is not None and TM_FLOAT:
+            # FP32 kernels need 128 - 160 registers: with part of the slots in tensor memory (one column each) shared memory no longer
+            # limits them to two CTAs per SM
+            S("    const size_t smtf = sizeof(float) * %d * %d;" % (tm0, BLOCK))
+            S("    if (!no_tmem) {")
+            launch_line("float, float, true", "smtf", "float")
+            S("      return cudaGetLastError();")
+            S("    }")
         launch_line("float, float, false", "smf", "float")
         S("  } else {")
         if tm0 is not None:
-            S(NO_TMEM)
             S("    if (!no_tmem) {         // FP64 amplitudes: tensor-memory kernel (two CTAs per SM)")
             launch_line("double, double, true", "smt", "double")
             S("      return cudaGetLastError();")
