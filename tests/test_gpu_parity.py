@@ -505,3 +505,30 @@ def test_host_buffer_entry_equals_device_entry(me, proc, n):
     pageable = mom.cpu()                                     # not page-locked: accepted, copies serialise
     assert torch.equal(ctx.me_compute_host(pageable, n, me.ME_FP64), ref)
     ctx.close()
+
+
+def test_host_buffer_entry_errors_and_empty_batch(me):
+    """me_compute_host follows the error contract of me_compute (include/me.h): ME_ENOTFILTERED before a helicity mask exists,
+    ME_EINVAL for a null buffer or an unknown precision, n = 0 is a no-op; a failed call leaves the context usable."""
+    import ctypes
+    import torch
+    cfg = inputs.CONFIGS[1]
+    ctx = me.MEContext(1)
+    n = 64
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    host = mom.cpu().pin_memory()
+    with pytest.raises(me.MEError) as ei:
+        ctx.me_compute_host(host, n)
+    assert ei.value.status == me.ME_ENOTFILTERED
+    ctx.me_filter_helicities(mom, 32)
+    out = torch.empty(n, dtype=torch.float64, pin_memory=True)
+    L, st = me.lib(), ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    hp, op = ctypes.c_void_p(host.data_ptr()), ctypes.c_void_p(out.data_ptr())
+    assert L.me_compute_host(ctx._h, None, n, int(me.ME_FP64), op, st) == me.ME_EINVAL
+    assert L.me_compute_host(ctx._h, hp, n, int(me.ME_FP64), None, st) == me.ME_EINVAL
+    assert L.me_compute_host(ctx._h, hp, n, 7, op, st) == me.ME_EINVAL
+    assert L.me_compute_host(ctx._h, hp, -1, int(me.ME_FP64), op, st) == me.ME_EINVAL
+    assert L.me_compute_host(ctx._h, hp, 0, int(me.ME_FP64), op, st) == me.ME_OK
+    got = ctx.me_compute_host(host, n, me.ME_FP64, out=out)
+    assert got.data_ptr() == out.data_ptr() and torch.equal(got, ctx.me_compute(mom, n, me.ME_FP64).cpu())
+    ctx.close()
