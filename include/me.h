@@ -23,7 +23,23 @@
  * Pointers named d_* are DEVICE pointers, everything else is HOST memory.  The caller
  * owns every buffer it passes; the library owns me_ctx and its internal scratch.
  * No function throws or aborts; every function returns an me_status.
- * Every entry point runs on the CUDA device that was current at me_create time.
+ *
+ * Devices.  A context belongs to the CUDA device that was current at me_create: its tables, colour matrix and scratch live
+ * there.  Every entry point that takes a context runs on that device; if another device is current at the call it is
+ * switched for the duration of the call and restored on return.  Buffers passed in must be reachable from that device.
+ * One process may hold contexts on several devices.
+ *
+ * Concurrency.  A context is NOT thread-safe: one host thread at a time per context (use one context per thread).  From
+ * one thread, calls on one context may be issued on any streams: a call on another stream than the previous call of the same
+ * context first waits (on the device, cudaStreamWaitEvent) for that call, because they share the context's scratch
+ * (jamp staging of g g -> t t~ g g g, cached currents of ME_OPT_SHARE_CURRENTS, the workspace of me_filter_helicities /
+ * me_select_helicity_color) and helicity lists.  Results are therefore correct on any mix of streams, but calls on ONE
+ * context do not overlap on the GPU; to run several batches concurrently (several producers sharing
+ * one GPU) create one context per stream.  me_set_helicities / me_filter_helicities wait for the context's previous call on
+ * the host before they replace the lists.
+ *
+ * Alignment.  d_momenta, d_rnd: 16 bytes (what the vector loads need; cudaMalloc and torch give 256 or more); d_me, d_me_hel:
+ * 8 bytes.  Anything less returns ME_EALIGN.
  * ===================================================================================== */
 #ifndef PAPER_2303_18244_B200_ME_H
 #define PAPER_2303_18244_B200_ME_H
@@ -74,6 +90,9 @@ typedef struct {
                                    amplitude and colour-sum term evaluated exactly once */
   double flops_per_event_fixed[3]; /* helicity-independent flops per event (invariants, bases)   */
   double flops_executed_per_helicity[3]; /* flops the kernels actually issue (>= algorithmic: recomputation) */
+  double flops_per_event_shared;  /* ME_OPT_SHARE_CURRENTS: ALGORITHMIC flops per event of the sharing kernel over the full helicity
+                                     set (every current evaluated once per distinct helicity assignment of ITS OWN legs, in the walk
+                                     order of the kernel), fixed part included; 0 where no such kernel exists                          */
 } me_info;
 
 /* Create a context for `process` on the current CUDA device.  Builds the colour matrix and
@@ -91,7 +110,8 @@ me_status me_get_info(const me_ctx* ctx, me_info* out);
  * on the first n events of d_momenta; helicity h is "good" iff
  *     max_events  ME_h(evt) / sum_h' ME_h'(evt)  >  1e-12.
  * mask_out[w] bit b <=> helicity index 64*w+b is good.  The mask is stored in the context and
- * returned.  Synchronises `stream`.  n must be >= 1; the buffer must hold ceil(n/P) pages.
+ * returned.  Synchronises `stream`.  n must be >= 1; the buffer must hold ceil(n/P) pages.  The per-helicity fractions are
+ * reduced on the device (workspace of (ncomb + 1) n doubles owned by the context); only ncomb doubles reach the host.
  * d_momenta layout: see me_compute. */
 me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
                                uint64_t mask_out[2], int* ngood_out, void* stream);
@@ -100,8 +120,15 @@ me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
  * ME_OPT_PARITY_PAIRING: for the pure-QCD processes |M_h|^2 = |M_{~h}|^2 where ~h flips
  * every helicity (parity invariance, tree level, real momenta), so me_compute evaluates one helicity of every good
  * pair and counts it twice: half the work, same number up to rounding (~1e-14).  Ignored for e+ e- -> mu+ mu- and
- * whenever the installed mask is not closed under h -> ~h.  me_compute_helicities is unaffected. */
-typedef enum { ME_OPT_PARITY_PAIRING = 0 } me_option;
+ * whenever the installed mask is not closed under h -> ~h.  me_compute_helicities is unaffected.
+ * ME_OPT_SHARE_CURRENTS (second half: "sharing sub-tree currents across helicity
+ * combinations"): a gluon sub-tree current depends only on the helicities of its own gluons, a one-gluon quark current on one
+ * quark and one gluon helicity.  With the option on, g g -> t t~ g g runs a kernel that walks the good helicities in a
+ * reflected Gray order (quark helicities fastest) and re-evaluates a current only when one of ITS helicities changed since the
+ * previous step; three-gluon sub-trees are parked in an L2-resident scratch owned by the context.  Same diagrams, same
+ * amplitudes, same number up to rounding order (~1e-15).  Ignored by the other processes.  me_info.flops_per_event_shared is
+ * the algorithmic flop count with the option on.  me_compute_helicities / me_compute_jamps are unaffected. */
+typedef enum { ME_OPT_PARITY_PAIRING = 0, ME_OPT_SHARE_CURRENTS = 1 } me_option;
 me_status me_set_option(me_ctx* ctx, me_option option, int value);
 
 /* Install a helicity mask without filtering (e.g. one returned by an earlier context). */
@@ -109,9 +136,8 @@ me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
 
 /* The hot path.  Asynchronous on `stream`
  * (a cudaStream_t passed as void*; null = default stream).  No host<->device copy, no
- * synchronisation (except a one-off scratch allocation for ME_GG_TTXGGG the first time a
- * larger n is seen; that process is evaluated in slices of 65536 events so the scratch
- * never exceeds 3.8 GB).
+ * synchronisation (except a one-off scratch allocation for ME_GG_TTXGGG, and for ME_GG_TTXGG with
+ * ME_OPT_SHARE_CURRENTS, the first time; the scratch is bounded whatever n is).
  *   d_momenta : DEVICE, FP64 in every precision mode, AoSoA [ceil(n/P)][npar][4][P] with
  *               P = me_info.page and component order (E,px,py,pz); event e lives at page e/P,
  *               lane e%P.  The last page must be allocated in full; lanes >= n are read
@@ -140,7 +166,7 @@ me_status me_compute_host(me_ctx* ctx, const double* h_momenta, int64_t n, me_pr
 
 /* Same pass, but also returns the per-helicity colour-summed |M_h|^2 (not averaged) for ALL
  * ncomb helicities (masked ones evaluate too): d_me_hel is DEVICE FP64 [ncomb][n].
- * Used by the filter and by the parity tests.  d_me may be null. */
+ * Used by the filter and by the parity tests.  d_me may be null.  Asynchronous on `stream`. */
 me_status me_compute_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
                                 me_precision precision, double* d_me, double* d_me_hel, void* stream);
 
@@ -150,8 +176,9 @@ me_status me_compute_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
  * me_philox_uniform).  d_ihel[e] = helicity index drawn with probability ME_h / sum_h ME_h over the installed good
  * helicities; d_icol[e] = colour-flow index drawn with probability |J_s|^2 / sum_s |J_s|^2 at that helicity; both by
  * inverse CDF in index order with FP64 left-to-right sums (first k with cum_k >= u * total).  FP64 throughout; every
- * kernel stays in lockstep (the helicity enters as data).  d_ihel, d_icol: DEVICE int32 [n].  Allocates and frees a
- * temporary buffer and synchronises `stream`.  Errors as me_compute. */
+ * kernel stays in lockstep (the helicity enters as data).  d_ihel, d_icol: DEVICE int32 [n].  Asynchronous on `stream`
+ * (the workspace, max(ncomb, 2 ncolor) x n doubles, is owned by the context and grown on first use: that one call
+ * synchronises).  Errors as me_compute. */
 me_status me_select_helicity_color(me_ctx* ctx, const double* d_momenta, int64_t n, uint64_t seed, uint64_t first_event,
                                    int32_t* d_ihel, int32_t* d_icol, void* stream);
 
@@ -159,7 +186,7 @@ me_status me_select_helicity_color(me_ctx* ctx, const double* d_momenta, int64_t
  * cross-section", line 45 the idea of offloading them).
  *   w_i = flux * d_weight[i] * d_me[i]   (flux = 1/(2 s) for a fixed-energy collision; d_weight from me_rambo)
  *   sums_out (HOST) = { sum_i w_i, sum_i w_i^2, max_i w_i }: sigma = sums[0]/n, its standard error from sums[1]
- *   d_accept[i] (DEVICE uint8 [n], nullable) = 1 iff u_i * wmax < w_i, with u_i = u53 of Philox4x32-10 at counter
+ *   d_accept[i] (DEVICE uint8 [n], nullable: the flags are then not stored, *naccept_out is still produced) = 1 iff u_i * wmax < w_i, with u_i = u53 of Philox4x32-10 at counter
  *   (event lo32, event hi32, 0x554E5754, 0), key = seed, event = first_event + i; wmax <= 0 selects the batch maximum;
  *   *naccept_out = number of accepted events.
  * Reductions are fixed-order trees without atomics (bit-identical run to run).  Allocates temporaries and

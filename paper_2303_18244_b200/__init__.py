@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_PKG, "libme_b200.so")
 ME_OK, ME_EINVAL, ME_EPROCESS, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA = range(7)
 ME_EPEM_MUPMUM, ME_GG_TTX, ME_GG_TTXG, ME_GG_TTXGG, ME_GG_TTXGGG = range(5)
 ME_FP64, ME_MIXED, ME_FP32 = range(3)
-ME_OPT_PARITY_PAIRING = 0
+ME_OPT_PARITY_PAIRING, ME_OPT_SHARE_CURRENTS = 0, 1
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
 EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute", "me_compute_host",
@@ -30,7 +30,8 @@ class me_info(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int) for k in ("npar", "ninitial", "ndiagrams", "ncomb", "ncolor", "color_denom", "avg_denom",
                                             "page", "nkernels", "namplitudes")] + \
                [("mass", ctypes.c_double * 8), ("flops_per_helicity", ctypes.c_double * 3),
-                ("flops_per_event_fixed", ctypes.c_double * 3), ("flops_executed_per_helicity", ctypes.c_double * 3)]
+                ("flops_per_event_fixed", ctypes.c_double * 3), ("flops_executed_per_helicity", ctypes.c_double * 3),
+                ("flops_per_event_shared", ctypes.c_double)]
 
 
 class MEError(RuntimeError):

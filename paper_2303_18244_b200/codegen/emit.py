@@ -15,13 +15,66 @@ of csrc/hel_amp.cuh as written.
 """
 from .topology import Topology
 
-# real flops of the routines in hel_amp.cuh, as written
-FLOPS = dict(row_slash=64, slash_col=64, row_col=30, wdot=30, kdot=14, quark_step=131, v3_current=156,
-             v4_dots=96, v4_current=56, bilinear=72, gluon_pol=3, spinor=8, jamp_entry=2)
+# real flops of the routines in hel_amp.cuh, as written.  Not free parameters: tests/flopcount/count_flops.cpp instantiates the
+# routines on the host with an operator-counting scalar and tests/test_abi_and_host.py compares every entry with what it counts
+# (gluon_pol: the multiplication by the compile-time sign +-1 of eps / eps* is folded; spinor: either helicity branch).
+FLOPS = dict(row_slash=64, slash_col=64, row_col=30, wdot=30, kdot=14, quark_step=127, v3_current=156,
+             v4_dots=96, v4_current=56, bilinear=72, gluon_pol=3, spinor=6, jamp_entry=2)
 
 
 def particle_of(label):
     return label if label < 2 else label + 2
+
+
+# --- propagator denominators in double-double arithmetic (csrc/hel_amp.cuh "Propagator denominators")
+DD_DOT_FLOPS = 4 * 2 + 3 * 17      # four error-free products, three double-double additions
+DD_ADD_FLOPS = 17
+
+
+def dd_sum(terms):
+    """terms = [(sign, expression of type DD)] -> (nested dd_add / dd_sub expression, flops)"""
+    sign, expr = terms[0]
+    out = expr if sign > 0 else "dd_neg(%s)" % expr
+    for sign, expr in terms[1:]:
+        out = "%s(%s, %s)" % ("dd_add" if sign > 0 else "dd_sub", out, expr)
+    return out, DD_ADD_FLOPS * (len(terms) - 1)
+
+
+def dd_invariant_lines(labels, tlabels, sgn, part):
+    """declarations of the exact pairwise invariants: d{i}_{j} = p_i.p_j, dt{l} = p_t.p_l, sq{l} = p_l^2, sqt = p_t^2 - m_t^2
+    (labels: gluon labels that occur in a propagator; tlabels: those that occur in a quark propagator) -> (lines, flops)"""
+    out, fl = [], 0
+    labels = sorted(labels)
+    for a, i in enumerate(labels):
+        out.append("const DD sq%d = dd_dot(pd%d, pd%d);" % (i, part(i), part(i))); fl += DD_DOT_FLOPS
+        for j in labels[a + 1:]:
+            out.append("const DD d%d_%d = dd_dot(pd%d, pd%d);" % (i, j, part(i), part(j))); fl += DD_DOT_FLOPS
+    if tlabels:
+        out.append("const DD sqt = dd_offshell(pd2, mt_d);"); fl += DD_DOT_FLOPS + 2 + DD_ADD_FLOPS
+    for l in sorted(tlabels):
+        out.append("const DD dt%d = dd_dot(pd2, pd%d);" % (l, part(l))); fl += DD_DOT_FLOPS
+    return out, fl
+
+
+def dd_k2(b, sgn):
+    """K^2 of the gluon set b (labels), K = sum_l sgn(l) p_l: sum_l p_l^2 + 2 sum_{i<j} sgn_i sgn_j p_i.p_j -> (DD expression, flops)"""
+    terms = [(+1, "sq%d" % l) for l in b]
+    pairs = [(sgn(b[i]) * sgn(b[j]), "d%d_%d" % (b[i], b[j])) for i in range(len(b)) for j in range(i + 1, len(b))]
+    if pairs:
+        pe, pf = dd_sum(pairs)
+        terms.append((+1, "dd_mul2(%s)" % pe))
+    else:
+        pf = 0
+    e, f = dd_sum(terms)
+    return e, f + pf
+
+
+def dd_q2(b, sgn):
+    """(p_t - K)^2 - m_t^2 = (p_t^2 - m_t^2) + K^2 - 2 sum_l sgn(l) p_t.p_l -> (DD expression, flops)"""
+    ke, kf = dd_k2(b, sgn)
+    le, lf = dd_sum([(sgn(l), "dt%d" % l) for l in b])
+    e, f = dd_sum([(+1, "sqt"), (+1, ke), (-1, "dd_mul2(%s)" % le)])
+    return e, f + kf + lf
 
 
 def bits(m):
@@ -151,43 +204,24 @@ class KernelEmitter:
         for m in need_K | self.used_iK2 | self.used_iQ:
             labs_needed.update(bits(m))
         fixed = 0
-        # pairwise invariants
-        pairs = set()
+        # exact invariants (double-double) of the gluons that occur in a propagator
+        labs, tl = set(), set()
         for m in self.used_iK2 | self.used_iQ:
-            b = bits(m)
-            for i in range(len(b)):
-                for j in range(i + 1, len(b)):
-                    pairs.add((b[i], b[j]))
-        for (i, j) in sorted(pairs):
-            A("const double d%d_%d = pdot(pd%d, pd%d);" % (i, j, particle_of(i), particle_of(j)))
-            fixed += 7
-        tl = set()
+            labs.update(bits(m))
         for m in self.used_iQ:
             tl.update(bits(m))
-        for l in sorted(tl):
-            A("const double dt%d = pdot(pd2, pd%d);" % (l, particle_of(l)))
-            fixed += 7
-
-        def k2expr(m):
-            b = bits(m)
-            terms = []
-            for i in range(len(b)):
-                for j in range(i + 1, len(b)):
-                    s = sgn(b[i]) * sgn(b[j])
-                    terms.append(("+" if s > 0 else "-") + "d%d_%d" % (b[i], b[j]))
-            return "2.0*(" + "".join(terms).lstrip("+") + ")"
-
+        lines, fl = dd_invariant_lines(labs, tl, sgn, particle_of)
+        for l in lines:
+            A(l)
+        fixed += fl
         for m in sorted(self.used_iK2):
-            A("const R iK2_%d = (R)(1.0/(%s));" % (m, k2expr(m)))
-            fixed += 2 + len(bits(m)) * (len(bits(m)) - 1) // 2
+            e, fl = dd_k2(bits(m), sgn)
+            A("const R iK2_%d = (R)(1.0 / dd_value(%s));" % (m, e))
+            fixed += fl + 2
         for m in sorted(self.used_iQ):
-            b = bits(m)
-            lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
-            if len(b) == 1:
-                A("const R iQ_%d = (R)(1.0/(-2.0*(%s)));" % (m, lin))
-            else:
-                A("const R iQ_%d = (R)(1.0/(%s-2.0*(%s)));" % (m, k2expr(m), lin))
-            fixed += 4 + len(b) * (len(b) + 1) // 2
+            e, fl = dd_q2(bits(m), sgn)
+            A("const R iQ_%d = (R)(1.0 / dd_value(%s));" % (m, e))
+            fixed += fl + 2
         for m in sorted(need_K):
             b = bits(m)
             comps = []
@@ -295,7 +329,7 @@ def emit_single_kernel_process(n, name):
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, T.ncol * T.ncol, ", ".join(str(float(x)) for row in T.color_num for x in row)))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr};"
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr, false, nullptr, 0.0};"
       % (name, n, T.ndiagrams, K.namp, T.ncol, T.color_denom, float(per_hel), float(per_hel), float(per_hel),
          float(per_hel), float(per_hel), float(per_hel), float(K.fixed_flops), name, name))
     S("}  // namespace me")

@@ -19,7 +19,7 @@ jamps in per-thread shared-memory slots [slot][thread] (north_star "jamp staging
 """
 from itertools import permutations
 
-from .emit import FLOPS, colour_sum_lines
+from .emit import FLOPS, colour_sum_lines, dd_invariant_lines, dd_k2, dd_q2
 from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
@@ -557,33 +557,19 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     for k in range(NPAR):
         S("    const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
     fixed = 0
-    for i in range(N):
-        for j in range(i + 1, N):
-            S("    const double d%d_%d = pdot(pd%d, pd%d);" % (i, j, part(i), part(j))); fixed += 7
-    for l in range(N):
-        S("    const double dt%d = pdot(pd2, pd%d);" % (l, part(l))); fixed += 7
-
-    def k2expr(m):
-        b = [i for i in range(N) if m >> i & 1]
-        terms = []
-        for i in range(len(b)):
-            for j in range(i + 1, len(b)):
-                terms.append(("+" if sgn(b[i]) * sgn(b[j]) > 0 else "-") + "d%d_%d" % (b[i], b[j]))
-        return "2.0*(" + "".join(terms).lstrip("+") + ")"
-
+    lines, fl = dd_invariant_lines(range(N), range(N), sgn, part)      # exact invariants (hel_amp.cuh "Propagator denominators")
+    for l in lines:
+        S("    " + l)
+    fixed += fl
     for l in range(N):
         S("    stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
     S("    stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
     for m, slot in lay.IK2.items():
-        S("    sm[ME_EO(%d)] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+        e, fl = dd_k2([i for i in range(N) if m >> i & 1], sgn)
+        S("    sm[ME_EO(%d)] = (R)(1.0 / dd_value(%s));" % (slot, e)); fixed += fl + 2
     for m, slot in lay.IQ.items():
-        b = [i for i in range(N) if m >> i & 1]
-        lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
-        if len(b) == 1:
-            S("    sm[ME_EO(%d)] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
-        else:
-            S("    sm[ME_EO(%d)] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
-        fixed += 8
+        e, fl = dd_q2([i for i in range(N) if m >> i & 1], sgn)
+        S("    sm[ME_EO(%d)] = (R)(1.0 / dd_value(%s));" % (slot, e)); fixed += fl + 2
     for l in range(N):
         S("    { GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GBS[l]))
         fixed += 22
@@ -668,7 +654,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr};"
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr, false, nullptr, 0.0};"
       % (name, N, 123, namp, ncol, color_denom, float(per_hel), float(per_hel), float(per_hel),
          float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name))
     S("}  // namespace me")

@@ -16,6 +16,7 @@ gluons (from the t~ end); (|L|,|mid|,|R|) = (0,5,0) 510, (0,4,1)+(1,4,0) 450, (0
 """
 from itertools import permutations
 
+from .emit import dd_invariant_lines, dd_k2, dd_q2
 from .emit_orbit import Inst, FL, c_leaf, c_v3, c_v4, c_step, c_close, ONE, mask_of, SlotAlloc, eo, sum_expr
 from .topology import color_matrix
 
@@ -708,33 +709,18 @@ def prologue_lines(lay):
     A("const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % NPAR)
     for k in range(NPAR):
         A("const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
-    for i in range(N):
-        for j in range(i + 1, N):
-            A("const double d%d_%d = pdot(pd%d, pd%d);" % (i, j, part(i), part(j))); fixed += 7
-    for l in range(N):
-        A("const double dt%d = pdot(pd2, pd%d);" % (l, part(l))); fixed += 7
-
-    def k2expr(m):
-        b = [i for i in range(N) if m >> i & 1]
-        terms = []
-        for i in range(len(b)):
-            for j in range(i + 1, len(b)):
-                terms.append(("+" if sgn(b[i]) * sgn(b[j]) > 0 else "-") + "d%d_%d" % (b[i], b[j]))
-        return "2.0*(" + "".join(terms).lstrip("+") + ")"
-
+    lines, fl = dd_invariant_lines(range(N), range(N), sgn, part)      # exact invariants (hel_amp.cuh "Propagator denominators")
+    out.extend(lines)
+    fixed += fl
     for l in range(N):
         A("stp<R>(sm, %d, pcast<R>(%s));" % (lay.MOM + 4 * l, "pd%d" % part(l) if sgn(l) > 0 else "pneg(pd%d)" % part(l)))
     A("stp<R>(sm, %d, pcast<R>(pd2));" % lay.PT)
     for m, slot in lay.IK2.items():
-        A("sm[ME_EO(%d)] = (R)(1.0/(%s));" % (slot, k2expr(m))); fixed += 8
+        e, fl = dd_k2([i for i in range(N) if m >> i & 1], sgn)
+        A("sm[ME_EO(%d)] = (R)(1.0 / dd_value(%s));" % (slot, e)); fixed += fl + 2
     for m, slot in lay.IQ.items():
-        b = [i for i in range(N) if m >> i & 1]
-        lin = "".join(("+" if sgn(l) > 0 else "-") + "dt%d" % l for l in b).lstrip("+")
-        if len(b) == 1:
-            A("sm[ME_EO(%d)] = (R)(1.0/(-2.0*(%s)));" % (slot, lin))
-        else:
-            A("sm[ME_EO(%d)] = (R)(1.0/(%s-2.0*(%s)));" % (slot, k2expr(m), lin))
-        fixed += 8
+        e, fl = dd_q2([i for i in range(N) if m >> i & 1], sgn)
+        A("sm[ME_EO(%d)] = (R)(1.0 / dd_value(%s));" % (slot, e)); fixed += fl + 2
     for l in range(N):
         A("{ GluonBasis<R> gb = gluon_basis(pcast<R>(pd%d)); gb.bx *= (R)%d; gb.by *= (R)%d; stgb<R>(sm, %d, gb); }" % (part(l), -sgn(l), -sgn(l), lay.GBS[l]))
         fixed += 22
@@ -969,8 +955,8 @@ def emit_orbit5_process(name="gg_ttxggg"):
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) { return launch_multi(precision, a, parts_%s, %d, %d, color_num_%s); }"
       % (name, name, len(kinfo), ncol, name))
-    S("static size_t scratch_%s(int precision, long npad) { return multi_scratch_bytes(precision, npad, %d); }" % (name, ncol))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s};"
+    S("static size_t scratch_%s(int precision, long npad, int, int) { return multi_scratch_bytes(precision, npad, %d); }" % (name, ncol))
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, true, nullptr, 0.0};"
       % (name, N, 1240, namp, ncol, color_denom, len(kinfo) + 1, float(algo), float(algo), float(algo),
          float(executed), float(executed), float(executed), float(fixed), name, name, name))
     S("}  // namespace me")

@@ -15,17 +15,10 @@ namespace me {
 #define CS_WARPS 8
 #define CS_ROWS (CS_NCOL / CS_WARPS)   // 15
 
-// colour-matrix numerators (exact small integers); 115 KB in FP64, too large for the constant bank
-__device__ double c_color_d[CS_NCOL * CS_NCOL];
-__device__ float c_color_f[CS_NCOL * CS_NCOL];
-
-template <typename RC> __device__ __forceinline__ RC cmat(int i);
-template <> __device__ __forceinline__ double cmat<double>(int i) { return __ldg(&c_color_d[i]); }
-template <> __device__ __forceinline__ float cmat<float>(int i) { return __ldg(&c_color_f[i]); }
-
+// (the colour-matrix numerators, exact small integers, 115 KB in FP64, live in device buffers owned by the context: cm)
 // RJ: staging type, RC: arithmetic type of the contraction
 template <typename RJ, typename RC>
-__global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restrict__ gj, long npad, long n, long hs, int nh,
+__global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RC* __restrict__ cm, const RJ* __restrict__ gj, long npad, long n, long hs, int nh,
                                                              const unsigned char* __restrict__ hels, int first,
                                                              double norm_hel, double inv_avg,
                                                              double* __restrict__ me_out, double* __restrict__ me_hel) {
@@ -49,7 +42,7 @@ __global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RJ* __restric
       const RC xr = sx[2 * j][lane], xi = sx[2 * j + 1][lane];
 #pragma unroll
       for (int r = 0; r < CS_ROWS; ++r) {
-        const RC c = cmat<RC>((row0 + r) * CS_NCOL + j);
+        const RC c = __ldg(&cm[(row0 + r) * CS_NCOL + j]);
         yr[r] += c * xr; yi[r] += c * xi;
       }
     }
@@ -80,7 +73,6 @@ size_t multi_scratch_bytes(int precision, long npad, int ncol) {
   return (size_t)ME_HEL_CHUNK * ncol * 2 * np * (precision == 2 ? sizeof(float) : sizeof(double));
 }
 
-static bool g_color_loaded = false;
 // tensor-core colour sums (FP64: DMMA, FP32: TF32 split); ME_COLOR_FMA=1 in the environment selects the plain-FMA kernels (A/B timing)
 static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
 // ME_COLOR_MMA_SYNC=1 selects the warp-level TF32 kernel (color_sum_tf32.cu) instead of the tcgen05 one (A/B timing)
@@ -110,14 +102,7 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
 static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
                                       const double* color_num_host) {
   if (ncol != CS_NCOL) return cudaErrorInvalidValue;
-  if (!g_color_loaded) {
-    static float cf[CS_NCOL * CS_NCOL];
-    for (int i = 0; i < CS_NCOL * CS_NCOL; ++i) cf[i] = (float)color_num_host[i];
-    cudaError_t e = cudaMemcpyToSymbol(c_color_d, color_num_host, sizeof(double) * CS_NCOL * CS_NCOL);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_color_f, cf, sizeof(float) * CS_NCOL * CS_NCOL);
-    if (e != cudaSuccess) return e;
-    g_color_loaded = true;
-  }
+  if (a.color_d == nullptr || a.color_f == nullptr) return cudaErrorInvalidValue;   // uploaded by me_create on the context's device
   const unsigned cgrid = (unsigned)(a.npad / 32);
   for (int base = 0; base < a.nhel; base += ME_HEL_CHUNK) {
     const int nh = a.nhel - base < ME_HEL_CHUNK ? a.nhel - base : ME_HEL_CHUNK;
@@ -142,23 +127,21 @@ static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long h
     const size_t smd = sizeof(double) * (2 * CS_NCOL + CS_WARPS) * 32, smf = sizeof(float) * (2 * CS_NCOL + CS_WARPS) * 32;
     cudaFuncSetAttribute(k_color_sum<double, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smd);
     if (precision == 0 && g_use_dmma) {
-      const double* cm = nullptr;
-      cudaError_t e2 = cudaGetSymbolAddress((void**)&cm, c_color_d);
-      if (e2 == cudaSuccess) e2 = launch_color_sum_dmma(cm, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      cudaError_t e2 = launch_color_sum_dmma(a.nsm, a.color_d, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
       if (e2 != cudaSuccess) return e2;
     } else if (precision != 0 && g_use_dmma) {      // FP32 colour sum (float and mixed mode) on the tensor cores, TF32 hi/lo split
-      const float* cf = nullptr;
-      cudaError_t e2 = cudaGetSymbolAddress((void**)&cf, c_color_f);
-      if (e2 == cudaSuccess && g_use_tcgen05)
-        e2 = launch_color_sum_tcgen05(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
-      else if (e2 == cudaSuccess) e2 = launch_color_sum_tf32(precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      const float* cf = a.color_f;
+      cudaError_t e2 = cudaSuccess;
+      if (g_use_tcgen05)
+        e2 = launch_color_sum_tcgen05(a.nsm, precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
+      else e2 = launch_color_sum_tf32(a.nsm, precision == 1, cf, a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.stream);
       if (e2 != cudaSuccess) return e2;
     } else if (precision == 0)
-      k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<double, double><<<cgrid, 32 * CS_WARPS, smd, a.stream>>>(a.color_d, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     else if (precision == 1)
-      k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<double, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>(a.color_f, (const double*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     else
-      k_color_sum<float, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>((const float*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
+      k_color_sum<float, float><<<cgrid, 32 * CS_WARPS, smf, a.stream>>>(a.color_f, (const float*)a.scratch, a.npad, a.n, hs, nh, a.hels + base, first, a.norm_hel, a.inv_avg, a.me_out, a.me_hel);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }

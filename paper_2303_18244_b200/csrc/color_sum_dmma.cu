@@ -112,14 +112,8 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
   }
 }
 
-cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
+cudaError_t launch_color_sum_dmma(int sms, const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
                                   double norm_hel, double inv_avg, double* me_out, double* me_hel, cudaStream_t stream) {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  }
   const size_t smem = sizeof(double) * CD_RB * CD_KS * 32;
   cudaError_t e = cudaFuncSetAttribute(k_color_sum_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;

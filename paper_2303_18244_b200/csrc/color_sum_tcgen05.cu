@@ -211,15 +211,9 @@ __global__ void __launch_bounds__(TC_M, 2) k_color_sum_tcgen05(const float* __re
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TC_TMEM_COLS) : "memory");
 }
 
-cudaError_t launch_color_sum_tcgen05(int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
+cudaError_t launch_color_sum_tcgen05(int sms, int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
                                      const unsigned char* hels, int first, double norm_hel, double inv_avg, double* me_out, double* me_hel,
                                      cudaStream_t stream) {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  }
   const long ntiles = (npad + TC_M - 1) / TC_M;
   const unsigned grid = (unsigned)(ntiles < 2L * sms ? ntiles : 2L * sms);
   cudaError_t e;

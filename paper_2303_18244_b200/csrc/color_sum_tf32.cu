@@ -114,15 +114,9 @@ __global__ void __launch_bounds__(32 * CT_WARPS, 1) k_color_sum_tf32(const float
   }
 }
 
-cudaError_t launch_color_sum_tf32(int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
+cudaError_t launch_color_sum_tf32(int sms, int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
                                   const unsigned char* hels, int first, double norm_hel, double inv_avg, double* me_out, double* me_hel,
                                   cudaStream_t stream) {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  }
   const size_t smem = sizeof(uint4) * CT_RT * CT_KS * 32;
   const long ntiles = (npad + 8 * CT_WARPS - 1) / (8 * CT_WARPS);
   const unsigned grid = (unsigned)(ntiles < sms ? ntiles : sms);

@@ -43,6 +43,44 @@ template <typename R> ME_DEV P4<R> pneg(const P4<R>& a) { return {-a.e, -a.x, -a
 ME_DEV double pdot(const P4<double>& a, const P4<double>& b) { return a.e * b.e - a.x * b.x - a.y * b.y - a.z * b.z; }
 template <typename R> ME_DEV P4<R> pcast(const P4<double>& a) { return {(R)a.e, (R)a.x, (R)a.y, (R)a.z}; }
 
+#ifndef ME_HOST_FLOP_COUNT
+// ------------------------------------------------------------------------------------
+// Propagator denominators (helicity-independent, once per event, FP64 in every precision mode).  Without cuts some events
+// have an invariant s_ij ~ 1e-6 s: (p_i + p_j)^2 formed in plain binary64 then carries a relative error eps * E^2 / s_ij, and
+// the shortcut 2 p_i.p_j (which assumes exactly massless legs) differs from it by (p_i^2 + p_j^2) / s_ij, where p_i^2 ~ eps E^2 is
+// the rounding of the input energy itself: both are 1e-10 effects on such events against north_star's 1e-11.  The invariants are
+// therefore formed in double-double arithmetic (error-free products with FMA, compensated sums) from the binary64 inputs AS
+// GIVEN, own squares p_i^2 and p_t^2 - m^2 included: K^2 and q^2 - m^2 are exact to rounding for the inputs the caller
+// passed, which is what the oracle evaluated in long double computes.  ~1 kflop per event.
+// ------------------------------------------------------------------------------------
+struct DD { double hi, lo; };
+ME_DEV DD dd_two_sum(double a, double b) {
+  const double s = __dadd_rn(a, b), bb = __dadd_rn(s, -a);
+  return {s, __dadd_rn(__dadd_rn(a, -__dadd_rn(s, -bb)), __dadd_rn(b, -bb))};
+}
+ME_DEV DD dd_two_prod(double a, double b) {
+  const double p = __dmul_rn(a, b);
+  return {p, __fma_rn(a, b, -p)};
+}
+ME_DEV DD dd_add(const DD& a, const DD& b) {
+  const DD s = dd_two_sum(a.hi, b.hi);
+  const double lo = __dadd_rn(__dadd_rn(a.lo, b.lo), s.lo);
+  const double hi = __dadd_rn(s.hi, lo);
+  return {hi, __dadd_rn(lo, -__dadd_rn(hi, -s.hi))};
+}
+ME_DEV DD dd_neg(const DD& a) { return {-a.hi, -a.lo}; }
+ME_DEV DD dd_sub(const DD& a, const DD& b) { return dd_add(a, dd_neg(b)); }
+ME_DEV DD dd_mul2(const DD& a) { return {2.0 * a.hi, 2.0 * a.lo}; }       // exact
+ME_DEV double dd_value(const DD& a) { return __dadd_rn(a.hi, a.lo); }
+// Minkowski product a.b of two binary64 four-vectors
+ME_DEV DD dd_dot(const P4<double>& a, const P4<double>& b) {
+  const DD t = dd_two_prod(a.e, b.e), x = dd_two_prod(a.x, b.x), y = dd_two_prod(a.y, b.y), z = dd_two_prod(a.z, b.z);
+  return dd_sub(dd_sub(dd_sub(t, x), y), z);
+}
+// a.a - m^2
+ME_DEV DD dd_offshell(const P4<double>& a, double m) { return dd_sub(dd_dot(a, a), dd_two_prod(m, m)); }
+#endif
+
 // ------------------------------------------------------------------------------------
 // External gluons (step a3).  eps(p,lam) = (-lam e1 - i e2)/sqrt2 with real e1,e2 that do
 // not depend on the helicity, so the basis is built once per event and a helicity flip is
@@ -275,6 +313,7 @@ template <typename R> ME_DEV W4<R> bilinear(const W4<R>& r, const W4<R>& c) {
 
 }  // namespace me
 
+#ifndef ME_HOST_FLOP_COUNT   // tests/flopcount instantiates the arithmetic routines on the host; storage helpers are CUDA-only
 // ------------------------------------------------------------------------------------
 // Per-thread shared-memory slots.  Slots are stored in PAIRS: slot s of thread t is element
 //     2 * ((s >> 1) * ME_SM_STRIDE + t) + (s & 1)        (ME_SM_STRIDE = threads per CTA)
@@ -521,6 +560,8 @@ ME_DEV void tm_free(uint32_t base, uint32_t ncols) {
 }
 }  // namespace me
 
+#endif  // ME_HOST_FLOP_COUNT
+
 // ------------------------------------------------------------------------------------
 // Helpers of the orbit-looped kernels (codegen/emit_orbit.py): operands addressed through a
 // per-instance table of shared-memory offsets, two-sided quark line, dual currents.
@@ -529,10 +570,12 @@ namespace me {
 template <typename R> ME_DEV Cx<R> cxs(const Cx<R>& c, R s) { return {c.re * s, c.im * s}; }
 template <typename R> ME_DEV R lam_of(int h, int bit) { return ((h >> bit) & 1) ? (R)1 : (R)-1; }
 // polarisation from a basis whose b part is pre-signed (+ for outgoing eps*, - for incoming eps)
-template <typename R> ME_DEV W4<R> gluon_pol_s(const R* p, R lam) {
-  const GluonBasis<R> g = ldgb<R>(p);
+template <typename R> ME_DEV W4<R> gluon_pol_from(const GluonBasis<R>& g, R lam) {
   return {(R)0, (R)0, -lam * g.ax, g.bx, -lam * g.ay, g.by, -lam * g.az, (R)0};
 }
+#ifndef ME_HOST_FLOP_COUNT
+template <typename R> ME_DEV W4<R> gluon_pol_s(const R* p, R lam) { return gluon_pol_from<R>(ldgb<R>(p), lam); }
+#endif
 // column current grown from the t~ end: chi' = (q-slash + m) X * iden  (X = V-slash chi already formed)
 template <typename R> ME_DEV W4<R> col_step(const W4<R>& X, const P4<R>& q, R m, R iden) {
   const R A = (q.e - q.z) * iden, B = (q.e + q.z) * iden, qx = q.x * iden, qy = q.y * iden, ms = m * iden;

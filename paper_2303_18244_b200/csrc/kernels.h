@@ -22,8 +22,12 @@ struct LaunchArgs {
   double* me_out;             // [n] or null
   double* me_hel;             // [ncomb][n] or null
   double* jamp_out;           // [ncol][2][n] or null (single helicity expected)
-  void* scratch;              // process-specific device scratch (gg->tt~ggg jamp staging)
+  void* scratch;              // process-specific device scratch (gg->tt~ggg jamp staging; cached currents of the sharing kernel)
   size_t scratch_bytes;
+  const double* color_d;      // device colour-matrix numerators [ncol*ncol] (processes with a separate colour-sum kernel), else null
+  const float* color_f;
+  int nsm;                    // multiprocessors of the context's device
+  int share;                  // 1: kernel variant that shares sub-tree currents across helicities (hels is then in walk order)
   cudaStream_t stream;
 };
 
@@ -35,7 +39,10 @@ struct ProcTable {
   double fixed_flops;
   const double* color_num;        // [ncol*ncol] host
   cudaError_t (*launch)(int precision, const LaunchArgs&);
-  size_t (*scratch_bytes)(int precision, long npad);   // may be null
+  size_t (*scratch_bytes)(int precision, long npad, int share, int nsm);   // may be null; may return 0
+  bool needs_color_matrix;        // the context uploads color_num for a separate colour-sum kernel
+  const unsigned char* gray_rank; // [ncomb] position of every helicity in the walk of the current-sharing kernel, or null (no such kernel)
+  double flops_shared_event;      // algorithmic flops per event of the sharing kernel over the full helicity set (0: none)
 };
 
 extern const ProcTable tab_gg_ttx, tab_gg_ttxg, tab_gg_ttxgg, tab_gg_ttxggg;
@@ -52,6 +59,8 @@ cudaError_t run_fma_peak(int fp64, double* tflops);
 cudaError_t run_unweight(const double* d_wt, const double* d_me, long n, double flux, uint64_t seed, uint64_t first_event, double wmax_in,
                          double sums[3], unsigned char* d_accept, long long* naccept, cudaStream_t st);
 cudaError_t launch_select_hel(const double* me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* ihel, cudaStream_t s);
+// fractions of me_filter_helicities: tot[i] = sum_h me_hel[h][i] (index order), maxfrac[h] = max_i me_hel[h][i] / tot[i]
+cudaError_t launch_helicity_fractions(const double* me_hel, int ncomb, long n, double* tot, double* maxfrac, cudaStream_t s);
 cudaError_t launch_select_col(double* jamp, int ncol, long n, uint64_t seed, uint64_t first_event, int* icol, cudaStream_t s);
 
 }  // namespace me

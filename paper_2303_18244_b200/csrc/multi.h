@@ -22,16 +22,17 @@ struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); };
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host);
 size_t multi_scratch_bytes(int precision, long npad, int ncol);
+// (colour-sum launchers: cmat = device pointer owned by the context, sms = multiprocessors of its device)
 // FP32 colour sum on the tensor cores, TF32 hi/lo split (color_sum_tf32.cu); cmat = device pointer to float numerators
-cudaError_t launch_color_sum_tf32(int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
+cudaError_t launch_color_sum_tf32(int sms, int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
                                   const unsigned char* hels, int first, double norm_hel, double inv_avg, double* me_out, double* me_hel,
                                   cudaStream_t stream);
 // the same contraction on tcgen05 / TMEM (color_sum_tcgen05.cu): the default FP32 / mixed colour sum
-cudaError_t launch_color_sum_tcgen05(int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
+cudaError_t launch_color_sum_tcgen05(int sms, int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
                                      const unsigned char* hels, int first, double norm_hel, double inv_avg, double* me_out, double* me_hel,
                                      cudaStream_t stream);
 // FP64 colour sum on the tensor cores (color_sum_dmma.cu); cmat = device pointer to the [ncol*ncol] numerators
-cudaError_t launch_color_sum_dmma(const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
+cudaError_t launch_color_sum_dmma(int sms, const double* cmat, const double* gj, long npad, long n, long hs, int nh, const unsigned char* hels, int first,
                                   double norm_hel, double inv_avg, double* me_out, double* me_hel, cudaStream_t stream);
 
 }  // namespace me

@@ -86,6 +86,31 @@ __global__ void k_select_col(double* __restrict__ jamp, int ncol, long n, uint64
   }
   icol[e] = inverse_cdf(jamp + e, ncol, 2 * n, u2);
 }
+// me_filter_helicities (reading Q7): tot[i] = sum_h ME_h(i) in index order, then per helicity the maximum over the filter events of
+// ME_h(i) / tot[i] (IEEE division; a maximum does not depend on the reduction order: bit-identical to the plain host loops)
+__global__ void k_hel_total(const double* __restrict__ me_hel, int ncomb, long n, double* __restrict__ tot) {
+  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  double t = 0;
+  for (int h = 0; h < ncomb; ++h) t += me_hel[(long)h * n + e];
+  tot[e] = t;
+}
+__global__ void __launch_bounds__(256) k_hel_maxfrac(const double* __restrict__ me_hel, long n, const double* __restrict__ tot, double* __restrict__ maxfrac) {
+  __shared__ double sh[8];
+  const double* row = me_hel + (long)blockIdx.x * n;
+  double m = 0;
+  for (long e = threadIdx.x; e < n; e += 256) { const double f = row[e] / tot[e]; if (f > m) m = f; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) { for (int k = 1; k < 8; ++k) m = fmax(m, sh[k]); maxfrac[blockIdx.x] = m; }
+}
+cudaError_t launch_helicity_fractions(const double* me_hel, int ncomb, long n, double* tot, double* maxfrac, cudaStream_t s) {
+  k_hel_total<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(me_hel, ncomb, n, tot);
+  k_hel_maxfrac<<<ncomb, 256, 0, s>>>(me_hel, n, tot, maxfrac);
+  return cudaGetLastError();
+}
 cudaError_t launch_select_hel(const double* me_hel, int ncomb, long n, uint64_t seed, uint64_t first_event, int* ihel, cudaStream_t s) {
   k_select_hel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(me_hel, ncomb, n, seed, first_event, ihel);
   return cudaGetLastError();
@@ -141,12 +166,21 @@ __global__ void __launch_bounds__(ME_RED_THREADS) k_accept(const double* __restr
     uint32_t r[4];
     philox4x32_10((uint32_t)ev, (uint32_t)(ev >> 32), ME_UNWT_TAG, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), r);
     a = u53(r[0], r[1]) * wmax < w[e] ? 1 : 0;
-    accept[e] = (unsigned char)a;
+    if (accept != nullptr) accept[e] = (unsigned char)a;
   }
   const unsigned b = __ballot_sync(0xffffffffu, a);
   if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = __popc(b);
   __syncthreads();
   if (threadIdx.x == 0) { int c = 0; for (int k = 0; k < ME_RED_THREADS / 32; ++k) c += sh[k]; part[blockIdx.x] = (unsigned long long)c; }
+}
+// part[0] = sum of the per-block accept counts (integers: exact in any order)
+__global__ void __launch_bounds__(ME_RED_THREADS) k_count_final(unsigned long long* __restrict__ part, long nblocks) {
+  __shared__ unsigned long long sh[ME_RED_THREADS];
+  unsigned long long c = 0;
+  for (long b = threadIdx.x; b < nblocks; b += ME_RED_THREADS) c += part[b];
+  sh[threadIdx.x] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) { for (int k = 1; k < ME_RED_THREADS; ++k) c += sh[k]; part[0] = c; }
 }
 cudaError_t run_unweight(const double* d_wt, const double* d_me, long n, double flux, uint64_t seed, uint64_t first_event, double wmax_in,
                          double sums[3], unsigned char* d_accept, long long* naccept, cudaStream_t st) {
@@ -162,15 +196,14 @@ cudaError_t run_unweight(const double* d_wt, const double* d_me, long n, double 
     e = cudaMemcpyAsync(sums, d_out, sizeof(double) * 3, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   }
-  if (e == cudaSuccess && d_accept != nullptr) {
+  if (e == cudaSuccess && (d_accept != nullptr || naccept != nullptr)) {      // the count is produced with or without the flags
     const double wmax = wmax_in > 0 ? wmax_in : sums[2];
     k_accept<<<(unsigned)nb, ME_RED_THREADS, 0, st>>>(d_w, n, wmax, seed, first_event, d_accept, d_cnt);
-    unsigned long long* h = new unsigned long long[nb];
-    e = cudaMemcpyAsync(h, d_cnt, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost, st);
+    k_count_final<<<1, ME_RED_THREADS, 0, st>>>(d_cnt, nb);
+    unsigned long long total = 0;
+    e = cudaMemcpyAsync(&total, d_cnt, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    long long c = 0; for (long b = 0; b < nb; ++b) c += (long long)h[b];
-    delete[] h;
-    if (naccept != nullptr) *naccept = c;
+    if (naccept != nullptr) *naccept = (long long)total;
   }
   if (e == cudaSuccess) e = cudaGetLastError();
   cudaFree(d_w); cudaFree(d_part); cudaFree(d_out); cudaFree(d_cnt);
@@ -203,10 +236,12 @@ __global__ void k_rambo(RamboMasses masses, double sqs, const double* __restrict
 #pragma unroll
   for (int k = 0; k < NF; ++k) {
     const double bq = b1 * q[k][1] + b2 * q[k][2] + b3 * q[k][3];
-    p[k][0] = x * (gam * q[k][0] + bq);
     p[k][1] = x * (q[k][1] + b1 * q[k][0] + a * bq * b1);
     p[k][2] = x * (q[k][2] + b2 * q[k][0] + a * bq * b2);
     p[k][3] = x * (q[k][3] + b3 * q[k][0] + a * bq * b3);
+    // massless energy as |p| rather than x (gam q0 + b.q): same number algebraically, on shell to rounding whatever the boost
+    // amplifies (reading Q12a; the propagator denominators of the ME kernels assume on-shell legs)
+    p[k][0] = sqrt(p[k][1] * p[k][1] + p[k][2] * p[k][2] + p[k][3] * p[k][3]);
   }
   double w = w0;
   if (massive) {

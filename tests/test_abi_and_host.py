@@ -115,6 +115,32 @@ def test_generated_flop_counts_are_recorded(melib):
     assert 1.5e4 < s["gg_ttxgg"]["flops_per_helicity"] < 6e4
 
 
+def test_flops_tables_match_the_device_routines(tmp_path):
+    """the generator's per-routine flop tables (codegen/emit.py FLOPS, emit_orbit.py FL, emit_orbit5.py FL5) are not free
+    parameters: tests/flopcount/count_flops.cpp instantiates the routines of csrc/hel_amp.cuh on the host with a scalar type
+    that counts every +, -, *, / it executes (SURVEY.md section 8(d) rule), and every table entry must equal that count"""
+    from paper_2303_18244_b200.codegen import emit, emit_orbit, emit_orbit5
+    exe = tmp_path / "count_flops"
+    subprocess.run(["g++", "-std=c++17", "-O0", "-I", os.path.join(ROOT, "tests", "flopcount"), "-I", os.path.join(ROOT, "paper_2303_18244_b200", "csrc"),
+                    os.path.join(ROOT, "tests", "flopcount", "count_flops.cpp"), "-o", str(exe)], check=True)
+    counted = {}
+    for line in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.splitlines():
+        name, v = line.split()
+        counted[name] = int(v)
+    assert counted["spinor_ubar_plus"] == counted["spinor_ubar_minus"] == counted["spinor_v_plus"] == counted["spinor_v_minus"]
+    assert counted["v4_current"] == counted["v4_current_1"] == counted["v4_current_2"]
+    alias = dict(quark_step="quark_step2", spinor="spinor_ubar_plus")
+    for table in (emit.FLOPS, emit_orbit.FL, emit_orbit5.FL5):
+        for key, val in table.items():
+            if key == "jamp_entry":          # one complex add into an accumulator
+                assert val == 2
+                continue
+            assert val == counted[alias.get(key, key)], (key, val, counted[alias.get(key, key)])
+    # literals the emitters use next to the tables: momentum sums (4 per padd / psub) and the per-event bases
+    assert counted["padd"] == counted["psub"] == 4 and counted["wadd"] == counted["wsub"] == 8
+    assert counted["gluon_basis"] <= 22 and counted["spinor_basis"] <= 20      # `fixed` charges 22 per gluon basis, 40 for two spinor bases
+
+
 # ------------------------------------------------------------------ host logic
 def test_aosoa_roundtrip_and_padding():
     import inputs

@@ -2,11 +2,10 @@
 element on the same seeded events (BASELINE.json north_star: helicity masks bit-exact, relative |M|^2
 error <= 1e-11 in FP64 and <= 1e-4 in FP32/mixed).
 
-FP64 tolerance: 1e-11 for every event with s_min/s >= 1e-3, where s_min is the
-smallest |2 p_i.p_j| over parton pairs; below that, the propagator 1/s_ij itself carries a relative
-rounding error eps*s/s_ij in ANY binary64 implementation (the oracle's own double-vs-long-double
-difference shows the same scaling), so such events are judged against 1e-14 * s/s_min and counted.
-The FP64 reference is the oracle run in long double.
+FP64 tolerance (tests/parity_rules.py, lines 388-390): the reference is the oracle in long
+double; an event is judged against max(1e-11, 10 x the oracle's own double-vs-long-double difference on that event), so
+only events on which ANY binary64 evaluation loses digits (tiny s_ij, no cuts) may exceed 1e-11, and each is counted.
+The same rule on ALL events of the five configs: tests/full_parity_report.py -> profiles/r2_parity_full.md.
 """
 import math
 
@@ -14,6 +13,8 @@ import numpy as np
 import pytest
 
 import inputs
+import parity_rules as pr
+from brute_force import explicit_colour_me_hel
 
 pytestmark = pytest.mark.gpu
 
@@ -48,27 +49,17 @@ def to_aos(mom, n, cfg):
     return inputs.aosoa_to_aos(mom.cpu().numpy(), n, cfg["npar"], 32)
 
 
-def smin_over_s(p):
-    npar = p.shape[1]
-    d = lambda a, b: a[:, 0] * b[:, 0] - (a[:, 1:] * b[:, 1:]).sum(1)
-    out = np.full(p.shape[0], np.inf)
-    for i in range(npar):
-        for j in range(i + 1, npar):
-            if (i, j) == (2, 3):
-                continue
-            out = np.minimum(out, np.abs(2 * d(p[:, i], p[:, j])))
-    return out / (SQRT_S ** 2)
-
-
-def check_fp64(out, ref_ld, p, label):
-    rel = np.abs(out / ref_ld - 1)
-    cond = smin_over_s(p)
-    tol = np.where(cond >= 1e-3, TOL64, np.maximum(TOL64, 1e-14 / cond))
-    nill = int((rel > TOL64).sum())
-    print("%s fp64: max rel %.2e, median %.2e, events above 1e-11 (ill-conditioned, s_min/s<1e-3): %d of %d"
-          % (label, rel.max(), np.median(rel), nill, rel.size))
-    assert (rel <= tol).all(), (label, rel.max(), cond[np.argmax(rel / tol)])
-    assert nill <= max(2, rel.size // 1000), "too many events above 1e-11"
+def check_fp64(out, ref_ld, ref_d, p, label):
+    """every event within max(1e-11, 10 x the oracle's own double-vs-long-double spread); the events above 1e-11 are few
+    (the oracle's own count sets the scale: ~1e-4 of a batch) and printed with their s_min/s"""
+    j = pr.judge_fp64(out, ref_ld, ref_d)
+    cond = pr.smin_over_s(p)
+    print("%s fp64: max rel %.2e, median %.2e, events above 1e-11: %d of %d (oracle double vs long double above 1e-11: %d)"
+          % (label, j["rel"].max(), np.median(j["rel"]), j["above"].size, out.size, j["oracle_above"].size))
+    for i in j["above"]:
+        print("   event %d: s_min/s %.1e, GPU %.2e, oracle spread %.2e" % (i, cond[i], j["rel"][i], j["spread"][i]))
+    assert j["failed"].size == 0, (label, [(int(i), j["rel"][i], j["spread"][i], cond[i]) for i in j["failed"][:5]])
+    assert j["above"].size <= max(2, 3 * j["oracle_above"].size, out.size // 2000), "too many events above 1e-11"
 
 
 # ---------------------------------------------------------------------------------- support kernels
@@ -120,7 +111,7 @@ def test_parity_small(me, orc, proc):
     assert ngood == bin(mask).count("1")
     ref_ld = orc.me(proc, p, long_double=True)
     out = ctx.me_compute(mom, n, me.ME_FP64).cpu().numpy()
-    check_fp64(out, ref_ld, p, cfg["name"])
+    check_fp64(out, ref_ld, ref, p, cfg["name"])
     for name in ("mixed", "fp32"):
         o = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
         rel = np.abs(o / ref_ld - 1)
@@ -244,36 +235,44 @@ def test_bad_parameters_rejected(me):
 
 
 # ---------------------------------------------------------------------------------- full BASELINE.json sizes
+# events compared with the ORACLE in this test (all precisions): everything for the two small processes, a leading block plus a
+# random sample for the others, sized so that the oracle (long double + double) takes about a minute in total on the GPU box.
+# The same comparison on ALL events of every config is tests/full_parity_report.py (~20 min), kept as profiles/r2_parity_full.md.
+FULL_ORACLE_EVENTS = {0: None, 1: None, 2: 98304, 3: 12288, 4: 384}
+
+
 @pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
-def test_full_size_sampled_parity_and_properties(me, orc, proc):
-    """The launch configuration bench.py times: whole config on the device; sampled events against the oracle,
-    any-size properties on all of them (finite, positive, closed-form cross sections for cfg 1 and 2)."""
+def test_full_size_parity_and_properties(me, orc, proc):
+    """The launch configuration bench.py times: the whole config on the device in every precision; every precision is compared
+    with the oracle (never with another GPU result) on the events of FULL_ORACLE_EVENTS; any-size properties hold on all of
+    them (finite, positive, closed-form cross sections for cfg 1 and 2)."""
     cfg = inputs.CONFIGS[proc]
     n = cfg["events"]
     ctx = me.MEContext(proc)
     _, mom, wt = gen_events(me, ctx, cfg, n)
     mask, _ = ctx.me_filter_helicities(mom, 32)
     assert mask == EXPECTED_MASK[proc]
-    nsample = 64 if proc == 4 else 384
-    idx = np.unique(np.concatenate([[0, 1, 31, 32, n - 2, n - 1], np.random.default_rng(proc).choice(n, nsample, replace=False)]))
-    p_all = to_aos(mom, n, cfg)
-    ref_ld = orc.me(proc, p_all[idx], long_double=True)
+    m = FULL_ORACLE_EVENTS[proc]
+    if m is None:
+        idx = np.arange(n)
+    else:       # first pages, last page, and a seeded random sample spread over every CTA wave
+        idx = np.unique(np.concatenate([np.arange(m // 2), np.arange(n - 32, n), np.random.default_rng(proc).choice(n, m // 2, replace=False)]))
+    p = to_aos(mom, n, cfg)[idx]
+    ref_ld = orc.me(proc, p, long_double=True)
+    ref_d = orc.me(proc, p)
     res = {}
     for name in cfg["precisions"]:
         out = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
         assert np.isfinite(out).all() and (out > 0).all()
         res[name] = out
         if name == "fp64":
-            check_fp64(out[idx], ref_ld, p_all[idx], cfg["name"] + " full-size sample")
+            check_fp64(out[idx], ref_ld, ref_d, p, cfg["name"] + " full size (%d events vs oracle)" % idx.size)
         else:
-            rel = np.abs(out[idx] / ref_ld - 1)
-            assert rel.max() <= TOL32
-            rel_all = np.abs(out / res["fp64"] - 1)
-            nbad = int((rel_all > TOL32).sum())
-            print("%s %s full size: max rel vs fp64 %.2e, events above 1e-4: %d of %d, batch-mean ratio-1 = %.2e"
-                  % (cfg["name"], name, rel_all.max(), nbad, n, out.mean() / res["fp64"].mean() - 1))
-            assert nbad <= n // 100000 + 1                      # never silently dropped: counted and bounded
-            assert abs(out.mean() / res["fp64"].mean() - 1) < 1e-5
+            j = pr.judge_fp32(out[idx], ref_ld)
+            print("%s %s full size: %d events vs oracle, max rel %.2e, above 1e-4: %d, batch-mean ratio-1 = %.2e"
+                  % (cfg["name"], name, idx.size, j["rel"].max(), j["above"].size, j["mean_ratio"]))
+            assert j["above"].size == 0, (name, j["rel"].max())
+            assert abs(j["mean_ratio"]) < 1e-5                  # PAPER.md line 81: cross sections agree to ~1e-5
     if proc in (0, 1):
         w = wt.cpu().numpy()
         x = w * res["fp64"] / (2 * SQRT_S ** 2)
@@ -309,17 +308,33 @@ def test_parity_pairing_option(me, orc, proc):
         assert np.array_equal(ctx.me_compute(mom, n).cpu().numpy(), full)
     p = to_aos(mom, n, cfg)
     ref_ld = orc.me(proc, p[:100], long_double=True)
-    check_fp64(ctx.me_compute(mom, n).cpu().numpy()[:100], ref_ld, p[:100], cfg["name"] + " parity-paired")
+    check_fp64(ctx.me_compute(mom, n).cpu().numpy()[:100], ref_ld, orc.me(proc, p[:100]), p[:100], cfg["name"] + " parity-paired")
     ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
     assert np.array_equal(ctx.me_compute(mom, n).cpu().numpy(), full)
     ctx.close()
 
 
 # ---------------------------------------------------------------------------------- helicity / colour selection
+def select_uniforms(orc, seed, event):
+    """the two uniforms of include/me.h me_select_helicity_color, re-derived from the oracle's raw Philox words"""
+    w = orc.philox4x32_10([event & 0xFFFFFFFF, event >> 32, 0x53454C45, 0], [seed & 0xFFFFFFFF, seed >> 32])
+    u53 = lambda a, b: ((a >> 5) * 67108864.0 + (b >> 6) + 0.5) / 9007199254740992.0
+    return u53(w[0], w[1]), u53(w[2], w[3])
+
+
+def boundary_distance(w, u, k1, k2):
+    """smallest |u * total - cum_k| / total over the CDF boundaries k that separate the choices k1 and k2"""
+    cum = np.cumsum(w)
+    lo, hi = min(k1, k2), max(k1, k2)
+    return float(np.abs(u * cum[-1] - cum[lo:hi]).min() / cum[-1])
+
+
+
 @pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
 def test_select_helicity_color_matches_oracle(me, orc, proc):
-    """integer outputs: bit-exact against the oracle's choice on the same events, seed and counters.  A mismatch is only
-    tolerated where the uniform falls within 1e-9 of a CDF boundary (the two FP64 evaluations of ME_h differ by ~1e-13)."""
+    """integer outputs: bit-exact against the oracle's choice on the same events, seed and counters.  A mismatch is accepted
+    only where it is PROVEN to sit on a CDF boundary: |u * total - cum_k| / total < 1e-9 for a boundary k between the two
+    choices (the two FP64 evaluations of ME_h / |J_s|^2 differ by ~1e-13); anything else fails."""
     import torch
     cfg = inputs.CONFIGS[proc]
     n = 90 if proc == 4 else 500
@@ -336,7 +351,16 @@ def test_select_helicity_color_matches_oracle(me, orc, proc):
     assert icol.min() >= 0 and icol.max() < ctx.info.ncolor
     bad = np.nonzero((ihel != rh) | (icol != rc))[0]
     print("%s: %d of %d selections differ from the oracle" % (cfg["name"], bad.size, n))
-    assert bad.size <= 1, bad
+    if bad.size:
+        _, mh = orc.me(proc, p[bad], per_helicity=True)
+        for row, e in enumerate(bad):
+            u1, u2 = select_uniforms(orc, 424242, first + int(e))
+            if ihel[e] != rh[e]:
+                w = np.where([(mask >> h) & 1 for h in range(mh.shape[1])], mh[row], 0.0)
+                assert boundary_distance(w, u1, int(ihel[e]), int(rh[e])) < 1e-9, ("helicity", int(e), int(ihel[e]), int(rh[e]))
+            else:
+                w = np.abs(orc.jamps(proc, p[e], int(rh[e]))) ** 2
+                assert boundary_distance(w, u2, int(icol[e]), int(rc[e])) < 1e-9, ("colour", int(e), int(icol[e]), int(rc[e]))
     # the draw really varies: more than one helicity is chosen over the batch
     assert len(set(ihel.tolist())) > 1
     # a second call with the same seed reproduces the draw bit for bit; another seed changes it
@@ -350,8 +374,9 @@ def test_select_helicity_color_matches_oracle(me, orc, proc):
 # ---------------------------------------------------------------------------------- cross section + unweighting
 @pytest.mark.parametrize("proc,n", [(0, 16384), (1, 50000), (3, 3001)])
 def test_unweight_matches_oracle(me, orc, proc, n):
-    """sums within rounding of the exactly rounded host sums; accept flags (bytes) equal the oracle's except where
-    u*wmax and w agree to 1e-9 (the oracle's w uses the oracle's ME, the GPU's the GPU's: they differ by ~1e-13)."""
+    """sums within rounding of the exactly rounded host sums; accept flags (bytes) equal the oracle's; a differing flag is
+    accepted only where |u * wmax - w| / wmax < 1e-9 is verified for that event (the oracle's w uses the oracle's ME, the
+    GPU's the GPU's: they differ by ~1e-13)."""
     cfg = inputs.CONFIGS[proc]
     ctx = me.MEContext(proc)
     rnd, mom, wt = gen_events(me, ctx, cfg, n)
@@ -365,7 +390,17 @@ def test_unweight_matches_oracle(me, orc, proc, n):
     ref_me = orc.me(proc, p)
     r1, r2, rmax, racc = orc.unweight(wt.cpu().numpy(), ref_me, flux, seed=31337, first_event=17)
     assert abs(s1 / r1 - 1) < 1e-11 and abs(s2 / r2 - 1) < 1e-11 and abs(wmax / rmax - 1) < 1e-11
-    assert (acc != racc).sum() <= 1
+    diff = np.nonzero(acc != racc)[0]
+    if diff.size:
+        u = np.zeros(n)
+        import ctypes
+        orc.lib().orc_tagged_uniform(ctypes.c_uint64(31337), ctypes.c_uint64(17), ctypes.c_long(n), ctypes.c_uint32(0x554E5754),
+                                     u.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+        w = flux * wt.cpu().numpy() * ref_me
+        for e in diff:
+            assert abs(u[e] * rmax - w[e]) / rmax < 1e-9, ("accept flag", int(e), u[e] * rmax, w[e])
+    # the count is produced without the flag buffer as well (include/me.h: d_accept nullable)
+    assert me.me_unweight(wt, me_dev, flux, seed=31337, first_event=17, want_accept=False)[4] == nacc
     # deterministic reductions: bit-identical on a second call
     t1, t2, tmax, acc2, _ = me.me_unweight(wt, me_dev, flux, seed=31337, first_event=17)
     assert (t1, t2, tmax) == (s1, s2, wmax) and np.array_equal(acc2.cpu().numpy().astype(bool), acc)
@@ -532,3 +567,101 @@ def test_host_buffer_entry_errors_and_empty_batch(me):
     got = ctx.me_compute_host(host, n, me.ME_FP64, out=out)
     assert got.data_ptr() == out.data_ptr() and torch.equal(got, ctx.me_compute(mom, n, me.ME_FP64).cpu())
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- GPU against a definition with no diagram list
+@pytest.mark.parametrize("proc,hels", [(1, range(16)), (2, range(32)), (3, (0, 5, 27, 38, 44, 63)), (4, (3, 77, 120))])
+def test_gpu_against_brute_force_explicit_colour(me, proc, hels):
+    """per-helicity |M_h|^2 of the CUDA path against tests/brute_force.py: a colour-dressed off-shell recursion with explicit
+    f^{abc}, T^a_{ij} and 4x4 gamma matrices, external states from their eigenvalue equations; no diagram enumeration and no
+    colour-flow basis, and the oracle (whose enumerator has the same structure as the generator's) is not involved at all."""
+    import torch
+    cfg = inputs.CONFIGS[proc]
+    n = proc + 1
+    ctx = me.MEContext(proc)
+    _, mom, _ = gen_events(me, ctx, cfg, 3, first_event=6000 + proc)
+    p = to_aos(mom, 3, cfg)
+    _, mh = ctx.me_compute_helicities(mom, 3)
+    mh = mh.cpu().numpy()                                       # [ncomb][3]
+    e = 1
+    scale = mh[:, e].max()
+    npar = cfg["npar"]
+    for ih in hels:
+        hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
+        ref = explicit_colour_me_hel(n, p[e], hel)
+        assert abs(mh[ih, e] - ref) < 1e-10 * max(ref, 1e-6 * scale), (proc, ih, mh[ih, e], ref)
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------- concurrency contract (include/me.h)
+def test_streams_and_contexts_sharing_the_gpu(me):
+    """PAPER.md line 65 / Fig. 1: several producers sharing one GPU.  (a) one context per stream, each stream its own slice of
+    the batch, all in flight together: bit-identical to the single-stream results (g g -> t t~ g g and the staged
+    g g -> t t~ g g g).  (b) ONE context called from several streams: the library orders the calls on the device (they share
+    the context's scratch), so the results are still bit-identical."""
+    import torch
+    for proc, nb, ns in ((3, 4096, 4), (4, 512, 3)):
+        cfg = inputs.CONFIGS[proc]
+        n = nb * ns
+        ctxs = [me.MEContext(proc) for _ in range(ns)]
+        _, mom, _ = gen_events(me, ctxs[0], cfg, n)
+        for c in ctxs:
+            c.me_set_helicities(EXPECTED_MASK[proc])
+        words = ctxs[0].momenta_numel(nb)
+        for prec in (me.ME_FP64, me.ME_FP32):
+            ref = ctxs[0].me_compute(mom, n, prec).cpu().numpy()
+            streams = [torch.cuda.Stream() for _ in range(ns)]
+            torch.cuda.synchronize()
+            for variant in ("contexts", "one context"):
+                outs = []
+                for rep in range(2):
+                    for k, st in enumerate(streams):
+                        c = ctxs[k] if variant == "contexts" else ctxs[0]
+                        outs.append(c.me_compute(mom[k * words:(k + 1) * words], nb, prec, stream=st))
+                torch.cuda.synchronize()
+                for i, o in enumerate(outs):
+                    k = i % ns
+                    assert np.array_equal(o.cpu().numpy(), ref[k * nb:(k + 1) * nb]), (proc, prec, variant, k)
+        for c in ctxs:
+            c.close()
+
+
+def test_filter_on_a_large_batch_and_mask_reuse(me, orc):
+    """the per-helicity fractions of me_filter_helicities are reduced on the device: same mask as the oracle's plain loops on
+    5000 filter events; a mask handed to a second context gives bit-identical MEs"""
+    for proc in (0, 1, 2):
+        cfg = inputs.CONFIGS[proc]
+        n = 5000
+        ctx = me.MEContext(proc)
+        _, mom, _ = gen_events(me, ctx, cfg, n)
+        mask, ngood = ctx.me_filter_helicities(mom, n)
+        _, ref_h = orc.me(proc, to_aos(mom, n, cfg), per_helicity=True)
+        assert mask == orc.helicity_mask(ref_h) == EXPECTED_MASK[proc]
+        c2 = me.MEContext(proc)
+        c2.me_set_helicities(mask)
+        assert np.array_equal(c2.me_compute(mom, n).cpu().numpy(), ctx.me_compute(mom, n).cpu().numpy())
+        ctx.close(); c2.close()
+
+
+def test_second_device_if_present(me):
+    """a context belongs to the device current at me_create (include/me.h "Devices"): a second GPU gets its own colour matrix
+    and scratch, and a call made while another device is current still runs on the context's device"""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    cfg = inputs.CONFIGS[4]
+    n = 96
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            ctx = me.MEContext(4)
+            rnd = me.me_philox_uniform(cfg["seed"], 0, n, cfg["nfinal"], device="cuda:%d" % dev)
+            mom, _ = ctx.me_rambo(SQRT_S, rnd)
+            ctx.me_set_helicities(EXPECTED_MASK[4])
+        with torch.cuda.device(0):                       # current device differs from the context's for dev = 1
+            s = torch.cuda.Stream(device=dev)
+            o = ctx.me_compute(mom, n, stream=s)
+            s.synchronize()
+            outs.append(o.cpu().numpy())
+        ctx.close()
+    assert np.array_equal(outs[0], outs[1]) and (outs[0] > 0).all()
