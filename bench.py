@@ -7,9 +7,14 @@ amplitudes, jamps, colour sum, helicity sum) over one batch of seeded synthetic 
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--quick]
 
-N > 1 is launched by torch.distributed.run (one rank per GPU); every rank takes its own page-aligned shard
-of N x 524288 events (weak scaling, no data-path collective).
+N > 1: one rank per GPU, every rank takes its own page-aligned shard of N x 524288 events (weak scaling, no data-path
+collective, SURVEY.md §8(e)).  Launched by torch.distributed.run (RANK / WORLD_SIZE in the environment) it is one of the ranks;
+started plainly as `python bench.py --gpus N` it re-executes itself under torch.distributed.run with N ranks on 127.0.0.1.
 `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+
+Numbers that come from a profile rather than from this run (DRAM traffic per launch, executed-flop counts by opcode) are read
+from the committed table profiles/r2_kernel_metrics.csv (written from ncu captures; the commands are in the .md beside it),
+keyed by kernel, workload and batch size, and are labelled with that source in the JSON line.
 """
 import argparse
 import json
@@ -78,6 +83,37 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def profile_metrics():
+    """rows of profiles/r2_kernel_metrics.csv: {(process name, precision, option, events): {column: float}}"""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r2_kernel_metrics.csv")
+    out = {}
+    if os.path.exists(path):
+        with open(path) as f:
+            for row in csv.DictReader(l for l in f if not l.startswith("#")):
+                key = (row["process"], row["precision"], row["option"], int(row["events"]))
+                out[key] = {k: float(v) for k, v in row.items() if k not in ("process", "precision", "option", "events", "kernel", "source") and v != ""}
+                out[key]["source"] = row["source"]; out[key]["kernel"] = row["kernel"]
+    return out
+
+
+def ncu_flops_per_event(m):
+    """executed flops per event from the ncu opcode counts of one launch: add + mul + 2 fma (thread-level, predicated-on), both
+    precisions added (the FP32 kernels form their propagator denominators in FP64), plus the tensor-core flops by instruction shape"""
+    return (m.get("dadd", 0) + m.get("dmul", 0) + 2 * m.get("dfma", 0) + m.get("fadd", 0) + m.get("fmul", 0) + 2 * m.get("ffma", 0)
+            + m.get("tensor_flops", 0)) / m["events_per_launch"]
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start N ranks on this node (127.0.0.1) and return their exit code"""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def oracle_rate(proc, p, target_seconds=15.0):
     """MEs/s of the oracle as it stands on all host cores, on a bounded sample of the events in p."""
     import oracle
@@ -133,8 +169,11 @@ def main():
     ap.add_argument("--config", type=int, default=HEADLINE, choices=[1, 2, 3, 4],
                     help="index into inputs.CONFIGS of the timed workload (default 3 = g g -> t t~ g g, the BASELINE.json metric; "
                          "others are for profiling a single process, e.g. --quick --config 4)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the short batch-size / shared-GPU sweep of the default run")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
     if args.impl == "reference":
         return run_reference(args)
 
@@ -210,48 +249,115 @@ def main():
     ctx, mom = setup(HL, n, first)
     info = ctx.info
     ngood = bin(ctx.me_filter_helicities(mom, 32)[0]).count("1")
-    flops_alg = info.flops_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
-    flops_exe = info.flops_executed_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
+    # algorithmic flops per event of the DEFAULT path: with current sharing (on by default where a sharing kernel exists, include/me.h
+    # ME_OPT_SHARE_CURRENTS) every current is counted once per distinct helicity assignment of its own legs (SURVEY.md line 493:
+    # "re-count algorithmic flops when enabled"); flops_unshared is the count with every current once per helicity
+    flops_unshared = info.flops_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
+    shared_default = info.flops_per_event_shared > 0 and ngood == info.ncomb
+    flops_alg = info.flops_per_event_shared if shared_default else flops_unshared
+    flops_exe = flops_alg if shared_default else info.flops_executed_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
     results = {}
+    prof = profile_metrics()
     with ClockSampler(local) as clk:
         total_ms, per = timed(ctx, mom, n, me.ME_FP64, args.steps, args.warmup)
     clocks = clk.summary()
     total_ms = allmax(total_ms)
     value = per_gpu * world * args.steps / (total_ms * 1e-3)
     ms_kernel = statistics.mean(per)
-    per_step_launches = info.nkernels * ((ngood + 31) // 32 if HL == 4 else 1)    # cfg 5: 3 diagram kernels + colour sum per 32-helicity chunk (ME_HEL_CHUNK)
+    per_step_launches = me.launches_per_pass(info, ngood)
     launches = args.steps * per_step_launches
     results[cfg["name"]] = {"fp64": {"MEs_per_s": n * args.steps / (sum(per) * 1e-3), "ms_per_step": ms_kernel}}
     # measured FMA-chain peaks (register-resident microkernel, same box, same run)
     peak_meas = {"fp64": me.me_fma_peak(1), "fp32": me.me_fma_peak(0)}
-    ach = flops_alg * n / (ms_kernel * 1e-3) * 1e-12
-    roofline = {"bound": "alu", "kernel": "k_%s<double,double,TM=true>" % cfg["name"] + (" (+ colour sum)" if HL == 4 else ""), "achieved": ach, "peak": PEAK_TFLOPS["fp64"], "unit": "TFLOP/s",
-                "frac": ach / PEAK_TFLOPS["fp64"],
-                # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel at the full config, from the committed
-                # ncu --set full capture (profiles/r1_ttxgg_fp64_tmem.md: 101.6 MB read + 5.5 MB written); algorithmic bytes = 200 B/event = 104.9 MB
-                "traffic": 107.1e6 if (HL == 3 and n == 524288) else None,
-                "traffic_source": "profiles/r1_ttxgg_fp64_tmem.md" if (HL == 3 and n == 524288) else None,
+
+    def roof(pname, ms, flops_per_event, option="-"):
+        """roofline numbers of one timed variant: algorithmic flops / CUDA-event time against the derived and the measured FMA peak;
+        where the committed ncu table has this (process, precision, option, n), also the executed flops by opcode and the DRAM traffic"""
+        pk = "fp32" if pname == "fp32" else "fp64"
+        ach = flops_per_event * n / (ms * 1e-3) * 1e-12
+        r = {"achieved": ach, "peak": PEAK_TFLOPS[pk], "frac": ach / PEAK_TFLOPS[pk], "peak_measured_fma_chain": peak_meas[pk],
+             "frac_of_measured": ach / peak_meas[pk], "flops_per_event_algorithmic": flops_per_event}
+        m = prof.get((cfg["name"], pname, option, n))
+        if m is not None:
+            fe = ncu_flops_per_event(m)
+            r.update({"flops_per_event_ncu": fe, "frac_ncu": fe * n / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
+                      "traffic": m.get("dram_bytes"), "traffic_algorithmic": m.get("algorithmic_bytes"), "profile_source": m["source"], "kernel": m["kernel"]})
+        return r
+
+    roofline = {"bound": "alu", "unit": "TFLOP/s", "kernel": "k_%s<double,double,TM=true,SH=%s>" % (cfg["name"], "true" if shared_default else "false") + (" (+ colour sum)" if HL == 4 else ""),
+                "flops_per_event_unshared_algorithm": flops_unshared,
+                "frac_counting_unshared_algorithm": flops_unshared * n / (ms_kernel * 1e-3) * 1e-12 / PEAK_TFLOPS["fp64"],
+                "traffic": None, "traffic_source": None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (B200_PROFILING.md clocks; no FP64 entry in MEASURED_PEAKS.json)",
-                "peak_measured_fma_chain": peak_meas["fp64"], "frac_of_measured": ach / peak_meas["fp64"],
-                "flops_per_event_algorithmic": flops_alg, "flops_per_event_executed": flops_exe,
-                "achieved_executed": flops_exe * n / (ms_kernel * 1e-3) * 1e-12}
+                "flops_per_event_executed": flops_exe, "achieved_executed": flops_exe * n / (ms_kernel * 1e-3) * 1e-12,
+                "frac_executed": flops_exe * n / (ms_kernel * 1e-3) * 1e-12 / PEAK_TFLOPS["fp64"]}
+    roofline.update(roof("fp64", ms_kernel, flops_alg, option="shared_currents" if shared_default else "-"))
+    if "profile_source" in roofline:        # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch at this batch size, from the committed ncu capture
+        roofline["traffic_source"] = roofline["profile_source"]
     # other precisions of the headline workload
     for pname in [q for q in ("mixed", "fp32") if q in cfg["precisions"]]:
         t, pp = timed(ctx, mom, n, me.PRECISIONS[pname], args.steps, args.warmup)
         launches += args.steps * per_step_launches
         ms = statistics.mean(pp)
         results[cfg["name"]][pname] = {"MEs_per_s": n / (ms * 1e-3), "ms_per_step": ms}
-    a32 = flops_alg * n / (results[cfg["name"]]["fp32"]["ms_per_step"] * 1e-3) * 1e-12
-    roofline["fp32"] = {"achieved": a32, "peak": PEAK_TFLOPS["fp32"], "frac": a32 / PEAK_TFLOPS["fp32"],
-                        "peak_measured_fma_chain": peak_meas["fp32"], "frac_of_measured": a32 / peak_meas["fp32"]}
-    # optional exact symmetry (include/me.h ME_OPT_PARITY_PAIRING): half the helicities, same number; NOT the headline
-    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
-    t, pp = timed(ctx, mom, n, me.ME_FP64, args.steps, args.warmup)
-    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
-    launches += args.steps * info.nkernels * ((ngood // 2 + 31) // 32 if HL == 4 else 1)
-    results[cfg["name"]]["fp64_parity_pairing"] = {"MEs_per_s": n / (statistics.mean(pp) * 1e-3), "ms_per_step": statistics.mean(pp)}
+        roofline[pname] = roof(pname, ms, flops_alg, option="shared_currents" if shared_default else "-")
+    # options of include/me.h that reduce the work exactly; reported beside the headline, NEVER as the headline
+    #   ME_OPT_PARITY_PAIRING: half the helicities, each counted twice;
+    #   ME_OPT_SHARE_CURRENTS: sub-tree currents re-evaluated only when their own helicities change (own algorithmic flop count)
+    def timed_option(key, opts, pname, flops_per_event, nhel_pass):
+        nonlocal launches
+        defaults = {me.ME_OPT_PARITY_PAIRING: 0, me.ME_OPT_SHARE_CURRENTS: 1}
+        for o, v in opts.items():
+            ctx.me_set_option(o, v)
+        t, pp = timed(ctx, mom, n, me.PRECISIONS[pname], args.steps, args.warmup)
+        for o in opts:
+            ctx.me_set_option(o, defaults[o])
+        launches += args.steps * me.launches_per_pass(info, nhel_pass)
+        ms = statistics.mean(pp)
+        results[cfg["name"]][key] = {"MEs_per_s": n / (ms * 1e-3), "ms_per_step": ms}
+        if flops_per_event:
+            results[cfg["name"]][key]["roofline"] = roof(pname, ms, flops_per_event, option="-")
+    timed_option("fp64_parity_pairing", {me.ME_OPT_PARITY_PAIRING: 1}, "fp64", None, ngood // 2)
+    if shared_default:          # the same workload with current sharing switched off: every current once per helicity
+        for pname in cfg["precisions"]:
+            timed_option("%s_unshared" % pname, {me.ME_OPT_SHARE_CURRENTS: 0}, pname, flops_unshared, ngood)
+    if world == 1 and not args.sweep and not args.no_sweep and HL == 3:
+        # short form of --sweep in every default run (PAPER.md line 65, Fig. 1; SURVEY.md section 8(f) item 1): throughput against batch
+        # size, and 1 / 2 / 4 / 8 producers sharing the GPU, each with its own context and stream and a batch of 8192 events
+        sw = {"batch": {}, "streams_x_8192": {}}
+        nb = 8192
+        while nb <= n:
+            t, pp = timed(ctx, mom, nb, me.ME_FP64, 3, 1)
+            launches += 4 * per_step_launches
+            sw["batch"][str(nb)] = nb / (min(pp) * 1e-3)
+            nb *= 4
+        ctxs = [ctx] + [me.MEContext(HL) for _ in range(7)]
+        for c in ctxs[1:]:
+            c.me_set_helicities(ctx.me_filter_helicities(mom, 32)[0])
+        words = ctx.momenta_numel(8192)
+        outs = [torch.empty(8192, dtype=torch.float64, device="cuda") for _ in range(8)]
+        sts = [torch.cuda.Stream() for _ in range(8)]
+        for ns in (1, 2, 4, 8):
+            best = 1e30
+            for rep in range(4):
+                torch.cuda.synchronize()
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for k in range(ns):
+                    sts[k].wait_event(e0)
+                    ctxs[k].me_compute(mom[k * words:(k + 1) * words], 8192, me.ME_FP64, out=outs[k], stream=sts[k])
+                for k in range(ns):
+                    torch.cuda.current_stream().wait_stream(sts[k])
+                e1.record(); e1.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+                launches += ns * per_step_launches
+            sw["streams_x_8192"][str(ns)] = ns * 8192 / (best * 1e-3)
+        for c in ctxs[1:]:
+            c.close()
+        results["sweep_fp64_MEs_per_s"] = sw
     if args.sweep and world == 1:
         sweep = {"batch": {}, "streams": {}}
+        sweep_ctxs = [ctx]
         nb = 8192
         while nb <= n:
             t, pp = timed(ctx, mom, nb, me.ME_FP64, 5, 2)
@@ -263,6 +369,8 @@ def main():
                 if ns * nb > n:
                     continue
                 streams = [torch.cuda.Stream() for _ in range(ns)]
+                while len(sweep_ctxs) < ns:            # one context per producer: calls on ONE context are ordered on the device (include/me.h)
+                    sweep_ctxs.append(me.MEContext(HL)); sweep_ctxs[-1].me_set_helicities(ctx.me_filter_helicities(mom, 32)[0])
                 ppages = ctx.momenta_numel(nb)
                 outs = [torch.empty(nb, dtype=torch.float64, device="cuda") for _ in range(ns)]
                 torch.cuda.synchronize()
@@ -272,7 +380,7 @@ def main():
                     e0.record()
                     for k, st in enumerate(streams):
                         st.wait_event(e0)
-                        ctx.me_compute(mom[k * ppages:(k + 1) * ppages], nb, me.ME_FP64, out=outs[k], stream=st)
+                        sweep_ctxs[k].me_compute(mom[k * ppages:(k + 1) * ppages], nb, me.ME_FP64, out=outs[k], stream=st)
                     for st in streams:
                         torch.cuda.current_stream().wait_stream(st)
                     e1.record(); e1.synchronize()
@@ -294,7 +402,7 @@ def main():
            "d2h_bytes_per_step": n * 8, "api": "C-ABI me_compute_host (pinned host momenta -> sliced H2D overlapped with the kernels -> pinned host MEs)"}
     # me_compute_host cuts the batch in slices of 6 x 128 events per SM, one me_compute (per_step_launches kernels) each
     host_slice = 6 * 128 * torch.cuda.get_device_properties(local).multi_processor_count
-    launches += args.steps * per_step_launches * ((n + host_slice - 1) // host_slice)
+    launches += (args.steps + 3) * per_step_launches * ((n + host_slice - 1) // host_slice)
     line = {
         "metric": "matrix elements/sec (%s, FP64)" % cfg["label"], "value": value, "unit": "MEs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -319,6 +427,7 @@ def main():
             cx, mm = setup(proc, c["events"], 0)
             ng = bin(cx.me_filter_helicities(mm, 32)[0]).count("1")
             fl = cx.info.flops_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
+            fx = cx.info.flops_executed_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
             results[c["name"]] = {}
             reps = 2 if proc == 4 else 5
             for pname in c["precisions"]:
@@ -326,7 +435,15 @@ def main():
                 ms = statistics.mean(pp)
                 pk = "fp32" if pname == "fp32" else "fp64"
                 results[c["name"]][pname] = {"MEs_per_s": c["events"] / (ms * 1e-3), "ms_per_step": ms,
-                                             "frac_of_%s_peak" % pk: fl * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk]}
+                                             "flops_per_event_algorithmic": fl, "flops_per_event_executed": fx,
+                                             "frac_of_%s_peak" % pk: fl * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
+                                             "frac_of_%s_peak_executed" % pk: fx * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk]}
+                m = prof.get((c["name"], pname, "-", c["events"]))
+                if m is not None:
+                    fe = ncu_flops_per_event(m)
+                    results[c["name"]][pname].update({"flops_per_event_ncu": fe, "frac_ncu": fe * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
+                                                      "traffic": m.get("dram_bytes"), "traffic_algorithmic": m.get("algorithmic_bytes"), "profile_source": m["source"]})
+                launches += (reps + 1) * me.launches_per_pass(cx.info, ng)
             cx.close(); del mm
     line["results"] = results
     if rank == 0:
@@ -336,4 +453,4 @@ def main():
 
 
 if __name__ == "__main__":
-    main()
+    sys.exit(main() or 0)

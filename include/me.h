@@ -116,14 +116,14 @@ me_status me_get_info(const me_ctx* ctx, me_info* out);
 me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
                                uint64_t mask_out[2], int* ngood_out, void* stream);
 
-/* Options (default 0 = off).
+/* Options.  ME_OPT_PARITY_PAIRING is off by default, ME_OPT_SHARE_CURRENTS is on by default.
  * ME_OPT_PARITY_PAIRING: for the pure-QCD processes |M_h|^2 = |M_{~h}|^2 where ~h flips
  * every helicity (parity invariance, tree level, real momenta), so me_compute evaluates one helicity of every good
  * pair and counts it twice: half the work, same number up to rounding (~1e-14).  Ignored for e+ e- -> mu+ mu- and
  * whenever the installed mask is not closed under h -> ~h.  me_compute_helicities is unaffected.
  * ME_OPT_SHARE_CURRENTS (second half: "sharing sub-tree currents across helicity
  * combinations"): a gluon sub-tree current depends only on the helicities of its own gluons, a one-gluon quark current on one
- * quark and one gluon helicity.  With the option on, g g -> t t~ g g runs a kernel that walks the good helicities in a
+ * quark and one gluon helicity.  With the option on (the default), g g -> t t~ g g runs a kernel that walks the good helicities in a
  * reflected Gray order (quark helicities fastest) and re-evaluates a current only when one of ITS helicities changed since the
  * previous step; three-gluon sub-trees are parked in an L2-resident scratch owned by the context.  Same diagrams, same
  * amplitudes, same number up to rounding order (~1e-15).  Ignored by the other processes.  me_info.flops_per_event_shared is

@@ -127,6 +127,15 @@ def me_fma_peak(fp64):
     return v.value
 
 
+def launches_per_pass(info, nhel):
+    """kernels one me_compute pass launches for `nhel` helicities: one for the single-kernel processes; for the staged process
+    (info.nkernels > 1: diagram kernels + colour sum per helicity chunk of 32, plus the memset that clears the staging buffer is not
+    a kernel of ours and is not counted)"""
+    if info.nkernels <= 1:
+        return 1
+    return info.nkernels * ((nhel + 31) // 32)
+
+
 class MEContext:
     """Owns one me_ctx (include/me.h).  Methods mirror the C entry points."""
 

@@ -24,6 +24,7 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
 NPAR = 6
+NSCVEC = 8          # current sharing: vectors parked per thread in the L2-resident scratch (two ordered currents per three-gluon sub-tree)
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 MERGE_ORDERED = True   # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
 MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: T.w - w.T)
@@ -36,6 +37,35 @@ UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_
 def lam_bit(label, npar=NPAR):
     p = label if label < 2 else label + 2
     return npar - 1 - p
+
+
+# ---- current sharing across helicities (include/me.h ME_OPT_SHARE_CURRENTS, second half).
+# The sharing kernel walks the helicities in a reflected Gray order whose fastest bits are the quark helicities, so that a current
+# made of gluons only survives as many steps as possible.  Position p of the Gray code (0 = flips every other step) -> helicity bit.
+T_BIT, TB_BIT = NPAR - 1 - 2, NPAR - 1 - 3
+GRAY_BITS = [T_BIT, TB_BIT, lam_bit(3), lam_bit(2), lam_bit(1), lam_bit(0)]      # t, t~, g3, g2, g1, g0 (g0 slowest: parity pairing keeps the first half)
+
+
+def gray_walk():
+    """the 64 helicity indices in walk order"""
+    out = []
+    for i in range(1 << NPAR):
+        g = i ^ (i >> 1)
+        out.append(sum(((g >> pos) & 1) << hb for pos, hb in enumerate(GRAY_BITS)))
+    return out
+
+
+def walk_count(mask, walk=None):
+    """steps of the walk (the first one included) on which a current that depends on the helicity bits `mask` is re-evaluated"""
+    walk = walk or gray_walk()
+    return 1 + sum(1 for a, b in zip(walk, walk[1:]) if (a ^ b) & mask)
+
+
+def dep_mask(gluons=(), t=False, tb=False):
+    m = 0
+    for l in gluons:
+        m |= 1 << lam_bit(l)
+    return m | (1 << T_BIT if t else 0) | (1 << TB_BIT if tb else 0)
 
 
 class SlotAlloc:
@@ -121,6 +151,8 @@ class Inst:
         self.zcount = 0
         self.tm0 = getattr(lay, "TM0", None)      # slots >= tm0 live in tensor memory in the FP64 kernels (None: no TMEM)
         self.inflight = []         # 4-vector loads issued, not yet converted (TMEM loads are asynchronous)
+        self.cond = []             # (helicity-bit mask, flops) of the parts the sharing kernel re-evaluates only when one of those helicities changed
+        self._cond_open = None
 
     tbname = "tb"          # name of the parameter-table row pointer in the emitted loop body
 
@@ -139,6 +171,20 @@ class Inst:
             self.lines.append("const W4<R> %s = xldw_get<R, TM>(%s_x);" % (name, name))
         self.inflight = []
         self.lines.append(s)
+
+    # ---- current sharing: the code between begin_cond / end_cond depends on the helicity bits `mask` only; the sharing
+    # instantiation (SH) skips it on the steps of the walk that leave them unchanged (the result it left behind is still valid)
+    def begin_cond(self, mask):
+        assert self._cond_open is None
+        self._cond_open = (mask, self.flops)
+        self.L("if (!SH || (chg & %s)) {" % self.P(mask))
+
+    def end_cond(self, close=True):
+        mask, f0 = self._cond_open
+        self._cond_open = None
+        self.cond.append((mask, self.flops - f0))
+        if close:
+            self.L("}")
 
     # ---- operand helpers
     def leaf(self, name, l):
@@ -327,6 +373,7 @@ def build_groups(stride):
         for it in instances[1:]:
             assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
             assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
+        tmpl.cond_all = [it.cond for it in instances]
         groups.append((name, tmpl, [it.params for it in instances]))
 
     labels = list(range(N))
@@ -338,19 +385,23 @@ def build_groups(stride):
     insts = []
     for (a, b) in lay.PAIR:
         I = Inst(lay, stride)
+        I.begin_cond(dep_mask([a, b]))
         I.leaf("ea", a); I.leaf("eb", b)
         I.kvec("ka", [a]); I.kvec("kb", [b])
         I.L("const W4<R> t = v3_current(ea, eb, ka, kb, %s);" % I.ik2(a, b)); I.flops += FL["v3_current"]
         I.stw(lay.PAIR[(a, b)], "t")
+        I.end_cond()
         insts.append(I)
     add_group("pairs", insts)
     # ---- A2: one-gluon row currents from the t end
     insts = []
     for l in labels:
         I = Inst(lay, stride)
+        I.begin_cond(dep_mask([l], t=True))
         I.leaf("el", l); I.qvec("q", [l])
         I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL["quark_step2"]
         I.stw(lay.Q1 + 8 * l, "t")
+        I.end_cond()
         insts.append(I)
     add_group("q1", insts)
     # ---- A3: one-gluon column currents from the t~ end: chi_w = (qslash+m)/(q^2-m^2) eps_w-slash v, q = p_t - K_{all but w}
@@ -358,61 +409,56 @@ def build_groups(stride):
     for w in labels:
         rest = [l for l in labels if l != w]
         I = Inst(lay, stride)
+        I.begin_cond(dep_mask([w], tb=True))
         I.leaf("ew", w); I.qvec("q", rest)
         I.L("const W4<R> t = col_step(slash_col(ew, vv), q, mt, %s);" % I.iq(*rest)); I.flops += FL["slash_col"] + FL["col_step"]
         I.stw(lay.CHI + 8 * w, "t")
+        I.end_cond()
         insts.append(I)
     add_group("chi1", insts)
-    # ---- B1: three-gluon sub-trees on {a,b,c} (6 terms) closing three ways with the remaining gluon w
+    # ---- B1: three-gluon sub-trees on {a,b,c} closing three ways with the remaining gluon w
     insts = []
-    for w in labels:
+    for vi, w in enumerate(labels):
         a, b, c = [l for l in labels if l != w]
         I = Inst(lay, stride)
-        I.leaf("ea", a); I.leaf("eb", b); I.leaf("ec", c); I.leaf("ew", w)
-        I.kvec("ka", [a]); I.kvec("kb", [b]); I.kvec("kc", [c]); I.kvec("kw", [w])
-        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc), kabc = padd(kab, kc);"); I.flops += 16
+        # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three channels,
+        # and the Jacobi identity col1 = col0 + col2 leaves two independent currents s0, s2 instead of six terms.  They depend
+        # on the helicities of a, b, c only: the sharing kernel parks them in its L2-resident scratch (vectors 2 vi, 2 vi + 1)
+        cols = [c_v3(cpair(a, b), c_leaf(c)), c_v3(cpair(a, c), c_leaf(b)), c_v3(cpair(b, c), c_leaf(a))] + \
+               [c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c)) for k in range(3)]
+        assert all(not _cdiff(cols[3 + k], cols[k], {}) for k in range(3)) and not _cdiff(cols[1], cols[0], _pscale(cols[2], -1))
+        I.L("W4<R> s0, s2;")
+        I.begin_cond(dep_mask([a, b, c]))
+        I.leaf("ea", a); I.leaf("eb", b); I.leaf("ec", c)
+        I.kvec("ka", [a]); I.kvec("kb", [b]); I.kvec("kc", [c])
+        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc);"); I.flops += 12
         I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pac", lay.PAIR[(a, c)]); I.ldw("pbc", lay.PAIR[(b, c)])
-        I.ldw("chiw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
-        # the last gluon w closes the sub-tree three ways: on the t~ end (colour T.w), on the t end (w.T), or through a
-        # three-gluon vertex on the bare line, whose colour is the commutator T.w - w.T.  MERGE_V3 folds the dual current dd of
-        # the third into the other two: two dot products and two jamp groups per term instead of three
-        I.L("const W4<R> dd = v3_dual(ew, jtt, kabc, kw, %s);" % I.ik2(a, b, c, w)); I.flops += FL["v3_dual"]
-        if MERGE_V3:
-            I.L("const W4<R> j1 = wadd(bilinear(ub, chiw), dd), j2 = wsub(bilinear(q1w, vv), dd);"); I.flops += 2 * FL["bilinear"] + 16
-        else:
-            I.L("const W4<R> j1 = bilinear(ub, chiw);"); I.L("const W4<R> j2 = bilinear(q1w, vv);"); I.flops += 2 * FL["bilinear"]
-        ik3 = I.ik2(a, b, c)
-        I.L("const R ik3 = %s;" % ik3)
-        terms = [("t0", "v3_current(pab, ec, kab, kc, ik3)", c_v3(cpair(a, b), c_leaf(c))),
-                 ("t1", "v3_current(pac, eb, kac, kb, ik3)", c_v3(cpair(a, c), c_leaf(b))),
-                 ("t2", "v3_current(pbc, ea, kbc, ka, ik3)", c_v3(cpair(b, c), c_leaf(a)))]
+        I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL["v4_dots"]
-        for k in range(3):
-            terms.append(("t%d" % (3 + k), "v4_current(%d, dots, ea, eb, ec)" % k, c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c))))
-        if MERGE_TRIPLE:
-            # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three
-            # channels, and the Jacobi identity col1 = col0 + col2 leaves two independent currents instead of six terms
-            cols = [t[2] for t in terms]
-            assert all(not _cdiff(cols[3 + k], cols[k], {}) for k in range(3)) and not _cdiff(cols[1], cols[0], _pscale(cols[2], -1))
-            I.L("const W4<R> t14 = wadd(%s, %s);" % (terms[1][1], terms[4][1]))
-            I.L("const W4<R> s0 = wadd(wadd(%s, %s), t14), s2 = wadd(wadd(%s, %s), t14);" % (terms[0][1], terms[3][1], terms[2][1], terms[5][1]))
-            I.flops += 3 * (FL["v3_current"] + FL["v4_current"]) + 5 * 8
-            I.namp += 4 * 3                              # diagram terms folded into the two ordered currents
-            terms = [("s0", None, cols[0]), ("s2", None, cols[2])]
-        for i, (nm, expr, col) in enumerate(terms):
-            if expr is None:
-                I.L("{")
-            else:
-                I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["v3_current"] if i < 3 else FL["v4_current"]
-            if MERGE_V3:
-                I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2);" % (nm, nm)); I.flops += 2 * FL["wdot"]
-                I.namp += 1                                                   # V3(t, eps_w) on the bare line is inside a1 and a2
-            else:
-                I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2), a3 = wdot(%s, dd);" % (nm, nm, nm)); I.flops += 3 * FL["wdot"]
+        I.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
+        I.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
+        I.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
+        I.flops += 3 * (FL["v3_current"] + FL["v4_current"]) + 5 * 8
+        I.namp += 4 * 3                              # diagram terms folded into the two ordered currents
+        vec = I.P(2 * vi)
+        I.L("if constexpr (SH) { sc_stw<R>(sc, %s, s0); sc_stw<R>(sc, %s + 1, s2); }" % (vec, vec))
+        I.end_cond(close=False)
+        I.L("} else {")
+        I.L("  s0 = sc_ldw<R>(sc, %s); s2 = sc_ldw<R>(sc, %s + 1);" % (vec, vec))
+        I.L("}")
+        # the last gluon w closes the sub-tree three ways: on the t~ end (colour T.w), on the t end (w.T), or through a
+        # three-gluon vertex on the bare line, whose colour is the commutator T.w - w.T: its dual current dd is folded into the
+        # other two, which leaves two dot products and two jamp groups per ordered current
+        I.leaf("ew", w); I.kvec("kabc", [a, b, c]); I.kvec("kw", [w])
+        I.ldw("chiw", lay.CHI + 8 * w); I.ldw("q1w", lay.Q1 + 8 * w)
+        I.L("const W4<R> dd = v3_dual(ew, jtt, kabc, kw, %s);" % I.ik2(a, b, c, w)); I.flops += FL["v3_dual"]
+        I.L("const W4<R> j1 = wadd(bilinear(ub, chiw), dd), j2 = wsub(bilinear(q1w, vv), dd);"); I.flops += 2 * FL["bilinear"] + 16
+        for nm, col in (("s0", cols[0]), ("s2", cols[2])):
+            I.L("{")
+            I.L("  const Cx<R> a1 = wdot(%s, j1), a2 = wdot(%s, j2);" % (nm, nm)); I.flops += 2 * FL["wdot"]
+            I.namp += 1                                                   # V3(t, eps_w) on the bare line is inside a1 and a2
             I.jamp("a1", c_close(ONE, col, cchi(w)), pidx)                    # ubar . t-slash . chi_w
             I.jamp("a2", c_close(cq1(w), col, ONE), pidx)                     # q1(w) . t-slash . v
-            if not MERGE_V3:
-                I.jamp("a3", c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)   # V3(t, eps_w) on the bare line
             I.flush_jamps()
             I.L("}")
         insts.append(I)
@@ -534,10 +580,13 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
             S("  {%s}," % ", ".join(str(v) for v in r))
         S("};")
     S("// TM: slots >= %d (gluon-pair currents, row currents, jamps) live in tensor memory, %d columns per CTA: two CTAs per SM in FP64" % (lay.TM0, lay.tm_cols))
-    S("template <typename R, typename RC, bool TM>")
+    S("// SH: current sharing across helicities (include/me.h ME_OPT_SHARE_CURRENTS): hels is in walk order (reflected Gray code, quark helicities")
+    S("// fastest); a current whose own helicities did not change since the previous step is not re-evaluated (pairs, one-gluon quark currents:")
+    S("// their slots still hold it; three-gluon sub-trees: reloaded from the L2-resident scratch `scratch`, %d vectors per thread)" % NSCVEC)
+    S("template <typename R, typename RC, bool TM, bool SH>")
     S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
       " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out,"
-      " const int* __restrict__ helpe) {" % (block, name))
+      " const int* __restrict__ helpe, void* __restrict__ scratch) {" % (block, name))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
@@ -577,9 +626,14 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    sbtb = spinor_basis(pcast<R>(pd3), mt);")
     fixed += 40
     S("  }")
+    S("  R* sc = nullptr;")
+    S("  if constexpr (SH) sc = reinterpret_cast<R*>(scratch) + ((size_t)blockIdx.x * (%d * 8 * ME_SM_STRIDE) + 2 * threadIdx.x);" % NSCVEC)
     S("  double acc = 0;")
+    S("  int hprev = -1;")
     S("  for (int ih = 0; ih < nhel; ++ih) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
+    S("    const int chg = (SH && hprev >= 0) ? (h ^ hprev) : %d;      // helicities that changed since the previous step" % ((1 << NPAR) - 1))
+    S("    hprev = h;")
     S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
     S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
@@ -638,27 +692,47 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.nslots, block, lay.TM0, block))
     S("  // FP64 amplitudes (double and mixed): tensor-memory kernel, two CTAs per SM; ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
-    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event")
+    S("  const bool sh = a.share != 0 && a.hel_per_event == nullptr && a.scratch != nullptr && !no_tmem;")
+    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event, a.scratch")
     S("#define ME_LAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
     S("    K<<<grid, %d, SMEM, a.stream>>>(ME_ARGS); } while (0)" % block)
-    S("  if (precision == 0) {")
-    S("    if (no_tmem) ME_LAUNCH((k_%s<double, double, false>), smd); else ME_LAUNCH((k_%s<double, double, true>), smt);" % (name, name))
+    S("  if (sh) {")
+    S("    if (precision == 0) ME_LAUNCH((k_%s<double, double, true, true>), smt);" % name)
+    S("    else if (precision == 1) ME_LAUNCH((k_%s<double, float, true, true>), smt);" % name)
+    S("    else ME_LAUNCH((k_%s<float, float, false, true>), smf);" % name)
+    S("  } else if (precision == 0) {")
+    S("    if (no_tmem) ME_LAUNCH((k_%s<double, double, false, false>), smd); else ME_LAUNCH((k_%s<double, double, true, false>), smt);" % (name, name))
     S("  } else if (precision == 1) {")
-    S("    if (no_tmem) ME_LAUNCH((k_%s<double, float, false>), smd); else ME_LAUNCH((k_%s<double, float, true>), smt);" % (name, name))
+    S("    if (no_tmem) ME_LAUNCH((k_%s<double, float, false, false>), smd); else ME_LAUNCH((k_%s<double, float, true, false>), smt);" % (name, name))
     S("  } else {")
-    S("    ME_LAUNCH((k_%s<float, float, false>), smf);" % name)
+    S("    ME_LAUNCH((k_%s<float, float, false, false>), smf);" % name)
     S("  }")
     S("#undef ME_LAUNCH")
     S("#undef ME_ARGS")
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr, false, nullptr, 0.0};"
+    # current sharing: scratch of one CTA = NSCVEC vectors x 8 reals x threads; rank of every helicity in the walk; algorithmic flops per event
+    walk = gray_walk()
+    rank = [walk.index(h) for h in range(1 << NPAR)]
+    S("static const unsigned char gray_rank_%s[%d] = {%s};" % (name, 1 << NPAR, ", ".join(str(r) for r in rank)))
+    S("static size_t scratch_%s(int precision, long npad, int share, int) {" % name)
+    S("  if (!share) return 0;")
+    S("  return (size_t)((npad + %d - 1) / %d) * %d * 8 * %d * (precision == 2 ? sizeof(float) : sizeof(double));" % (block, block, NSCVEC, block))
+    S("}")
+    nh = 1 << NPAR
+    shared = 0
+    for _, t, rows in groups:
+        for conds in t.cond_all:
+            always = t.flops - sum(f for _, f in conds)
+            shared += always * nh + sum(f * walk_count(m, walk) for m, f in conds)
+    shared_event = shared + nh * (cs_flops + 2 * FL["spinor"] + FL["bilinear"]) + fixed
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, false, gray_rank_%s, %r};"
       % (name, N, 123, namp, ncol, color_denom, float(per_hel), float(per_hel), float(per_hel),
-         float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name))
+         float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name, name, name, float(shared_event)))
     S("}  // namespace me")
     info = dict(n=N, ndiagrams=123, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=per_hel,
-                flops_executed_per_helicity=per_hel, fixed_flops=fixed, colour_flops=cs_flops, smem_slots=lay.nslots, tm_slot0=lay.TM0, tm_cols=lay.tm_cols, block=block,
+                flops_executed_per_helicity=per_hel, fixed_flops=fixed, flops_shared_event=shared_event, gray_walk=walk, colour_flops=cs_flops, smem_slots=lay.nslots, tm_slot0=lay.TM0, tm_cols=lay.tm_cols, block=block,
                 shapes={g: len(r) for g, _, r in groups}, color_num=color_num)
     return "\n".join(src) + "\n", info

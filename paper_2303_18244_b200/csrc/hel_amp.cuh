@@ -537,6 +537,25 @@ template <typename R, bool TM> ME_DEV void xstsb(R* sm, uint32_t tm, int off, co
   if constexpr (TM) xstw<R, TM>(sm, tm, off, W4<R>{g.a, g.b, g.c, g.wp, g.wm, (R)0, (R)0, (R)0});
   else stsb<R>(sm + off, g);
 }
+// ------------------------------------------------------------------------------------
+// Current sharing across helicities (ME_OPT_SHARE_CURRENTS): a three-gluon sub-tree current depends on three gluon helicities
+// only; the kernel parks it in a global scratch that stays resident in the 126 MB L2 (64 FP64 slots per thread do not fit on
+// chip next to the rest) and reloads it on the steps of the helicity walk that leave those three helicities unchanged.
+// Layout per CTA: [8-slot vector][4 pairs][ME_SM_STRIDE threads] of R2 (one coalesced 16-byte access per thread and pair, the
+// vector index is an immediate offset); ld / st .cg: L2 only.
+// ------------------------------------------------------------------------------------
+template <typename R> ME_DEV void sc_stw(R* sc, int vec, const W4<R>& w) {
+  typedef typename Pair2<R>::T R2;
+  R2* q = reinterpret_cast<R2*>(sc) + vec * 4 * ME_SM_STRIDE;
+  R2 a, b, c, d; a.x = w.r0; a.y = w.i0; b.x = w.r1; b.y = w.i1; c.x = w.r2; c.y = w.i2; d.x = w.r3; d.y = w.i3;
+  __stcg(q, a); __stcg(q + ME_SM_STRIDE, b); __stcg(q + 2 * ME_SM_STRIDE, c); __stcg(q + 3 * ME_SM_STRIDE, d);
+}
+template <typename R> ME_DEV W4<R> sc_ldw(const R* sc, int vec) {
+  typedef typename Pair2<R>::T R2;
+  const R2* q = reinterpret_cast<const R2*>(sc) + vec * 4 * ME_SM_STRIDE;
+  const R2 a = __ldcg(q), b = __ldcg(q + ME_SM_STRIDE), c = __ldcg(q + 2 * ME_SM_STRIDE), d = __ldcg(q + 3 * ME_SM_STRIDE);
+  return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+}
 // all earlier tcgen05.st of this thread are complete (needed before a tcgen05.ld that may read what they wrote)
 template <bool TM> ME_DEV void xwait_st() {
   if constexpr (TM) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");

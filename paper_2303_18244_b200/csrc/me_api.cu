@@ -96,6 +96,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
   me_ctx* c = new (std::nothrow) me_ctx();      // value-initialised: every pointer null, every flag false
   if (c == nullptr) return ME_ENOMEM;
   c->process = process; c->prm = *prm;
+  c->share = true;               // ME_OPT_SHARE_CURRENTS is on by default (exact, faster); it only acts where a sharing kernel exists
   me_info& I = c->info; memset(&I, 0, sizeof(I));
   I.page = ME_PAGE; I.ninitial = 2;
   const double PI = 3.14159265358979323846;
@@ -210,7 +211,7 @@ static me_status mark_ran(me_ctx* c, cudaStream_t st) {
 // hels_gray != null selects the kernel that shares sub-tree currents across helicities (it walks the list in that order)
 static me_status run(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, const unsigned char* hels, int nhel, double inv_avg,
                      double* d_me, double* d_me_hel, double* d_jamp, void* stream, const int* hel_per_event = nullptr, bool share = false,
-                     bool ordered = true) {
+                     bool ordered = true, size_t scratch_offset = 0, size_t scratch_total = 0) {
   if ((int)prec < 0 || (int)prec > 2) return ME_EINVAL;
   if (((uintptr_t)d_mom & 15) || ((uintptr_t)d_me & 7) || ((uintptr_t)d_me_hel & 7)) return ME_EALIGN;
   me::LaunchArgs a;
@@ -222,11 +223,13 @@ static me_status run(me_ctx* c, const double* d_mom, int64_t n, me_precision pre
   me_status ms = ordered ? order_after_previous(c, a.stream) : ME_OK;
   if (ms != ME_OK) return ms;
   if (c->tab != nullptr && c->tab->scratch_bytes != nullptr) {
+    // (me_compute_host runs alternate slices on two streams: it sizes a scratch of two slots and hands each slice its own)
     const size_t need = c->tab->scratch_bytes((int)prec, a.npad, a.share, c->nsm);
     if (need > 0) {
-      ms = ensure_buffer(&c->scratch, &c->scratch_bytes, need, c->ran ? c->last_stream : a.stream, "scratch alloc");
+      if (scratch_offset + need > (scratch_total > 0 ? scratch_total : need)) return ME_EINVAL;
+      ms = ensure_buffer(&c->scratch, &c->scratch_bytes, scratch_total > 0 ? scratch_total : need, c->ran ? c->last_stream : a.stream, "scratch alloc");
       if (ms != ME_OK) return ms;
-      a.scratch = c->scratch; a.scratch_bytes = c->scratch_bytes;
+      a.scratch = (char*)c->scratch + scratch_offset; a.scratch_bytes = need;
     }
   }
   cudaError_t e = c->tab != nullptr ? c->tab->launch((int)prec, a) : me::launch_epem((int)prec, a, c->epem);
@@ -373,7 +376,12 @@ extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, 
   const int64_t unit = (int64_t)c->nsm * ME_BLOCK * 6, slice = (slice_units > 0 ? slice_units : 1) * unit;
   const unsigned char* hels; int nhel; double inv_avg; bool share;
   hel_list(c, &hels, &nhel, &inv_avg, &share);
-  const bool one_stream = c->tab != nullptr && c->tab->scratch_bytes != nullptr && c->tab->scratch_bytes((int)prec, slice, share, c->nsm) > 0;
+  // the staged process (scratch used by several kernels in sequence) keeps its slices on one stream; the sharing kernel only
+  // needs a private scratch per slice in flight: two slots
+  const bool one_stream = c->tab != nullptr && c->tab->scratch_bytes != nullptr && c->tab->scratch_bytes((int)prec, slice, 0, c->nsm) > 0;
+  size_t slot_bytes = 0;
+  if (!one_stream && c->tab != nullptr && c->tab->scratch_bytes != nullptr)      // one slot = what a full slice needs
+    slot_bytes = (c->tab->scratch_bytes((int)prec, slice, share, c->nsm) + 255) / 256 * 256;
   const size_t ev_words = (size_t)c->info.npar * 4;            // doubles per event
   if (c->h_slice < (size_t)slice) {
     ME_CUDA(cudaStreamSynchronize(c->s_h2d), "host sync"); ME_CUDA(cudaStreamSynchronize(c->s_d2h), "host sync");
@@ -411,7 +419,7 @@ extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, 
     HOST_TRY(cudaStreamWaitEvent(cs, c->ev_h2d[b], 0), "host wait");
     if (k >= 2) HOST_TRY(cudaStreamWaitEvent(cs, c->ev_d2h[b], 0), "host wait");             // the MEs of slice k - 2 have left
     if (e == cudaSuccess && ms == ME_OK)          // the slices are ordered by the events of this function (ordered = false)
-      ms = run(c, c->h_mom[b], m, prec, hels, nhel, inv_avg, c->h_me[b], nullptr, nullptr, (void*)cs, nullptr, share, false);
+      ms = run(c, c->h_mom[b], m, prec, hels, nhel, inv_avg, c->h_me[b], nullptr, nullptr, (void*)cs, nullptr, share, false, b * slot_bytes, 2 * slot_bytes);
     HOST_TRY(cudaEventRecord(c->ev_comp[b], cs), "host compute");
     HOST_TRY(cudaStreamWaitEvent(c->s_d2h, c->ev_comp[b], 0), "host wait");
     HOST_TRY(cudaMemcpyAsync(h_me + first, c->h_me[b], sizeof(double) * m, cudaMemcpyDeviceToHost, c->s_d2h), "host d2h");

@@ -141,6 +141,26 @@ def test_flops_tables_match_the_device_routines(tmp_path):
     assert counted["gluon_basis"] <= 22 and counted["spinor_basis"] <= 20      # `fixed` charges 22 per gluon basis, 40 for two spinor bases
 
 
+def test_helicity_walk_of_the_sharing_kernel():
+    """ME_OPT_SHARE_CURRENTS: the walk is a permutation of the 64 helicities in which consecutive steps differ in exactly one
+    helicity, the quark helicities flip most often, particle 0 last (parity pairing keeps the first half); the re-evaluation
+    counts that enter flops_per_event_shared follow from it"""
+    from paper_2303_18244_b200.codegen import emit_orbit as eo
+    walk = eo.gray_walk()
+    assert sorted(walk) == list(range(64))
+    flips = [a ^ b for a, b in zip(walk, walk[1:])]
+    assert all(bin(f).count("1") == 1 for f in flips)
+    count = {b: sum(1 for f in flips if f == 1 << b) for b in range(6)}
+    assert count[eo.T_BIT] == 32 and count[eo.TB_BIT] == 16 and count[5] == 1          # t fastest, then t~; gluon 0 (bit 5) slowest
+    assert all(not (h >> 5) & 1 for h in walk[:32])
+    # a gluon pair is re-evaluated 1 + flips(a) + flips(b) times, a current of all four gluons 16 times
+    assert eo.walk_count(eo.dep_mask([0, 1])) == 1 + count[5] + count[4]
+    assert eo.walk_count(eo.dep_mask([0, 1, 2, 3])) == 16
+    assert eo.walk_count(eo.dep_mask([2], t=True)) == 1 + 32 + count[eo.lam_bit(2)]
+    src, info = eo.emit_orbit_process()
+    assert 0.6 * 64 * info["flops_per_helicity"] < info["flops_shared_event"] < 0.85 * 64 * info["flops_per_helicity"]
+
+
 # ------------------------------------------------------------------ host logic
 def test_aosoa_roundtrip_and_padding():
     import inputs

@@ -59,7 +59,9 @@ def check_fp64(out, ref_ld, ref_d, p, label):
     for i in j["above"]:
         print("   event %d: s_min/s %.1e, GPU %.2e, oracle spread %.2e" % (i, cond[i], j["rel"][i], j["spread"][i]))
     assert j["failed"].size == 0, (label, [(int(i), j["rel"][i], j["spread"][i], cond[i]) for i in j["failed"][:5]])
-    assert j["above"].size <= max(2, 3 * j["oracle_above"].size, out.size // 2000), "too many events above 1e-11"
+    # with the propagator denominators formed exactly (csrc/hel_amp.cuh) the CUDA path is at least as well conditioned as the
+    # oracle's own double evaluation: never more events above 1e-11 than the oracle shows against its long double
+    assert j["above"].size <= j["oracle_above"].size, "more events above 1e-11 than the oracle's own double evaluation"
 
 
 # ---------------------------------------------------------------------------------- support kernels
@@ -665,3 +667,60 @@ def test_second_device_if_present(me):
             outs.append(o.cpu().numpy())
         ctx.close()
     assert np.array_equal(outs[0], outs[1]) and (outs[0] > 0).all()
+
+
+# ---------------------------------------------------------------------------------- option: current sharing (second half)
+def test_share_currents_option(me, orc):
+    """ME_OPT_SHARE_CURRENTS: g g -> t t~ g g walks the helicities in Gray order and re-evaluates a sub-tree current only when
+    one of its own helicities changed.  Same diagrams and amplitudes: the result must match the oracle under the FP64 rule and
+    the plain kernel to rounding, in every precision, for ragged sizes, with parity pairing, for an arbitrary helicity mask
+    (steps of the walk that change several bits) and through the host-buffer entry; the other processes ignore the option."""
+    import torch
+    cfg = inputs.CONFIGS[3]
+    n = 1000
+    ctx = me.MEContext(3)
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    p = to_aos(mom, n, cfg)
+    ctx.me_filter_helicities(mom, 32)
+    assert 0 < ctx.info.flops_per_event_shared < 64 * ctx.info.flops_per_helicity[0]
+    ctx.me_set_option(me.ME_OPT_SHARE_CURRENTS, 0)                  # the option is on by default
+    plain = {name: ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy() for name in ("fp64", "mixed", "fp32")}
+    ctx.me_set_option(me.ME_OPT_SHARE_CURRENTS, 1)
+    ref_ld, ref_d = orc.me(3, p, long_double=True), orc.me(3, p)
+    shared = ctx.me_compute(mom, n).cpu().numpy()
+    check_fp64(shared, ref_ld, ref_d, p, "gg_ttxgg shared currents")
+    for name, tol in (("fp64", 1e-12), ("mixed", 5e-6), ("fp32", 1e-4)):
+        out = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
+        assert np.abs(out / plain[name] - 1).max() < tol, name
+        assert np.abs(out / ref_ld - 1).max() < (1e-11 if name == "fp64" else 1e-4) or name == "fp64"
+        assert np.array_equal(ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy(), out)          # deterministic
+        for m in (1, 31, 129, 517):                                                                      # ragged sizes: prefix bit for bit
+            assert np.array_equal(ctx.me_compute(mom, m, me.PRECISIONS[name]).cpu().numpy(), out[:m]), (name, m)
+    # host-buffer entry with the option on
+    host = mom.cpu().pin_memory()
+    assert np.array_equal(ctx.me_compute_host(host, n).numpy(), shared)
+    # both options together
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 1)
+    both = ctx.me_compute(mom, n).cpu().numpy()
+    assert np.abs(both / plain["fp64"] - 1).max() < 1e-12
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
+    # an arbitrary mask: consecutive walk steps then differ in several helicities
+    mask = 0x5A3C96E178D2B40F & ((1 << 64) - 1)
+    ctx.me_set_helicities(mask)
+    got = ctx.me_compute(mom, n).cpu().numpy()
+    ctx.me_set_option(me.ME_OPT_SHARE_CURRENTS, 0)
+    want = ctx.me_compute(mom, n).cpu().numpy()
+    assert np.abs(got / want - 1).max() < 1e-12
+    _, ref_h = orc.me(3, p[:64], per_helicity=True)
+    sel = np.array([(mask >> h) & 1 for h in range(64)], dtype=bool)
+    assert np.abs(got[:64] / (ref_h[:, sel].sum(1) / 512) - 1).max() < 1e-10
+    ctx.close()
+    # ignored elsewhere
+    for proc in (0, 2, 4):
+        c = me.MEContext(proc)
+        _, mm, _ = gen_events(me, c, inputs.CONFIGS[proc], 64)
+        c.me_set_helicities(EXPECTED_MASK[proc])
+        a = c.me_compute(mm, 64).cpu().numpy()
+        c.me_set_option(me.ME_OPT_SHARE_CURRENTS, 0)
+        assert np.array_equal(c.me_compute(mm, 64).cpu().numpy(), a)
+        c.close()
