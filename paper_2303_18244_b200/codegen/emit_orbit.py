@@ -24,13 +24,15 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
 NPAR = 6
-NSCVEC = 8          # current sharing: vectors parked per thread in the L2-resident scratch (two ordered currents per three-gluon sub-tree)
+NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
+NSCVEC = 14         # and the six colour-ordered four-gluon currents that close on the bare quark line
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 MERGE_ORDERED = True   # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
 MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: T.w - w.T)
 MERGE_TRIPLE = True   # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
 UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
+UNROLL_SH = dict(pairs=1, q1=1, chi1=1)      # FP64 sharing kernel (as loops the FP32 kernel is 17 % slower: table loads in front of its cheaper arithmetic)
 UNROLL32 = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=2, q1_pair_chi=12, pair_pair=3, pair_v4=6)    # FP32 (8 warps/SM, registers to spare)
 
 
@@ -368,8 +370,10 @@ def build_groups(stride):
     pidx = {p: i for i, p in enumerate(perms)}
     groups = []      # (name, template Inst, [param rows])
 
-    def add_group(name, instances):
+    def add_group(name, instances, mode="both"):
+        """mode: 'both' | 'plain' (kernel instantiations without current sharing) | 'sh' (sharing instantiations only)"""
         tmpl = instances[0]
+        tmpl.mode = mode
         for it in instances[1:]:
             assert it.lines == tmpl.lines, "instances of %s differ in shape" % name
             assert it.jamp_codes == tmpl.jamp_codes, "instances of %s differ in colour coefficients" % name
@@ -532,7 +536,7 @@ def build_groups(stride):
         I.jamp("a1", c_close(ONE, c_v3(cpair(a, b), cpair(c, d)), ONE), pidx)
         I.flush_jamps()
         insts.append(I)
-    add_group("pair_pair", insts)
+    add_group("pair_pair", insts, mode="plain")
     # ---- B5: four-gluon vertex (pair, eps_c, eps_d) on the bare line, three colour structures
     insts = []
     for (a, b) in lay.PAIR:
@@ -545,7 +549,73 @@ def build_groups(stride):
             I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(a, b), c_leaf(c), c_leaf(d)), ONE), pidx)
         I.flush_jamps()
         insts.append(I)
-    add_group("pair_v4", insts)
+    add_group("pair_v4", insts, mode="plain")
+    # ---- B4 + B5 of the sharing kernel: the 21 four-gluon currents that close on the bare line (V3(pair, pair'), V4(pair, eps, eps)) depend
+    # on the gluon helicities only, and their colour factors are multilinear Lie polynomials in the four generators, a six-dimensional
+    # space with basis D_pi = [[[T0, T_pi1], T_pi2], T_pi3] (the coefficient of D_pi is the coefficient of the string 0 pi1 pi2 pi3).  So
+    #     sum_T c_T (V_T . jtt) = sum_pi D_pi (U_pi . jtt),   U_pi = sum_T alpha_pi(T) V_T :
+    # six colour-ordered currents per gluon-helicity assignment (re-evaluated 16 times per event, parked in the L2-resident scratch)
+    # and six dot products with ubar gamma v per helicity
+    I = Inst(lay, stride)
+    pis = list(permutations((1, 2, 3)))
+    basis = [_pcomm(_pcomm(_pcomm(c_leaf(0), c_leaf(q[0])), c_leaf(q[1])), c_leaf(q[2])) for q in pis]
+    terms = []            # (emit function -> expression of V_T, colour polynomial X_T)
+    I.begin_cond(dep_mask([0, 1, 2, 3]))
+    I.L("W4<R> " + ", ".join("U%d" % k for k in range(6)) + ";")
+    started = [False] * 6
+
+    def accumulate(expr, X):
+        alpha = [X.get((0,) + q, 0) for q in pis]
+        chk = {}
+        for al, D in zip(alpha, basis):
+            for st, v in D.items():
+                chk[st] = chk.get(st, 0) + al * v
+        assert not _cdiff(X, chk, {}), "colour factor outside the span of the left-normed brackets"
+        I.L("{ const W4<R> V = %s;" % expr)
+        for k, al in enumerate(alpha):
+            if al == 0:
+                continue
+            assert al in (1, -1), al
+            if not started[k]:
+                I.L("  U%d = %s;" % (k, "V" if al > 0 else "wsub(W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0}, V)"))
+                started[k] = True
+                I.flops += 0 if al > 0 else 8
+            else:
+                I.L("  U%d = %s(U%d, V);" % (k, "wadd" if al > 0 else "wsub", k)); I.flops += 8
+        I.L("}")
+
+    ik4 = I.ik2(0, 1, 2, 3)
+    I.L("const R ik4 = %s;" % ik4)
+    for (a, b), (c, d) in (((0, 1), (2, 3)), ((0, 2), (1, 3)), ((0, 3), (1, 2))):
+        I.L("{")
+        I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pcd", lay.PAIR[(c, d)])
+        I.kvec("kab", [a, b]); I.kvec("kcd", [c, d])
+        I.flops += FL["v3_current"]
+        accumulate("v3_current(pab, pcd, kab, kcd, ik4)", c_v3(cpair(a, b), cpair(c, d)))
+        I.namp += 1
+        I.L("}")
+    for (a, b) in lay.PAIR:
+        c, d = [l for l in labels if l not in (a, b)]
+        I.L("{")
+        I.ldw("pab", lay.PAIR[(a, b)]); I.leaf("ec", c); I.leaf("ed", d)
+        I.L("const V4Dots<R> dots = v4_dots(pab, ec, ed, ik4);"); I.flops += FL["v4_dots"]
+        for k in range(3):
+            I.flops += FL["v4_current"]
+            accumulate("v4_current(%d, dots, pab, ec, ed)" % k, c_v4(k, cpair(a, b), c_leaf(c), c_leaf(d)))
+            I.namp += 1
+        I.L("}")
+    assert all(started)
+    for k in range(6):
+        I.L("sc_stw<R>(sc, %d, U%d);" % (NSCVEC_TRIPLES + k, k))
+    I.end_cond()
+    for k in range(6):
+        I.L("const W4<R> u%d = sc_ldw<R>(sc, %d);" % (k, NSCVEC_TRIPLES + k))
+    I.L("const Cx<R> " + ", ".join("q%d = wdot(u%d, jtt)" % (k, k) for k in range(6)) + ";"); I.flops += 6 * FL["wdot"]
+    for k in range(6):
+        I.jamp("q%d" % k, c_close(ONE, basis[k], ONE), pidx)
+    I.namp -= 6                       # the six ordered amplitudes are sums of the 21 diagram terms counted above
+    I.flush_jamps()
+    add_group("quad_bare", [I], mode="sh")
     return lay, perms, groups
 
 
@@ -555,8 +625,9 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     cs_lines, cs_flops = colour_sum_lines(color_num, ncol, color_denom)
-    namp = sum(t.namp * len(rows) for _, t, rows in groups)
-    flops = sum(t.flops * len(rows) for _, t, rows in groups)
+    namp = sum(t.namp * len(rows) for _, t, rows in groups if t.mode != "sh")
+    assert namp == sum(t.namp * len(rows) for _, t, rows in groups if t.mode != "plain")       # both instantiations cover the same diagram terms
+    flops = sum(t.flops * len(rows) for _, t, rows in groups if t.mode != "sh")
     per_hel = flops + cs_flops + 2 * FL["spinor"] + FL["bilinear"]
     sgn = lambda l: 1 if l < 2 else -1
     part = lambda l: l if l < 2 else l + 2
@@ -647,12 +718,19 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    }")
     for gname, tmpl, rows in groups:
         S("    // ---- %s: %d instances" % (gname, len(rows)))
-        S("#pragma unroll(sizeof(R) == 8 ? %d : %d)" % (UNROLL.get(gname, 1), UNROLL32.get(gname, 1)))
+        if tmpl.mode != "both":
+            S("    if constexpr (%sSH) {" % ("" if tmpl.mode == "sh" else "!"))
+        if gname in UNROLL_SH:      # executed on few steps of the walk in the sharing kernel: a compact loop costs nothing there and keeps the body small
+            S("#pragma unroll(sizeof(R) == 8 ? (SH ? %d : %d) : %d)" % (UNROLL_SH[gname], UNROLL.get(gname, 1), UNROLL32.get(gname, 1)))
+        else:
+            S("#pragma unroll(sizeof(R) == 8 ? %d : %d)" % (UNROLL.get(gname, 1), UNROLL32.get(gname, 1)))
         S("    for (int it = 0; it < %d; ++it) {" % len(rows))
         S("      const int* tb = tab_%s_%s[it];" % (name, gname))
         for l in tmpl.lines:
             S("      " + l)
         S("    }")
+        if tmpl.mode != "both":
+            S("    }")
     S("    RC cr[%d], ci[%d];" % (ncol, ncol))
     S("    if constexpr (TM) {")
     S("      XW<R, TM> jx[%d];" % (ncol // 4))
@@ -724,6 +802,8 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     nh = 1 << NPAR
     shared = 0
     for _, t, rows in groups:
+        if t.mode == "plain":
+            continue
         for conds in t.cond_all:
             always = t.flops - sum(f for _, f in conds)
             shared += always * nh + sum(f * walk_count(m, walk) for m, f in conds)
@@ -734,5 +814,5 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("}  // namespace me")
     info = dict(n=N, ndiagrams=123, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=per_hel,
                 flops_executed_per_helicity=per_hel, fixed_flops=fixed, flops_shared_event=shared_event, gray_walk=walk, colour_flops=cs_flops, smem_slots=lay.nslots, tm_slot0=lay.TM0, tm_cols=lay.tm_cols, block=block,
-                shapes={g: len(r) for g, _, r in groups}, color_num=color_num)
+                shapes={g: len(r) for g, t, r in groups if t.mode != "sh"}, color_num=color_num)
     return "\n".join(src) + "\n", info
