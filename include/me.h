@@ -93,6 +93,7 @@ typedef struct {
   double flops_per_event_shared;  /* ME_OPT_SHARE_CURRENTS: ALGORITHMIC flops per event of the sharing kernel over the full helicity
                                      set (every current evaluated once per distinct helicity assignment of ITS OWN legs, in the walk
                                      order of the kernel), fixed part included; 0 where no such kernel exists                          */
+  double flops_executed_per_event_shared; /* the same with what the sharing kernels actually issue (recomputation included)           */
 } me_info;
 
 /* Create a context for `process` on the current CUDA device.  Builds the colour matrix and
@@ -126,8 +127,10 @@ me_status me_filter_helicities(me_ctx* ctx, const double* d_momenta, int64_t n,
  * quark and one gluon helicity.  With the option on (the default), g g -> t t~ g g runs a kernel that walks the good helicities in a
  * reflected Gray order (quark helicities fastest) and re-evaluates a current only when one of ITS helicities changed since the
  * previous step; three-gluon sub-trees are parked in an L2-resident scratch owned by the context.  Same diagrams, same
- * amplitudes, same number up to rounding order (~1e-15).  Ignored by the other processes.  me_info.flops_per_event_shared is
- * the algorithmic flop count with the option on.  me_compute_helicities / me_compute_jamps are unaffected. */
+ * amplitudes, same number up to rounding order (~1e-14).  g g -> t t~ g g g groups the helicities by their gluon helicities (one CTA
+ * loops over the four quark-helicity assignments of a group): its last diagram kernel forms the colour-ordered four-gluon
+ * currents once per group and needs no local jamp accumulators.  Ignored by the other processes.  me_info.flops_per_event_shared
+ * is the algorithmic flop count with the option on.  me_compute_helicities / me_compute_jamps are unaffected. */
 typedef enum { ME_OPT_PARITY_PAIRING = 0, ME_OPT_SHARE_CURRENTS = 1 } me_option;
 me_status me_set_option(me_ctx* ctx, me_option option, int value);
 

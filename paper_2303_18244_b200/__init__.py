@@ -31,7 +31,7 @@ class me_info(ctypes.Structure):
                                             "page", "nkernels", "namplitudes")] + \
                [("mass", ctypes.c_double * 8), ("flops_per_helicity", ctypes.c_double * 3),
                 ("flops_per_event_fixed", ctypes.c_double * 3), ("flops_executed_per_helicity", ctypes.c_double * 3),
-                ("flops_per_event_shared", ctypes.c_double)]
+                ("flops_per_event_shared", ctypes.c_double), ("flops_executed_per_event_shared", ctypes.c_double)]
 
 
 class MEError(RuntimeError):

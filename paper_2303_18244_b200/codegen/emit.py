@@ -329,7 +329,7 @@ def emit_single_kernel_process(n, name):
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, T.ncol * T.ncol, ", ".join(str(float(x)) for row in T.color_num for x in row)))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr, false, nullptr, 0.0};"
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, nullptr, false, nullptr, 0.0, 0, 0.0};"
       % (name, n, T.ndiagrams, K.namp, T.ncol, T.color_denom, float(per_hel), float(per_hel), float(per_hel),
          float(per_hel), float(per_hel), float(per_hel), float(K.fixed_flops), name, name))
     S("}  // namespace me")

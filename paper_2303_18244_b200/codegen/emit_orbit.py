@@ -808,7 +808,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
             always = t.flops - sum(f for _, f in conds)
             shared += always * nh + sum(f * walk_count(m, walk) for m, f in conds)
     shared_event = shared + nh * (cs_flops + 2 * FL["spinor"] + FL["bilinear"]) + fixed
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, false, gray_rank_%s, %r};"
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, 1, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, false, gray_rank_%s, %r, 0, 0.0};"
       % (name, N, 123, namp, ncol, color_denom, float(per_hel), float(per_hel), float(per_hel),
          float(per_hel), float(per_hel), float(per_hel), float(fixed), name, name, name, name, float(shared_event)))
     S("}  // namespace me")

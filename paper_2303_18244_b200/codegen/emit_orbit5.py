@@ -22,6 +22,9 @@ from .topology import color_matrix
 
 N = 5
 NPAR = 7
+HEL_PER_CTA = 4  # helicities looped inside one CTA (csrc/multi.h ME_HEL_PER_CTA); the sharing kernels rely on the grouping of the list:
+                 # entries 4 g .. 4 g + 3 share their gluon helicities (the four quark-helicity assignments, 255 = absent)
+T_BIT, TB_BIT = NPAR - 1 - 2, NPAR - 1 - 3
 BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
 MERGE_ORDERED = True  # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
 MERGE_TRIPLE = True  # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
@@ -50,7 +53,7 @@ class Layout5:
     """per-thread shared-memory slots of one kernel (units of R), paired layout of hel_amp.cuh"""
     npar = NPAR
 
-    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5), scratch=False, tm=()):
+    def __init__(self, want_pairs, want_iq_mid, jacc, ferm_smem=False, want_q1chi=True, want_chi=False, ik2_sizes=(2, 3, 4, 5), scratch=False, tm=(), jtt4=False, nu=0, nu_smem=0):
         # tm: categories ("PAIR", "CHI") that the FP64 kernel keeps in tensor memory (hel_amp.cuh "Tensor memory as a per-thread
         # scratchpad"); they are allocated last, from the even slot TM0 on, so that the shared-memory part is contiguous
         A = SlotAlloc()
@@ -60,6 +63,9 @@ class Layout5:
         self.MOM = A.vec(4 * N)
         self.PT = A.vec(4)
         self.GBS = [A.vec(5) for _ in range(N)]
+        self.JTT4 = A.vec(8 * HEL_PER_CTA) if jtt4 else None      # ubar gamma v of the helicities of the CTA's group (sharing kernel o2s)
+        # colour-ordered currents of the sharing kernel o2s: U[(w, k)], the first nu_smem of every w in shared memory, the rest in TMEM
+        self.U = {(w, k): A.vec(8) for w in range(N) for k in range(nu_smem)}
         self.PAIR = {}
         pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
         if want_pairs and "PAIR" not in tm:
@@ -93,6 +99,8 @@ class Layout5:
             if "J" in tm:
                 assert jacc % 4 == 0
                 self.J = A.vec(2 * jacc)
+            if "U" in tm:
+                self.U.update({(w, k): A.vec(8) for w in range(N) for k in range(nu_smem, nu)})
             self.tm_cols = 32
             while self.tm_cols < 2 * (A.n - self.TM0):
                 self.tm_cols *= 2                      # tcgen05.alloc takes a power of two >= 32
@@ -697,6 +705,131 @@ def build_k3(stride, pidx, jacc=0, tm=()):
 
 
 # ------------------------------------------------------------------------------------------
+# kernel 3, sharing form (include/me.h ME_OPT_SHARE_CURRENTS): the same diagrams as build_k3, organised
+# around what depends on the gluon helicities only.  For the last gluon w the 21 four-gluon currents on quad = rest_of(w) (three
+# V3(pair, pair'), eighteen V4(pair, eps, eps)) have colour factors in the six-dimensional space of multilinear Lie polynomials in the
+# four generators; expanded on the left-normed brackets D_pi = [[[q0, q_pi1], q_pi2], q_pi3] they become six colour-ordered currents
+#     U_pi = sum_T alpha_pi(T) V_T          (alpha_pi(T) = coefficient of the string q0 q_pi1 q_pi2 q_pi3 in the colour factor of T)
+# that are formed ONCE for the (up to four) quark-helicity assignments a CTA loops over (pre-groups, run before the helicity loop), and
+# each helicity costs twelve dot products U_pi . x1, U_pi . x2 with the two end vectors per last gluon.  Every colour flow of a
+# (w, helicity) block is then complete in registers: the 48 flows go out by one RED pair each and no local jamp accumulators exist.
+# The thirty currents stay on chip for the whole group (20 in tensor memory next to the pair currents, 10 in shared memory: one
+# 128-thread CTA per SM in FP64, two in FP32 with one TMEM column per slot); the helicity loop stays outermost, so that all reductions
+# into one staging row happen close in time (with the loop over w outside, the rows of four helicities per CTA no longer fit the L2
+# and every reduction became a DRAM read-modify-write: 35 GB per launch instead of 9).
+# ------------------------------------------------------------------------------------------
+NU_SMEM = 2          # colour-ordered currents per last gluon kept in shared memory; the other four in tensor memory
+
+
+def build_k3s(stride, pidx):
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=0, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "U"), nu=6, nu_smem=NU_SMEM)
+    groups = []
+    add_group = _grouper(groups)
+    phase_a(lay, stride, add_group, want_pairs=True)          # the ten pair currents: gluon helicities only, once per group
+    pis = list(permutations((1, 2, 3)))
+    bases = {}
+    insts = []
+    for w in range(N):
+        quad = rest_of(w)
+        I = Inst5(lay, stride)
+        # c_v3(x, y) = -[x, y]: three nested c_v3 give -[[[q0, a], b], c]; the coefficient of the string q0 a b c in it is -1
+        basis = [c_v3(c_v3(c_v3(c_leaf(quad[0]), c_leaf(quad[q[0]])), c_leaf(quad[q[1]])), c_leaf(quad[q[2]])) for q in pis]
+        bases[w] = basis
+        I.L("W4<R> " + ", ".join("U%d" % k for k in range(6)) + ";")
+        I.L("const R ik4 = %s;" % I.ik2(*quad))
+        started = [False] * 6
+
+        def accumulate(expr, X):
+            alpha = [-X.get((quad[0], quad[q[0]], quad[q[1]], quad[q[2]]), 0) for q in pis]
+            chk = {}
+            for al, D in zip(alpha, basis):
+                for st, v in D.items():
+                    chk[st] = chk.get(st, 0) + al * v
+            assert not _cdiff(X, chk, {}), "colour factor outside the span of the left-normed brackets"
+            I.L("{ const W4<R> V = %s;" % expr)
+            for k, al in enumerate(alpha):
+                if al == 0:
+                    continue
+                assert al in (1, -1), al
+                if not started[k]:
+                    I.L("  U%d = %s;" % (k, "V" if al > 0 else "wsub(W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0}, V)"))
+                    started[k] = True
+                    I.flops += 0 if al > 0 else 8
+                else:
+                    I.L("  U%d = %s(U%d, V);" % (k, "wadd" if al > 0 else "wsub", k)); I.flops += 8
+            I.L("}")
+
+        a0 = quad[0]
+        for b0 in quad[1:]:
+            p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
+            I.L("{")
+            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.kvec("k1", list(p1)); I.kvec("k2", list(p2))
+            I.flops += FL5["v3_current"]
+            accumulate("v3_current(p1, p2, k1, k2, ik4)", c_v3(cpair(*p1), cpair(*p2)))
+            I.L("}")
+        for p in [(quad[i], quad[j]) for i in range(4) for j in range(i + 1, 4)]:
+            l1, l2 = [l for l in quad if l not in p]
+            I.L("{")
+            I.ldw("pp", lay.PAIR[p]); I.leaf("e1", l1); I.leaf("e2", l2)
+            I.L("const V4Dots<R> dots = v4_dots(pp, e1, e2, ik4);"); I.flops += FL5["v4_dots"]
+            for k in range(3):
+                I.flops += FL5["v4_current"]
+                accumulate("v4_current(%d, dots, pp, e1, e2)" % k, c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
+            I.L("}")
+        assert all(started)
+        for k in range(6):
+            I.stw(lay.U[(w, k)], "U%d" % k)
+        insts.append(I)
+    add_group("ubuild", insts, 1)
+    for _, t, _, _ in groups:
+        t.pre = True                                              # run once per group of helicities, before the helicity loop
+        t.group_flops = t.flops; t.flops = 0
+    # ---- per helicity: the two end vectors of w (bilinears of the fermion ends with the dual of V3(quad, eps_w) folded in) and 12 dots
+    insts = []
+    for w in range(N):
+        quad = rest_of(w)
+        I = Inst5(lay, stride)
+        I.leaf("ew", w); I.kvec("kw", [w]); I.kvec("kq", quad)
+        f0 = I.flops
+        I.qvec("qw", [w]); I.qvec("qq", quad)
+        I.L("const W4<R> q1w = quark_step2(ub, ew, qw, mt, %s), chw = col_step(slash_col(ew, vv), qq, mt, %s);" % (I.iq(w), I.iq(*quad)))
+        I.flops += FL5["quark_step2"] + FL5["slash_col"] + FL5["col_step"]
+        I.redundant += I.flops - f0                    # kernel 2 forms the same ten one-gluon quark currents
+        I.L("const W4<R> x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
+        I.L("const W4<R> x1 = wadd(bilinear(ub, chw), x3), x2 = wsub(bilinear(q1w, vv), x3);")
+        I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"] + 2 * FL5["wadd"]
+        for k0 in (0, 3):                              # three currents in flight at a time
+            for k in range(k0, k0 + 3):
+                I.ldw("u%d" % k, lay.U[(w, k)])
+            I.L("const Cx<R> " + ", ".join("a1_%d = wdot(u%d, x1), a2_%d = wdot(u%d, x2)" % (k, k, k, k) for k in range(k0, k0 + 3)) + ";")
+        I.flops += 12 * FL5["wdot"]
+        for k in range(6):
+            I.jamp("a1_%d" % k, c_close(ONE, bases[w][k], cchi(w)), pidx)
+            I.jamp("a2_%d" % k, c_close(cq1(w), bases[w][k], ONE), pidx)
+        I.namp += 63 - 12                      # 21 four-gluon terms x three closings, carried by the twelve ordered amplitudes
+        I.flush_direct()
+        insts.append(I)
+    add_group("quads", insts, 1)
+    # ---- V4(pair, pair', eps_m) on the bare line
+    insts = []
+    for m in range(N):
+        quad = rest_of(m)
+        a0 = quad[0]
+        for b0 in quad[1:]:
+            p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
+            I = Inst5(lay, stride)
+            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.leaf("em", m)
+            I.L("const V4Dots<R> dots = v4_dots(p1, p2, em, %s);" % I.ik2(*range(N))); I.flops += FL5["v4_dots"]
+            for k in range(3):
+                I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, p1, p2, em), jtt);" % (k, k)); I.flops += FL5["v4_current"] + FL5["wdot"]
+                I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(*p1), cpair(*p2), c_leaf(m)), ONE), pidx)
+            I.flush_direct()
+            insts.append(I)
+    add_group("pair_pair_v4", insts, 1)
+    return lay, groups
+
+
+# ------------------------------------------------------------------------------------------
 # source emission
 # ------------------------------------------------------------------------------------------
 def prologue_lines(lay):
@@ -737,6 +870,20 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
     fetch the same instructions (two independent 128-thread CTAs drift apart and thrash the instruction cache)"""
     src = []
     S = src.append
+
+    def emit_groups(gs):
+        for gname, tmpl, rows, unroll in gs:
+            S("    // ---- %s: %d instances" % (gname, len(rows)))
+            S("#pragma unroll %d" % unroll)
+            S("    for (int it = 0; it < %d; ++it) {" % len(rows))
+            S("      const int* tb = tab_%s_o%s_%s[it];" % (name, ki, gname))
+            for l in tmpl.lines:
+                if "@SUB:" in l:
+                    sname = l.split("@SUB:")[1].split("@")[0]
+                    l = l.replace("@SUB:%s@" % sname, "tab_%s_o%s_%s_%s" % (name, ki, gname, sname))
+                S("      " + l)
+            S("    }")
+
     namp = sum(t.namp * len(rows) for _, t, rows, _ in groups)
     S("// GENERATED by paper_2303_18244_b200/codegen (orbit-looped emitter, emit_orbit5.py) — do not edit.")
     S("// g g -> t t~ g g g, diagram kernel %s: %d amplitude terms in %d looped shapes; %d shared-memory slots per thread." % (ki, namp, len(groups), lay.nslots))
@@ -799,9 +946,21 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("  for (int s = 0; s < %d; ++s) xstw<R, TM>(sm, tm, ME_EO(%d) + s * 8 * ME_SM_STRIDE, W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0});" % (lay.jacc // 4, lay.J))
     else:
         S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
+    has_pre = any(getattr(t, "pre", False) for _, t, _, _ in groups)
     S("  const int hc_end = !live ? 0 : (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
+    if has_pre:
+        # sharing kernel: the helicities of this CTA share their gluon helicities (the host groups the list: include/me.h); what depends on
+        # the gluons only is formed once, with the first valid helicity of the group, before the helicity loop
+        S("  int h0 = 255;")
+        S("  if (helpe != nullptr) h0 = helpe[e < n ? e : n - 1];")
+        S("  else for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) if (h0 == 255 && hels[hc] != 255) h0 = hels[hc];")
+        S("  if (h0 != 255 && live) {")
+        S("    const int h = h0;")
+        emit_groups([g for g in groups if getattr(g[1], "pre", False)])
+        S("  }")
     S("  for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
+    S("    if (h == 255) continue;                       // padding of a grouped helicity list")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
     if lay.FERM is not None:
         S("    {")
@@ -820,17 +979,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
         S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
         S("    const W4<R> jtt = bilinear(ub, vv);")
-    for gname, tmpl, rows, unroll in groups:
-        S("    // ---- %s: %d instances" % (gname, len(rows)))
-        S("#pragma unroll %d" % unroll)
-        S("    for (int it = 0; it < %d; ++it) {" % len(rows))
-        S("      const int* tb = tab_%s_o%s_%s[it];" % (name, ki, gname))
-        for l in tmpl.lines:
-            if "@SUB:" in l:
-                sname = l.split("@SUB:")[1].split("@")[0]
-                l = l.replace("@SUB:%s@" % sname, "tab_%s_o%s_%s_%s" % (name, ki, gname, sname))
-            S("      " + l)
-        S("    }")
+    emit_groups([g for g in groups if not getattr(g[1], "pre", False)])
     S("  }")
     if tm0 is not None:
         S("  if constexpr (TM) tm_free(tm_base, (sizeof(R) == 8 ? %du : %du) * %d);" % (lay.tm_cols, max(32, lay.tm_cols // 2), BLOCK // 128))
@@ -891,7 +1040,8 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
     S("}  // namespace me")
     flops = sum(t.flops * len(rows) for _, t, rows, _ in groups)
     redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
-    return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, fixed=fixed, slots=lay.nslots, tm_slot0=tm0, tm_cols=getattr(lay, "tm_cols", 0),
+    group_flops = sum(getattr(t, "group_flops", 0) * len(rows) for _, t, rows, _ in groups)
+    return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, group_flops=group_flops, fixed=fixed, slots=lay.nslots, tm_slot0=tm0, tm_cols=getattr(lay, "tm_cols", 0),
                                        shapes={g: len(r) for g, _, r, _ in groups})
 
 
@@ -921,6 +1071,11 @@ def emit_orbit5_process(name="gg_ttxggg"):
             src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="tm" if K3D_FLOAT else "double")
             files["gen_%s_o%dd.cu" % (name, ki)] = src2
             info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, flops=info2["flops"], redundant=info2["redundant"])
+    # sharing form of the last kernel (build_k3s): used when the helicity list is grouped by gluon helicities (ME_OPT_SHARE_CURRENTS)
+    lay3, groups3 = build_k3s(BLOCK1, pidx)
+    src3, info3 = emit_kernel(name, "2s", lay3, groups3, BLOCK1, only="tm")
+    files["gen_%s_o2s.cu" % name] = src3
+    assert info3["amplitudes"] == kinfo[-1]["amplitudes"], (info3["amplitudes"], kinfo[-1]["amplitudes"])
     namp = sum(k["amplitudes"] for k in kinfo)
     assert namp == 1890, namp
     # colour sum in its symmetric form (S§8(d)): per part  sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), as for the smaller
@@ -948,19 +1103,36 @@ def emit_orbit5_process(name="gg_ttxggg"):
     S("// GENERATED by paper_2303_18244_b200/codegen (emit_orbit5.py) — do not edit.  g g -> t t~ g g g process table.")
     S("#include \"kernels.h\"")
     S("#include \"multi.h\"")
+    S("#include <stdlib.h>")
     S("namespace me {")
     for ki in range(len(kinfo)):
         S("extern const MultiKernel mk_%s_o%d;" % (name, ki))
+    S("extern const MultiKernel mk_%s_o2s;" % name)
     S("static const MultiKernel* const parts_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo)))))
+    S("static const MultiKernel* const parts_sh_%s[%d] = {%s, &mk_%s_o2s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo) - 1)), name))
+    # current sharing: the helicity list is ordered by gluon helicities, the four quark-helicity assignments of each adjacent (rank table);
+    # flops per event with it on, over the full helicity set: kernel o2 per helicity -> per group of four + per helicity
+    fmask = (1 << T_BIT) | (1 << TB_BIT)
+    order = sorted(range(1 << NPAR), key=lambda h: (h & ~fmask, h & fmask))
+    rank = [order.index(h) for h in range(1 << NPAR)]
+    S("static const unsigned char gray_rank_%s[%d] = {%s};" % (name, 1 << NPAR, ", ".join(str(r) for r in rank)))
+    k2 = kinfo[-1]
+    a2 = k2["flops"] - k2["redundant"] - pa["pairs"]                   # algorithmic part of kernel o2 per helicity (the pairs are counted once, elsewhere)
+    nhel, ngroups = 1 << NPAR, (1 << NPAR) // HEL_PER_CTA
+    shared_event = nhel * (algo - a2) + ngroups * (info3["group_flops"] - pa["pairs"]) + nhel * (info3["flops"] - info3["redundant"]) + fixed
+    executed_shared = executed - k2["flops"] + info3["flops"] + info3["group_flops"] / HEL_PER_CTA
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
-    S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) { return launch_multi(precision, a, parts_%s, %d, %d, color_num_%s); }"
-      % (name, name, len(kinfo), ncol, name))
+    S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
+    S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // the sharing kernel exists in its tensor-memory form only")
+    S("  return launch_multi(precision, a, (a.share && !no_tmem) ? parts_sh_%s : parts_%s, %d, %d, color_num_%s);" % (name, name, len(kinfo), ncol, name))
+    S("}")
     S("static size_t scratch_%s(int precision, long npad, int, int) { return multi_scratch_bytes(precision, npad, %d); }" % (name, ncol))
-    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, true, nullptr, 0.0};"
+    S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, true, gray_rank_%s, %r, %d, %r};"
       % (name, N, 1240, namp, ncol, color_denom, len(kinfo) + 1, float(algo), float(algo), float(algo),
-         float(executed), float(executed), float(executed), float(fixed), name, name, name))
+         float(executed), float(executed), float(executed), float(fixed), name, name, name, name, float(shared_event), fmask, float(executed_shared)))
     S("}  // namespace me")
     files["gen_%s_table.cu" % name] = "\n".join(src) + "\n"
     info = dict(n=N, ndiagrams=1240, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=algo,
-                flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK)
+                flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK,
+                flops_shared_event=shared_event, flops_executed_per_helicity_shared=executed_shared, kernel_o2s=info3)
     return files, info

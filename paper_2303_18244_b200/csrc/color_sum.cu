@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(32 * CS_WARPS) k_color_sum(const RC* __restric
 #pragma unroll
       for (int k = 0; k < CS_WARPS; ++k) s += red[k][lane];
       const double meh = (double)s;
-      if (me_hel != nullptr && e < n) me_hel[(long)hels[hc] * hs + e] = meh * norm_hel * 0.5;
+      if (me_hel != nullptr && e < n && hels[hc] != 255) me_hel[(long)hels[hc] * hs + e] = meh * norm_hel * 0.5;
       acc += meh;
     }
   }

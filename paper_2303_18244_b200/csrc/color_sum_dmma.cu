@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
       for (int o = 4; o < 32; o <<= 1) { p0 += __shfl_xor_sync(0xffffffffu, p0, o); p1 += __shfl_xor_sync(0xffffffffu, p1, o); }
       if (lane < 4) {
         const long e = e0 + 2 * lane;
-        if (me_hel != nullptr) {
+        if (me_hel != nullptr && hels[hc] != 255) {
           if (e < n) me_hel[(long)hels[hc] * hs + e] = p0 * norm_hel * 0.5;
           if (e + 1 < n) me_hel[(long)hels[hc] * hs + e + 1] = p1 * norm_hel * 0.5;
         }

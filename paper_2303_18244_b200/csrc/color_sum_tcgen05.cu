@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(TC_M, 2) k_color_sum_tcgen05(const float* __re
         TC_STEP(curA, pc)
         TC_STEP(curB, pc + 1)
       }
-      if (e < n && me_hel != nullptr) me_hel[(long)hels[hc] * hs + e] = (double)p * norm_hel * 0.5;
+      if (e < n && me_hel != nullptr && hels[hc] != 255) me_hel[(long)hels[hc] * hs + e] = (double)p * norm_hel * 0.5;
       me_acc += (double)p;
       p = 0.f;
     }

@@ -43,6 +43,9 @@ struct ProcTable {
   bool needs_color_matrix;        // the context uploads color_num for a separate colour-sum kernel
   const unsigned char* gray_rank; // [ncomb] position of every helicity in the walk of the current-sharing kernel, or null (no such kernel)
   double flops_shared_event;      // algorithmic flops per event of the sharing kernel over the full helicity set (0: none)
+  int group_mask;                 // != 0: helicity bits (the quark helicities) that vary WITHIN a group of the sharing list; the entries with equal
+                                  // remaining (gluon) bits are adjacent and padded with 255 to ME_HEL_PER_CTA entries (one CTA loops over one group)
+  double flops_executed_shared;   // flops per helicity the sharing kernels issue over the full helicity set (0: as flops_executed)
 };
 
 extern const ProcTable tab_gg_ttx, tab_gg_ttxg, tab_gg_ttxgg, tab_gg_ttxggg;

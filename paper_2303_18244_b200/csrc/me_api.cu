@@ -4,6 +4,7 @@
 #include <stdlib.h>
 #include "../../include/me.h"
 #include "kernels.h"
+#define ME_HEL_PER_CTA_HOST 4     // = ME_HEL_PER_CTA of csrc/multi.h (helicities one CTA of a staged diagram kernel loops over)
 
 #include <cmath>
 #include <cstdio>
@@ -24,8 +25,9 @@ struct me_ctx {
   int ngood;
   unsigned char* d_hels_half;    // parity pairing: one helicity of every good pair {h, ~h}
   int nhalf;                     // 0 = pairing not applicable to the current mask
-  unsigned char* d_hels_gray;    // ME_OPT_SHARE_CURRENTS: the good helicities in the order the sharing kernel walks them
-  unsigned char* d_hels_gray_half;
+  unsigned char* d_hels_gray;    // ME_OPT_SHARE_CURRENTS: the good helicities in the order the sharing kernels walk them (grouped and
+  unsigned char* d_hels_gray_half;   // padded with 255 where the process groups by gluon helicities); ngray / ngray_half entries
+  int ngray, ngray_half;
   bool pairing;                  // option ME_OPT_PARITY_PAIRING
   bool share;                    // option ME_OPT_SHARE_CURRENTS
   uint64_t mask[2];
@@ -123,6 +125,7 @@ extern "C" me_status me_create(me_process process, const me_sm_params* prm, me_c
     c->norm_hel = std::pow(gs2, n) * 2.0 / t->color_denom;
     for (int k = 0; k < 3; ++k) { I.flops_per_helicity[k] = t->flops_per_helicity[k]; I.flops_executed_per_helicity[k] = t->flops_executed[k]; I.flops_per_event_fixed[k] = t->fixed_flops; }
     I.flops_per_event_shared = t->flops_shared_event;
+    I.flops_executed_per_event_shared = t->flops_executed_shared > 0 ? t->flops_executed_shared * I.ncomb + t->fixed_flops : t->flops_shared_event;
   }
   c->inv_avg = 1.0 / I.avg_denom;
   cudaError_t e = cudaGetDevice(&c->device);
@@ -266,8 +269,9 @@ extern "C" me_status me_set_helicities(me_ctx* c, const uint64_t mask[2]) {
   }
   // current sharing (ME_OPT_SHARE_CURRENTS): the same lists in the walk order of the sharing kernel, a reflected Gray code
   // whose fastest bits are the two quark helicities (consecutive helicities differ in as few, and as rarely in gluon, bits as possible)
+  c->ngray = c->ngray_half = 0;
   if (c->tab != nullptr && c->tab->gray_rank != nullptr) {
-    unsigned char tmp[128];
+    unsigned char tmp[128], out[128];
     for (int pass = 0; pass < 2; ++pass) {
       const unsigned char* src = pass == 0 ? good : half; const int m = pass == 0 ? ng : c->nhalf;
       if (m == 0) continue;
@@ -277,7 +281,18 @@ extern "C" me_status me_set_helicities(me_ctx* c, const uint64_t mask[2]) {
         while (j >= 0 && c->tab->gray_rank[tmp[j]] > c->tab->gray_rank[v]) { tmp[j + 1] = tmp[j]; --j; }
         tmp[j + 1] = v;
       }
-      ME_CUDA(cudaMemcpy(pass == 0 ? c->d_hels_gray : c->d_hels_gray_half, tmp, m, cudaMemcpyHostToDevice), "me_set_helicities");
+      int len = 0;
+      if (c->tab->group_mask == 0) { memcpy(out, tmp, m); len = m; }
+      else {                                    // groups of equal gluon helicities, each padded with 255 to ME_HEL_PER_CTA entries
+        const int keep = ~c->tab->group_mask;
+        for (int i = 0; i < m; ++i) {
+          if (i > 0 && (tmp[i] & keep) != (tmp[i - 1] & keep)) while (len % ME_HEL_PER_CTA_HOST) out[len++] = 255;
+          out[len++] = tmp[i];
+        }
+        while (len % ME_HEL_PER_CTA_HOST) out[len++] = 255;
+      }
+      ME_CUDA(cudaMemcpy(pass == 0 ? c->d_hels_gray : c->d_hels_gray_half, out, len, cudaMemcpyHostToDevice), "me_set_helicities");
+      (pass == 0 ? c->ngray : c->ngray_half) = len;
     }
   }
   return ME_OK;
@@ -324,8 +339,8 @@ extern "C" me_status me_filter_helicities(me_ctx* c, const double* d_mom, int64_
 // twice; with current sharing (processes that have such a kernel) the list in walk order
 static void hel_list(const me_ctx* c, const unsigned char** hels, int* nhel, double* inv_avg, bool* share) {
   *share = c->share && c->tab != nullptr && c->tab->gray_rank != nullptr;
-  if (c->pairing && c->nhalf > 0) { *hels = *share ? c->d_hels_gray_half : c->d_hels_half; *nhel = c->nhalf; *inv_avg = 2.0 * c->inv_avg; }
-  else { *hels = *share ? c->d_hels_gray : c->d_hels_good; *nhel = c->ngood; *inv_avg = c->inv_avg; }
+  if (c->pairing && c->nhalf > 0) { *hels = *share ? c->d_hels_gray_half : c->d_hels_half; *nhel = *share ? c->ngray_half : c->nhalf; *inv_avg = 2.0 * c->inv_avg; }
+  else { *hels = *share ? c->d_hels_gray : c->d_hels_good; *nhel = *share ? c->ngray : c->ngood; *inv_avg = c->inv_avg; }
 }
 
 extern "C" me_status me_compute(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, double* d_me, void* stream) {

@@ -724,3 +724,35 @@ def test_share_currents_option(me, orc):
         c.me_set_option(me.ME_OPT_SHARE_CURRENTS, 0)
         assert np.array_equal(c.me_compute(mm, 64).cpu().numpy(), a)
         c.close()
+
+
+def test_share_currents_staged_process(me, orc):
+    """ME_OPT_SHARE_CURRENTS for g g -> t t~ g g g: the helicity list is grouped by gluon helicities (padded groups of four), the last
+    diagram kernel forms its colour-ordered four-gluon currents once per group.  On / off agree to rounding in every precision, also
+    for an irregular mask (incomplete groups: padding entries) and with parity pairing; the default (on) is what every other test of
+    this process runs against the oracle."""
+    cfg = inputs.CONFIGS[4]
+    n = 161
+    ctx = me.MEContext(4)
+    _, mom, _ = gen_events(me, ctx, cfg, n)
+    p = to_aos(mom, n, cfg)
+    full = EXPECTED_MASK[4]
+    irregular = full & ~0x0F0000000000000000000000F000F1 & ~(1 << 77) & ~(0x7 << 100)
+    _, ref_h = orc.me(4, p[:24], per_helicity=True)
+    for mask in (full, irregular):
+        ctx.me_set_helicities(mask)
+        for pairing in (0, 1):
+            ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, pairing)
+            for name, tol in (("fp64", 1e-12), ("mixed", 5e-6), ("fp32", 1e-4)):
+                ctx.me_set_option(me.ME_OPT_SHARE_CURRENTS, 0)
+                off = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
+                ctx.me_set_option(me.ME_OPT_SHARE_CURRENTS, 1)
+                on = ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy()
+                assert np.isfinite(on).all() and (on > 0).all()
+                assert np.abs(on / off - 1).max() < tol, (hex(mask), pairing, name, np.abs(on / off - 1).max())
+                assert np.array_equal(ctx.me_compute(mom, n, me.PRECISIONS[name]).cpu().numpy(), on)
+            ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
+        sel = np.array([(mask >> h) & 1 for h in range(128)], dtype=bool)
+        got = ctx.me_compute(mom, n).cpu().numpy()[:24]
+        assert np.abs(got / (ref_h[:, sel].sum(1) / 1536) - 1).max() < 1e-10
+    ctx.close()
