@@ -255,7 +255,7 @@ def main():
     flops_unshared = info.flops_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
     shared_default = info.flops_per_event_shared > 0 and ngood == info.ncomb
     flops_alg = info.flops_per_event_shared if shared_default else flops_unshared
-    flops_exe = flops_alg if shared_default else info.flops_executed_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
+    flops_exe = info.flops_executed_per_event_shared if shared_default else info.flops_executed_per_helicity[0] * ngood + info.flops_per_event_fixed[0]
     results = {}
     prof = profile_metrics()
     with ClockSampler(local) as clk:
@@ -426,8 +426,10 @@ def main():
             c = inputs.CONFIGS[proc]
             cx, mm = setup(proc, c["events"], 0)
             ng = bin(cx.me_filter_helicities(mm, 32)[0]).count("1")
-            fl = cx.info.flops_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
-            fx = cx.info.flops_executed_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
+            fl_un = cx.info.flops_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
+            sh = cx.info.flops_per_event_shared > 0 and ng == cx.info.ncomb          # default path shares currents: its own algorithmic count
+            fl = cx.info.flops_per_event_shared if sh else fl_un
+            fx = cx.info.flops_executed_per_event_shared if sh else cx.info.flops_executed_per_helicity[0] * ng + cx.info.flops_per_event_fixed[0]
             results[c["name"]] = {}
             reps = 2 if proc == 4 else 5
             for pname in c["precisions"]:
@@ -435,10 +437,11 @@ def main():
                 ms = statistics.mean(pp)
                 pk = "fp32" if pname == "fp32" else "fp64"
                 results[c["name"]][pname] = {"MEs_per_s": c["events"] / (ms * 1e-3), "ms_per_step": ms,
-                                             "flops_per_event_algorithmic": fl, "flops_per_event_executed": fx,
+                                             "flops_per_event_algorithmic": fl, "flops_per_event_executed": fx, "flops_per_event_unshared_algorithm": fl_un,
+                                             "frac_counting_unshared_algorithm": fl_un * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
                                              "frac_of_%s_peak" % pk: fl * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
                                              "frac_of_%s_peak_executed" % pk: fx * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk]}
-                m = prof.get((c["name"], pname, "-", c["events"]))
+                m = prof.get((c["name"], pname, "shared_currents" if sh else "-", c["events"]))
                 if m is not None:
                     fe = ncu_flops_per_event(m)
                     results[c["name"]][pname].update({"flops_per_event_ncu": fe, "frac_ncu": fe * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],

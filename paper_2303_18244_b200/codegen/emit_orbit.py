@@ -27,9 +27,9 @@ NPAR = 6
 NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
 NSCVEC = 14         # and the six colour-ordered four-gluon currents that close on the bare quark line
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
-MERGE_ORDERED = True   # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
-MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: T.w - w.T)
-MERGE_TRIPLE = True   # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
+# The amplitudes are formed in colour-ordered combinations throughout (each is still a sum of whole diagram terms): two-gluon quark currents
+# with the pair current folded into the two stepwise ones; the V3 closing of the last gluon folded into the two quark-end closings
+# (colour T.w - w.T); three-gluon sub-trees as two ordered currents (V4 pieces in their channels, Jacobi identity).
 # partial unrolling lets the operand loads of the next instance overlap the arithmetic of the current one
 UNROLL = dict(pairs=6, q1=4, chi1=4, triples=1, rows2=1, q1_pair_chi=12, pair_pair=3, pair_v4=6)      # FP64 (255 registers, 4 warps/SM)
 UNROLL_SH = dict(pairs=1, q1=1, chi1=1)      # FP64 sharing kernel (as loops the FP32 kernel is 17 % slower: table loads in front of its cheaper arithmetic)
@@ -478,38 +478,24 @@ def build_groups(stride):
         I.ldw("chic", lay.CHI + 8 * c); I.ldw("chid", lay.CHI + 8 * d)
         I.qvec("q", [a, b])
         I.L("const R iq2 = %s;" % I.iq(a, b))
-        if MERGE_ORDERED:
-            # colour-ordered two-gluon currents: the pair current (a commutator, colour ab - ba) is folded into the two stepwise
-            # currents, on the row side before the common propagator and on the column side before the dot product; the nine
-            # diagram terms of this block become four colour-ordered amplitudes, one colour flow each
-            col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
-            assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
-            for col in (col_ab, col_ba):
-                assert not _cdiff(c_close(col, cpair(c, d), ONE), c_close(col, c_leaf(c), cchi(d)), c_close(col, c_leaf(d), cchi(c)))
-            I.L("const W4<R> sp = row_slash(ub, pab), xp = slash_col(pcd, vv);"); I.flops += FL["row_slash"] + FL["slash_col"]
-            I.L("const W4<R> rab = row_step(wadd(row_slash(q1a, eb), sp), q, mt, iq2), rba = row_step(wsub(row_slash(q1b, ea), sp), q, mt, iq2);")
-            I.flops += 2 * (FL["row_slash"] + 8 + FL["col_step"])
-            I.L("const W4<R> xcd = wadd(slash_col(ec, chid), xp), xdc = wsub(slash_col(ed, chic), xp);"); I.flops += 2 * (FL["slash_col"] + 8)
-            I.L("const Cx<R> a1 = row_col(rab, xcd), a2 = row_col(rab, xdc), a3 = row_col(rba, xcd), a4 = row_col(rba, xdc);"); I.flops += 4 * FL["row_col"]
-            I.jamp("a1", c_close(col_ab, c_leaf(c), cchi(d)), pidx)
-            I.jamp("a2", c_close(col_ab, c_leaf(d), cchi(c)), pidx)
-            I.jamp("a3", c_close(col_ba, c_leaf(c), cchi(d)), pidx)
-            I.jamp("a4", c_close(col_ba, c_leaf(d), cchi(c)), pidx)
-            I.namp += 5
-            I.flush_jamps()
-        else:
-            I.L("const W4<R> xp = slash_col(pcd, vv), xcd = slash_col(ec, chid), xdc = slash_col(ed, chic);"); I.flops += 3 * FL["slash_col"]
-            rows = [("ra", "quark_step2(ub, pab, q, mt, iq2)", c_step(ONE, cpair(a, b))),
-                    ("rb", "quark_step2(q1a, eb, q, mt, iq2)", c_step(cq1(a), c_leaf(b))),
-                    ("rc", "quark_step2(q1b, ea, q, mt, iq2)", c_step(cq1(b), c_leaf(a)))]
-            for nm, expr, col in rows:
-                I.L("{ const W4<R> %s = %s;" % (nm, expr)); I.flops += FL["quark_step2"]
-                I.L("  const Cx<R> a1 = row_col(%s, xp), a2 = row_col(%s, xcd), a3 = row_col(%s, xdc);" % (nm, nm, nm)); I.flops += 3 * FL["row_col"]
-                I.jamp("a1", c_close(col, cpair(c, d), ONE), pidx)
-                I.jamp("a2", c_close(col, c_leaf(c), cchi(d)), pidx)
-                I.jamp("a3", c_close(col, c_leaf(d), cchi(c)), pidx)
-                I.flush_jamps()
-                I.L("}")
+        # colour-ordered two-gluon currents: the pair current (a commutator, colour ab - ba) is folded into the two stepwise
+        # currents, on the row side before the common propagator and on the column side before the dot product; the nine
+        # diagram terms of this block become four colour-ordered amplitudes, one colour flow each
+        col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
+        assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
+        for col in (col_ab, col_ba):
+            assert not _cdiff(c_close(col, cpair(c, d), ONE), c_close(col, c_leaf(c), cchi(d)), c_close(col, c_leaf(d), cchi(c)))
+        I.L("const W4<R> sp = row_slash(ub, pab), xp = slash_col(pcd, vv);"); I.flops += FL["row_slash"] + FL["slash_col"]
+        I.L("const W4<R> rab = row_step(wadd(row_slash(q1a, eb), sp), q, mt, iq2), rba = row_step(wsub(row_slash(q1b, ea), sp), q, mt, iq2);")
+        I.flops += 2 * (FL["row_slash"] + 8 + FL["col_step"])
+        I.L("const W4<R> xcd = wadd(slash_col(ec, chid), xp), xdc = wsub(slash_col(ed, chic), xp);"); I.flops += 2 * (FL["slash_col"] + 8)
+        I.L("const Cx<R> a1 = row_col(rab, xcd), a2 = row_col(rab, xdc), a3 = row_col(rba, xcd), a4 = row_col(rba, xdc);"); I.flops += 4 * FL["row_col"]
+        I.jamp("a1", c_close(col_ab, c_leaf(c), cchi(d)), pidx)
+        I.jamp("a2", c_close(col_ab, c_leaf(d), cchi(c)), pidx)
+        I.jamp("a3", c_close(col_ba, c_leaf(c), cchi(d)), pidx)
+        I.jamp("a4", c_close(col_ba, c_leaf(d), cchi(c)), pidx)
+        I.namp += 5
+        I.flush_jamps()
         insts.append(I)
     add_group("rows2", insts)
     # ---- B3: q1(x) . pair(y,z)-slash . chi_w

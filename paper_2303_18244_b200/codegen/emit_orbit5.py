@@ -2,9 +2,9 @@
 120 colour flows.  Same ideas as emit_orbit.py (shapes looped over gluon relabellings with table-driven
 operands, two-sided quark line, bilinear / dual-current factorisations), plus what the size of the process forces:
 
-  * the diagrams are split across FIVE kernels (north_star: "splitting the diagrams across kernels"; three for the
-    three-gluon sub-trees, one for the 2+2 / 2+1 quark ends, one for four-gluon sub-trees made of pairs), each small
-    enough to stay in the instruction cache; every kernel loops over the helicities of the current chunk;
+  * the diagrams are split across THREE kernels (north_star: "splitting the diagrams across kernels": o0 the three-gluon
+    sub-trees, o1 the 2+2 / 2+1 quark ends, o2 the four-gluon sub-trees made of pairs); every kernel loops over the helicities
+    of the current chunk (ME_HEL_PER_CTA per CTA, grid.y over the chunk);
   * the 120 jamps do not fit on chip: each block instance accumulates the <= 36 colour flows it touches in
     per-thread shared-memory slots and adds them once into the global staging buffer gj[hel][flow][re/im][event]
     that the batched colour-sum kernel (csrc/color_sum.cu) contracts with the colour matrix.
@@ -25,28 +25,18 @@ NPAR = 7
 HEL_PER_CTA = 4  # helicities looped inside one CTA (csrc/multi.h ME_HEL_PER_CTA); the sharing kernels rely on the grouping of the list:
                  # entries 4 g .. 4 g + 3 share their gluon helicities (the four quark-helicity assignments, 255 = absent)
 T_BIT, TB_BIT = NPAR - 1 - 2, NPAR - 1 - 3
-BLOCK = 96       # threads per CTA of kernel o3 (290 FP64 slots per thread)
-MERGE_ORDERED = True  # two-gluon quark currents in colour-ordered form (pair current folded into the two stepwise ones)
-MERGE_TRIPLE = True  # three-gluon sub-trees as two colour-ordered currents (V4 pieces folded into their channels, Jacobi identity)
-MERGE_V3 = True   # fold the V3 closing of the last gluon into the two quark-end closings (colour: Q.w - w.Q)
-K2_DIRECT = True  # kernel o1: amplitude combinations go straight to the staging buffer instead of through local accumulators
-K3_JACC = 0      # local jamp accumulators of kernel o2; 0: every amplitude combination goes straight to the staging buffer (48 = one set per last gluon, 96 threads: measured equal in FP64, 4 % slower in FP32)
-K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over
-BLOCK1 = 128     # kernels o0..o2 and o4 (212 / 214 slots)
+# Measured and rejected variants are not kept as switches; what was tried and by how much it lost is in DESIGN.md section 8
+# (a 256-thread CTA with a barrier per scope for kernel o0; a nested (u, w) loop in kernel o0; the tensor-memory layout for the FP32
+# instantiations of o0 / o1; direct reductions instead of accumulators in kernel o2; accumulators instead of direct reductions in o1).
+K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees are spread over (1 as run; tests/test_abi_and_host.py
+                 # checks with 2 and 3 that the algorithmic flop count does not depend on the split)
+BLOCK1 = 128     # threads per CTA of every diagram kernel
 FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
-K1_SHARE_UW = False      # kernel o0: nested table-driven loop over the (u, w) halves of the closing vectors (8.5 k instead of 10.6 k SASS instructions);
-                         # re-measured with the tensor-memory kernels: FP64 94.0 vs 91.6 ms per pass, FP32 48.7 vs 46.5 ms: off
-K1_SYNC = False          # FP64 variant of kernel o0 (k_..._o0d): one 256-thread CTA, named barrier at every scope so that the eight warps fetch the
-                         # same instructions; measured 9.55 ms per chunk against 9.40 ms for two free-running 128-thread CTAs: off
-TM_FLOAT = False          # kernels o0 and o1 with their tensor-memory layout in FP32 as well (three CTAs per SM instead of two; the FP32 kernels need
-                          # only 128 - 160 registers): measured slower, o0 5.49 vs 4.57 ms and o1 2.86 vs 2.66 ms per chunk (FP32 pass 49.0 vs 44.6 ms): off
-K3D_FLOAT = True          # the accumulator variant of kernel o2 also serves FP32 (96 TMEM columns, shared memory as before: two CTAs per SM)
-K3D_JACC = 48            # FP64 variant of kernel o2 (own kernel, k_..._o2d): local accumulators, kept in tensor memory
-TM_K3 = ("J",)            # kernel o2 FP64: 48 local jamp accumulators (one set per last gluon) = 96 slots = 192 columns; ("PAIR",) with
-                          # K3_JACC = 0 gives two CTAs per SM but leaves the kernel bound by the L2 throughput of its 1320 RED pairs per helicity
+K3D_JACC = 48            # accumulator kernel o2d (current sharing off): one set of local jamp accumulators per last gluon, kept in tensor memory
+TM_K3 = ("J",)            # FP64: 96 slots = 192 columns, one CTA per SM; FP32: one column per slot, two CTAs per SM
 
 
 class Layout5:
@@ -157,14 +147,23 @@ class Inst5(Inst):
             self.flops += 2
         self.emit_accumulate(ups)
 
+    RED_BATCH = 8
+
     def flush_direct(self):
         """pending jamp updates go straight into the global staging buffer, one fire-and-forget reduction per colour flow
         (all amplitudes that feed a flow are combined in registers first).  For blocks in which a flow is touched once: a
         shared-memory accumulator there is a read-modify-write plus a flush for nothing."""
-        for sigma, u, z in self.grouped_updates():
-            re, im = self.unit_times(u, z)
-            self.L("{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)(%s)); atomicAdd(g + npad32, (RJ)(%s)); }" % (self.P(2 * sigma), re, im))
-            self.flops += 2
+        ups = self.grouped_updates()
+        # the row offsets come from the instance table (indexed constant loads, long latency) and feed integer address arithmetic:
+        # they are formed in batches ahead of the reductions that use them, so that the loads of a batch are in flight together
+        for b0 in range(0, len(ups), self.RED_BATCH):
+            batch = ups[b0:b0 + self.RED_BATCH]
+            self.L("{ const unsigned " + ", ".join("ro%d = (unsigned)%s * npad32" % (i, self.P(2 * sigma)) for i, (sigma, u, z) in enumerate(batch)) + ";")
+            for i, (sigma, u, z) in enumerate(batch):
+                re, im = self.unit_times(u, z)
+                self.L("  { RJ* g = gj + ro%d; atomicAdd(g, (RJ)(%s)); atomicAdd(g + npad32, (RJ)(%s)); }" % (i, re, im))
+                self.flops += 2
+            self.L("}")
 
     def inner_loop(self, name, inners):
         """nested table-driven loop over `inners` (Inst5(inner=True) objects of identical shape) inside this instance"""
@@ -249,7 +248,7 @@ def emit_pair(I, name, a, b, ea, eb, ka, kb):
 
 
 def emit_rows2(I, a, b, pab, ea, eb):
-    """the three row currents with gluons {a,b} attached (a<b): returns [(name, colour)]"""
+    """the two colour-ordered row currents with gluons {a,b} attached (a<b): returns [(name, colour)]"""
     if I.lay.Q1 is not None:
         I.ldw("q1a", I.lay.Q1 + 8 * a); I.ldw("q1b", I.lay.Q1 + 8 * b)
     else:                                 # no Q1 slots: the two one-gluon row currents are formed here
@@ -260,40 +259,31 @@ def emit_rows2(I, a, b, pab, ea, eb):
     I.qvec("qr", [a, b])
     I.L("const R iqr = %s;" % I.iq(a, b))
     I.fv("ub")
-    if MERGE_ORDERED:
-        # colour-ordered form: the pair current (a commutator, colour ab - ba) is folded into the two stepwise currents in
-        # front of their common propagator: two currents, one colour string each, instead of three
-        col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
-        assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
-        I.L("const W4<R> spr = row_slash(ub, %s);" % pab)
-        I.L("const W4<R> rb = row_step(wadd(row_slash(q1a, %s), spr), qr, mt, iqr), rc = row_step(wsub(row_slash(q1b, %s), spr), qr, mt, iqr);" % (eb, ea))
-        I.flops += 3 * FL5["row_slash"] + 2 * (FL5["wadd"] + FL5["col_step"])
-        return [("rb", col_ab), ("rc", col_ba)]
-    I.L("const W4<R> ra = quark_step2(ub, %s, qr, mt, iqr), rb = quark_step2(q1a, %s, qr, mt, iqr), rc = quark_step2(q1b, %s, qr, mt, iqr);" % (pab, eb, ea))
-    I.flops += 3 * FL5["quark_step2"]
-    return [("ra", c_step(ONE, cpair(a, b))), ("rb", c_step(cq1(a), c_leaf(b))), ("rc", c_step(cq1(b), c_leaf(a)))]
+    # colour-ordered form: the pair current (a commutator, colour ab - ba) is folded into the two stepwise currents in
+    # front of their common propagator: two currents, one colour string each, instead of three
+    col_ab, col_ba = c_step(cq1(a), c_leaf(b)), c_step(cq1(b), c_leaf(a))
+    assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
+    I.L("const W4<R> spr = row_slash(ub, %s);" % pab)
+    I.L("const W4<R> rb = row_step(wadd(row_slash(q1a, %s), spr), qr, mt, iqr), rc = row_step(wsub(row_slash(q1b, %s), spr), qr, mt, iqr);" % (eb, ea))
+    I.flops += 3 * FL5["row_slash"] + 2 * (FL5["wadd"] + FL5["col_step"])
+    return [("rb", col_ab), ("rc", col_ba)]
 
 
 def emit_cols2(I, c, d, pcd, ec, ed, tag=""):
-    """the three column currents with gluons {c,d} attached (c<d), grown from the t~ end"""
+    """the two colour-ordered column currents with gluons {c,d} attached (c<d), grown from the t~ end"""
     I.ldw("chc" + tag, I.lay.CHI + 8 * c); I.ldw("chd" + tag, I.lay.CHI + 8 * d)
     row_side = rest_of(c, d)
     I.qvec("qc" + tag, row_side)
     I.L("const R iqc%s = %s;" % (tag, I.iq(*row_side)))
     I.fv("vv")
-    if MERGE_ORDERED:
-        col_cd, col_dc = c_step(c_leaf(c), cchi(d)), c_step(c_leaf(d), cchi(c))
-        assert not _cdiff(c_step(cpair(c, d), ONE), col_cd, col_dc)
-        I.L("const W4<R> spc%s = slash_col(%s, vv);" % (tag, pcd))
-        I.L("const W4<R> cb%s = col_step(wadd(slash_col(%s, chd%s), spc%s), qc%s, mt, iqc%s), cc%s = col_step(wsub(slash_col(%s, chc%s), spc%s), qc%s, mt, iqc%s);"
-            % (tag, ec, tag, tag, tag, tag, tag, ed, tag, tag, tag, tag))
-        I.flops += 3 * FL5["slash_col"] + 2 * (FL5["wadd"] + FL5["col_step"])
-        return [("cb" + tag, col_cd), ("cc" + tag, col_dc)]
-    I.L("const W4<R> ca%s = col_step(slash_col(%s, vv), qc%s, mt, iqc%s), cb%s = col_step(slash_col(%s, chd%s), qc%s, mt, iqc%s),"
-        " cc%s = col_step(slash_col(%s, chc%s), qc%s, mt, iqc%s);" % (tag, pcd, tag, tag, tag, ec, tag, tag, tag, tag, ed, tag, tag, tag))
-    I.flops += 3 * (FL5["slash_col"] + FL5["col_step"])
-    # colour of a column step: -(gluon)(previous column)
-    return [("ca" + tag, c_step(cpair(c, d), ONE)), ("cb" + tag, c_step(c_leaf(c), cchi(d))), ("cc" + tag, c_step(c_leaf(d), cchi(c)))]
+    # colour of a column step: -(gluon)(previous column); colour-ordered as in emit_rows2
+    col_cd, col_dc = c_step(c_leaf(c), cchi(d)), c_step(c_leaf(d), cchi(c))
+    assert not _cdiff(c_step(cpair(c, d), ONE), col_cd, col_dc)
+    I.L("const W4<R> spc%s = slash_col(%s, vv);" % (tag, pcd))
+    I.L("const W4<R> cb%s = col_step(wadd(slash_col(%s, chd%s), spc%s), qc%s, mt, iqc%s), cc%s = col_step(wsub(slash_col(%s, chc%s), spc%s), qc%s, mt, iqc%s);"
+        % (tag, ec, tag, tag, tag, tag, tag, ed, tag, tag, tag, tag))
+    I.flops += 3 * FL5["slash_col"] + 2 * (FL5["wadd"] + FL5["col_step"])
+    return [("cb" + tag, col_cd), ("cc" + tag, col_dc)]
 
 
 def phase_a(lay, stride, add_group, want_pairs):
@@ -334,7 +324,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
+def build_k1(stride, pidx, part=None, nparts=3):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
@@ -354,15 +344,11 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
         # the six three-gluon terms on M (registers for the whole block); their inputs die in this scope
         tcol = [c_v3(cpair(a, b), c_leaf(c)), c_v3(cpair(a, c), c_leaf(b)), c_v3(cpair(b, c), c_leaf(a))] + \
                [c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c)) for k in range(3)]
-        if MERGE_TRIPLE:
-            # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three
-            # channels, and the Jacobi identity col1 = col0 + col2 leaves two independent currents instead of six terms
-            assert all(not _cdiff(tcol[3 + k], tcol[k], {}) for k in range(3)) and not _cdiff(tcol[1], tcol[0], {st: -v for st, v in tcol[2].items()})
-            tnames, tcol = ["s0", "s2"], [tcol[0], tcol[2]]
-            I.L("W4<R> s0, s2; P4<R> kM;")
-        else:
-            tnames = ["t%d" % k for k in range(6)]
-            I.L("W4<R> t0, t1, t2, t3, t4, t5; P4<R> kM;")
+        # colour-ordered form of the three-gluon sub-tree: the four-gluon-vertex pieces carry the colours of the three
+        # channels, and the Jacobi identity col1 = col0 + col2 leaves two independent currents instead of six terms
+        assert all(not _cdiff(tcol[3 + k], tcol[k], {}) for k in range(3)) and not _cdiff(tcol[1], tcol[0], {st: -v for st, v in tcol[2].items()})
+        tnames, tcol = ["s0", "s2"], [tcol[0], tcol[2]]
+        I.L("W4<R> s0, s2; P4<R> kM;")
         I.L("{")
         for nm, l in (("ea", a), ("eb", b), ("ec", c)):
             I.leaf(nm, l)
@@ -375,15 +361,10 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
         I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once (as pxy of its own block) would do
         I.L("const R ik3 = %s;" % I.ik2(a, b, c))
         I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
-        if MERGE_TRIPLE:
-            I.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
-            I.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
-            I.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
-            I.flops += 5 * FL5["wadd"]
-        else:
-            I.L("t0 = v3_current(pab, ec, kab, kc, ik3); t1 = v3_current(pac, eb, kac, kb, ik3); t2 = v3_current(pbc, ea, kbc, ka, ik3);")
-            I.L("t3 = v4_current(0, dots, ea, eb, ec); t4 = v4_current(1, dots, ea, eb, ec); t5 = v4_current(2, dots, ea, eb, ec);")
-        I.flops += 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
+        I.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
+        I.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
+        I.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
+        I.flops += 5 * FL5["wadd"] + 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
         I.L("}")
         if part is not None and part > 0:             # the split kernels each rebuild pxy and the six terms: all of it overhead
             I.redundant = I.flops
@@ -396,7 +377,7 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             idx = counter[0]; counter[0] += 1
             if part is not None and idx // (18 // nparts) != part:
                 return
-            T.L("{ if (sizeof(R) == 8) ME_FENCE; ME_SCOPE_SYNC;")      # FP64 only: stops load hoisting that would spill
+            T.L("{ if (sizeof(R) == 8) ME_FENCE;")      # FP64 only: stops load hoisting that would spill
             for fn in prelude:
                 fn(T)
             T.fv(*[nm for nm in ("ub", "vv", "jtt") if nm in xexpr])
@@ -445,26 +426,18 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             fetch = lambda nm: (lambda T_: T_.ldw(nm, lay.TMP))
             T.L("{"); mk_chi("chw", w, ew)(T); park("chw")(T); T.L("}")
             # quad = V3(t, eps_u) closing three ways with the last gluon w: on the t~ end (colour Q.w), on the t end (w.Q), or through a
-            # three-gluon vertex on the bare line (colour Q.w - w.Q).  MERGE_V3 folds the current of the third, y3, into the
-            # other two: two scopes instead of three
+            # three-gluon vertex on the bare line (colour Q.w - w.Q): the current of the third, y3, is folded into the other two
+            # (two scopes instead of three)
             y3 = lambda T_: (T_.fv("jtt"), T_.L("const W4<R> y3 = v3_dual(%s, jtt, padd(kM, %s), %s, ik5);" % (ew, ku, kw)))
-            if MERGE_V3:
-                dots_with(T, [fetch("chw"), ik4, y3], "v3_dual(%s, wadd(bilinear(ub, chw), y3), kM, %s, ik4)" % (eu, ku),
-                          2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(ONE, quad(col), cchi(w)))
-                dots_with(T, [mk_q1("q1w", w, ew), ik4, y3], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
-                          2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(cq1(w), quad(col), ONE))
-                idx3 = counter[0]; counter[0] += 1
-                if part is None or idx3 // (18 // nparts) == part:
-                    T.namp += 6                   # the six V3-closing terms are inside the twelve above
-                if part is None or (idx3 - 1) // (18 // nparts) == part:
-                    T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
-            else:
-                dots_with(T, [fetch("chw"), ik4], "v3_dual(%s, bilinear(ub, chw), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                          lambda col: c_close(ONE, quad(col), cchi(w)))
-                dots_with(T, [mk_q1("q1w", w, ew), ik4], "v3_dual(%s, bilinear(q1w, vv), kM, %s, ik4)" % (eu, ku), FL5["v3_dual"] + FL5["bilinear"],
-                          lambda col: c_close(cq1(w), quad(col), ONE))
-                dots_with(T, [ik4], "v3_dual(%s, v3_dual(%s, jtt, padd(kM, %s), %s, ik5), kM, %s, ik4)" % (eu, ew, ku, kw, ku), 2 * FL5["v3_dual"] + 4,
-                          lambda col: c_close(ONE, c_v3(quad(col), c_leaf(w)), ONE))
+            dots_with(T, [fetch("chw"), ik4, y3], "v3_dual(%s, wadd(bilinear(ub, chw), y3), kM, %s, ik4)" % (eu, ku),
+                      2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(ONE, quad(col), cchi(w)))
+            dots_with(T, [mk_q1("q1w", w, ew), ik4, y3], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
+                      2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(cq1(w), quad(col), ONE))
+            idx3 = counter[0]; counter[0] += 1
+            if part is None or idx3 // (18 // nparts) == part:
+                T.namp += 6                   # the six V3-closing terms are inside the twelve above
+            if part is None or (idx3 - 1) // (18 // nparts) == part:
+                T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
             # ubar . t-slash . chi2: eps_u attached to chi1(w)
             dots_with(T, [qc, fetch("chw")], "bilinear(ub, col_step(slash_col(%s, chw), qc, mt, iqc))" % eu, stc,
                       lambda col: c_close(ONE, col, c_step(c_leaf(u), cchi(w))))
@@ -475,21 +448,8 @@ def build_k1(stride, pidx, part=None, nparts=3, share_uw=False):
             dots_with(T, [qr, fetch("q1u")], "bilinear(quark_step2(q1u, %s, qr, mt, iqr), vv)" % ew, str_,
                       lambda col: c_close(c_step(cq1(u), c_leaf(w)), col, ONE))
 
-        if share_uw:
-            # one nested table-driven loop of two iterations instead of two copies of six scopes; its jamp updates go to the
-            # block's accumulators.  Measured: 10.6 k -> 8.5 k SASS instructions, but the table-driven operand and accumulator
-            # offsets cost more than the instruction fetch they save (FP64 150 ms vs 144 ms per 65536 events): off by default
-            inners = []
-            for (u, w) in ((x, y), (y, x)):
-                J = Inst5(lay, stride, inner=True, parent=I)
-                J.leaf("eu", u); J.leaf("ew", w); J.kvec("ku", [u]); J.kvec("kw", [w])
-                J.redundant += J.flops                # ex, ey, kx, ky exist in the block
-                uw_vectors(J, u, w, "eu", "ew", "ku", "kw")
-                inners.append(J)
-            I.inner_loop("uw", inners)
-        else:
-            uw_vectors(I, x, y, "ex", "ey", "kx", "ky")
-            uw_vectors(I, y, x, "ey", "ex", "ky", "kx")
+        uw_vectors(I, x, y, "ex", "ey", "kx", "ky")
+        uw_vectors(I, y, x, "ey", "ex", "ky", "kx")
         # V3(t, pair(x,y)) on the bare line
         dots_with(I, [], "v3_dual(pxy, jtt, kM, padd(kx, ky), ik5)", FL5["v3_dual"] + 4, lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
         # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
@@ -529,8 +489,9 @@ def spair(p):
 # ------------------------------------------------------------------------------------------
 def build_k2(stride, pidx):
     # 226 slots per thread -> 128 threads per CTA: no Q1 slots (the row-side one-gluon currents are formed where they are
-    # used: 5 per ten uses would do, +14 % flops), only the pair propagators, 8 local jamp accumulators flushed per sub-block
-    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=0 if K2_DIRECT else 8, want_q1chi=False, want_chi=True, ik2_sizes=(2,), tm=TM_K2)
+    # used: 5 per ten uses would do, +14 % flops), only the pair propagators; no local jamp accumulators: every (sub-)block touches each
+    # colour flow once, its amplitudes are combined per flow in registers and added straight into the staging buffer
+    lay = Layout5(want_pairs=True, want_iq_mid=True, jacc=0, want_q1chi=False, want_chi=True, ik2_sizes=(2,), tm=TM_K2)
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
@@ -554,28 +515,19 @@ def build_k2(stride, pidx):
             I.namp += (9 - len(rows) * len(cols)) + (3 - len(rows))     # diagram terms folded into the colour-ordered currents
             xs = ["x%d" % k for k in range(len(cols))]
             I.L("const W4<R> " + ", ".join("%s = slash_col(em, %s)" % (xn, cn) for xn, (cn, _) in zip(xs, cols)) + ";"); I.flops += len(cols) * FL5["slash_col"]
-            for ri, (rn, rcol) in enumerate(rows):
-                if K2_DIRECT:       # the amplitudes of this sub-block are combined per colour flow and added once
-                    I.L("const Cx<R> " + ", ".join("a%d_%d = row_col(%s, %s)" % (k, ri, rn, xn) for k, xn in enumerate(xs)) + ";"); I.flops += len(xs) * FL5["row_col"]
-                    for k, (cn, ccol) in enumerate(cols):
-                        I.jamp("a%d_%d" % (k, ri), c_close(rcol, c_leaf(m), ccol), pidx)
-                    continue
-                I.L("{ const Cx<R> " + ", ".join("a%d = row_col(%s, %s)" % (k, rn, xn) for k, xn in enumerate(xs)) + ";"); I.flops += len(xs) * FL5["row_col"]
+            for ri, (rn, rcol) in enumerate(rows):       # the amplitudes of this sub-block are combined per colour flow and added once
+                I.L("const Cx<R> " + ", ".join("a%d_%d = row_col(%s, %s)" % (k, ri, rn, xn) for k, xn in enumerate(xs)) + ";"); I.flops += len(xs) * FL5["row_col"]
                 for k, (cn, ccol) in enumerate(cols):
-                    I.jamp("a%d" % k, c_close(rcol, c_leaf(m), ccol), pidx)
-                I.flush_jamps()
-                I.L("}")
+                    I.jamp("a%d_%d" % (k, ri), c_close(rcol, c_leaf(m), ccol), pidx)
             # (2,2,1): rows . pair(c,d)-slash . chi1(m)
             I.ldw("chm", lay.CHI + 8 * m)
             I.L("const W4<R> xp = slash_col(pcd, chm);"); I.flops += FL5["slash_col"]
             I.L("{ const Cx<R> " + ", ".join("a%d = row_col(%s, xp)" % (k, rn) for k, (rn, _) in enumerate(rows)) + ";"); I.flops += len(rows) * FL5["row_col"]
             for k, (rn, rcol) in enumerate(rows):
                 I.jamp("a%d" % k, c_close(rcol, cpair(c, d), cchi(m)), pidx)
-            I.flush_direct() if K2_DIRECT else I.flush_jamps()
+            I.flush_direct()
             I.L("}")
             I.L("}")
-            if not K2_DIRECT:
-                I.flush_global()
         insts.append(I)
     add_group("rows2", insts, 1)
     # ---- cols2 loop: B = {c,d}; q1(x) . pair(P)-slash . chi2(B)
@@ -599,10 +551,8 @@ def build_k2(stride, pidx):
             I.L("const Cx<R> " + ", ".join("a%d = row_col(r, %s)" % (k, cn) for k, (cn, _) in enumerate(cols)) + ";"); I.flops += len(cols) * FL5["row_col"]
             for k, (cn, ccol) in enumerate(cols):
                 I.jamp("a%d" % k, c_close(cq1(x), cpair(*p), ccol), pidx)
-            I.flush_direct() if K2_DIRECT else I.flush_jamps()
+            I.flush_direct()
             I.L("}")
-            if not K2_DIRECT:
-                I.flush_global()
         insts.append(I)
     add_group("cols2", insts, 1)
     return lay, groups
@@ -629,26 +579,18 @@ def build_k3(stride, pidx, jacc=0, tm=()):
         I.redundant += I.flops - f0                    # kernel 2 forms the same ten currents
         I.L("const R ik4 = %s;" % I.ik2(*quad))
         # the last gluon w closes a sub-tree Q three ways: on the t~ end (colour Q.w), on the t end (w.Q), or through a three-gluon
-        # vertex on the bare line, whose colour is the commutator Q.w - w.Q: its current x3 is folded into the other two
-        # (MERGE_V3), which leaves two dot products and two jamp groups per sub-tree term instead of three
+        # vertex on the bare line, whose colour is the commutator Q.w - w.Q: its current x3 is folded into the other two,
+        # which leaves two dot products and two jamp groups per sub-tree term instead of three
         I.L("const W4<R> x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
-        if MERGE_V3:
-            I.L("const W4<R> x1 = wadd(bilinear(ub, chw), x3), x2 = wsub(bilinear(q1w, vv), x3);"); I.flops += 2 * FL5["wadd"]
-        else:
-            I.L("const W4<R> x1 = bilinear(ub, chw), x2 = bilinear(q1w, vv);")
-        I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"]
+        I.L("const W4<R> x1 = wadd(bilinear(ub, chw), x3), x2 = wsub(bilinear(q1w, vv), x3);")
+        I.flops += 2 * FL5["wadd"] + 2 * FL5["bilinear"] + FL5["v3_dual"]
 
     def close3(I, w, tname, col, k=""):
-        """amplitudes of one four-gluon sub-tree term with the three ends; the caller flushes"""
-        if MERGE_V3:
-            I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2);" % (k, tname, k, tname)); I.flops += 2 * FL5["wdot"]
-            I.namp += 1                 # the V3 closing is inside a1 and a2
-        else:
-            I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2), a3%s = wdot(%s, x3);" % (k, tname, k, tname, k, tname)); I.flops += 3 * FL5["wdot"]
+        """amplitudes of one four-gluon sub-tree term with the two ends (the V3 closing on the bare line is inside both); the caller flushes"""
+        I.L("const Cx<R> a1%s = wdot(%s, x1), a2%s = wdot(%s, x2);" % (k, tname, k, tname)); I.flops += 2 * FL5["wdot"]
+        I.namp += 1                 # the V3 closing is inside a1 and a2
         I.jamp("a1%s" % k, c_close(ONE, col, cchi(w)), pidx)
         I.jamp("a2%s" % k, c_close(cq1(w), col, ONE), pidx)
-        if not MERGE_V3:
-            I.jamp("a3%s" % k, c_close(ONE, c_v3(col, c_leaf(w)), ONE), pidx)
 
     # one instance per last gluon w: the three end vectors are formed once, then two nested table-driven loops run over the
     # 3 + 6 four-gluon sub-trees (unrolled they were ~8 k instructions and instruction-fetch bound; as 45 independent small
@@ -863,11 +805,10 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, sync=False, delegate_all=False):
-    """only: None (float and double instances of one template), 'double' (FP64-only variant; ki is then a tag like '2d');
-    delegate_double: tag of the FP64-only variant this kernel's launcher hands double / mixed precision to;
-    sync: one 256-thread CTA per SM whose eight warps meet at a named barrier at every scope of the loop bodies, so that they
-    fetch the same instructions (two independent 128-thread CTAs drift apart and thrash the instruction cache)"""
+def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
+    """only: None (FP64 instances with part of the slots in tensor memory or all in shared memory, FP32 in shared memory) or 'tm' (every
+    instance in its tensor-memory layout; ki is then a tag like '2d'); delegate: tag of the tensor-memory variant this kernel's
+    launcher hands every precision to unless ME_NO_TMEM=1"""
     src = []
     S = src.append
 
@@ -892,7 +833,6 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
     if tm0 is not None:
         assert BLOCK in (128, 256)
         S("#define ME_TM_SLOT0 %d" % tm0)
-    S("#define ME_SCOPE_SYNC %s" % ('asm volatile("bar.sync 1, %0;" ::"r"(nlive) : "memory")' if sync else ""))
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("#include \"multi.h\"")
@@ -925,9 +865,6 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("    tm_base = tm_alloc(&tm_slot, tm_cols * %d);" % (BLOCK // 128))
         S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16) + (threadIdx.x >> 7) * tm_cols;      // this warp's quarter of the 128 lanes (and half of the columns)")
         S("  }")
-    if sync:
-        S("  const long left = npad - (long)blockIdx.x * blockDim.x;")
-        S("  const unsigned nlive = (unsigned)(left < (long)blockDim.x ? left : (long)blockDim.x);      // threads of the live warps (npad is a multiple of 32)")
     S("  const R mt = (R)mt_d;")
     S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 65536 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
@@ -984,10 +921,10 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
     if tm0 is not None:
         S("  if constexpr (TM) tm_free(tm_base, (sizeof(R) == 8 ? %du : %du) * %d);" % (lay.tm_cols, max(32, lay.tm_cols // 2), BLOCK // 128))
     S("}")
-    if delegate_double is not None:
-        S("extern const MultiKernel mk_%s_o%s;" % (name, delegate_double))
+    if delegate is not None:
+        S("extern const MultiKernel mk_%s_o%s;" % (name, delegate))
     S("static cudaError_t launch_o%s(int precision, const MultiArgs& a) {" % ki)
-    S("  // few helicities per CTA: many short CTAs, so the last partial wave costs little (65536 events are only 4.6 waves of 96-thread CTAs)")
+    S("  // few helicities per CTA: many short CTAs, so the last partial wave costs little")
     S("  const dim3 grid((unsigned)((a.npad + %d - 1) / %d), (unsigned)((a.nh + ME_HEL_PER_CTA - 1) / ME_HEL_PER_CTA));" % (BLOCK, BLOCK))
     NO_TMEM = "    static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // A/B timing: shared-memory-only kernels"
     def launch_line(inst, smem, cast):
@@ -996,13 +933,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         S("      k_%s_o%s<%s><<<grid, %d, %s, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (%s*)a.gj, a.hel_per_event, a.n);" % (name, ki, inst, BLOCK, smem, cast))
     S("  const size_t smf = sizeof(float) * %d * %d, smd = sizeof(double) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK, lay.nslots, BLOCK, tm0 or 0, BLOCK))
     S("  (void)smf; (void)smd; (void)smt;")
-    if only == "double":
-        assert tm0 is not None
-        S("  if (precision == 2) return cudaErrorInvalidValue;")
-        S("  {")
-        launch_line("double, double, true", "smt", "double")
-        S("  }")
-    elif only == "tm":
+    if only == "tm":
         assert tm0 is not None
         S("  const size_t smtf = sizeof(float) * %d * %d;" % (tm0, BLOCK))
         S("  if (precision == 2) {")
@@ -1011,20 +942,12 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate_double=None, s
         launch_line("double, double, true", "smt", "double")
         S("  }")
     else:
-        if delegate_double is not None:
+        if delegate is not None:
             S(NO_TMEM)
-            S("  if (%s!no_tmem) return mk_%s_o%s.launch(precision, a);     // the variant with local accumulators in tensor memory" % ("" if delegate_all else "precision != 2 && ", name, delegate_double))
-        if tm0 is not None and delegate_double is None:
+            S("  if (!no_tmem) return mk_%s_o%s.launch(precision, a);     // the variant with local accumulators in tensor memory" % (name, delegate))
+        if tm0 is not None and delegate is None:
             S(NO_TMEM)
         S("  if (precision == 2) {")
-        if tm0 is not None and TM_FLOAT:
-            # FP32 kernels need 128 - 160 registers: with part of the slots in tensor memory (one column each) shared memory no longer
-            # limits them to two CTAs per SM
-            S("    const size_t smtf = sizeof(float) * %d * %d;" % (tm0, BLOCK))
-            S("    if (!no_tmem) {")
-            launch_line("float, float, true", "smtf", "float")
-            S("      return cudaGetLastError();")
-            S("    }")
         launch_line("float, float, false", "smf", "float")
         S("  } else {")
         if tm0 is not None:
@@ -1051,24 +974,16 @@ def emit_orbit5_process(name="gg_ttxggg"):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     files, kinfo = {}, []
-    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS, share_uw=K1_SHARE_UW)) for i in range(K1_PARTS)) + (build_k2, build_k3)
-    blocks = (BLOCK1,) * (len(builders) - 1) + (BLOCK if (K3_JACC and not TM_K3) else BLOCK1,)
+    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
     for ki, b in enumerate(builders):
-        lay, groups = b(blocks[ki], pidx)
+        lay, groups = b(BLOCK1, pidx)
         last = ki == len(builders) - 1
-        k1_sync = K1_SYNC and K1_PARTS == 1 and ki == 0
-        src, info = emit_kernel(name, ki, lay, groups, blocks[ki], delegate_double="%dd" % ki if ((last and K3D_JACC) or k1_sync) else None,
-                                delegate_all=last and K3D_JACC and K3D_FLOAT)
+        src, info = emit_kernel(name, ki, lay, groups, BLOCK1, delegate="%dd" % ki if last else None)
         files["gen_%s_o%d.cu" % (name, ki)] = src
         kinfo.append(info)
-        if k1_sync:                # FP64-only variant of kernel o0: one 256-thread CTA per SM, warps kept in step by scope barriers
-            lay2, groups2 = build_k1(256, pidx, 0, 1)
-            src2, info2 = emit_kernel(name, "0d", lay2, groups2, 256, only="double", sync=True)
-            files["gen_%s_o0d.cu" % name] = src2
-            info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, block=256)
-        if last and K3D_JACC:      # FP64-only variant of the last kernel: local jamp accumulators in tensor memory (see TM_K3)
+        if last:      # variant of the last kernel with local jamp accumulators in tensor memory (see TM_K3); the plain one is its ME_NO_TMEM=1 fallback
             lay2, groups2 = build_k3(BLOCK1, pidx, jacc=K3D_JACC, tm=TM_K3)
-            src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="tm" if K3D_FLOAT else "double")
+            src2, info2 = emit_kernel(name, "%dd" % ki, lay2, groups2, BLOCK1, only="tm")
             files["gen_%s_o%dd.cu" % (name, ki)] = src2
             info["fp64_variant"] = dict(slots=lay2.nslots, tm_slot0=lay2.TM0, tm_cols=lay2.tm_cols, flops=info2["flops"], redundant=info2["redundant"])
     # sharing form of the last kernel (build_k3s): used when the helicity list is grouped by gluon helicities (ME_OPT_SHARE_CURRENTS)
@@ -1085,12 +1000,9 @@ def emit_orbit5_process(name="gg_ttxggg"):
     head = 2 * FL5["spinor"] + FL5["bilinear"]
     executed = sum(k["flops"] for k in kinfo) + len(kinfo) * head + cs_executed
     # algorithmic: every current once -> drop the tagged recomputation and the repeated phase A / spinors of kernels 2,3
-    phase_a_repeat = 0
-    for k, b in zip(kinfo, builders):
-        pass
     # the pairs, q1 and chi1 loops as they would run once (reference layout with all slots)
     ref_groups = []
-    phase_a(Layout5(want_pairs=True, want_iq_mid=True, jacc=12), BLOCK, _grouper(ref_groups), want_pairs=True)
+    phase_a(Layout5(want_pairs=True, want_iq_mid=True, jacc=12), BLOCK1, _grouper(ref_groups), want_pairs=True)
     pa = {g: t.flops * len(rows) for g, t, rows, _ in ref_groups}
     # needed once: the 10 pairs (untagged as pxy of the first kernel; kernels 2 and 3 both run the pairs loop again), the 5 + 5
     # one-gluon quark currents (chi1: kernel 2's loop; q1: every use is a tagged rebuild, so one set is taken back out of the
@@ -1133,6 +1045,6 @@ def emit_orbit5_process(name="gg_ttxggg"):
     S("}  // namespace me")
     files["gen_%s_table.cu" % name] = "\n".join(src) + "\n"
     info = dict(n=N, ndiagrams=1240, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=algo,
-                flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK,
+                flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK1,
                 flops_shared_event=shared_event, flops_executed_per_helicity_shared=executed_shared, kernel_o2s=info3)
     return files, info
