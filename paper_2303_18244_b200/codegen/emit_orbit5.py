@@ -664,7 +664,7 @@ NU_SMEM = 2          # colour-ordered currents per last gluon kept in shared mem
 
 
 def build_k3s(stride, pidx):
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=0, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "U"), nu=6, nu_smem=NU_SMEM)
+    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "U"), nu=6, nu_smem=NU_SMEM)      # jacc: the 24 ordered contact amplitudes
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)          # the ten pair currents: gluon helicities only, once per group
@@ -752,22 +752,63 @@ def build_k3s(stride, pidx):
         I.flush_direct()
         insts.append(I)
     add_group("quads", insts, 1)
-    # ---- V4(pair, pair', eps_m) on the bare line
-    insts = []
-    for m in range(N):
-        quad = rest_of(m)
-        a0 = quad[0]
-        for b0 in quad[1:]:
-            p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
-            I = Inst5(lay, stride)
-            I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.leaf("em", m)
-            I.L("const V4Dots<R> dots = v4_dots(p1, p2, em, %s);" % I.ik2(*range(N))); I.flops += FL5["v4_dots"]
-            for k in range(3):
-                I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, p1, p2, em), jtt);" % (k, k)); I.flops += FL5["v4_current"] + FL5["wdot"]
-                I.jamp("b%d" % k, c_close(ONE, c_v4(k, cpair(*p1), cpair(*p2), c_leaf(m)), ONE), pidx)
-            I.flush_direct()
-            insts.append(I)
-    add_group("pair_pair_v4", insts, 1)
+    # ---- V4(pair, pair', eps_m) on the bare line.  Their 45 colour factors are multilinear Lie polynomials in the five generators: expanded
+    # on the 24 left-normed brackets E_rho = [[[[0, r1], r2], r3], r4] (coefficient = coefficient of the string 0 r1 r2 r3 r4) the 45 amplitudes
+    # add up to 24 ordered amplitudes Z_rho, accumulated in shared memory (table-driven slots), and every one of the 120 colour flows leaves
+    # with ONE reduction pair as a combination of the Z_rho that contain it (360 pairs per helicity before: the reductions, not the arithmetic,
+    # bound this kernel: 4.7 TB/s of reduction payload into the L2 in FP64 and FP32 alike)
+    rhos = list(permutations((1, 2, 3, 4)))
+    ebasis = [c_v3(c_v3(c_v3(c_v3(c_leaf(0), c_leaf(q[0])), c_leaf(q[1])), c_leaf(q[2])), c_leaf(q[3])) for q in rhos]
+    assert all(E[(0,) + q] == 1 for E, q in zip(ebasis, rhos))
+    for m_class in (True, False):               # m = gluon 0 (three instances) / m != 0 (twelve): two shapes of the update pattern
+        insts = []
+        for m in range(N):
+            if (m == 0) != m_class:
+                continue
+            quad = rest_of(m)
+            a0 = quad[0]
+            for b0 in quad[1:]:
+                p1 = (a0, b0); p2 = spair([l for l in quad if l not in p1])
+                I = Inst5(lay, stride)
+                I.ldw("p1", lay.PAIR[p1]); I.ldw("p2", lay.PAIR[p2]); I.leaf("em", m)
+                I.L("const V4Dots<R> dots = v4_dots(p1, p2, em, %s);" % I.ik2(*range(N))); I.flops += FL5["v4_dots"]
+                ups = []
+                for k in range(3):
+                    I.L("const Cx<R> b%d = wdot(v4_current(%d, dots, p1, p2, em), jtt);" % (k, k)); I.flops += FL5["v4_current"] + FL5["wdot"]
+                    X = c_v4(k, cpair(*p1), cpair(*p2), c_leaf(m))
+                    alpha = [X.get((0,) + q, 0) for q in rhos]
+                    chk = {}
+                    for al, E in zip(alpha, ebasis):
+                        for st, v in E.items():
+                            chk[st] = chk.get(st, 0) + al * v
+                    assert not _cdiff(X, chk, {}) and all(al in (0, 1, -1) for al in alpha)
+                    for sign in (1, -1):             # plus terms first: the same code for every instance of the class, the slots from the table
+                        for r, al in enumerate(alpha):
+                            if al == sign:
+                                o = I.P(eo(lay.J + 2 * r, stride))
+                                ups.append((o, "%sb%d.re" % ("" if sign > 0 else "-", k), "%sb%d.im" % ("" if sign > 0 else "-", k)))
+                                I.flops += 2
+                    I.namp += 1
+                I.jamp_codes.extend(1 if u[1].startswith("-") else 0 for u in ups)     # (shape check of the looped instances)
+                # an ordered amplitude may receive several of the three terms of one instance: its updates must not be split over batches that
+                # read before an earlier one has written; batches of distinct slots only
+                seen, batch = set(), []
+                for u_ in ups:
+                    slot = I.params[int(u_[0][3:-1])]
+                    if slot in seen:
+                        I.emit_accumulate(batch); seen, batch = set(), []
+                    seen.add(slot); batch.append(u_)
+                I.emit_accumulate(batch)
+                insts.append(I)
+        add_group("contact_m0" if m_class else "contact", insts, 1)
+    I = Inst5(lay, stride)
+    for r in range(24):
+        I.L("R zr%d, zi%d; cget<R>(sm + %d, zr%d, zi%d); cset<R>(sm + %d, (R)0, (R)0);" % (r, r, eo(lay.J + 2 * r, stride), r, r, eo(lay.J + 2 * r, stride)))
+        I.L("const Cx<R> Z%d = {zr%d, zi%d};" % (r, r, r))
+        I.jamp("Z%d" % r, c_close(ONE, ebasis[r], ONE), pidx)
+    I.namp -= 24
+    I.flush_direct()
+    add_group("contact_flush", [I], 1)
     return lay, groups
 
 
