@@ -25,7 +25,8 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 N = 4
 NPAR = 6
 NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
-NSCVEC = 14         # and the six colour-ordered four-gluon currents that close on the bare quark line
+NSCVEC_QUAD_END = 14  # the six colour-ordered four-gluon currents that close on the bare quark line,
+NSCVEC = 26         # and the two column-side combinations of each of the six rows2 instances
 FL = dict(FLOPS, col_step=63, quark_step2=127, v3_dual=158)
 # The amplitudes are formed in colour-ordered combinations throughout (each is still a sum of whole diagram terms): two-gluon quark currents
 # with the pair current folded into the two stepwise ones; the V3 closing of the last gluon folded into the two quark-end closings
@@ -469,13 +470,26 @@ def build_groups(stride):
     add_group("triples", insts)
     # ---- B2: the three row currents with gluons {a,b} attached, each closing three ways on {c,d}
     insts = []
-    for (a, b) in lay.PAIR:
+    for ri, (a, b) in enumerate(lay.PAIR):
         c, d = [l for l in labels if l not in (a, b)]
         I = Inst(lay, stride)
-        I.leaf("ea", a); I.leaf("eb", b); I.leaf("ec", c); I.leaf("ed", d)
-        I.ldw("pab", lay.PAIR[(a, b)]); I.ldw("pcd", lay.PAIR[(c, d)])
-        I.ldw("q1a", lay.Q1 + 8 * a); I.ldw("q1b", lay.Q1 + 8 * b)
+        # the two column-side combinations depend on the t~ helicity and the gluons c, d only: the sharing kernel parks them in its scratch
+        I.L("W4<R> xcd, xdc;")
+        I.begin_cond(dep_mask([c, d], tb=True))
+        I.leaf("ec", c); I.leaf("ed", d)
+        I.ldw("pcd", lay.PAIR[(c, d)])
         I.ldw("chic", lay.CHI + 8 * c); I.ldw("chid", lay.CHI + 8 * d)
+        I.L("const W4<R> xp = slash_col(pcd, vv);"); I.flops += FL["slash_col"]
+        I.L("xcd = wadd(slash_col(ec, chid), xp); xdc = wsub(slash_col(ed, chic), xp);"); I.flops += 2 * (FL["slash_col"] + 8)
+        vec = I.P(NSCVEC_QUAD_END + 2 * ri)
+        I.L("if constexpr (SH) { sc_stw<R>(sc, %s, xcd); sc_stw<R>(sc, %s + 1, xdc); }" % (vec, vec))
+        I.end_cond(close=False)
+        I.L("} else {")
+        I.L("  xcd = sc_ldw<R>(sc, %s); xdc = sc_ldw<R>(sc, %s + 1);" % (vec, vec))
+        I.L("}")
+        I.leaf("ea", a); I.leaf("eb", b)
+        I.ldw("pab", lay.PAIR[(a, b)])
+        I.ldw("q1a", lay.Q1 + 8 * a); I.ldw("q1b", lay.Q1 + 8 * b)
         I.qvec("q", [a, b])
         I.L("const R iq2 = %s;" % I.iq(a, b))
         # colour-ordered two-gluon currents: the pair current (a commutator, colour ab - ba) is folded into the two stepwise
@@ -485,10 +499,9 @@ def build_groups(stride):
         assert not _cdiff(c_step(ONE, cpair(a, b)), col_ab, col_ba)
         for col in (col_ab, col_ba):
             assert not _cdiff(c_close(col, cpair(c, d), ONE), c_close(col, c_leaf(c), cchi(d)), c_close(col, c_leaf(d), cchi(c)))
-        I.L("const W4<R> sp = row_slash(ub, pab), xp = slash_col(pcd, vv);"); I.flops += FL["row_slash"] + FL["slash_col"]
+        I.L("const W4<R> sp = row_slash(ub, pab);"); I.flops += FL["row_slash"]
         I.L("const W4<R> rab = row_step(wadd(row_slash(q1a, eb), sp), q, mt, iq2), rba = row_step(wsub(row_slash(q1b, ea), sp), q, mt, iq2);")
         I.flops += 2 * (FL["row_slash"] + 8 + FL["col_step"])
-        I.L("const W4<R> xcd = wadd(slash_col(ec, chid), xp), xdc = wsub(slash_col(ed, chic), xp);"); I.flops += 2 * (FL["slash_col"] + 8)
         I.L("const Cx<R> a1 = row_col(rab, xcd), a2 = row_col(rab, xdc), a3 = row_col(rba, xcd), a4 = row_col(rba, xdc);"); I.flops += 4 * FL["row_col"]
         I.jamp("a1", c_close(col_ab, c_leaf(c), cchi(d)), pidx)
         I.jamp("a2", c_close(col_ab, c_leaf(d), cchi(c)), pidx)
@@ -626,6 +639,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("#include <stdlib.h>")
+    S("#define ME_SHARE_SLICE 524288L     // events per launch of the sharing kernel (%d KB of scratch per CTA in FP64)" % (NSCVEC * 8 * block * 8 // 1024))
     S("namespace me {")
     for gname, tmpl, rows in groups:
         nf = len(tmpl.params)
@@ -756,15 +770,25 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.nslots, block, lay.TM0, block))
     S("  // FP64 amplitudes (double and mixed): tensor-memory kernel, two CTAs per SM; ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
-    S("  const bool sh = a.share != 0 && a.hel_per_event == nullptr && a.scratch != nullptr && !no_tmem;")
+    S("  const bool sh = a.share != 0 && a.hel_per_event == nullptr && a.scratch != nullptr && !no_tmem && a.me_hel == nullptr && a.jamp_out == nullptr && a.me_out != nullptr;")
     S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event, a.scratch")
     S("#define ME_LAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
     S("    K<<<grid, %d, SMEM, a.stream>>>(ME_ARGS); } while (0)" % block)
-    S("  if (sh) {")
-    S("    if (precision == 0) ME_LAUNCH((k_%s<double, double, true, true>), smt);" % name)
-    S("    else if (precision == 1) ME_LAUNCH((k_%s<double, float, true, true>), smt);" % name)
-    S("    else ME_LAUNCH((k_%s<float, float, false, true>), smf);" % name)
+    S("  if (sh) {       // slices of at most ME_SHARE_SLICE events, one after the other on the stream: the scratch (one region per CTA) stays bounded")
+    S("    for (long start = 0; start < a.npad; start += ME_SHARE_SLICE) {")
+    S("      const long np = a.npad - start < ME_SHARE_SLICE ? a.npad - start : ME_SHARE_SLICE, nn = a.n - start < np ? a.n - start : np;")
+    S("      const unsigned sgrid = (unsigned)((np + %d - 1) / %d);" % (block, block))
+    S("#define ME_SARGS a.mom + (start / ME_PAGE) * (%d * 4 * ME_PAGE), nn, np, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out + start, nullptr, nullptr, nullptr, a.scratch" % NPAR)
+    S("#define ME_SLAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
+    S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
+    S("    K<<<sgrid, %d, SMEM, a.stream>>>(ME_SARGS); } while (0)" % block)
+    S("      if (precision == 0) ME_SLAUNCH((k_%s<double, double, true, true>), smt);" % name)
+    S("      else if (precision == 1) ME_SLAUNCH((k_%s<double, float, true, true>), smt);" % name)
+    S("      else ME_SLAUNCH((k_%s<float, float, false, true>), smf);" % name)
+    S("#undef ME_SLAUNCH")
+    S("#undef ME_SARGS")
+    S("    }")
     S("  } else if (precision == 0) {")
     S("    if (no_tmem) ME_LAUNCH((k_%s<double, double, false, false>), smd); else ME_LAUNCH((k_%s<double, double, true, false>), smt);" % (name, name))
     S("  } else if (precision == 1) {")
@@ -783,7 +807,8 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("static const unsigned char gray_rank_%s[%d] = {%s};" % (name, 1 << NPAR, ", ".join(str(r) for r in rank)))
     S("static size_t scratch_%s(int precision, long npad, int share, int) {" % name)
     S("  if (!share) return 0;")
-    S("  return (size_t)((npad + %d - 1) / %d) * %d * 8 * %d * (precision == 2 ? sizeof(float) : sizeof(double));" % (block, block, NSCVEC, block))
+    S("  const long np = npad < ME_SHARE_SLICE ? npad : ME_SHARE_SLICE;")
+    S("  return (size_t)((np + %d - 1) / %d) * %d * 8 * %d * (precision == 2 ? sizeof(float) : sizeof(double));" % (block, block, NSCVEC, block))
     S("}")
     nh = 1 << NPAR
     shared = 0

@@ -715,8 +715,18 @@ def test_share_currents_option(me, orc):
     sel = np.array([(mask >> h) & 1 for h in range(64)], dtype=bool)
     assert np.abs(got[:64] / (ref_h[:, sel].sum(1) / 512) - 1).max() < 1e-10
     ctx.close()
+    # more events than one launch of the sharing kernel takes (524288: its scratch is bounded): slices equal separate calls bit for bit
+    big, cut = 524288 + 4133, 524288
+    ctx = me.MEContext(3)
+    _, mom, _ = gen_events(me, ctx, cfg, big)
+    ctx.me_set_helicities(EXPECTED_MASK[3])
+    whole = ctx.me_compute(mom, big, me.ME_FP32).cpu().numpy()
+    head = ctx.me_compute(mom, cut, me.ME_FP32).cpu().numpy()
+    tail = ctx.me_compute(mom[ctx.momenta_numel(cut):], big - cut, me.ME_FP32).cpu().numpy()
+    assert np.array_equal(whole[:cut], head) and np.array_equal(whole[cut:], tail) and (whole > 0).all()
+    ctx.close()
     # ignored elsewhere
-    for proc in (0, 2, 4):
+    for proc in (0, 2):
         c = me.MEContext(proc)
         _, mm, _ = gen_events(me, c, inputs.CONFIGS[proc], 64)
         c.me_set_helicities(EXPECTED_MASK[proc])
