@@ -98,10 +98,18 @@ def profile_metrics():
 
 
 def ncu_flops_per_event(m):
-    """executed flops per event from the ncu opcode counts of one launch: add + mul + 2 fma (thread-level, predicated-on), both
-    precisions added (the FP32 kernels form their propagator denominators in FP64), plus the tensor-core flops by instruction shape"""
-    return (m.get("dadd", 0) + m.get("dmul", 0) + 2 * m.get("dfma", 0) + m.get("fadd", 0) + m.get("fmul", 0) + 2 * m.get("ffma", 0)
-            + m.get("tensor_flops", 0)) / m["events_per_launch"]
+    """executed ALU flops per event from the ncu opcode counts of one launch: add + mul + 2 fma (thread-level, predicated-on), both
+    precisions added (the FP32 kernels form their propagator denominators in FP64).  The tensor-core flops of the colour-sum
+    kernels (instruction count x instruction shape) are another unit with another peak: reported beside, never added in."""
+    return (m.get("dadd", 0) + m.get("dmul", 0) + 2 * m.get("dfma", 0) + m.get("fadd", 0) + m.get("fmul", 0) + 2 * m.get("ffma", 0)) / m["events_per_launch"]
+
+
+def ncu_fields(m, n, ms, peak):
+    """the keys a result row takes from its row of profiles/r2_kernel_metrics.csv"""
+    fe = ncu_flops_per_event(m)
+    return {"flops_per_event_ncu": fe, "frac_ncu": fe * n / (ms * 1e-3) * 1e-12 / peak,
+            "tensor_flops_per_event_ncu": m.get("tensor_flops", 0) / m["events_per_launch"],
+            "traffic": m.get("dram_bytes"), "traffic_algorithmic": m.get("algorithmic_bytes"), "profile_source": m["source"]}
 
 
 def respawn_under_torchrun(args):
@@ -279,9 +287,7 @@ def main():
              "frac_of_measured": ach / peak_meas[pk], "flops_per_event_algorithmic": flops_per_event}
         m = prof.get((cfg["name"], pname, option, n))
         if m is not None:
-            fe = ncu_flops_per_event(m)
-            r.update({"flops_per_event_ncu": fe, "frac_ncu": fe * n / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
-                      "traffic": m.get("dram_bytes"), "traffic_algorithmic": m.get("algorithmic_bytes"), "profile_source": m["source"], "kernel": m["kernel"]})
+            r.update(ncu_fields(m, n, ms, PEAK_TFLOPS[pk])); r["kernel"] = m["kernel"]
         return r
 
     roofline = {"bound": "alu", "unit": "TFLOP/s", "kernel": "k_%s<double,double,TM=true,SH=%s>" % (cfg["name"], "true" if shared_default else "false") + (" (+ colour sum)" if HL == 4 else ""),
@@ -443,9 +449,7 @@ def main():
                                              "frac_of_%s_peak_executed" % pk: fx * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk]}
                 m = prof.get((c["name"], pname, "shared_currents" if sh else "-", c["events"]))
                 if m is not None:
-                    fe = ncu_flops_per_event(m)
-                    results[c["name"]][pname].update({"flops_per_event_ncu": fe, "frac_ncu": fe * c["events"] / (ms * 1e-3) * 1e-12 / PEAK_TFLOPS[pk],
-                                                      "traffic": m.get("dram_bytes"), "traffic_algorithmic": m.get("algorithmic_bytes"), "profile_source": m["source"]})
+                    results[c["name"]][pname].update(ncu_fields(m, c["events"], ms, PEAK_TFLOPS[pk]))
                 launches += (reps + 1) * me.launches_per_pass(cx.info, ng)
             cx.close(); del mm
     line["results"] = results
