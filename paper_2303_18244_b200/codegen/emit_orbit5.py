@@ -33,6 +33,9 @@ K1_PARTS = 1     # kernels the 18 closing vectors of the three-gluon sub-trees a
 BLOCK1 = 128     # threads per CTA of every diagram kernel
 FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
+K1_UW_LOOP = False   # kernel o0: the two (u, w) halves of the closing vectors as a nested table-driven loop
+K1_PRE = True        # sharing form o0s of kernel o0 (gluon-only currents of the three-gluon sub-trees once per group of helicities)
+K1S_UW_LOOP = True   # ... with the nested (u, w) loop in its FP64 form
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
 K3D_JACC = 48            # accumulator kernel o2d (current sharing off): one set of local jamp accumulators per last gluon, kept in tensor memory
@@ -324,7 +327,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None, nparts=3):
+def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
@@ -333,14 +336,26 @@ def build_k1(stride, pidx, part=None, nparts=3):
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=False)
-    insts = []
-    for M in [(a, b, c) for a in range(N) for b in range(a + 1, N) for c in range(b + 1, N)]:
+    insts, pre_insts = [], []
+    for vi, M in enumerate([(a, b, c) for a in range(N) for b in range(a + 1, N) for c in range(b + 1, N)]):
         a, b, c = M
         x, y = rest_of(a, b, c)
         I = Inst5(lay, stride)
         I.leaf("ex", x); I.leaf("ey", y); I.kvec("kx", [x]); I.kvec("ky", [y])
         I.L("const R ik5 = %s;" % I.ik2(*range(N)))
-        emit_pair(I, "pxy", x, y, "ex", "ey", "kx", "ky")
+        # pre: the two ordered currents of the sub-tree and the pair current of the other two gluons depend on the gluon helicities
+        # only: the sharing form of the kernel builds them once per group of helicities (G) and parks them in the L2-resident
+        # current cache (vectors 3 vi .. 3 vi + 2); the block reloads them
+        G = Inst5(lay, stride) if pre else I
+        if pre:
+            G.L("W4<R> pxy;")
+            G.L("{")
+            G.leaf("ex", x); G.leaf("ey", y); G.kvec("kx", [x]); G.kvec("ky", [y])
+            G.L("const W4<R> t = v3_current(ex, ey, kx, ky, %s); pxy = t;" % G.ik2(x, y)); G.flops += FL5["v3_current"]
+            G.L("}")
+            I.L("const W4<R> pxy = sc_ldw<R>(sc, %s + 2);" % I.P(3 * vi))
+        else:
+            emit_pair(I, "pxy", x, y, "ex", "ey", "kx", "ky")
         # the six three-gluon terms on M (registers for the whole block); their inputs die in this scope
         tcol = [c_v3(cpair(a, b), c_leaf(c)), c_v3(cpair(a, c), c_leaf(b)), c_v3(cpair(b, c), c_leaf(a))] + \
                [c_v4(k, c_leaf(a), c_leaf(b), c_leaf(c)) for k in range(3)]
@@ -349,23 +364,37 @@ def build_k1(stride, pidx, part=None, nparts=3):
         assert all(not _cdiff(tcol[3 + k], tcol[k], {}) for k in range(3)) and not _cdiff(tcol[1], tcol[0], {st: -v for st, v in tcol[2].items()})
         tnames, tcol = ["s0", "s2"], [tcol[0], tcol[2]]
         I.L("W4<R> s0, s2; P4<R> kM;")
-        I.L("{")
+        if pre:
+            G.L("W4<R> s0, s2;")
+        G.L("{")
         for nm, l in (("ea", a), ("eb", b), ("ec", c)):
-            I.leaf(nm, l)
+            G.leaf(nm, l)
         for nm, l in (("ka", a), ("kb", b), ("kc", c)):
-            I.kvec(nm, [l])
-        I.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc);"); I.flops += 12
-        I.L("kM = padd(kab, kc);"); I.flops += 4
-        emit_pair(I, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(I, "pac", a, c, "ea", "ec", "ka", "kc")
-        emit_pair(I, "pbc", b, c, "eb", "ec", "kb", "kc")
-        I.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once (as pxy of its own block) would do
-        I.L("const R ik3 = %s;" % I.ik2(a, b, c))
-        I.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); I.flops += FL5["v4_dots"]
-        I.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
-        I.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
-        I.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
-        I.flops += 5 * FL5["wadd"] + 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
-        I.L("}")
+            G.kvec(nm, [l])
+        G.L("const P4<R> kab = padd(ka, kb), kac = padd(ka, kc), kbc = padd(kb, kc);"); G.flops += 12
+        if not pre:
+            I.L("kM = padd(kab, kc);"); I.flops += 4
+        emit_pair(G, "pab", a, b, "ea", "eb", "ka", "kb"); emit_pair(G, "pac", a, c, "ea", "ec", "ka", "kc")
+        emit_pair(G, "pbc", b, c, "eb", "ec", "kb", "kc")
+        G.redundant += 3 * FL5["v3_current"]          # every pair is formed in 4 blocks; once (as pxy of its own block) would do
+        G.L("const R ik3 = %s;" % G.ik2(a, b, c))
+        G.L("const V4Dots<R> dots = v4_dots(ea, eb, ec, ik3);"); G.flops += FL5["v4_dots"]
+        G.L("const W4<R> t14 = wadd(v3_current(pac, eb, kac, kb, ik3), v4_current(1, dots, ea, eb, ec));")
+        G.L("s0 = wadd(wadd(v3_current(pab, ec, kab, kc, ik3), v4_current(0, dots, ea, eb, ec)), t14);")
+        G.L("s2 = wadd(wadd(v3_current(pbc, ea, kbc, ka, ik3), v4_current(2, dots, ea, eb, ec)), t14);")
+        G.flops += 5 * FL5["wadd"] + 3 * FL5["v3_current"] + 3 * FL5["v4_current"]
+        G.L("}")
+        if pre:
+            vec = G.P(3 * vi)
+            G.L("sc_stw<R>(sc, %s, s0); sc_stw<R>(sc, %s + 1, s2); sc_stw<R>(sc, %s + 2, pxy);" % (vec, vec, vec))
+            pre_insts.append(G)
+            vec = I.P(3 * vi)
+            I.L("s0 = sc_ldw<R>(sc, %s); s2 = sc_ldw<R>(sc, %s + 1);" % (vec, vec))
+            I.L("{")
+            for nm, l in (("ka", a), ("kb", b), ("kc", c)):
+                I.kvec(nm, [l])
+            I.L("kM = padd(padd(ka, kb), kc);"); I.flops += 8
+            I.L("}")
         if part is not None and part > 0:             # the split kernels each rebuild pxy and the six terms: all of it overhead
             I.redundant = I.flops
 
@@ -448,8 +477,20 @@ def build_k1(stride, pidx, part=None, nparts=3):
             dots_with(T, [qr, fetch("q1u")], "bilinear(quark_step2(q1u, %s, qr, mt, iqr), vv)" % ew, str_,
                       lambda col: c_close(c_step(cq1(u), c_leaf(w)), col, ONE))
 
-        uw_vectors(I, x, y, "ex", "ey", "kx", "ky")
-        uw_vectors(I, y, x, "ey", "ex", "ky", "kx")
+        if K1_UW_LOOP if uw_loop is None else uw_loop:
+            # one nested table-driven loop of two iterations instead of two copies of five scopes; its jamp updates go to the
+            # block's accumulators (slots from the table)
+            inners = []
+            for (u, w) in ((x, y), (y, x)):
+                J = Inst5(lay, stride, inner=True, parent=I)
+                J.leaf("eu", u); J.leaf("ew", w); J.kvec("ku", [u]); J.kvec("kw", [w])
+                J.redundant += J.flops                # ex, ey, kx, ky exist in the block
+                uw_vectors(J, u, w, "eu", "ew", "ku", "kw")
+                inners.append(J)
+            I.inner_loop("uw", inners)
+        else:
+            uw_vectors(I, x, y, "ex", "ey", "kx", "ky")
+            uw_vectors(I, y, x, "ey", "ex", "ky", "kx")
         # V3(t, pair(x,y)) on the bare line
         dots_with(I, [], "v3_dual(pxy, jtt, kM, padd(kx, ky), ik5)", FL5["v3_dual"] + 4, lambda col: c_close(ONE, c_v3(col, cpair(x, y)), ONE))
         # V4(t, eps_x, eps_y) on the bare line, three structures (duals of the contact term)
@@ -464,6 +505,13 @@ def build_k1(stride, pidx, part=None, nparts=3):
         assert counter[0] == 18
         I.flush_global()
         insts.append(I)
+    if pre:
+        add_group("tripre", pre_insts, 1)
+        t = groups[-1][1]
+        t.pre = True                      # run once per group of helicities, before the helicity loop
+        t.group_flops = t.flops; t.flops = 0
+        t.group_redundant = t.redundant; t.redundant = 0
+        t.cache_vectors = 3 * len(pre_insts)
     add_group("triples", insts, 1)
     return lay, groups
 
@@ -891,7 +939,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
             S("};")
     S("template <typename R, typename RJ, bool TM>")
     S("__global__ void __launch_bounds__(%d) k_%s_o%s(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
-      " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n) {" % (BLOCK, name, ki))
+      " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n, void* __restrict__ cache) {" % (BLOCK, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
@@ -906,6 +954,9 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
         S("    tm_base = tm_alloc(&tm_slot, tm_cols * %d);" % (BLOCK // 128))
         S("    tm = tm_base + ((uint32_t)(threadIdx.x & 96) << 16) + (threadIdx.x >> 7) * tm_cols;      // this warp's quarter of the 128 lanes (and half of the columns)")
         S("  }")
+    ncache = max([getattr(t, "cache_vectors", 0) for _, t, _, _ in groups])
+    if ncache:      # this CTA's region of the current cache: [vector][4 pairs of reals][thread]
+        S("  R* const sc = reinterpret_cast<R*>(cache) + ((size_t)(blockIdx.y * gridDim.x + blockIdx.x) * (%d * 8 * ME_SM_STRIDE) + 2 * threadIdx.x);" % ncache)
     S("  const R mt = (R)mt_d;")
     S("  const unsigned npad32 = (unsigned)npad;   // a slice holds <= 65536 events: 240 rows x npad elements fit 32 bits (cheap RED addresses)")
     S("  SpinorBasis<R> sbt, sbtb;")
@@ -971,7 +1022,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
     def launch_line(inst, smem, cast):
         S("      cudaFuncSetAttribute(k_%s_o%s<%s>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)%s);" % (name, ki, inst, smem))
         S("      cudaFuncSetAttribute(k_%s_o%s<%s>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);" % (name, ki, inst))
-        S("      k_%s_o%s<%s><<<grid, %d, %s, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (%s*)a.gj, a.hel_per_event, a.n);" % (name, ki, inst, BLOCK, smem, cast))
+        S("      k_%s_o%s<%s><<<grid, %d, %s, a.stream>>>(a.mom, a.npad, a.hels, a.nh, a.mt, (%s*)a.gj, a.hel_per_event, a.n, a.cache);" % (name, ki, inst, BLOCK, smem, cast))
     S("  const size_t smf = sizeof(float) * %d * %d, smd = sizeof(double) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, BLOCK, lay.nslots, BLOCK, tm0 or 0, BLOCK))
     S("  (void)smf; (void)smd; (void)smt;")
     if only == "tm":
@@ -982,6 +1033,13 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
         S("  } else {")
         launch_line("double, double, true", "smt", "double")
         S("  }")
+    elif only == "f32":          # this form of the kernel serves FP32 only (the FP64 form of the same step is another kernel)
+        S("  if (precision != 2) return cudaErrorInvalidValue;")
+        launch_line("float, float, false", "smf", "float")
+    elif only == "f64tm":        # ... and this one FP64 amplitudes in the tensor-memory layout only (sharing kernels: never run with ME_NO_TMEM=1)
+        assert tm0 is not None
+        S("  if (precision == 2) return mk_%s_o%s.launch(precision, a);" % (name, delegate))
+        launch_line("double, double, true", "smt", "double")
     else:
         if delegate is not None:
             S(NO_TMEM)
@@ -1006,7 +1064,8 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
     redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
     group_flops = sum(getattr(t, "group_flops", 0) * len(rows) for _, t, rows, _ in groups)
     return "\n".join(src) + "\n", dict(amplitudes=namp, flops=flops, redundant=redundant, group_flops=group_flops, fixed=fixed, slots=lay.nslots, tm_slot0=tm0, tm_cols=getattr(lay, "tm_cols", 0),
-                                       shapes={g: len(r) for g, _, r, _ in groups})
+                                       shapes={g: len(r) for g, _, r, _ in groups}, cache_vectors=ncache,
+                                       group_redundant=sum(getattr(t, "group_redundant", 0) * len(rows) for _, t, rows, _ in groups))
 
 
 def emit_orbit5_process(name="gg_ttxggg"):
@@ -1032,6 +1091,20 @@ def emit_orbit5_process(name="gg_ttxggg"):
     src3, info3 = emit_kernel(name, "2s", lay3, groups3, BLOCK1, only="tm")
     files["gen_%s_o2s.cu" % name] = src3
     assert info3["amplitudes"] == kinfo[-1]["amplitudes"], (info3["amplitudes"], kinfo[-1]["amplitudes"])
+    # sharing form of the first kernel: the gluon-only currents of the three-gluon sub-trees once per group of helicities
+    info0s = None
+    if K1_PRE and K1_PARTS == 1:
+        # FP64: with the two (u, w) halves as a nested loop (70 KB loop body instead of 93 KB: instruction fetch); FP32: without (measured
+        # 41.6 ms per pass against 44.3 ms with the nested loop, whose table-driven accumulator offsets cost more than the fetch saves)
+        lay0, groups0 = build_k1(BLOCK1, pidx, uw_loop=K1S_UW_LOOP, pre=True)
+        src0, info0s = emit_kernel(name, "0s", lay0, groups0, BLOCK1, only="f64tm" if K1S_UW_LOOP else None, delegate="0f" if K1S_UW_LOOP else None)
+        files["gen_%s_o0s.cu" % name] = src0
+        assert info0s["amplitudes"] == kinfo[0]["amplitudes"]
+        if K1S_UW_LOOP:
+            lay0f, groups0f = build_k1(BLOCK1, pidx, uw_loop=False, pre=True)
+            src0f, info0f = emit_kernel(name, "0f", lay0f, groups0f, BLOCK1, only="f32")
+            files["gen_%s_o0f.cu" % name] = src0f
+            assert info0f["cache_vectors"] == info0s["cache_vectors"]
     namp = sum(k["amplitudes"] for k in kinfo)
     assert namp == 1890, namp
     # colour sum in its symmetric form (S§8(d)): per part  sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), as for the smaller
@@ -1061,8 +1134,13 @@ def emit_orbit5_process(name="gg_ttxggg"):
     for ki in range(len(kinfo)):
         S("extern const MultiKernel mk_%s_o%d;" % (name, ki))
     S("extern const MultiKernel mk_%s_o2s;" % name)
+    if info0s is not None:
+        S("extern const MultiKernel mk_%s_o0s;" % name)
     S("static const MultiKernel* const parts_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo)))))
-    S("static const MultiKernel* const parts_sh_%s[%d] = {%s, &mk_%s_o2s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo) - 1)), name))
+    sh_names = ["o%d" % ki for ki in range(len(kinfo) - 1)] + ["o2s"]
+    if info0s is not None:
+        sh_names[0] = "o0s"
+    S("static const MultiKernel* const parts_sh_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_%s" % (name, k) for k in sh_names)))
     # current sharing: the helicity list is ordered by gluon helicities, the four quark-helicity assignments of each adjacent (rank table);
     # flops per event with it on, over the full helicity set: kernel o2 per helicity -> per group of four + per helicity
     fmask = (1 << T_BIT) | (1 << TB_BIT)
@@ -1074,12 +1152,24 @@ def emit_orbit5_process(name="gg_ttxggg"):
     nhel, ngroups = 1 << NPAR, (1 << NPAR) // HEL_PER_CTA
     shared_event = nhel * (algo - a2) + ngroups * (info3["group_flops"] - pa["pairs"]) + nhel * (info3["flops"] - info3["redundant"]) + fixed
     executed_shared = executed - k2["flops"] + info3["flops"] + info3["group_flops"] / HEL_PER_CTA
+    cache_vectors = 0
+    if info0s is not None:     # kernel o0 per helicity -> per group of four + per helicity
+        k0 = kinfo[0]
+        shared_event += -nhel * (k0["flops"] - k0["redundant"]) + nhel * (info0s["flops"] - info0s["redundant"]) \
+            + ngroups * (info0s["group_flops"] - info0s["group_redundant"])
+        executed_shared += -k0["flops"] + info0s["flops"] + info0s["group_flops"] / HEL_PER_CTA
+        cache_vectors = info0s["cache_vectors"]
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // the sharing kernel exists in its tensor-memory form only")
-    S("  return launch_multi(precision, a, (a.share && !no_tmem) ? parts_sh_%s : parts_%s, %d, %d, color_num_%s);" % (name, name, len(kinfo), ncol, name))
+    S("  if (a.share && !no_tmem) return launch_multi(precision, a, parts_sh_%s, %d, %d, color_num_%s, %d);" % (name, len(kinfo), ncol, name, cache_vectors))
+    S("  return launch_multi(precision, a, parts_%s, %d, %d, color_num_%s, 0);" % (name, len(kinfo), ncol, name))
     S("}")
-    S("static size_t scratch_%s(int precision, long npad, int, int) { return multi_scratch_bytes(precision, npad, %d); }" % (name, ncol))
+    S("// staging buffer of one helicity chunk; with current sharing also the current cache of kernel o0s behind it (%d vectors per thread)" % cache_vectors)
+    S("static size_t scratch_%s(int precision, long npad, int share, int) {" % name)
+    S("  const size_t staging = multi_scratch_bytes(precision, npad, %d);" % ncol)
+    S("  return share ? (staging + 255) / 256 * 256 + multi_cache_bytes(precision, npad, %d) : staging;" % cache_vectors)
+    S("}")
     S("extern const ProcTable tab_%s = {%d, %d, %d, %d, %d, %d, {%r, %r, %r}, {%r, %r, %r}, %r, color_num_%s, launch_%s, scratch_%s, true, gray_rank_%s, %r, %d, %r};"
       % (name, N, 1240, namp, ncol, color_denom, len(kinfo) + 1, float(algo), float(algo), float(algo),
          float(executed), float(executed), float(executed), float(fixed), name, name, name, name, float(shared_event), fmask, float(executed_shared)))
@@ -1087,5 +1177,5 @@ def emit_orbit5_process(name="gg_ttxggg"):
     files["gen_%s_table.cu" % name] = "\n".join(src) + "\n"
     info = dict(n=N, ndiagrams=1240, namp=namp, ncol=ncol, color_denom=color_denom, flops_per_helicity=algo,
                 flops_executed_per_helicity=executed, fixed_flops=fixed, colour_flops=cs_flops, kernels=kinfo, block=BLOCK1,
-                flops_shared_event=shared_event, flops_executed_per_helicity_shared=executed_shared, kernel_o2s=info3)
+                flops_shared_event=shared_event, flops_executed_per_helicity_shared=executed_shared, kernel_o2s=info3, kernel_o0s=info0s)
     return files, info

@@ -78,12 +78,31 @@ static const bool g_use_dmma = getenv("ME_COLOR_FMA") == nullptr;
 // ME_COLOR_MMA_SYNC=1 selects the warp-level TF32 kernel (color_sum_tf32.cu) instead of the tcgen05 one (A/B timing)
 static const bool g_use_tcgen05 = getenv("ME_COLOR_MMA_SYNC") == nullptr;
 
+// one region per CTA of a diagram kernel: grid = (slice / 128 threads) x (chunk / ME_HEL_PER_CTA helicity groups)
+size_t multi_cache_bytes(int precision, long npad, int vectors) {
+  const long np = npad < ME_EVENT_SLICE ? npad : ME_EVENT_SLICE;
+  const long ctas = (np + 127) / 128 * (ME_HEL_CHUNK / ME_HEL_PER_CTA);
+  return (size_t)ctas * vectors * 8 * 128 * (precision == 2 ? sizeof(float) : sizeof(double));
+}
+
 static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
-                                      const double* color_num_host);
+                                      const double* color_num_host, void* cache);
 
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host) {
+  return launch_multi(precision, a, parts, nparts, ncol, color_num_host, 0);
+}
+
+cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
+                         const double* color_num_host, int cache_vectors) {
   const int npar = 7;   // g g -> t t~ g g g
+  // the current cache of the sharing kernels sits behind the staging buffer of the batch (sizes as scratch_bytes of the process table)
+  void* cache = nullptr;
+  if (cache_vectors > 0) {
+    const size_t off = (multi_scratch_bytes(precision, a.npad, ncol) + 255) / 256 * 256;
+    if (a.scratch == nullptr || a.scratch_bytes < off + multi_cache_bytes(precision, a.npad, cache_vectors)) return cudaErrorInvalidValue;
+    cache = (char*)a.scratch + off;
+  }
   for (long start = 0; start < a.n; start += ME_EVENT_SLICE) {
     LaunchArgs s = a;
     s.n = a.n - start < ME_EVENT_SLICE ? a.n - start : ME_EVENT_SLICE;
@@ -93,20 +112,20 @@ cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* 
     if (a.me_hel != nullptr) s.me_hel = a.me_hel + start;
     if (a.jamp_out != nullptr) s.jamp_out = a.jamp_out + start;
     if (a.hel_per_event != nullptr) s.hel_per_event = a.hel_per_event + start;
-    cudaError_t e = launch_multi_slice(precision, s, a.n, parts, nparts, ncol, color_num_host);
+    cudaError_t e = launch_multi_slice(precision, s, a.n, parts, nparts, ncol, color_num_host, cache);
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
 }
 
 static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long hs, const MultiKernel* const* parts, int nparts, int ncol,
-                                      const double* color_num_host) {
+                                      const double* color_num_host, void* cache) {
   if (ncol != CS_NCOL) return cudaErrorInvalidValue;
   if (a.color_d == nullptr || a.color_f == nullptr) return cudaErrorInvalidValue;   // uploaded by me_create on the context's device
   const unsigned cgrid = (unsigned)(a.npad / 32);
   for (int base = 0; base < a.nhel; base += ME_HEL_CHUNK) {
     const int nh = a.nhel - base < ME_HEL_CHUNK ? a.nhel - base : ME_HEL_CHUNK;
-    MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream, a.hel_per_event, a.n};
+    MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream, a.hel_per_event, a.n, cache};
     {   // every diagram kernel ADDS its colour flows into the staging buffer
       const size_t esz = precision == 2 ? sizeof(float) : sizeof(double);
       cudaError_t e = cudaMemsetAsync(a.scratch, 0, (size_t)nh * ncol * 2 * a.npad * esz, a.stream);

@@ -16,12 +16,17 @@ namespace me {
 struct MultiArgs {
   const double* mom; long npad; const unsigned char* hels; int nh; double mt; void* gj; cudaStream_t stream;
   const int* hel_per_event; long n;
+  void* cache;      // sharing kernels: L2-resident region for currents parked across the helicities of a CTA (null: not available)
 };
 struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); };
 
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host);
 size_t multi_scratch_bytes(int precision, long npad, int ncol);
+// bytes of the current cache behind the staging buffer: `vectors` four-vectors per thread and CTA of a diagram kernel (0: none)
+size_t multi_cache_bytes(int precision, long npad, int vectors);
+cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
+                         const double* color_num_host, int cache_vectors);
 // (colour-sum launchers: cmat = device pointer owned by the context, sms = multiprocessors of its device)
 // FP32 colour sum on the tensor cores, TF32 hi/lo split (color_sum_tf32.cu); cmat = device pointer to float numerators
 cudaError_t launch_color_sum_tf32(int sms, int staging_is_double, const float* cmat, const void* gj, long npad, long n, long hs, int nh,
