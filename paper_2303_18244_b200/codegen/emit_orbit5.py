@@ -35,9 +35,13 @@ FL5 = dict(FL, cx_comb=56, wadd=8, row_slash=64)
 # FP64 kernels: categories kept in tensor memory so that two 128-thread CTAs fit per SM (8 warps instead of 4)
 K1_UW_LOOP = False   # kernel o0: the two (u, w) halves of the closing vectors as a nested table-driven loop
 K1_PRE = True        # sharing form o0s of kernel o0 (gluon-only currents of the three-gluon sub-trees once per group of helicities)
+K1_CACHE_Q = (False, True)   # ... (FP64 form, FP32 form) with the one-gluon quark currents of a helicity in the current cache: one set per helicity
+                             # instead of six rebuilds per block.  Measured per pass: FP32 40.8 against 41.5 ms; FP64 81.2 against 80.4 ms (the
+                             # L2 latency of six more loads per block costs more than the 7 % of the arithmetic they save; through the L1: 81.8 ms)
 K1S_UW_LOOP = True   # ... with the nested (u, w) loop in its FP64 form
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
+K3S_CACHE_U = True       # sharing kernel o2s: the thirty ordered currents of a group in the L2-resident current cache (two CTAs per SM) instead of on chip (one)
 K3D_JACC = 48            # accumulator kernel o2d (current sharing off): one set of local jamp accumulators per last gluon, kept in tensor memory
 TM_K3 = ("J",)            # FP64: 96 slots = 192 columns, one CTA per SM; FP32: one column per slot, two CTAs per SM
 
@@ -327,7 +331,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False):
+def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False, cache_q=False):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
@@ -336,6 +340,25 @@ def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False):
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=False)
+    QV, CV = 30, 35             # current cache, sharing form: vectors 0..29 per group (three per block), 30..34 q1(l), 35..39 chi1(w) per helicity
+    if cache_q and pre:
+        qi, ci = [], []
+        for l in range(N):
+            I = Inst5(lay, stride)
+            I.leaf("el", l); I.qvec("q", [l]); I.fv("ub")
+            I.L("const W4<R> t = quark_step2(ub, el, q, mt, %s);" % I.iq(l)); I.flops += FL5["quark_step2"]
+            I.L("sc_stw<R>(sc, %s, t);" % I.P(QV + l))
+            I.redundant += I.flops       # the algorithmic count has one set of one-gluon quark currents already (kernel o1 / the q1 reference loop)
+            qi.append(I)
+            rest = rest_of(l)
+            I = Inst5(lay, stride)
+            I.leaf("ew", l); I.qvec("q", rest); I.fv("vv")
+            I.L("const W4<R> t = col_step(slash_col(ew, vv), q, mt, %s);" % I.iq(*rest)); I.flops += FL5["slash_col"] + FL5["col_step"]
+            I.L("sc_stw<R>(sc, %s, t);" % I.P(CV + l))
+            I.redundant += I.flops
+            ci.append(I)
+        add_group("q1c", qi, 1)
+        add_group("chi1c", ci, 1)
     insts, pre_insts = [], []
     for vi, M in enumerate([(a, b, c) for a in range(N) for b in range(a + 1, N) for c in range(b + 1, N)]):
         a, b, c = M
@@ -453,28 +476,39 @@ def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False):
             # chi1(w) is formed once and parked in the scratch vector for its three scopes; q1(u) takes the slot over for its second
             park = lambda nm: (lambda T_: T_.stw(lay.TMP, nm))
             fetch = lambda nm: (lambda T_: T_.ldw(nm, lay.TMP))
-            T.L("{"); mk_chi("chw", w, ew)(T); park("chw")(T); T.L("}")
             # quad = V3(t, eps_u) closing three ways with the last gluon w: on the t~ end (colour Q.w), on the t end (w.Q), or through a
             # three-gluon vertex on the bare line (colour Q.w - w.Q): the current of the third, y3, is folded into the other two
             # (two scopes instead of three)
             y3 = lambda T_: (T_.fv("jtt"), T_.L("const W4<R> y3 = v3_dual(%s, jtt, padd(kM, %s), %s, ik5);" % (ew, ku, kw)))
-            dots_with(T, [fetch("chw"), ik4, y3], "v3_dual(%s, wadd(bilinear(ub, chw), y3), kM, %s, ik4)" % (eu, ku),
+            if cache_q and pre:
+                # sharing form: the one-gluon quark currents come from the current cache (formed once per helicity by the q1c / chi1c loops
+                # instead of six times per block), which leaves the scratch vector to y3 (formed once instead of twice)
+                cached = lambda nm, base, l: (lambda T_: T_.L("const W4<R> %s = sc_ldw<R>(sc, %s);" % (nm, T_.P(base + l))))
+                get_chw, get_q1w, get_q1u, get_q1u2 = cached("chw", CV, w), cached("q1w", QV, w), cached("q1u", QV, u), cached("q1u", QV, u)
+                y3a = lambda T_: (y3(T_), park("y3")(T_)); y3b = fetch("y3")
+                post_q1u = None
+            else:
+                T.L("{"); mk_chi("chw", w, ew)(T); park("chw")(T); T.L("}")
+                get_chw, get_q1w, get_q1u, get_q1u2 = fetch("chw"), mk_q1("q1w", w, ew), mk_q1("q1u", u, eu), fetch("q1u")
+                y3a = y3b = y3
+                post_q1u = park("q1u")
+            dots_with(T, [get_chw, ik4, y3a], "v3_dual(%s, wadd(bilinear(ub, chw), y3), kM, %s, ik4)" % (eu, ku),
                       2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(ONE, quad(col), cchi(w)))
-            dots_with(T, [mk_q1("q1w", w, ew), ik4, y3], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
-                      2 * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + 4, lambda col: c_close(cq1(w), quad(col), ONE))
+            dots_with(T, [get_q1w, ik4, y3b], "v3_dual(%s, wsub(bilinear(q1w, vv), y3), kM, %s, ik4)" % (eu, ku),
+                      (2 if y3b is y3 else 1) * FL5["v3_dual"] + FL5["bilinear"] + FL5["wadd"] + (4 if y3b is y3 else 0), lambda col: c_close(cq1(w), quad(col), ONE))
             idx3 = counter[0]; counter[0] += 1
             if part is None or idx3 // (18 // nparts) == part:
                 T.namp += 6                   # the six V3-closing terms are inside the twelve above
-            if part is None or (idx3 - 1) // (18 // nparts) == part:
+            if (part is None or (idx3 - 1) // (18 // nparts) == part) and y3b is y3:
                 T.redundant += FL5["v3_dual"] + 4  # y3 is formed twice
             # ubar . t-slash . chi2: eps_u attached to chi1(w)
-            dots_with(T, [qc, fetch("chw")], "bilinear(ub, col_step(slash_col(%s, chw), qc, mt, iqc))" % eu, stc,
+            dots_with(T, [qc, get_chw], "bilinear(ub, col_step(slash_col(%s, chw), qc, mt, iqc))" % eu, stc,
                       lambda col: c_close(ONE, col, c_step(c_leaf(u), cchi(w))))
             # q1(u) . t-slash . chi1(w)
-            dots_with(T, [mk_q1("q1u", u, eu), fetch("chw")], "bilinear(q1u, chw)", FL5["bilinear"], lambda col: c_close(cq1(u), col, cchi(w)),
-                      post=park("q1u"))
+            dots_with(T, [get_q1u, get_chw], "bilinear(q1u, chw)", FL5["bilinear"], lambda col: c_close(cq1(u), col, cchi(w)),
+                      post=post_q1u)
             # q2 . t-slash . v: eps_w attached to q1(u)
-            dots_with(T, [qr, fetch("q1u")], "bilinear(quark_step2(q1u, %s, qr, mt, iqr), vv)" % ew, str_,
+            dots_with(T, [qr, get_q1u2], "bilinear(quark_step2(q1u, %s, qr, mt, iqr), vv)" % ew, str_,
                       lambda col: c_close(c_step(cq1(u), c_leaf(w)), col, ONE))
 
         if K1_UW_LOOP if uw_loop is None else uw_loop:
@@ -511,7 +545,7 @@ def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False):
         t.pre = True                      # run once per group of helicities, before the helicity loop
         t.group_flops = t.flops; t.flops = 0
         t.group_redundant = t.redundant; t.redundant = 0
-        t.cache_vectors = 3 * len(pre_insts)
+        t.cache_vectors = 3 * len(pre_insts) + (10 if cache_q else 0)
     add_group("triples", insts, 1)
     return lay, groups
 
@@ -711,8 +745,14 @@ def build_k3(stride, pidx, jacc=0, tm=()):
 NU_SMEM = 2          # colour-ordered currents per last gluon kept in shared memory; the other four in tensor memory
 
 
-def build_k3s(stride, pidx):
-    lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "U"), nu=6, nu_smem=NU_SMEM)      # jacc: the 24 ordered contact amplitudes
+def build_k3s(stride, pidx, cache_u=None):
+    cache_u = K3S_CACHE_U if cache_u is None else cache_u
+    if cache_u:
+        # the thirty ordered currents of a group live in the L2-resident current cache (vector 6 w + k): what stays on chip (pair currents and
+        # the 24 ordered contact amplitudes in tensor memory, 76 slots in shared memory) lets two CTAs share an SM
+        lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "J"))
+    else:
+        lay = Layout5(want_pairs=True, want_iq_mid=False, jacc=24, want_q1chi=False, ik2_sizes=(2, 4, 5), tm=("PAIR", "U"), nu=6, nu_smem=NU_SMEM)      # jacc: the 24 ordered contact amplitudes
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)          # the ten pair currents: gluon helicities only, once per group
@@ -767,18 +807,26 @@ def build_k3s(stride, pidx):
                 accumulate("v4_current(%d, dots, pp, e1, e2)" % k, c_v4(k, cpair(*p), c_leaf(l1), c_leaf(l2)))
             I.L("}")
         assert all(started)
-        for k in range(6):
-            I.stw(lay.U[(w, k)], "U%d" % k)
+        if cache_u:
+            I.L(" ".join("sc_stw<R>(sc, %s + %d, U%d);" % (I.P(6 * w), k, k) for k in range(6)))
+        else:
+            for k in range(6):
+                I.stw(lay.U[(w, k)], "U%d" % k)
         insts.append(I)
     add_group("ubuild", insts, 1)
     for _, t, _, _ in groups:
         t.pre = True                                              # run once per group of helicities, before the helicity loop
         t.group_flops = t.flops; t.flops = 0
+    if cache_u:
+        groups[-1][1].cache_vectors = 6 * N
     # ---- per helicity: the two end vectors of w (bilinears of the fermion ends with the dual of V3(quad, eps_w) folded in) and 12 dots
     insts = []
     for w in range(N):
         quad = rest_of(w)
         I = Inst5(lay, stride)
+        if cache_u:        # the first three ordered currents are requested before the end vectors are built, the other three before the first dots
+            ubase = I.P(6 * w)
+            I.L("const W4<R> " + ", ".join("u%d = sc_ldw<R>(sc, %s + %d)" % (k, ubase, k) for k in range(3)) + ";")
         I.leaf("ew", w); I.kvec("kw", [w]); I.kvec("kq", quad)
         f0 = I.flops
         I.qvec("qw", [w]); I.qvec("qq", quad)
@@ -788,9 +836,12 @@ def build_k3s(stride, pidx):
         I.L("const W4<R> x3 = v3_dual(ew, jtt, kq, kw, %s);" % I.ik2(*range(N)))
         I.L("const W4<R> x1 = wadd(bilinear(ub, chw), x3), x2 = wsub(bilinear(q1w, vv), x3);")
         I.flops += 2 * FL5["bilinear"] + FL5["v3_dual"] + 2 * FL5["wadd"]
+        if cache_u:
+            I.L("const W4<R> " + ", ".join("u%d = sc_ldw<R>(sc, %s + %d)" % (k, ubase, k) for k in range(3, 6)) + ";")
         for k0 in (0, 3):                              # three currents in flight at a time
-            for k in range(k0, k0 + 3):
-                I.ldw("u%d" % k, lay.U[(w, k)])
+            if not cache_u:
+                for k in range(k0, k0 + 3):
+                    I.ldw("u%d" % k, lay.U[(w, k)])
             I.L("const Cx<R> " + ", ".join("a1_%d = wdot(u%d, x1), a2_%d = wdot(u%d, x2)" % (k, k, k, k) for k in range(k0, k0 + 3)) + ";")
         I.flops += 12 * FL5["wdot"]
         for k in range(6):
@@ -850,9 +901,21 @@ def build_k3s(stride, pidx):
                 insts.append(I)
         add_group("contact_m0" if m_class else "contact", insts, 1)
     I = Inst5(lay, stride)
+    if I.in_tm(lay.J):
+        I.L("xwait_st<TM>();")
+    for r0 in range(0, 24, 4):
+        if I.in_tm(lay.J):     # four ordered amplitudes per tcgen05.ld x16, cleared with one tcgen05.st x16
+            o = eo(lay.J + 2 * r0, stride)
+            I.L("XW<R, TM> zx%d; xldw_issue<R, TM>(zx%d, sm, tm, %d);" % (r0, r0, o))
+            I.L("const W4<R> zw%d = xldw_get<R, TM>(zx%d);" % (r0, r0))
+            I.L("xstw<R, TM>(sm, tm, %d, W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0});" % o)
+            for k in range(4):
+                I.L("const Cx<R> Z%d = {zw%d.r%d, zw%d.i%d};" % (r0 + k, r0, k, r0, k))
+        else:
+            for r in range(r0, r0 + 4):
+                I.L("R zr%d, zi%d; cget<R>(sm + %d, zr%d, zi%d); cset<R>(sm + %d, (R)0, (R)0);" % (r, r, eo(lay.J + 2 * r, stride), r, r, eo(lay.J + 2 * r, stride)))
+                I.L("const Cx<R> Z%d = {zr%d, zi%d};" % (r, r, r))
     for r in range(24):
-        I.L("R zr%d, zi%d; cget<R>(sm + %d, zr%d, zi%d); cset<R>(sm + %d, (R)0, (R)0);" % (r, r, eo(lay.J + 2 * r, stride), r, r, eo(lay.J + 2 * r, stride)))
-        I.L("const Cx<R> Z%d = {zr%d, zi%d};" % (r, r, r))
         I.jamp("Z%d" % r, c_close(ONE, ebasis[r], ONE), pidx)
     I.namp -= 24
     I.flush_direct()
@@ -1096,15 +1159,16 @@ def emit_orbit5_process(name="gg_ttxggg"):
     if K1_PRE and K1_PARTS == 1:
         # FP64: with the two (u, w) halves as a nested loop (70 KB loop body instead of 93 KB: instruction fetch); FP32: without (measured
         # 41.6 ms per pass against 44.3 ms with the nested loop, whose table-driven accumulator offsets cost more than the fetch saves)
-        lay0, groups0 = build_k1(BLOCK1, pidx, uw_loop=K1S_UW_LOOP, pre=True)
+        lay0, groups0 = build_k1(BLOCK1, pidx, uw_loop=K1S_UW_LOOP, pre=True, cache_q=K1_CACHE_Q[0])
         src0, info0s = emit_kernel(name, "0s", lay0, groups0, BLOCK1, only="f64tm" if K1S_UW_LOOP else None, delegate="0f" if K1S_UW_LOOP else None)
         files["gen_%s_o0s.cu" % name] = src0
         assert info0s["amplitudes"] == kinfo[0]["amplitudes"]
         if K1S_UW_LOOP:
-            lay0f, groups0f = build_k1(BLOCK1, pidx, uw_loop=False, pre=True)
+            lay0f, groups0f = build_k1(BLOCK1, pidx, uw_loop=False, pre=True, cache_q=K1_CACHE_Q[1])
             src0f, info0f = emit_kernel(name, "0f", lay0f, groups0f, BLOCK1, only="f32")
             files["gen_%s_o0f.cu" % name] = src0f
-            assert info0f["cache_vectors"] == info0s["cache_vectors"]
+            info0s["cache_vectors"] = max(info0s["cache_vectors"], info0f["cache_vectors"])    # one region serves both forms
+            info0s["fp32_form"] = dict(flops=info0f["flops"], redundant=info0f["redundant"], cache_vectors=info0f["cache_vectors"])
     namp = sum(k["amplitudes"] for k in kinfo)
     assert namp == 1890, namp
     # colour sum in its symmetric form (S§8(d)): per part  sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), as for the smaller
@@ -1152,13 +1216,13 @@ def emit_orbit5_process(name="gg_ttxggg"):
     nhel, ngroups = 1 << NPAR, (1 << NPAR) // HEL_PER_CTA
     shared_event = nhel * (algo - a2) + ngroups * (info3["group_flops"] - pa["pairs"]) + nhel * (info3["flops"] - info3["redundant"]) + fixed
     executed_shared = executed - k2["flops"] + info3["flops"] + info3["group_flops"] / HEL_PER_CTA
-    cache_vectors = 0
+    cache_vectors = info3["cache_vectors"]      # one region serves the sharing kernels one after the other
     if info0s is not None:     # kernel o0 per helicity -> per group of four + per helicity
         k0 = kinfo[0]
         shared_event += -nhel * (k0["flops"] - k0["redundant"]) + nhel * (info0s["flops"] - info0s["redundant"]) \
             + ngroups * (info0s["group_flops"] - info0s["group_redundant"])
         executed_shared += -k0["flops"] + info0s["flops"] + info0s["group_flops"] / HEL_PER_CTA
-        cache_vectors = info0s["cache_vectors"]
+        cache_vectors = max(cache_vectors, info0s["cache_vectors"])
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // the sharing kernel exists in its tensor-memory form only")
