@@ -59,7 +59,8 @@ typedef enum {
   ME_ENOTFILTERED = 3, /* me_compute before me_filter_helicities / me_set_helicities */
   ME_EALIGN = 4,       /* d_momenta / d_me not 16-byte aligned */
   ME_ENOMEM = 5,       /* host or device allocation failed */
-  ME_ECUDA = 6         /* a CUDA call failed; me_strerror(ME_ECUDA) names the last one */
+  ME_ECUDA = 6,        /* a CUDA call failed; me_strerror(ME_ECUDA) names the last one */
+  ME_ETOOLARGE = 7     /* me_compute_static: n beyond ME_STATIC_MAX_EVENTS; me_strerror(ME_ETOOLARGE) says by how much */
 } me_status;
 
 typedef enum {
@@ -151,6 +152,23 @@ me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
  * Errors: ME_EINVAL, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA (launch failure). */
 me_status me_compute(me_ctx* ctx, const double* d_momenta, int64_t n, me_precision precision,
                      double* d_me, void* stream);
+
+/* The hot path for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
+ * g g -> t t~ g g only (ME_EPROCESS otherwise), at most ME_STATIC_MAX_EVENTS events per call.  Same arguments, layout and result as
+ * me_compute with ME_OPT_SHARE_CURRENTS on (ME_OPT_PARITY_PAIRING is honoured), same kernel; the kernel's current cache (SURVEY.md section
+ * 8(f) item 4: sub-tree currents parked across the helicity walk) is not the context's lazily allocated scratch but a file-scope
+ * `static __device__` array of the library, 64 CTAs x 208 KB = 13 MiB, which every GPU that loads the library holds until exit.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine; the first call on a device resolves the
+ * array's device address (cudaGetSymbolAddress, once per device).  Asynchronous on `stream`, no synchronisation, no copy.
+ * EVERY call on a device, from any context, uses the same array: calls that overlap on the GPU (different streams, threads or
+ * contexts) race on it and give wrong results; calls on one stream, or otherwise ordered on the device, are safe.  The array keeps
+ * the last call's contents; nothing in it has to start at zero (the first step of the helicity walk writes every vector it later
+ * reads), so the call clears nothing.  It is independent of the context's own scratch and stream ordering (include "Concurrency").
+ * n = 0 is a no-op.  Errors: ME_EINVAL, ME_EPROCESS, ME_ENOTFILTERED, ME_EALIGN, ME_ETOOLARGE (n > ME_STATIC_MAX_EVENTS; nothing is
+ * launched), ME_ECUDA. */
+#define ME_STATIC_MAX_EVENTS 8192
+me_status me_compute_static(me_ctx* ctx, const double* d_momenta, int64_t n, me_precision precision,
+                            double* d_me, void* stream);
 
 /* The same computation with HOST buffers: the end-to-end call ("e2e"; the paper's
  * data flow "momenta in, matrix elements out", section 2, as seen from a host-side event generator).

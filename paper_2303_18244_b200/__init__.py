@@ -11,13 +11,14 @@ import os
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libme_b200.so")
 
-ME_OK, ME_EINVAL, ME_EPROCESS, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA = range(7)
+ME_OK, ME_EINVAL, ME_EPROCESS, ME_ENOTFILTERED, ME_EALIGN, ME_ENOMEM, ME_ECUDA, ME_ETOOLARGE = range(8)
+ME_STATIC_MAX_EVENTS = 8192
 ME_EPEM_MUPMUM, ME_GG_TTX, ME_GG_TTXG, ME_GG_TTXGG, ME_GG_TTXGGG = range(5)
 ME_FP64, ME_MIXED, ME_FP32 = range(3)
 ME_OPT_PARITY_PAIRING, ME_OPT_SHARE_CURRENTS = 0, 1
 PRECISIONS = {"fp64": ME_FP64, "mixed": ME_MIXED, "fp32": ME_FP32}
 
-EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute", "me_compute_host",
+EXPORTS = ("me_create", "me_destroy", "me_get_info", "me_filter_helicities", "me_set_helicities", "me_compute", "me_compute_host", "me_compute_static",
            "me_compute_helicities", "me_compute_jamps", "me_set_option", "me_select_helicity_color", "me_unweight", "me_color_matrix", "me_philox_uniform", "me_rambo",
            "me_fma_peak", "me_strerror")
 
@@ -61,6 +62,7 @@ def lib():
         L.me_unweight.argtypes = [vp, vp, i64, dbl, u64, u64, dbl, ctypes.POINTER(dbl), vp, ctypes.POINTER(i64), vp]
         L.me_compute.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_host.argtypes = [vp, vp, i64, cint, vp, vp]
+        L.me_compute_static.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_compute_helicities.argtypes = [vp, vp, i64, cint, vp, vp, vp]
         L.me_compute_jamps.argtypes = [vp, vp, i64, cint, vp, vp]
         L.me_color_matrix.argtypes = [vp, ctypes.POINTER(dbl)]
@@ -199,6 +201,15 @@ class MEContext:
         if out is None:
             out = torch.empty(n, dtype=torch.float64, device=momenta.device)
         _check(lib().me_compute(self._h, _ptr(momenta, torch.float64), n, int(precision), _ptr(out, torch.float64), _stream(stream)))
+        return out
+
+    def me_compute_static(self, momenta, n, precision=ME_FP64, out=None, stream=None):
+        """me_compute without any allocation inside the library (include/me.h me_compute_static): pass `out` to allocate nothing here either"""
+        import torch
+        assert momenta.numel() >= self.momenta_numel(n)
+        if out is None:
+            out = torch.empty(n, dtype=torch.float64, device=momenta.device)
+        _check(lib().me_compute_static(self._h, _ptr(momenta, torch.float64), n, int(precision), _ptr(out, torch.float64), _stream(stream)))
         return out
 
     def me_compute_helicities(self, momenta, n, precision=ME_FP64, stream=None):

@@ -24,6 +24,7 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
 NPAR = 6
+STATIC_MAX_EVENTS = 8192   # me_compute_static: events one call takes (its current cache is a file-scope device array of 64 CTAs x 208 KB = 13 MiB)
 NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
 NSCVEC_QUAD_END = 14  # the six colour-ordered four-gluon currents that close on the bare quark line,
 NSCVEC = 26         # and the two column-side combinations of each of the six rows2 instances
@@ -639,6 +640,8 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("#include <stdlib.h>")
+    S("#include <mutex>")
+    S("#define ME_STATIC_MAX_DEVICES 64")
     S("#define ME_SHARE_SLICE 524288L     // events per launch of the sharing kernel (%d KB of scratch per CTA in FP64)" % (NSCVEC * 8 * block * 8 // 1024))
     S("namespace me {")
     for gname, tmpl, rows in groups:
@@ -798,6 +801,45 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  }")
     S("#undef ME_LAUNCH")
     S("#undef ME_ARGS")
+    S("  return cudaGetLastError();")
+    S("}")
+    # ---- the sharing kernel on a scratch that nobody allocates (include/me.h me_compute_static): a file-scope device array of a fixed size
+    static_ctas = STATIC_MAX_EVENTS // block
+    S("// Sharing kernel without any allocation: its current cache is this file-scope array (%d CTAs x %d vectors x 8 x %d threads of double:" % (static_ctas, NSCVEC, block))
+    S("// %.1f MiB that every GPU which loads the library holds until exit).  In host code the NAME of the array is a host-side stand-in, not" % (static_ctas * NSCVEC * 8 * block * 8 / 2.0 ** 20))
+    S("// a device address: the launcher below asks the runtime for the address once per device, with that device current.")
+    S("static __device__ __align__(256) unsigned char static_scratch_%s[%dUL * %d * 8 * %d * sizeof(double)];" % (name, static_ctas, NSCVEC, block))
+    S("extern const long static_max_events_%s = %dL;" % (name, STATIC_MAX_EVENTS))
+    S("cudaError_t launch_%s_static(int precision, const LaunchArgs& a) {" % name)
+    S("  if (a.npad > %dL || a.me_out == nullptr || a.hel_per_event != nullptr) return cudaErrorInvalidValue;" % STATIC_MAX_EVENTS)
+    S("  static void* addr[ME_STATIC_MAX_DEVICES];         // device address of the array on every device seen so far")
+    S("  static std::mutex mtx;")
+    S("  int dev = -1;")
+    S("  cudaError_t e = cudaGetDevice(&dev);")
+    S("  if (e != cudaSuccess) return e;")
+    S("  if (dev < 0 || dev >= ME_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;")
+    S("  void* ptr = nullptr;")
+    S("  {")
+    S("    std::lock_guard<std::mutex> lock(mtx);")
+    S("    if (addr[dev] == nullptr) {                      // set-up, once per device")
+    S("      e = cudaGetSymbolAddress((void**)&addr[dev], static_scratch_%s);" % name)
+    S("      if (e != cudaSuccess) { addr[dev] = nullptr; return e; }")
+    S("    }")
+    S("    ptr = addr[dev];")
+    S("  }")
+    S("  // nothing in the array has to start at zero: the first step of the helicity walk writes every vector before any step reads it")
+    S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
+    S("  const size_t smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.TM0, block))
+    S("#define ME_TARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, nullptr, nullptr, nullptr, ptr")
+    S("#define ME_TLAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
+    S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
+    S("    K<<<grid, %d, SMEM, a.stream>>>(ME_TARGS); } while (0)" % block)
+    S("  if (precision == 0) ME_TLAUNCH((k_%s<double, double, true, true>), smt);" % name)
+    S("  else if (precision == 1) ME_TLAUNCH((k_%s<double, float, true, true>), smt);" % name)
+    S("  else if (precision == 2) ME_TLAUNCH((k_%s<float, float, false, true>), smf);" % name)
+    S("  else return cudaErrorInvalidValue;")
+    S("#undef ME_TLAUNCH")
+    S("#undef ME_TARGS")
     S("  return cudaGetLastError();")
     S("}")
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))

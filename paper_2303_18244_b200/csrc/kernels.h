@@ -49,6 +49,10 @@ struct ProcTable {
 };
 
 extern const ProcTable tab_gg_ttx, tab_gg_ttxg, tab_gg_ttxgg, tab_gg_ttxggg;
+// g g -> t t~ g g, sharing kernel on a file-scope device array instead of a.scratch (include/me.h me_compute_static): no allocation;
+// a.hels in walk order (gray_rank), a.npad <= static_max_events_gg_ttxgg, only a.me_out is written
+cudaError_t launch_gg_ttxgg_static(int precision, const LaunchArgs& a);
+extern const long static_max_events_gg_ttxgg;
 
 // e+ e- -> mu+ mu-: couplings passed explicitly
 struct EpemCouplings { double gL, gR, mz, wz; };

@@ -71,6 +71,7 @@ extern "C" const char* me_strerror(me_status s) {
     case ME_ENOTFILTERED: return "helicities not filtered: call me_filter_helicities or me_set_helicities first";
     case ME_EALIGN: return "device buffer not 16-byte aligned";
     case ME_ENOMEM: return "out of memory";
+    case ME_ETOOLARGE: return g_errbuf;
     case ME_ECUDA: return g_errbuf;
   }
   return "unknown status";
@@ -352,6 +353,36 @@ extern "C" me_status me_compute(me_ctx* c, const double* d_mom, int64_t n, me_pr
   const unsigned char* hels; int nhel; double inv_avg; bool share;
   hel_list(c, &hels, &nhel, &inv_avg, &share);
   return run(c, d_mom, n, prec, hels, nhel, inv_avg, d_me, nullptr, nullptr, stream, nullptr, share);
+}
+
+// The hot path for callers that must not allocate (include/me.h): g g -> t t~ g g, currents shared across helicities, the current cache in
+// a file-scope device array of the generated kernel file.  Touches no buffer of the context except its helicity list (read) and creates,
+// grows or frees nothing; does not take part in the context's stream ordering (it does not use the context's scratch).
+extern "C" me_status me_compute_static(me_ctx* c, const double* d_mom, int64_t n, me_precision prec, double* d_me, void* stream) {
+  if (c == nullptr || n < 0) return ME_EINVAL;
+  if (c->process != ME_GG_TTXGG) return ME_EPROCESS;
+  if ((int)prec < 0 || (int)prec > 2) return ME_EINVAL;
+  if (n > (int64_t)me::static_max_events_gg_ttxgg) {
+    snprintf(g_errbuf, sizeof(g_errbuf), "me_compute_static: n = %lld exceeds ME_STATIC_MAX_EVENTS = %ld (the static scratch is sized for that)",
+             (long long)n, me::static_max_events_gg_ttxgg);
+    return ME_ETOOLARGE;
+  }
+  if (n == 0) return ME_OK;
+  if (d_mom == nullptr || d_me == nullptr) return ME_EINVAL;
+  if (!c->filtered) return ME_ENOTFILTERED;
+  if (((uintptr_t)d_mom & 15) || ((uintptr_t)d_me & 7)) return ME_EALIGN;
+  ME_ON_DEVICE(c);
+  me::LaunchArgs a;
+  a.mom = d_mom; a.n = n; a.npad = (n + ME_PAGE - 1) / ME_PAGE * ME_PAGE;
+  const bool half = c->pairing && c->nhalf > 0;           // the helicity list in walk order, as me_compute takes it with sharing on
+  a.hels = half ? c->d_hels_gray_half : c->d_hels_gray; a.nhel = half ? c->ngray_half : c->ngray;
+  a.mt = c->prm.mt; a.norm_hel = c->norm_hel; a.inv_avg = half ? 2.0 * c->inv_avg : c->inv_avg;
+  a.me_out = d_me; a.me_hel = nullptr; a.jamp_out = nullptr; a.stream = (cudaStream_t)stream;
+  a.scratch = nullptr; a.scratch_bytes = 0; a.hel_per_event = nullptr;
+  a.color_d = nullptr; a.color_f = nullptr; a.nsm = c->nsm; a.share = 1;
+  cudaError_t e = me::launch_gg_ttxgg_static((int)prec, a);
+  if (e != cudaSuccess) return cuda_fail(e, "me_compute_static");
+  return ME_OK;
 }
 
 static me_status host_init(me_ctx* c) {
