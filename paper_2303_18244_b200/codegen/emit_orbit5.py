@@ -41,6 +41,10 @@ K1_CACHE_Q = (False, True)   # ... (FP64 form, FP32 form) with the one-gluon qua
 K1S_UW_LOOP = True   # ... with the nested (u, w) loop in its FP64 form
 TM_K1 = ("FERM", "TMP", "J")   # kernel o0: spinor bases, ubar / v / ubar gamma v, the parked current and 36 local jamp accumulators = 120 slots
 TM_K2 = ("PAIR", "CHI")   # kernel o1: 10 gluon-pair currents + 5 column currents = 120 slots = 240 columns
+K1_INIT_STAGING = (True, False)   # kernel o0 / o0s (FP64 forms: True) and o0f (FP32: False) zero the staging rows of a helicity themselves instead of a
+                                  # memset in front of the pass.  Measured per pass: FP64 76.9 against 77.6 ms, FP32 40.3 against 40.1 ms.  (Plain stores on
+                                  # the first touch of a row, chosen by a flag from the instance table, were slower: 78.9 ms, the flush code doubles.)
+K2_CACHE_COLS = True     # kernel o1: the two column currents of every gluon pair parked in the current cache by the cols2 loop and reloaded by rows2
 K3S_CACHE_U = True       # sharing kernel o2s: the thirty ordered currents of a group in the L2-resident current cache (two CTAs per SM) instead of on chip (one)
 K3D_JACC = 48            # accumulator kernel o2d (current sharing off): one set of local jamp accumulators per last gluon, kept in tensor memory
 TM_K3 = ("J",)            # FP64: 96 slots = 192 columns, one CTA per SM; FP32: one column per slot, two CTAs per SM
@@ -193,6 +197,8 @@ class Inst5(Inst):
         """add the local accumulators into gj and clear them.  The add is a fire-and-forget reduction (RED.ADD, no
         read latency); every address is private to one thread, whose program order fixes the order of the adds, so
         the result is deterministic run to run."""
+        def out(sigma, re, im):
+            return "{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)%s); atomicAdd(g + npad32, (RJ)%s); }" % (self.P(2 * sigma), re, im)
         if self.in_tm(self.lay.J):
             # accumulators in tensor memory: four flows per tcgen05.ld x16, reduced into gj, cleared with one tcgen05.st x16
             items = sorted(self.local.items(), key=lambda t: t[1])
@@ -204,15 +210,15 @@ class Inst5(Inst):
                 self.L("{ XW<R, TM> jx; xldw_issue<R, TM>(jx, sm, tm, %d);" % o)
                 self.L("  const W4<R> jw = xldw_get<R, TM>(jx);")
                 for k, (sigma, loc) in enumerate(grp):
-                    self.L("  { RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)jw.r%d); atomicAdd(g + npad32, (RJ)jw.i%d); }" % (self.P(2 * sigma), k, k))
+                    self.L("  " + out(sigma, "jw.r%d" % k, "jw.i%d" % k))
                     self.flops += 2; self.redundant += 2
                 self.L("  xstw<R, TM>(sm, tm, %d, W4<R>{(R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0}); }" % o)
             self.local = {}
             return
         for sigma, loc in sorted(self.local.items(), key=lambda t: t[1]):
             o = eo(self.lay.J + 2 * loc, self.stride)
-            self.L("{ RJ* g = gj + (unsigned)%s * npad32; atomicAdd(g, (RJ)sm[%d]); atomicAdd(g + npad32, (RJ)sm[%d]); sm[%d] = 0; sm[%d] = 0; }"
-                   % (self.P(2 * sigma), o, o + 1, o, o + 1))
+            self.L(out(sigma, "sm[%d]" % o, "sm[%d]" % (o + 1)))
+            self.L("sm[%d] = 0; sm[%d] = 0;" % (o, o + 1))
             self.flops += 2; self.redundant += 2     # staging adds are overhead of the multi-kernel split, not of the method
         self.local = {}
 
@@ -276,15 +282,20 @@ def emit_rows2(I, a, b, pab, ea, eb):
     return [("rb", col_ab), ("rc", col_ba)]
 
 
-def emit_cols2(I, c, d, pcd, ec, ed, tag=""):
-    """the two colour-ordered column currents with gluons {c,d} attached (c<d), grown from the t~ end"""
+def emit_cols2(I, c, d, pcd, ec, ed, tag="", cached=None):
+    """the two colour-ordered column currents with gluons {c,d} attached (c<d), grown from the t~ end; cached = first vector of the
+    pair in the current cache: the currents are loaded from there (the cols2 loop of the same helicity has parked them) instead of built"""
+    col_cd, col_dc = c_step(c_leaf(c), cchi(d)), c_step(c_leaf(d), cchi(c))
+    if cached is not None:
+        vec = I.P(cached)
+        I.L("const W4<R> cb%s = sc_ldw<R>(sc, %s), cc%s = sc_ldw<R>(sc, %s + 1);" % (tag, vec, tag, vec))
+        return [("cb" + tag, col_cd), ("cc" + tag, col_dc)]
     I.ldw("chc" + tag, I.lay.CHI + 8 * c); I.ldw("chd" + tag, I.lay.CHI + 8 * d)
     row_side = rest_of(c, d)
     I.qvec("qc" + tag, row_side)
     I.L("const R iqc%s = %s;" % (tag, I.iq(*row_side)))
     I.fv("vv")
     # colour of a column step: -(gluon)(previous column); colour-ordered as in emit_rows2
-    col_cd, col_dc = c_step(c_leaf(c), cchi(d)), c_step(c_leaf(d), cchi(c))
     assert not _cdiff(c_step(cpair(c, d), ONE), col_cd, col_dc)
     I.L("const W4<R> spc%s = slash_col(%s, vv);" % (tag, pcd))
     I.L("const W4<R> cb%s = col_step(wadd(slash_col(%s, chd%s), spc%s), qc%s, mt, iqc%s), cc%s = col_step(wsub(slash_col(%s, chc%s), spc%s), qc%s, mt, iqc%s);"
@@ -331,7 +342,7 @@ def phase_a(lay, stride, add_group, want_pairs):
 # The 6 terms t_i stay in registers; 18 four-vectors X_j (bilinears of the fermion ends, dual currents of the
 # vertices that would extend t) are formed one after the other and each gives 6 amplitudes t_i . X_j.
 # ------------------------------------------------------------------------------------------
-def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False, cache_q=False):
+def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False, cache_q=False, init_staging=False):
     """part = None: all 18 vectors in one kernel; part = 0,1,2: six vectors each (the kernel then fits the
     instruction cache: the single kernel was ~12.5 k SASS instructions and stalled on instruction fetch)"""
     # no Q1 / CHI slots: the one-gluon quark currents are rebuilt where they are used (12 per block, ~15 % more flops), which
@@ -547,6 +558,9 @@ def build_k1(stride, pidx, part=None, nparts=3, uw_loop=None, pre=False, cache_q
         t.group_redundant = t.redundant; t.redundant = 0
         t.cache_vectors = 3 * len(pre_insts) + (10 if cache_q else 0)
     add_group("triples", insts, 1)
+    # the first kernel of a pass can zero the staging rows of a helicity itself, right before it adds into them (the lines are then in the L2
+    # for its first reductions), instead of a memset of the whole chunk in front of the pass
+    groups[-1][1].init_staging = bool(init_staging) and (part is None or part == 0)
     return lay, groups
 
 
@@ -569,7 +583,8 @@ def spair(p):
 # ------------------------------------------------------------------------------------------
 # kernel 2: amplitudes whose two ends carry (2 | 2), (2 | 1) or (1 | 2) gluons and whose middle is a gluon or a pair
 # ------------------------------------------------------------------------------------------
-def build_k2(stride, pidx):
+def build_k2(stride, pidx, cache_cols=None):
+    cache_cols = K2_CACHE_COLS if cache_cols is None else cache_cols
     # 226 slots per thread -> 128 threads per CTA: no Q1 slots (the row-side one-gluon currents are formed where they are
     # used: 5 per ten uses would do, +14 % flops), only the pair propagators; no local jamp accumulators: every (sub-)block touches each
     # colour flow once, its amplitudes are combined per flow in registers and added straight into the staging buffer
@@ -577,6 +592,7 @@ def build_k2(stride, pidx):
     groups = []
     add_group = _grouper(groups)
     phase_a(lay, stride, add_group, want_pairs=True)
+    pair_index = {p_: i_ for i_, p_ in enumerate(lay.PAIR)}
     # ---- rows2 loop: A = {a,b}; the three row currents on A meet (i) eps_m . chi2(B), (ii) pair(P) . chi1(w)
     insts = []
     for (a, b) in lay.PAIR:
@@ -592,8 +608,8 @@ def build_k2(stride, pidx):
             I.leaf("em", m); I.leaf("ec", c); I.leaf("ed", d)
             I.ldw("pcd", lay.PAIR[(c, d)])
             f0 = I.flops
-            cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
-            I.redundant += 2 * (I.flops - f0) // 3      # each chi2 set is formed for 3 masks A
+            cols = emit_cols2(I, c, d, "pcd", "ec", "ed", cached=2 * pair_index[(c, d)] if cache_cols else None)
+            I.redundant += I.flops - f0                 # the cols2 loop forms the same two currents of the pair (c, d): needed once per helicity
             I.namp += (9 - len(rows) * len(cols)) + (3 - len(rows))     # diagram terms folded into the colour-ordered currents
             xs = ["x%d" % k for k in range(len(cols))]
             I.L("const W4<R> " + ", ".join("%s = slash_col(em, %s)" % (xn, cn) for xn, (cn, _) in zip(xs, cols)) + ";"); I.flops += len(cols) * FL5["slash_col"]
@@ -611,7 +627,9 @@ def build_k2(stride, pidx):
             I.L("}")
             I.L("}")
         insts.append(I)
-    add_group("rows2", insts, 1)
+    rows2_insts = insts
+    if not cache_cols:
+        add_group("rows2", rows2_insts, 1)
     # ---- cols2 loop: B = {c,d}; q1(x) . pair(P)-slash . chi2(B)
     insts = []
     for (c, d) in lay.PAIR:
@@ -620,6 +638,9 @@ def build_k2(stride, pidx):
         I.leaf("ec", c); I.leaf("ed", d)
         I.ldw("pcd", lay.PAIR[(c, d)])
         cols = emit_cols2(I, c, d, "pcd", "ec", "ed")
+        if cache_cols:      # parked for the three rows2 sub-blocks that need the same two currents (this loop then runs first)
+            vec = I.P(2 * pair_index[(c, d)])
+            I.L("sc_stw<R>(sc, %s, %s); sc_stw<R>(sc, %s + 1, %s);" % (vec, cols[0][0], vec, cols[1][0]))
         I.namp += 3 * (3 - len(cols))
         for x in rest:
             p = spair([l for l in rest if l != x])
@@ -637,6 +658,9 @@ def build_k2(stride, pidx):
             I.L("}")
         insts.append(I)
     add_group("cols2", insts, 1)
+    if cache_cols:
+        groups[-1][1].cache_vectors = 2 * len(lay.PAIR)
+        add_group("rows2", rows2_insts, 1)
     return lay, groups
 
 
@@ -957,7 +981,7 @@ def prologue_lines(lay):
     return out, fixed
 
 
-def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
+def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None, delegate_init=False):
     """only: None (FP64 instances with part of the slots in tensor memory or all in shared memory, FP32 in shared memory) or 'tm' (every
     instance in its tensor-memory layout; ki is then a tag like '2d'); delegate: tag of the tensor-memory variant this kernel's
     launcher hands every precision to unless ME_NO_TMEM=1"""
@@ -1039,6 +1063,7 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
     else:
         S("  for (int s = 0; s < %d; ++s) sm[ME_EO(%d + s)] = 0;" % (2 * lay.jacc, lay.J))
     has_pre = any(getattr(t, "pre", False) for _, t, _, _ in groups)
+    init_staging = any(getattr(t, "init_staging", False) for _, t, _, _ in groups)
     S("  const int hc_end = !live ? 0 : (int)(blockIdx.y + 1) * ME_HEL_PER_CTA < nh ? (int)(blockIdx.y + 1) * ME_HEL_PER_CTA : nh;")
     if has_pre:
         # sharing kernel: the helicities of this CTA share their gluon helicities (the host groups the list: include/me.h); what depends on
@@ -1052,8 +1077,17 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
         S("  }")
     S("  for (int hc = (int)blockIdx.y * ME_HEL_PER_CTA; hc < hc_end; ++hc) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[hc];")
-    S("    if (h == 255) continue;                       // padding of a grouped helicity list")
     S("    RJ* gj = gjbase + (long)hc * %d * npad + e;" % (2 * 120))
+    if init_staging:
+        S("    if (h == 255) {                               // padding of a grouped helicity list: this kernel initialises the staging rows, these to zero")
+        S("      for (int r = 0; r < %d; ++r) gj[(unsigned)r * npad32] = (RJ)0;" % (2 * 120))
+        S("      continue;")
+        S("    }")
+        if True:
+            S("#pragma unroll 8")
+            S("    for (int r = 0; r < %d; ++r) gj[(unsigned)r * npad32] = (RJ)0;      // the rows of this helicity start at zero (no memset of the staging buffer)" % (2 * 120))
+    else:
+        S("    if (h == 255) continue;                       // padding of a grouped helicity list")
     if lay.FERM is not None:
         S("    {")
         if tm0 is not None and lay.FERM["sbt"] >= tm0:
@@ -1121,7 +1155,11 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None):
         S("  }")
     S("  return cudaGetLastError();")
     S("}")
-    S("extern const MultiKernel mk_%s_o%s = {launch_o%s};" % (name, ki, ki))
+    # bit p of the mask: the kernel this entry launches for precision p zeroes its staging rows itself
+    own = 7 if init_staging else 0
+    if only == "f64tm":
+        own = (own & 3) | (4 if delegate_init else 0)
+    S("extern const MultiKernel mk_%s_o%s = {launch_o%s, %d};" % (name, ki, ki, own))
     S("}  // namespace me")
     flops = sum(t.flops * len(rows) for _, t, rows, _ in groups)
     redundant = sum(getattr(t, "redundant", 0) * len(rows) for _, t, rows, _ in groups)
@@ -1137,7 +1175,7 @@ def emit_orbit5_process(name="gg_ttxggg"):
     color_num, color_denom = color_matrix(perms)
     ncol = len(perms)
     files, kinfo = {}, []
-    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS)) for i in range(K1_PARTS)) + (build_k2, build_k3)
+    builders = tuple((lambda st, px, i=i: build_k1(st, px, i, K1_PARTS, init_staging=K1_INIT_STAGING[0])) for i in range(K1_PARTS)) + ((lambda st, px: build_k2(st, px, cache_cols=False)), build_k3)
     for ki, b in enumerate(builders):
         lay, groups = b(BLOCK1, pidx)
         last = ki == len(builders) - 1
@@ -1159,16 +1197,24 @@ def emit_orbit5_process(name="gg_ttxggg"):
     if K1_PRE and K1_PARTS == 1:
         # FP64: with the two (u, w) halves as a nested loop (70 KB loop body instead of 93 KB: instruction fetch); FP32: without (measured
         # 41.6 ms per pass against 44.3 ms with the nested loop, whose table-driven accumulator offsets cost more than the fetch saves)
-        lay0, groups0 = build_k1(BLOCK1, pidx, uw_loop=K1S_UW_LOOP, pre=True, cache_q=K1_CACHE_Q[0])
-        src0, info0s = emit_kernel(name, "0s", lay0, groups0, BLOCK1, only="f64tm" if K1S_UW_LOOP else None, delegate="0f" if K1S_UW_LOOP else None)
+        lay0, groups0 = build_k1(BLOCK1, pidx, uw_loop=K1S_UW_LOOP, pre=True, cache_q=K1_CACHE_Q[0], init_staging=K1_INIT_STAGING[0])
+        src0, info0s = emit_kernel(name, "0s", lay0, groups0, BLOCK1, only="f64tm" if K1S_UW_LOOP else None, delegate="0f" if K1S_UW_LOOP else None,
+                                    delegate_init=K1_INIT_STAGING[1])
         files["gen_%s_o0s.cu" % name] = src0
         assert info0s["amplitudes"] == kinfo[0]["amplitudes"]
         if K1S_UW_LOOP:
-            lay0f, groups0f = build_k1(BLOCK1, pidx, uw_loop=False, pre=True, cache_q=K1_CACHE_Q[1])
+            lay0f, groups0f = build_k1(BLOCK1, pidx, uw_loop=False, pre=True, cache_q=K1_CACHE_Q[1], init_staging=K1_INIT_STAGING[1])
             src0f, info0f = emit_kernel(name, "0f", lay0f, groups0f, BLOCK1, only="f32")
             files["gen_%s_o0f.cu" % name] = src0f
             info0s["cache_vectors"] = max(info0s["cache_vectors"], info0f["cache_vectors"])    # one region serves both forms
             info0s["fp32_form"] = dict(flops=info0f["flops"], redundant=info0f["redundant"], cache_vectors=info0f["cache_vectors"])
+    # sharing-path form of the second kernel: column currents of a helicity through the current cache
+    info1s = None
+    if K2_CACHE_COLS and K1_PARTS == 1:
+        lay1, groups1 = build_k2(BLOCK1, pidx, cache_cols=True)
+        src1, info1s = emit_kernel(name, "1s", lay1, groups1, BLOCK1)
+        files["gen_%s_o1s.cu" % name] = src1
+        assert info1s["amplitudes"] == kinfo[1]["amplitudes"]
     namp = sum(k["amplitudes"] for k in kinfo)
     assert namp == 1890, namp
     # colour sum in its symmetric form (S§8(d)): per part  sum_r x_r (C_rr x_r + 2 sum_{c<r} C_rc x_c), as for the smaller
@@ -1200,10 +1246,14 @@ def emit_orbit5_process(name="gg_ttxggg"):
     S("extern const MultiKernel mk_%s_o2s;" % name)
     if info0s is not None:
         S("extern const MultiKernel mk_%s_o0s;" % name)
+    if info1s is not None:
+        S("extern const MultiKernel mk_%s_o1s;" % name)
     S("static const MultiKernel* const parts_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_o%d" % (name, ki) for ki in range(len(kinfo)))))
     sh_names = ["o%d" % ki for ki in range(len(kinfo) - 1)] + ["o2s"]
     if info0s is not None:
         sh_names[0] = "o0s"
+    if info1s is not None:
+        sh_names[1] = "o1s"
     S("static const MultiKernel* const parts_sh_%s[%d] = {%s};" % (name, len(kinfo), ", ".join("&mk_%s_%s" % (name, k) for k in sh_names)))
     # current sharing: the helicity list is ordered by gluon helicities, the four quark-helicity assignments of each adjacent (rank table);
     # flops per event with it on, over the full helicity set: kernel o2 per helicity -> per group of four + per helicity
@@ -1223,6 +1273,10 @@ def emit_orbit5_process(name="gg_ttxggg"):
             + ngroups * (info0s["group_flops"] - info0s["group_redundant"])
         executed_shared += -k0["flops"] + info0s["flops"] + info0s["group_flops"] / HEL_PER_CTA
         cache_vectors = max(cache_vectors, info0s["cache_vectors"])
+    if info1s is not None:     # same algorithm; the executed count loses the rebuilt column currents
+        executed_shared += -kinfo[1]["flops"] + info1s["flops"]
+        assert kinfo[1]["flops"] - kinfo[1]["redundant"] == info1s["flops"] - info1s["redundant"]
+        cache_vectors = max(cache_vectors, info1s["cache_vectors"])
     S("static const double color_num_%s[%d] = {%s};" % (name, ncol * ncol, ", ".join(str(float(x)) for row in color_num for x in row)))
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';   // the sharing kernel exists in its tensor-memory form only")

@@ -126,7 +126,7 @@ static cudaError_t launch_multi_slice(int precision, const LaunchArgs& a, long h
   for (int base = 0; base < a.nhel; base += ME_HEL_CHUNK) {
     const int nh = a.nhel - base < ME_HEL_CHUNK ? a.nhel - base : ME_HEL_CHUNK;
     MultiArgs m{a.mom, a.npad, a.hels + base, nh, a.mt, a.scratch, a.stream, a.hel_per_event, a.n, cache};
-    {   // every diagram kernel ADDS its colour flows into the staging buffer
+    if (!((parts[0]->zeroes_staging >> precision) & 1)) {   // every diagram kernel ADDS its colour flows into the staging buffer
       const size_t esz = precision == 2 ? sizeof(float) : sizeof(double);
       cudaError_t e = cudaMemsetAsync(a.scratch, 0, (size_t)nh * ncol * 2 * a.npad * esz, a.stream);
       if (e != cudaSuccess) return e;

@@ -18,7 +18,9 @@ struct MultiArgs {
   const int* hel_per_event; long n;
   void* cache;      // sharing kernels: L2-resident region for currents parked across the helicities of a CTA (null: not available)
 };
-struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); };
+// zeroes_staging: bit p set = the kernel launched for precision p zeroes the staging rows of a helicity itself before it adds into them;
+// when the first kernel of a pass says so the staging buffer is not zeroed (cudaMemsetAsync) in front of the pass
+struct MultiKernel { cudaError_t (*launch)(int precision, const MultiArgs&); int zeroes_staging; };
 
 cudaError_t launch_multi(int precision, const LaunchArgs& a, const MultiKernel* const* parts, int nparts, int ncol,
                          const double* color_num_host);
