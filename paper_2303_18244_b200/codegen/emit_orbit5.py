@@ -45,6 +45,8 @@ K1_INIT_STAGING = (True, False)   # kernel o0 / o0s (FP64 forms: True) and o0f (
                                   # memset in front of the pass.  Measured per pass: FP64 76.9 against 77.6 ms, FP32 40.3 against 40.1 ms.  (Plain stores on
                                   # the first touch of a row, chosen by a flag from the instance table, were slower: 78.9 ms, the flush code doubles.)
 K2_CACHE_COLS = True     # kernel o1: the two column currents of every gluon pair parked in the current cache by the cols2 loop and reloaded by rows2
+MIN_CTAS_F32 = {"2s": 3}  # kernel tag -> minimum CTAs per SM asked of the compiler for the FP32 instantiation (register cap).  o2s in FP32 is latency-bound and
+                          # small in shared / tensor memory: 168 registers (8 B of spill) and three CTAs per SM: FP32 pass 40.1 -> 39.2 ms; four (128 registers): 40.4 ms
 K3S_CACHE_U = True       # sharing kernel o2s: the thirty ordered currents of a group in the L2-resident current cache (two CTAs per SM) instead of on chip (one)
 K3D_JACC = 48            # accumulator kernel o2d (current sharing off): one set of local jamp accumulators per last gluon, kept in tensor memory
 TM_K3 = ("J",)            # FP64: 96 slots = 192 columns, one CTA per SM; FP32: one column per slot, two CTAs per SM
@@ -1025,8 +1027,10 @@ def emit_kernel(name, ki, lay, groups, BLOCK, only=None, delegate=None, delegate
                 S("  {%s}," % ", ".join(str(v) for v in r))
             S("};")
     S("template <typename R, typename RJ, bool TM>")
-    S("__global__ void __launch_bounds__(%d) k_%s_o%s(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
-      " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n, void* __restrict__ cache) {" % (BLOCK, name, ki))
+    minb = MIN_CTAS_F32.get(str(ki), 0)
+    bounds = "%d" % BLOCK if not minb else "%d, sizeof(R) == 4 ? %d : 1" % (BLOCK, minb)
+    S("__global__ void __launch_bounds__(%s) k_%s_o%s(const double* __restrict__ mom, long npad, const unsigned char* __restrict__ hels, int nh,"
+      " double mt_d, RJ* __restrict__ gjbase, const int* __restrict__ helpe, long n, void* __restrict__ cache) {" % (bounds, name, ki))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
