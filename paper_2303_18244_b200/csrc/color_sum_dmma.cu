@@ -45,24 +45,26 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
     const long e0 = (tile * CD_WARPS + w) * 8;
     if (e0 >= npad) continue;                              // npad is a multiple of 32: a warp is either fully in or out
     double me_acc0 = 0, me_acc1 = 0;
+    double bre[CD_PF], bim[CD_PF];                         // B fragments of the next batch of k-steps, always one batch ahead (also across helicities)
+#pragma unroll
+    for (int j = 0; j < CD_PF; ++j) {
+      const double* p = gj + e0 + (long)(2 * (4 * j + kr)) * npad + ec;
+      bre[j] = p[0]; bim[j] = p[npad];
+    }
     for (int hc = 0; hc < nh; ++hc) {
       const double* g = gj + (long)hc * (2 * CD_NCOL) * npad + e0;
       double acc[CD_RB][2][2];
 #pragma unroll
       for (int rb = 0; rb < CD_RB; ++rb) { acc[rb][0][0] = acc[rb][0][1] = acc[rb][1][0] = acc[rb][1][1] = 0; }
-      double bre[CD_PF], bim[CD_PF];
-#pragma unroll
-      for (int j = 0; j < CD_PF; ++j) {
-        const double* p = g + (long)(2 * (4 * j + kr)) * npad + ec;
-        bre[j] = p[0]; bim[j] = p[npad];
-      }
 #pragma unroll   // fully unrolled: the triangular skip below is then resolved at compile time (a predicated-off DMMA still costs its pipe slot)
       for (int kb = 0; kb < CD_KS; kb += CD_PF) {
         double nre[CD_PF], nim[CD_PF];
-        if (kb + CD_PF < CD_KS) {
+        const bool more = kb + CD_PF < CD_KS;              // (compile-time after unrolling)
+        if (more || hc + 1 < nh) {                         // the last batch of a helicity fetches the first batch of the next one: its latency hides behind the epilogue
+          const double* gn = more ? g + (long)(2 * 4 * (kb + CD_PF)) * npad : g + (long)(2 * CD_NCOL) * npad;
 #pragma unroll
           for (int j = 0; j < CD_PF; ++j) {
-            const double* p = g + (long)(2 * (4 * (kb + CD_PF + j) + kr)) * npad + ec;
+            const double* p = gn + (long)(2 * (4 * j + kr)) * npad + ec;
             nre[j] = p[0]; nim[j] = p[npad];
           }
         }
@@ -78,7 +80,7 @@ __global__ void __launch_bounds__(32 * CD_WARPS, 1) k_color_sum_dmma(const doubl
             dmma8x8x4(acc[rb][1][0], acc[rb][1][1], a, bim[j]);
           }
         }
-        if (kb + CD_PF < CD_KS) {
+        if (more || hc + 1 < nh) {
 #pragma unroll
           for (int j = 0; j < CD_PF; ++j) { bre[j] = nre[j]; bim[j] = nim[j]; }
         }
