@@ -24,6 +24,7 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
 NPAR = 6
+MIN_SEG_STEPS = 8          # helicity-segment split of small batches: steps of the helicity list per segment at least (every segment starts with a full evaluation)
 STATIC_MAX_EVENTS = 8192   # me_compute_static: events one call takes (its current cache is a file-scope device array of 64 CTAs x 208 KB = 13 MiB)
 NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
 NSCVEC_QUAD_END = 14  # the six colour-ordered four-gluon currents that close on the bare quark line,
@@ -657,10 +658,10 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("// SH: current sharing across helicities (include/me.h ME_OPT_SHARE_CURRENTS): hels is in walk order (reflected Gray code, quark helicities")
     S("// fastest); a current whose own helicities did not change since the previous step is not re-evaluated (pairs, one-gluon quark currents:")
     S("// their slots still hold it; three-gluon sub-trees: reloaded from the L2-resident scratch `scratch`, %d vectors per thread)" % NSCVEC)
-    S("template <typename R, typename RC, bool TM, bool SH>")
+    S("template <typename R, typename RC, bool TM, bool SH, bool SEG = false>")
     S("__global__ void __launch_bounds__(%d) k_%s(const double* __restrict__ mom, long n, long npad, const unsigned char* __restrict__ hels, int nhel,"
       " double mt_d, double norm_hel, double inv_avg, double* __restrict__ me_out, double* __restrict__ me_hel, double* __restrict__ jamp_out,"
-      " const int* __restrict__ helpe, void* __restrict__ scratch) {" % (block, name))
+      " const int* __restrict__ helpe, void* __restrict__ scratch, double* __restrict__ part) {" % (block, name))
     S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
     S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const long e0 = (long)blockIdx.x * blockDim.x + threadIdx.x;")
@@ -701,10 +702,19 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     fixed += 40
     S("  }")
     S("  R* sc = nullptr;")
-    S("  if constexpr (SH) sc = reinterpret_cast<R*>(scratch) + ((size_t)blockIdx.x * (%d * 8 * ME_SM_STRIDE) + 2 * threadIdx.x);" % NSCVEC)
+    S("  if constexpr (SH) sc = reinterpret_cast<R*>(scratch) + ((size_t)((SEG ? blockIdx.y * gridDim.x : 0u) + blockIdx.x) * (%d * 8 * ME_SM_STRIDE) + 2 * threadIdx.x);" % NSCVEC)
     S("  double acc = 0;")
     S("  int hprev = -1;")
-    S("  for (int ih = 0; ih < nhel; ++ih) {")
+    S("  // small batches: gridDim.y CTAs share the helicity list of an event block, each its own contiguous segment (the walk restarts with a")
+    S("  // full evaluation); the |M|^2 of every step goes to part[step][event] and k_sum_steps adds them in list order: the same sequence of")
+    S("  // additions as the loop below makes for gridDim.y = 1, so the result does not depend on the split, bit for bit")
+    S("  // (SEG = false: the kernel of the large batches, one segment, no per-step buffer: nothing of this costs it a register)")
+    S("  int ih_begin = 0, ih_end = nhel;")
+    S("  if constexpr (SEG) {")
+    S("    const int seg_len = (nhel + (int)gridDim.y - 1) / (int)gridDim.y;")
+    S("    ih_begin = (int)blockIdx.y * seg_len; ih_end = ih_begin + seg_len < nhel ? ih_begin + seg_len : nhel;")
+    S("  }")
+    S("  for (int ih = ih_begin; ih < ih_end; ++ih) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
     S("    const int chg = (SH && hprev >= 0) ? (h ^ hprev) : %d;      // helicities that changed since the previous step" % ((1 << NPAR) - 1))
     S("    hprev = h;")
@@ -763,10 +773,31 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
         S("    " + l)
     S("    const double meh = (double)cs;")
     S("    if (me_hel != nullptr && e0 < n) me_hel[(long)h * n + e0] = meh * norm_hel;")
-    S("    acc += meh;")
+    S("    if constexpr (SEG) { if (e0 < n) part[(long)ih * n + e0] = meh; }")
+    S("    else acc += meh;")
     S("  }")
-    S("  if (me_out != nullptr && e0 < n) me_out[e0] = acc * norm_hel * inv_avg;")
+    S("  if constexpr (!SEG) { if (me_out != nullptr && e0 < n) me_out[e0] = acc * norm_hel * inv_avg; }")
     S("  if constexpr (TM) tm_free(tm_base, %d);" % lay.tm_cols)
+    S("}")
+    S("// sum over the steps of the helicity list in list order (see the kernel above)")
+    S("static __global__ void k_sum_steps_%s(const double* __restrict__ part, int nhel, long n, double norm_hel, double inv_avg, double* __restrict__ me_out) {" % name)
+    S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
+    S("  if (e >= n) return;")
+    S("  double acc = 0;")
+    S("  for (int ih = 0; ih < nhel; ++ih) acc += part[(long)ih * n + e];")
+    S("  me_out[e] = acc * norm_hel * inv_avg;")
+    S("}")
+    S("// segments of the helicity list per event block: as many as fill the CTA slots of the device (two per SM), at least %d steps each" % MIN_SEG_STEPS)
+    S("static int segments_%s(long npad, int nhel, int nsm) {" % name)
+    S("  const long ctas = (npad + %d - 1) / %d;" % (block, block))
+    S("  long s = (2L * nsm) / ctas;")
+    S("  if (s > nhel / %d) s = nhel / %d;" % (MIN_SEG_STEPS, MIN_SEG_STEPS))
+    S("  return s < 1 ? 1 : (int)s;")
+    S("}")
+    S("// bytes of the current cache: one region per CTA, nseg segments per event block (0: kernel without sharing, no cache)")
+    S("static size_t cache_bytes_%s(int precision, long npad, int nseg) {" % name)
+    S("  const long np = npad < ME_SHARE_SLICE ? npad : ME_SHARE_SLICE;")
+    S("  return (size_t)((np + %d - 1) / %d) * nseg * %d * 8 * %d * (precision == 2 ? sizeof(float) : sizeof(double));" % (block, block, NSCVEC, block))
     S("}")
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
@@ -774,19 +805,33 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  // FP64 amplitudes (double and mixed): tensor-memory kernel, two CTAs per SM; ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
     S("  const bool sh = a.share != 0 && a.hel_per_event == nullptr && a.scratch != nullptr && !no_tmem && a.me_hel == nullptr && a.jamp_out == nullptr && a.me_out != nullptr;")
-    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event, a.scratch")
+    S("  // small batch, only me_out wanted: split the helicity list over gridDim.y (the per-step buffer sits behind the current cache in a.scratch)")
+    S("  const bool only_me = a.hel_per_event == nullptr && a.me_hel == nullptr && a.jamp_out == nullptr && a.me_out != nullptr;")
+    S("  const int nseg = (only_me && sh) ? segments_%s(a.npad, a.nhel, a.nsm) : 1;" % name)
+    S("  double* part = nullptr;")
+    S("  if (nseg > 1) {")
+    S("    const size_t off = (cache_bytes_%s(precision, a.npad, nseg) + 255) / 256 * 256;" % name)
+    S("    if (a.scratch_bytes < off + sizeof(double) * (size_t)a.nhel * a.n) return cudaErrorInvalidValue;")
+    S("    part = reinterpret_cast<double*>((char*)a.scratch + off);")
+    S("  }")
+    S("  const dim3 grid2(grid, (unsigned)nseg);")
+    S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event, a.scratch, part")
     S("#define ME_LAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
-    S("    K<<<grid, %d, SMEM, a.stream>>>(ME_ARGS); } while (0)" % block)
+    S("    K<<<grid2, %d, SMEM, a.stream>>>(ME_ARGS); } while (0)" % block)
     S("  if (sh) {       // slices of at most ME_SHARE_SLICE events, one after the other on the stream: the scratch (one region per CTA) stays bounded")
     S("    for (long start = 0; start < a.npad; start += ME_SHARE_SLICE) {")
     S("      const long np = a.npad - start < ME_SHARE_SLICE ? a.npad - start : ME_SHARE_SLICE, nn = a.n - start < np ? a.n - start : np;")
-    S("      const unsigned sgrid = (unsigned)((np + %d - 1) / %d);" % (block, block))
-    S("#define ME_SARGS a.mom + (start / ME_PAGE) * (%d * 4 * ME_PAGE), nn, np, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out + start, nullptr, nullptr, nullptr, a.scratch" % NPAR)
+    S("      const dim3 sgrid((unsigned)((np + %d - 1) / %d), (unsigned)nseg);      // (nseg > 1 only for batches far below one slice)" % (block, block))
+    S("#define ME_SARGS a.mom + (start / ME_PAGE) * (%d * 4 * ME_PAGE), nn, np, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out + start, nullptr, nullptr, nullptr, a.scratch, part" % NPAR)
     S("#define ME_SLAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
     S("    K<<<sgrid, %d, SMEM, a.stream>>>(ME_SARGS); } while (0)" % block)
-    S("      if (precision == 0) ME_SLAUNCH((k_%s<double, double, true, true>), smt);" % name)
+    S("      if (nseg > 1) {")
+    S("        if (precision == 0) ME_SLAUNCH((k_%s<double, double, true, true, true>), smt);" % name)
+    S("        else if (precision == 1) ME_SLAUNCH((k_%s<double, float, true, true, true>), smt);" % name)
+    S("        else ME_SLAUNCH((k_%s<float, float, false, true, true>), smf);" % name)
+    S("      } else if (precision == 0) ME_SLAUNCH((k_%s<double, double, true, true>), smt);" % name)
     S("      else if (precision == 1) ME_SLAUNCH((k_%s<double, float, true, true>), smt);" % name)
     S("      else ME_SLAUNCH((k_%s<float, float, false, true>), smf);" % name)
     S("#undef ME_SLAUNCH")
@@ -801,6 +846,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  }")
     S("#undef ME_LAUNCH")
     S("#undef ME_ARGS")
+    S("  if (nseg > 1) k_sum_steps_%s<<<(unsigned)((a.n + 255) / 256), 256, 0, a.stream>>>(part, a.nhel, a.n, a.norm_hel, a.inv_avg, a.me_out);" % name)
     S("  return cudaGetLastError();")
     S("}")
     # ---- the sharing kernel on a scratch that nobody allocates (include/me.h me_compute_static): a file-scope device array of a fixed size
@@ -830,7 +876,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  // nothing in the array has to start at zero: the first step of the helicity walk writes every vector before any step reads it")
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
     S("  const size_t smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.TM0, block))
-    S("#define ME_TARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, nullptr, nullptr, nullptr, ptr")
+    S("#define ME_TARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, nullptr, nullptr, nullptr, ptr, nullptr")
     S("#define ME_TLAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
     S("    K<<<grid, %d, SMEM, a.stream>>>(ME_TARGS); } while (0)" % block)
@@ -847,10 +893,12 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     walk = gray_walk()
     rank = [walk.index(h) for h in range(1 << NPAR)]
     S("static const unsigned char gray_rank_%s[%d] = {%s};" % (name, 1 << NPAR, ", ".join(str(r) for r in rank)))
-    S("static size_t scratch_%s(int precision, long npad, int share, int) {" % name)
+    S("// current cache (sharing on) + for small batches the per-step buffer of the helicity-segment split, sized for the full helicity list")
+    S("static size_t scratch_%s(int precision, long npad, int share, int nsm) {" % name)
     S("  if (!share) return 0;")
-    S("  const long np = npad < ME_SHARE_SLICE ? npad : ME_SHARE_SLICE;")
-    S("  return (size_t)((np + %d - 1) / %d) * %d * 8 * %d * (precision == 2 ? sizeof(float) : sizeof(double));" % (block, block, NSCVEC, block))
+    S("  const int nseg = segments_%s(npad, %d, nsm);" % (name, 1 << NPAR))
+    S("  const size_t cache = cache_bytes_%s(precision, npad, nseg);" % name)
+    S("  return nseg > 1 ? (cache + 255) / 256 * 256 + sizeof(double) * %d * (size_t)npad : cache;" % (1 << NPAR))
     S("}")
     nh = 1 << NPAR
     shared = 0

@@ -736,6 +736,28 @@ def test_share_currents_option(me, orc):
         c.close()
 
 
+def test_helicity_segments_of_small_batches(me):
+    """g g -> t t~ g g, small batches: the launcher splits the helicity list of an event block over several CTAs (segments of the walk, a
+    per-step buffer, a sum in list order) so that a few thousand events fill the device.  The sum runs over the same numbers in the same
+    order as the single-segment kernel of large batches: a batch small enough to be split equals the prefix of a batch that is not, bit for
+    bit, in every precision and with parity pairing (32 steps: fewer segments)."""
+    cfg = inputs.CONFIGS[3]
+    n_big = 40000                                           # 313 CTAs: more than the 2 x 148 CTA slots of a B200, one segment
+    ctx = me.MEContext(3)
+    _, mom, _ = gen_events(me, ctx, cfg, n_big)
+    ctx.me_filter_helicities(mom, 32)
+    for pairing in (0, 1):
+        ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, pairing)
+        for name in ("fp64", "mixed", "fp32"):
+            big = ctx.me_compute(mom, n_big, me.PRECISIONS[name]).cpu().numpy()
+            assert np.isfinite(big).all() and (big > 0).all()
+            for m in (32, 1000, 4096, 8192, 18000):        # 1 .. 141 CTAs: 8, 8, 8, 4, 2 segments (4, 4, 4, 4, 2 with pairing)
+                small = ctx.me_compute(mom, m, me.PRECISIONS[name]).cpu().numpy()
+                assert np.array_equal(small, big[:m]), (pairing, name, m)
+    ctx.me_set_option(me.ME_OPT_PARITY_PAIRING, 0)
+    ctx.close()
+
+
 def test_share_currents_staged_process(me, orc):
     """ME_OPT_SHARE_CURRENTS for g g -> t t~ g g g: the helicity list is grouped by gluon helicities (padded groups of four), the last
     diagram kernel forms its colour-ordered four-gluon currents once per group.  On / off agree to rounding in every precision, also
