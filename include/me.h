@@ -141,7 +141,9 @@ me_status me_set_helicities(me_ctx* ctx, const uint64_t mask[2]);
 /* The hot path.  Asynchronous on `stream`
  * (a cudaStream_t passed as void*; null = default stream).  No host<->device copy, no
  * synchronisation (except a one-off scratch allocation for ME_GG_TTXGGG, and for ME_GG_TTXGG with
- * ME_OPT_SHARE_CURRENTS, the first time; the scratch is bounded whatever n is).
+ * ME_OPT_SHARE_CURRENTS, the first time or when a later call needs more; the scratch is bounded whatever n is).
+ * The result of an event does not depend on the batch it is in: a batch of any size, sliced or (ME_GG_TTXGG, small batches) with the
+ * helicity list of an event block split over several thread blocks, gives every event the same bits.
  *   d_momenta : DEVICE, FP64 in every precision mode, AoSoA [ceil(n/P)][npar][4][P] with
  *               P = me_info.page and component order (E,px,py,pz); event e lives at page e/P,
  *               lane e%P.  The last page must be allocated in full; lanes >= n are read
