@@ -331,10 +331,11 @@ def main():
         # short form of --sweep in every default run (Fig. 1): throughput against batch
         # size, and 1 / 2 / 4 / 8 producers sharing the GPU, each with its own context and stream and a batch of 8192 events
         sw = {"batch": {}, "streams_x_8192": {}}
+        nsm = torch.cuda.get_device_properties(local).multi_processor_count
         nb = 8192
         while nb <= n:
             t, pp = timed(ctx, mom, nb, me.ME_FP64, 3, 1)
-            launches += 4 * per_step_launches
+            launches += 4 * me.launches_per_pass(info, ngood, nb, nsm)
             sw["batch"][str(nb)] = nb / (min(pp) * 1e-3)
             nb *= 4
         ctxs = [ctx] + [me.MEContext(HL) for _ in range(7)]
@@ -356,7 +357,7 @@ def main():
                     torch.cuda.current_stream().wait_stream(sts[k])
                 e1.record(); e1.synchronize()
                 best = min(best, e0.elapsed_time(e1))
-                launches += ns * per_step_launches
+                launches += ns * me.launches_per_pass(info, ngood, 8192, nsm)
             sw["streams_x_8192"][str(ns)] = ns * 8192 / (best * 1e-3)
         for c in ctxs[1:]:
             c.close()

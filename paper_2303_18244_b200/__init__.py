@@ -129,11 +129,16 @@ def me_fma_peak(fp64):
     return v.value
 
 
-def launches_per_pass(info, nhel):
+def launches_per_pass(info, nhel, n=None, nsm=None, shared=True):
     """kernels one me_compute pass launches for `nhel` helicities: one for the single-kernel processes; for the staged process
-    (info.nkernels > 1: diagram kernels + colour sum per helicity chunk of 32, plus the memset that clears the staging buffer is not
-    a kernel of ours and is not counted)"""
+    (info.nkernels > 1: diagram kernels + colour sum per helicity chunk of 32; the memset that clears the staging buffer in float mode
+    is not a kernel of ours and is not counted).  g g -> t t~ g g with current sharing on and a batch of n events that leaves CTA slots
+    of the nsm multiprocessors free: the helicity list is split over several CTAs and a second kernel sums the steps (two launches)."""
     if info.nkernels <= 1:
+        if info.npar == 6 and shared and n is not None and nsm is not None:
+            ctas = (n + info.page - 1) // info.page * info.page // 128 + (1 if ((n + info.page - 1) // info.page * info.page) % 128 else 0)
+            if min((2 * nsm) // max(ctas, 1), nhel // 8) > 1:
+                return 2
         return 1
     return info.nkernels * ((nhel + 31) // 32)
 
