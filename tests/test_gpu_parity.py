@@ -595,6 +595,36 @@ def test_gpu_against_brute_force_explicit_colour(me, proc, hels):
     ctx.close()
 
 
+@pytest.mark.parametrize("proc,hels", [(2, range(32)), (3, (0, 5, 27, 38, 63)), (4, (0, 77, 126))])
+def test_gpu_jamps_against_colour_ordered_recursion(me, proc, hels):
+    """every colour-flow amplitude of me_compute_jamps, one by one, against the colour-ordered Berends-Giele recursion of
+    tests/berends_giele.py (SURVEY.md line 408): no diagram list, no colour algebra, no oracle.  The library strips g_s^n and a global phase
+    (include/me.h), and the external states of the recursion come with their own phases: one complex constant per helicity
+    configuration, of modulus g_s^n, must relate all n! amplitudes."""
+    import itertools
+    import berends_giele as bg
+    from brute_force import GS
+    cfg = inputs.CONFIGS[proc]
+    n = proc + 1
+    npar = cfg["npar"]
+    ctx = me.MEContext(proc)
+    _, mom, _ = gen_events(me, ctx, cfg, 3, first_event=7000 + proc)
+    p = to_aos(mom, 3, cfg)
+    perms = list(itertools.permutations(range(n)))
+    e = 2
+    for ih in hels:
+        hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
+        A = bg.ordered_amplitudes(n, p[e], hel)
+        a = np.array([A[s] for s in perms])
+        j = ctx.me_compute_jamps(mom, 3, ih).cpu().numpy()       # [ncolor][2][3]
+        j = j[:, 0, e] + 1j * j[:, 1, e]
+        k = int(np.argmax(np.abs(j)))
+        c = a[k] / j[k]
+        assert abs(abs(c) / GS ** n - 1) < 1e-11, (proc, ih, abs(c), GS ** n)
+        assert np.abs(a - c * j).max() <= 1e-10 * np.abs(a).max(), (proc, ih, np.abs(a - c * j).max() / np.abs(a).max())
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------------- concurrency contract (include/me.h)
 def test_streams_and_contexts_sharing_the_gpu(me):
     """PAPER.md line 65 / Fig. 1: several producers sharing one GPU.  (a) one context per stream, each stream its own slice of

@@ -309,3 +309,49 @@ def test_brute_force_explicit_colour(orc, process, hels):
         hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
         ref = explicit_colour_me_hel(n, p[0], hel)
         assert abs(mh[0, ih] - ref) < 1e-10 * max(ref, 1e-6 * scale), (process, ih, mh[0, ih], ref)
+
+
+# ---------------------------------------------------------------------------------- colour-ordered recursion (SURVEY.md line 408)
+@pytest.mark.parametrize("n,hels", [(2, range(16)), (3, (0, 7, 21, 30)), (4, (5, 38))])
+def test_colour_ordered_recursion_against_explicit_colour(n, hels):
+    """pins the helper tests/berends_giele.py itself, with nothing of the oracle involved: the n! ordered amplitudes contracted with the
+    numeric colour matrix of their T-strings (explicit Gell-Mann matrices) equal the colour-dressed brute force of tests/brute_force.py"""
+    import berends_giele as bg
+    from brute_force import explicit_colour_me_hel
+    import oracle
+    p, _ = oracle.events(n - 1, 1, seed=600 + n - 1)          # (only the seeded event generator is taken from the oracle package)
+    perms, C = bg.colour_matrix(n)
+    assert np.abs(C - C.conj().T).max() < 1e-14 and np.abs(C.imag).max() < 1e-14
+    npar = n + 2
+    for ih in hels:
+        hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
+        A = bg.ordered_amplitudes(n, p[0], hel)
+        a = np.array([A[s] for s in perms])
+        ref = explicit_colour_me_hel(n, p[0], hel)
+        got = float((a.conj() @ C @ a).real)
+        assert abs(got - ref) <= 1e-12 * ref + 1e-22, (n, ih, got, ref)      # (helicities that vanish identically come out as ~1e-28)
+
+
+@pytest.mark.parametrize("process,hels", [(1, range(16)), (2, range(32)), (3, (0, 5, 27, 38, 63)), (4, (0, 77, 101, 126))])
+def test_jamps_against_colour_ordered_recursion(orc, process, hels):
+    """every colour-flow amplitude of the oracle, one by one, against the colour-ordered Berends-Giele recursion (no diagram list, no
+    colour algebra): equal up to the phase convention of the external states (one unit-modulus constant per helicity configuration),
+    in the basis order of reading C4/C5 (strings T^{s(1)}..T^{s(n)} in lexicographic order of s, s(1) next to the t)"""
+    import itertools
+    import berends_giele as bg
+    n = process + 1
+    npar = n + 2
+    p, _ = orc.events(process, 1, seed=600 + process)
+    perms = list(itertools.permutations(range(n)))
+    for ih in hels:
+        hel = [+1 if (ih >> (npar - 1 - k)) & 1 else -1 for k in range(npar)]
+        A = bg.ordered_amplitudes(n, p[0], hel)
+        a = np.array([A[s] for s in perms])
+        j = orc.jamps(process, p[0], ih)
+        k = int(np.argmax(np.abs(j)))
+        if np.abs(a).max() < 1e-12:                               # a helicity configuration that vanishes identically
+            assert np.abs(j).max() < 1e-12
+            continue
+        c = a[k] / j[k]
+        assert abs(abs(c) - 1) < 1e-12, (process, ih, c)          # the oracle's jamps carry g_s^n and every i of the rules
+        assert np.abs(a - c * j).max() <= 1e-11 * np.abs(a).max(), (process, ih, np.abs(a - c * j).max() / np.abs(a).max())
