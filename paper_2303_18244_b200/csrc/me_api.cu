@@ -456,7 +456,9 @@ extern "C" me_status me_compute_host(me_ctx* c, const double* h_mom, int64_t n, 
   int k = 0;
   for (int64_t first = 0; first < n && e == cudaSuccess && ms == ME_OK; ++k) {
     const int b = k & 1;
-    const int64_t m = n - first < slice ? n - first : slice;
+    // the first slice is a third of a unit (one wave of two CTAs per SM): the kernels start after 1/9 of the copy time of a full slice
+    const int64_t want = (k == 0 && n > slice) ? unit / 3 : slice;
+    const int64_t m = n - first < want ? n - first : want;
     const int64_t mpad = (m + ME_PAGE - 1) / ME_PAGE * ME_PAGE;
     cudaStream_t cs = (b == 1 && !one_stream) ? c->s_comp : st;
     if (k >= 2) HOST_TRY(cudaStreamWaitEvent(c->s_h2d, c->ev_comp[b], 0), "host wait");      // slice k - 2 no longer reads this buffer
