@@ -195,6 +195,7 @@ class KernelEmitter:
     def prologue(self):
         T, n = self.T, self.T.n
         full = T.full
+        self.smem_names = []
         P = []
         A = P.append
         sgn = lambda l: 1 if l < 2 else -1
@@ -230,15 +231,33 @@ class KernelEmitter:
             A("const P4<double> Kd%d = {%s};" % (m, ", ".join(comps)))
             fixed += 4 * (len(b) - 1)
             if m in self.used_K:
-                A("const P4<R> K%d = pcast<R>(Kd%d);" % (m, m))
+                if n in SMEM_KQ:      # FP64: parked in shared memory, reloaded at every use (volatile: the compiler must not keep it in a register)
+                    A("const P4<R> K%dr = pcast<R>(Kd%d);" % (m, m))
+                    A("if constexpr (sizeof(R) == 8) stp<R>(sm + ME_EO(%d), K%dr);" % (4 * len(self.smem_names), m)); self.smem_names.append("K%d" % m)
+                else:
+                    A("const P4<R> K%d = pcast<R>(Kd%d);" % (m, m))
             if m in self.used_q:
-                A("const P4<R> Q%d = pcast<R>(psub(pd2, Kd%d));" % (m, m))
+                if n in SMEM_KQ:
+                    A("const P4<R> Q%dr = pcast<R>(psub(pd2, Kd%d));" % (m, m))
+                    A("if constexpr (sizeof(R) == 8) stp<R>(sm + ME_EO(%d), Q%dr);" % (4 * len(self.smem_names), m)); self.smem_names.append("Q%d" % m)
+                else:
+                    A("const P4<R> Q%d = pcast<R>(psub(pd2, Kd%d));" % (m, m))
                 fixed += 4
+        self.smem_bases = []
+        base_slot = 4 * len(self.smem_names)
         for l in range(n):
-            A("const GluonBasis<R> gb%d = gluon_basis(pcast<R>(pd%d));" % (l, particle_of(l)))
+            if n in SMEM_KQ:
+                A("const GluonBasis<R> gb%dr = gluon_basis(pcast<R>(pd%d));" % (l, particle_of(l)))
+                A("if constexpr (sizeof(R) == 8) stgb<R>(sm, %d, gb%dr);" % (base_slot + 6 * len(self.smem_bases), l)); self.smem_bases.append(("gb%d" % l, "GluonBasis"))
+            else:
+                A("const GluonBasis<R> gb%d = gluon_basis(pcast<R>(pd%d));" % (l, particle_of(l)))
             fixed += 20
-        A("const SpinorBasis<R> sbt = spinor_basis(pcast<R>(pd2), mt);")
-        A("const SpinorBasis<R> sbtb = spinor_basis(pcast<R>(pd3), mt);")
+        for nm, pd in (("sbt", "pd2"), ("sbtb", "pd3")):
+            if n in SMEM_KQ:
+                A("const SpinorBasis<R> %sr = spinor_basis(pcast<R>(%s), mt);" % (nm, pd))
+                A("if constexpr (sizeof(R) == 8) stsb<R>(sm, %d, %sr);" % (base_slot + 6 * len(self.smem_bases), nm)); self.smem_bases.append((nm, "SpinorBasis"))
+            else:
+                A("const SpinorBasis<R> %s = spinor_basis(pcast<R>(%s), mt);" % (nm, pd))
         fixed += 40
         self.fixed_flops = fixed
         return ["    " + s for s in P]
@@ -261,6 +280,9 @@ def colour_sum_lines(C, ncol, denom):
     return out, flops
 
 
+SMEM_KQ = {3}      # gluon counts whose kernel parks the helicity-independent momenta K_m, Q_m in shared memory instead of registers
+
+
 def emit_single_kernel_process(n, name):
     """g g -> t t~ + (n-2) g evaluated by ONE kernel (n = 2,3,4): jamps in registers/local, in-kernel colour sum."""
     T = Topology(n)
@@ -277,6 +299,27 @@ def emit_single_kernel_process(n, name):
     S("#include \"hel_amp.cuh\"")
     S("#include \"kernels.h\"")
     S("namespace me {")
+    if K.smem_names:
+        S("// a four-momentum parked in shared memory (paired layout of hel_amp.cuh), loaded where it is used and not kept")
+        S("// (FP32: registers suffice, the value computed in the prologue is returned as it is)")
+        S("template <typename R> ME_DEV P4<R> ldpv(const R* p, const P4<R>& in_registers);")
+        S("template <> ME_DEV P4<double> ldpv<double>(const double* p, const P4<double>&) {")
+        S("  const unsigned a = (unsigned)__cvta_generic_to_shared(p); P4<double> v;")
+        S("  asm volatile(\"ld.volatile.shared.v2.f64 {%0, %1}, [%2];\" : \"=d\"(v.e), \"=d\"(v.x) : \"r\"(a));")
+        S("  asm volatile(\"ld.volatile.shared.v2.f64 {%%0, %%1}, [%%2 + %d];\" : \"=d\"(v.y), \"=d\"(v.z) : \"r\"(a));" % (16 * 128))
+        S("  return v;")
+        S("}")
+        S("template <> ME_DEV P4<float> ldpv<float>(const float*, const P4<float>& in_registers) { return in_registers; }")
+        S("// the same for the five numbers of a polarisation / spinor basis (both structs are five reals in the order ld5 / st5 store them)")
+        S("template <typename R, typename B> ME_DEV B ld5v(const R* p, const B& in_registers) {")
+        S("  if constexpr (sizeof(R) == 8) {")
+        S("    const unsigned a = (unsigned)__cvta_generic_to_shared(p); double v[5];")
+        S("    asm volatile(\"ld.volatile.shared.v2.f64 {%0, %1}, [%2];\" : \"=d\"(v[0]), \"=d\"(v[1]) : \"r\"(a));")
+        S("    asm volatile(\"ld.volatile.shared.v2.f64 {%%0, %%1}, [%%2 + %d];\" : \"=d\"(v[2]), \"=d\"(v[3]) : \"r\"(a));" % (16 * 128))
+        S("    asm volatile(\"ld.volatile.shared.f64 %%0, [%%1 + %d];\" : \"=d\"(v[4]) : \"r\"(a));" % (4 * 8 * 128))
+        S("    return B{(R)v[0], (R)v[1], (R)v[2], (R)v[3], (R)v[4]};")
+        S("  } else return in_registers;")
+        S("}")
     S("#define JR(s) Jr[s]")
     S("#define JI(s) Ji[s]")
     S("template <typename R, typename RC>")
@@ -285,11 +328,18 @@ def emit_single_kernel_process(n, name):
       " const int* __restrict__ helpe) {" % name)
     S("  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;")
     S("  if (e >= npad) return;")
+    if K.smem_names:
+        S("  extern __shared__ __align__(16) unsigned char smem_raw[];")
+        S("  R* sm = reinterpret_cast<R*>(smem_raw) + 2 * threadIdx.x;")
     S("  const double* pm = mom + (e >> 5) * (%d * 4 * 32) + (e & 31);" % npar)
     for k in range(npar):
         S("  const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
     S("  const R mt = (R)mt_d;")
     src.extend(pro)
+    for i, nm in enumerate(K.smem_names):
+        S("#define %s ldpv<R>(sm + ME_EO(%d), %sr)" % (nm, 4 * i, nm))
+    for i, (nm, ty) in enumerate(K.smem_bases):
+        S("#define %s ld5v<R, %s<R> >(sm + ME_EO(%d), %sr)" % (nm, ty, 4 * len(K.smem_names) + 6 * i, nm))
     S("  double acc = 0;")
     S("  for (int ih = 0; ih < nhel; ++ih) {")
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
@@ -317,14 +367,21 @@ def emit_single_kernel_process(n, name):
     S("    acc += meh;")
     S("  }")
     S("  if (me_out != nullptr && e < n) me_out[e] = acc * norm_hel * inv_avg;")
+    for nm in K.smem_names + [b for b, _ in K.smem_bases]:
+        S("#undef %s" % nm)
     S("}")
     per_hel = K.flops + cs_flops + 2 * FLOPS["spinor"]
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + ME_BLOCK - 1) / ME_BLOCK);")
     S("#define ME_ARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, a.me_hel, a.jamp_out, a.hel_per_event")
-    S("  if (precision == 0) k_%s<double, double><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)
-    S("  else if (precision == 1) k_%s<double, float><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)
-    S("  else k_%s<float, float><<<grid, ME_BLOCK, 0, a.stream>>>(ME_ARGS);" % name)
+    nsl = 4 * len(K.smem_names) + 6 * len(K.smem_bases)
+    S("  const size_t smd = sizeof(double) * %d * ME_BLOCK, smf = 0;" % nsl)
+    if nsl:
+        for inst, sm_ in (("double, double", "smd"), ("double, float", "smd"), ("float, float", "smf")):
+            S("  cudaFuncSetAttribute(k_%s<%s>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)%s);" % (name, inst, sm_))
+    S("  if (precision == 0) k_%s<double, double><<<grid, ME_BLOCK, smd, a.stream>>>(ME_ARGS);" % name)
+    S("  else if (precision == 1) k_%s<double, float><<<grid, ME_BLOCK, smd, a.stream>>>(ME_ARGS);" % name)
+    S("  else k_%s<float, float><<<grid, ME_BLOCK, smf, a.stream>>>(ME_ARGS);" % name)
     S("#undef ME_ARGS")
     S("  return cudaGetLastError();")
     S("}")
