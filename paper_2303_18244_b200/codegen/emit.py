@@ -336,6 +336,8 @@ def emit_single_kernel_process(n, name):
         S("  const P4<double> pd%d = {pm[%d], pm[%d], pm[%d], pm[%d]};" % (k, (4 * k) * 32, (4 * k + 1) * 32, (4 * k + 2) * 32, (4 * k + 3) * 32))
     S("  const R mt = (R)mt_d;")
     src.extend(pro)
+    if K.smem_names:
+        S("  ME_FENCE;      // the stores above are complete before the volatile loads below (their asm statements name no memory operand)")
     for i, nm in enumerate(K.smem_names):
         S("#define %s ldpv<R>(sm + ME_EO(%d), %sr)" % (nm, 4 * i, nm))
     for i, (nm, ty) in enumerate(K.smem_bases):
