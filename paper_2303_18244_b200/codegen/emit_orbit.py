@@ -24,6 +24,7 @@ from .topology import _pmul, _pcomm, _pscale, color_matrix
 
 N = 4
 NPAR = 6
+PARK_SB = True             # tensor-memory kernels: spinor bases of t and t~ in shared memory instead of 20 registers held across the helicity walk
 MIN_SEG_STEPS = 8          # helicity-segment split of small batches: steps of the helicity list per segment at least (every segment starts with a full evaluation)
 STATIC_MAX_EVENTS = 8192   # me_compute_static: events one call takes (its current cache is a file-scope device array of 64 CTAs x 208 KB = 13 MiB)
 NSCVEC_TRIPLES = 8  # current sharing: vectors parked per thread in the L2-resident scratch: two ordered currents per three-gluon sub-tree,
@@ -700,6 +701,10 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    sbt = spinor_basis(pcast<R>(pd2), mt);")
     S("    sbtb = spinor_basis(pcast<R>(pd3), mt);")
     fixed += 40
+    if PARK_SB:
+        S("    // tensor-memory kernels: the two spinor bases are parked in the shared memory behind the %d slots (slots >= %d are tensor memory" % (lay.TM0, lay.TM0))
+        S("    // there) and reloaded at the top of every step instead of holding 20 registers across the helicity walk")
+        S("    if constexpr (TM) { stsb<R>(sm + ME_EO(%d), sbt); stsb<R>(sm + ME_EO(%d), sbtb); }" % (lay.TM0, lay.TM0 + 6))
     S("  }")
     S("  R* sc = nullptr;")
     S("  if constexpr (SH) sc = reinterpret_cast<R*>(scratch) + ((size_t)((SEG ? blockIdx.y * gridDim.x : 0u) + blockIdx.x) * (%d * 8 * ME_SM_STRIDE) + 2 * threadIdx.x);" % NSCVEC)
@@ -718,8 +723,12 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("    const int h = helpe != nullptr ? helpe[e < n ? e : n - 1] : hels[ih];")
     S("    const int chg = (SH && hprev >= 0) ? (h ^ hprev) : %d;      // helicities that changed since the previous step" % ((1 << NPAR) - 1))
     S("    hprev = h;")
-    S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
-    S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
+    if PARK_SB:
+        S("    const W4<R> ub = spinor_ubar(TM ? ldsb<R>(sm + ME_EO(%d)) : sbt, lam_of<R>(h, %d));" % (lay.TM0, NPAR - 1 - 2))
+        S("    const W4<R> vv = spinor_v(TM ? ldsb<R>(sm + ME_EO(%d)) : sbtb, lam_of<R>(h, %d));" % (lay.TM0 + 6, NPAR - 1 - 3))
+    else:
+        S("    const W4<R> ub = spinor_ubar(sbt, lam_of<R>(h, %d));" % (NPAR - 1 - 2))
+        S("    const W4<R> vv = spinor_v(sbtb, lam_of<R>(h, %d));" % (NPAR - 1 - 3))
     S("    const W4<R> jtt = bilinear(ub, vv);")
     S("    if constexpr (TM) {")
     S("      const uint32_t zz[16] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};")
@@ -801,7 +810,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("}")
     S("static cudaError_t launch_%s(int precision, const LaunchArgs& a) {" % name)
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
-    S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.nslots, block, lay.TM0, block))
+    S("  const size_t smd = sizeof(double) * %d * %d, smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.nslots, block, lay.TM0 + (12 if PARK_SB else 0), block))
     S("  // FP64 amplitudes (double and mixed): tensor-memory kernel, two CTAs per SM; ME_NO_TMEM=1 selects the shared-memory-only kernel (A/B timing)")
     S("  static const bool no_tmem = getenv(\"ME_NO_TMEM\") != nullptr && getenv(\"ME_NO_TMEM\")[0] == '1';")
     S("  const bool sh = a.share != 0 && a.hel_per_event == nullptr && a.scratch != nullptr && !no_tmem && a.me_hel == nullptr && a.jamp_out == nullptr && a.me_out != nullptr;")
@@ -875,7 +884,7 @@ def emit_orbit_process(name="gg_ttxgg", block=128):
     S("  }")
     S("  // nothing in the array has to start at zero: the first step of the helicity walk writes every vector before any step reads it")
     S("  const unsigned grid = (unsigned)((a.npad + %d - 1) / %d);" % (block, block))
-    S("  const size_t smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.TM0, block))
+    S("  const size_t smf = sizeof(float) * %d * %d, smt = sizeof(double) * %d * %d;" % (lay.nslots, block, lay.TM0 + (12 if PARK_SB else 0), block))
     S("#define ME_TARGS a.mom, a.n, a.npad, a.hels, a.nhel, a.mt, a.norm_hel, a.inv_avg, a.me_out, nullptr, nullptr, nullptr, ptr, nullptr")
     S("#define ME_TLAUNCH(K, SMEM) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)); \\")
     S("    cudaFuncSetAttribute(K, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \\")
